@@ -1,0 +1,381 @@
+#!/usr/bin/env python
+"""bench.py -- SegPagedAttention on B200: useful TFLOP/s, roofline fraction, ms per layer.
+
+A "step" is one pass of the whole hot path over one batch of synthetic
+input, all through the C ABI (include/segpa.h):
+    segpa_append_pages   (a1: scatter the batch's K/V rows, resident in HBM, into per-head pages)
+    segpa_build_segments (a2-a5: page selection, translation, descriptor packing, tile schedule, H2D)
+    segpa_attention_fwd  (a6-a8: fused attention [+ split-KV combine]; heads merged by layout)
+Default workload: BASELINE.json configs[1] (Llama-3-8B-shaped layer).  `--config {1..5,4d}` selects
+another one for profiling.  Multi-GPU: the path does not shard (BASELINE north_star: one GPU, no
+collectives) -> N independent replicas, "scaling": "weak".
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "segpa_useful_tflops"
+UNIT = "TFLOP/s (useful: 4*D per attended (query, key, q-head) pair)"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return d, "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
+
+
+def get_workload(name: str):
+    from paper_2606_06256_b200 import workloads as wl
+    if name == "4d":
+        return wl.config4(decode_only=True)
+    return wl.CONFIGS[int(name)]()
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.samples = []
+        self.proc = None
+        self.idx = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------
+# oracle legs (cpu_baseline and --impl reference): the oracle as it stands on the host cores
+# ---------------------------------------------------------------------------------------------
+def oracle_sample(w, budget_rows: int, seed: int = 0, k_pool=None, v_pool=None, q=None):
+    """Times the oracle on a bounded row sample of layer 0 of `w`. Returns (tflops, seconds, cores, pairs, desc)."""
+    import torch  # noqa: F401
+    import oracle
+    from paper_2606_06256_b200 import workloads as wl
+    if k_pool is None:
+        k_pool, v_pool = wl.pool_values(w, "cpu")
+        q = wl.q_values(w, 0, "cpu")
+    rng = np.random.default_rng(seed)
+    T = w.T[0]
+    rows = np.sort(rng.choice(T, size=min(budget_rows, T), replace=False)).astype(np.int64)
+    table, offs, kv_lens, index = wl.csr_page_tables(w, 0)
+    segs = [(index[(s.kv_head, s.seq_id)], s.kv_head, s.head_class, s.window, s.n_sink, s.q_row_start, s.q_len)
+            for s in w.layer_segments(0)]
+    t0 = time.perf_counter()
+    res = oracle.oracle_attention(Hq=w.Hq, Hkv=w.Hkv, D=w.D, P=w.P, k_pool=k_pool, v_pool=v_pool, page_table=table,
+                                  pt_offsets=offs, kv_lens=kv_lens, segments=segs, q=q, T=T, scale=w.scale,
+                                  row_subset=rows)
+    dt = time.perf_counter() - t0
+    flops = res.pairs * 4 * w.D
+    desc = "%d uniformly sampled query rows of %d (all heads, layer 0) of %s; %d attended pairs" % (len(rows), T, w.name, res.pairs)
+    return flops / dt / 1e12, dt, oracle.num_threads(), res.pairs, desc
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = get_workload(args.config)
+    from paper_2606_06256_b200 import workloads as wl
+    k_pool, v_pool = wl.pool_values(w, "cpu")
+    q = wl.q_values(w, 0, "cpu")
+    rows = args.ref_rows
+    vals, times = [], []
+    for i in range(args.warmup + args.steps):
+        tf, dt, cores, pairs, desc = oracle_sample(w, rows, seed=i, k_pool=k_pool, v_pool=v_pool, q=q)
+        if i >= args.warmup:
+            vals.append(tf)
+            times.append(dt)
+    v = float(np.mean(vals))
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "note": "fp64 CPU oracle on a bounded row sample per step"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=dev)
+
+    os.environ.setdefault("SEGPA_KERNEL", "tc")
+    os.environ.setdefault("SEGPA_TC_TILES", str(args.tiles))
+    w = get_workload(args.config)
+    peaks, peaks_src = load_peaks()
+    k_pool, v_pool = wl.pool_values(w, dev)
+    qs = [wl.q_values(w, l, dev) for l in range(w.num_layers)]
+    outs = [torch.empty_like(q) for q in qs]
+    lses = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32, device=dev) for l in range(w.num_layers)]
+    # the batch's K/V rows, resident in HBM (what the QKV projections would have produced)
+    owners = [s for s in w.streams if s.shared_from is None]
+    aliased = [s for s in w.streams if s.shared_from is not None]
+    order = owners + aliased
+    rows = {}
+    for s in order:
+        pp = s.n_shared_prefix_pages
+        if s.kv_len - pp * w.P > 0:
+            rows[id(s)] = (wl.stream_rows(k_pool, s, w.P, pp), wl.stream_rows(v_pool, s, w.P, pp))
+    cache = H.create_cache(w, local_rank)
+    stream = torch.cuda.current_stream()
+    flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+    useful = sum(wl.useful_flops(w, l) for l in range(w.num_layers))
+    seg_objs = []
+    appended = [False]
+    launches = [0]
+
+    def append_all():
+        n = 0
+        if appended[0]:
+            for s in reversed(order):
+                B.segpa_free_stream(cache, s.layer, s.kv_head, s.seq_id)
+        for s in order:
+            pp = s.n_shared_prefix_pages
+            if pp > 0:
+                B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, None, None, pp * w.P, page_ids=s.page_ids[:pp])
+            if id(s) in rows:
+                kr, vr = rows[id(s)]
+                B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, kr, vr, kr.shape[0], page_ids=s.page_ids[pp:], stream=stream)
+                n += 1
+        appended[0] = True
+        return n
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(timed):
+        """one pass of the hot path; returns (step_ms, fwd_ms, n_launches) when timed"""
+        e0, e1 = ev(), ev()
+        fa, fb = [], []
+        e0.record(stream)
+        n = append_all()
+        for l in range(w.num_layers):
+            segs = H.build_layer(cache, w, l, stream=stream)
+            seg_objs.append(segs)
+            a, b = ev(), ev()
+            a.record(stream)
+            B.segpa_attention_fwd(cache, segs, qs[l], w.scale, outs[l], lses[l], stream=stream)
+            b.record(stream)
+            fa.append(a)
+            fb.append(b)
+            n += B.segpa_last_launch_count(cache)
+        e1.record(stream)
+        e1.synchronize()
+        return e0.elapsed_time(e1), sum(a.elapsed_time(b) for a, b in zip(fa, fb)), n
+
+    def free_segs():
+        torch.cuda.synchronize()
+        for s in seg_objs:
+            B.segpa_free_segments(cache, s)
+        seg_objs.clear()
+
+    for _ in range(args.warmup):
+        step(False)
+        flush_buf.fill_(1)
+    free_segs()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    step_ms, fwd_ms = [], []
+    wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush_buf.fill_(1)                      # L2 flush between timed iterations (outside the events)
+        torch.cuda.synchronize()
+        sm, fm, n = step(True)
+        step_ms.append(sm)
+        fwd_ms.append(fm)
+        launches[0] += n
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    free_segs()
+    total_ms = float(sum(step_ms))
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * useful / (ms_per_step * 1e-3) / 1e12
+    fwd_mean = float(np.mean(fwd_ms))
+
+    # ---- e2e through the host-buffer entry point: H2D of the step's K/V rows and Q, D2H of out + LSE
+    h_rows = {k: (a.cpu().pin_memory(), b.cpu().pin_memory()) for k, (a, b) in rows.items()}
+    h_q = [q.cpu().pin_memory() for q in qs]
+    h_out = [torch.empty_like(q).pin_memory() for q in h_q]
+    h_lse = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32).pin_memory() for l in range(w.num_layers)]
+    h2d = sum(a.numel() * 2 * 2 for a, _ in h_rows.values()) + sum(q.numel() * 2 for q in h_q)
+    d2h = sum(o.numel() * 2 for o in h_out) + sum(x.numel() * 4 for x in h_lse)
+
+    def e2e_step():
+        for k, (a, b) in h_rows.items():
+            rows[k][0].copy_(a, non_blocking=True)
+            rows[k][1].copy_(b, non_blocking=True)
+        append_all()
+        for l in range(w.num_layers):
+            segs = H.build_layer(cache, w, l, stream=stream)
+            seg_objs.append(segs)
+            B.segpa_attention_fwd_host(cache, segs, h_q[l], w.scale, h_out[l], h_lse[l], stream=stream)
+        torch.cuda.synchronize()
+
+    e2e_step()
+    free_segs()
+    n_e2e = max(2, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        e2e_step()
+    e2e_s = (time.perf_counter() - t0) / n_e2e
+    free_segs()
+    if dist is not None:
+        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_val = world * useful / e2e_s / 1e12
+
+    # ---- plan statistics / algorithmic bytes for the roofline
+    segs0 = H.build_layer(cache, w, 0)
+    st0 = B.segpa_segments_stats(segs0)
+    alg_bytes = 0
+    for l in range(w.num_layers):
+        sg = segs0 if l == 0 else H.build_layer(cache, w, l)
+        st = B.segpa_segments_stats(sg)
+        cov_rows = sum(s.q_len * w.G for s in w.layer_segments(l))
+        alg_bytes += st["visible_kv_tokens"] * w.D * 2 * 2 + cov_rows * w.D * 2 * 2 + cov_rows * 4
+    torch.cuda.synchronize()
+    decode_shaped = args.config == "4d"
+    if decode_shaped:
+        roof = {"bound": "hbm", "achieved": alg_bytes / (fwd_mean * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    else:
+        roof = {"bound": "tensor", "achieved": useful / (fwd_mean * 1e-3) / 1e12, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s"}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["kernel"] = "attention_tc_kernel (segpa_attention_fwd), avg of %d launches-groups timed with CUDA events" % args.steps
+    roof["peak_source"] = peaks_src + (", burst figure" if not decode_shaped else "")
+    roof["algorithmic_bytes"] = alg_bytes
+    roof["useful_flops"] = useful
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": w.name, "Hq": w.Hq, "Hkv": w.Hkv, "D": w.D, "page_size": w.P, "layers": w.num_layers,
+                       "q_rows": int(sum(w.T)), "segments": len(w.segments), "l2_flush_between_steps": True,
+                       "step": "append_pages + build_segments + attention_fwd per layer", "tiles_per_item": int(os.environ["SEGPA_TC_TILES"]),
+                       "replicas": world},
+            "fwd_ms_per_step": fwd_mean, "us_per_layer": 1e3 * fwd_mean / w.num_layers,
+            "pct_of_bf16_peak": 100.0 * (useful / (fwd_mean * 1e-3) / 1e12) / peaks["bf16_tflops"],
+            "plan": {k: st0[k] for k in ("n_tiles", "n_items", "n_split_tiles", "kv_blocks", "workspace_bytes")},
+            "roofline": roof, "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": 1e3 * e2e_s},
+            "gpu_launches": int(launches[0]), "wall_s_timed_region": wall}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        tf, dt, cores, pairs, desc = oracle_sample(w, args.cpu_rows, seed=0, k_pool=k_pool.cpu(), v_pool=v_pool.cpu(), q=qs[0].cpu())
+        line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc + "; %.1f s" % dt}
+    B.segpa_destroy(cache)
+    if rank == 0:
+        print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="2")
+    ap.add_argument("--tiles", type=int, default=1)
+    ap.add_argument("--cpu-rows", type=int, default=384, help="rows in the cpu_baseline oracle sample")
+    ap.add_argument("--ref-rows", type=int, default=128, help="rows per step of the --impl reference oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

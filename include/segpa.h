@@ -1,0 +1,264 @@
+/*
+ * segpa.h -- C ABI of the B200-native SegPagedAttention library (libsegpa.so).
+ *
+ * SegPagedAttention is the storage and execution substrate of RedKnot (arxiv 2606.06256,
+ * PAPER.md:233-284, Sec. 4.3, Algorithm 2): the KV cache is decomposed per (layer, KV head) into
+ * head segments stored in pages; a per-layer metadata pass selects, per KV head, the pages its
+ * policy makes visible (GLOBAL: the full range; LOCAL: sink pages + recent-window pages),
+ * translates them to physical pages and packs (h, B_h, |U_h|, p); then ONE fused variable-length
+ * attention runs over all heads' page lists, with no dense [B,H,L,D] tensor and no mask.
+ *
+ * Conventions
+ *   - Plain C, no exceptions cross this boundary; every call returns a segpa_status_t and applies
+ *     nothing on error.  segpa_last_error() gives a human-readable reason.
+ *   - "device" pointers are CUDA device pointers on the cache's device; "host" pointers are
+ *     ordinary host memory, copied during the call (the caller may free them on return).
+ *   - cuda_stream arguments are a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - bf16 = IEEE bfloat16 bit patterns (uint16_t).
+ *   - A cache is not thread-safe; use one host thread per cache at a time.
+ *   - There is no CPU fallback: on a box without a CUDA device, segpa_create_cache with
+ *     device >= 0 fails with SEGPA_ERR_CUDA.  device == -1 creates a PLANNING-ONLY cache (host
+ *     bookkeeping, builder and scheduler work; no device memory; append_pages accepts attach
+ *     calls only; attention_fwd returns SEGPA_ERR_STATE).
+ *
+ * Terms
+ *   stream   = (layer, kv_head, seq_id): the ordered tokens of ONE KV head of one request, of
+ *              length kv_len, backed by ceil(kv_len / page_size) physical pages; token j lives in
+ *              page pt[j / page_size], slot j % page_size.  It is the concatenation of the paper's
+ *              head segments (l, h, s), each mapped to consecutive virtual pages by T_seg and to
+ *              physical pages by T_page; here virtual page v of a stream is simply
+ *              index v of its page table.
+ *   segment  = execution segment: one (request, KV head) unit of a layer's attention call, i.e.
+ *              one tuple (h, B_h, |U_h|, p) of the per-layer varlen metadata M_l,
+ *              plus its query rows.
+ */
+#ifndef SEGPA_H_
+#define SEGPA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SEGPA_VERSION 1
+
+typedef enum {
+    SEGPA_OK = 0,
+    SEGPA_ERR_INVALID = 1,     /* bad argument; message says which */
+    SEGPA_ERR_OOM = 2,         /* page pool or device/host memory exhausted */
+    SEGPA_ERR_CUDA = 3,        /* a CUDA call failed (also: no device) */
+    SEGPA_ERR_UNSUPPORTED = 4, /* shape outside what the kernels are built for */
+    SEGPA_ERR_STATE = 5        /* call not valid in this state (e.g. fwd on a planning-only cache) */
+} segpa_status_t;
+
+typedef enum { SEGPA_GLOBAL = 0, SEGPA_LOCAL = 1 } segpa_head_class_t;
+
+typedef struct segpa_cache segpa_cache_t;       /* opaque */
+typedef struct segpa_segments segpa_segments_t; /* opaque; owned by the cache that built it */
+
+/* ------------------------------------------------------------------------------------------- */
+/* Per-head paged KV pool ("head-segmented KV layout"; "allocates     */
+/* pages per head, so local heads occupy only their short windows").                            */
+/* ------------------------------------------------------------------------------------------- */
+
+typedef struct {
+    int32_t num_layers;   /* >= 1 */
+    int32_t num_q_heads;  /* Hq; multiple of num_kv_heads; G = Hq / Hkv <= 16 */
+    int32_t num_kv_heads; /* Hkv */
+    int32_t head_dim;     /* D: 64 or 128 */
+    int32_t page_size;    /* P tokens per page: 16 or 32 */
+    int32_t device;       /* CUDA device ordinal, or -1 = planning-only cache */
+    int64_t num_pages;    /* pool capacity in pages; one page holds P tokens of ONE KV head */
+    void *k_pool;         /* optional caller-owned device memory of segpa_pool_bytes() bytes, */
+    void *v_pool;         /*   else NULL (library allocates). Contents are library-private.     */
+} segpa_cache_desc_t;
+
+/* Bytes needed for each of k_pool / v_pool when the caller owns them ((num_pages + 1) pages: the
+ * extra page is the library's always-zero page). */
+int64_t segpa_pool_bytes(const segpa_cache_desc_t *desc);
+
+/*
+ * Create a cache.  The pool is zero-filled.  Physical page layout is private to the library
+ * (a page is stored as the shared-memory image the attention kernel consumes, so that one bulk
+ * copy moves a page).
+ * Errors: INVALID (null, counts < 1, Hq % Hkv != 0), UNSUPPORTED (head_dim, page_size, G > 16,
+ * device is not compute capability 10.x), CUDA, OOM.
+ */
+segpa_status_t segpa_create_cache(const segpa_cache_desc_t *desc, segpa_cache_t **out);
+
+/*
+ * Extend the stream (layer, kv_head, seq_id) by n_tokens tokens (creating it if absent).
+ *
+ *  - COPY mode (k_src and v_src non-NULL): device bf16 rows; row t of the new tokens is at
+ *    k_src + t * src_row_stride_elems (D contiguous elements).  Rows are scattered into the
+ *    stream's pages by a kernel on cuda_stream.  If the stream's last page is partial the new
+ *    tokens first fill it; further pages are taken from page_ids (host int32, in order,
+ *    n_page_ids of them, each must be free) or, if page_ids == NULL, from the allocator.
+ *    Slots of a newly started page beyond the stream's end are zero-filled (masked probabilities
+ *    multiply them, so they must stay finite).
+ *  - ATTACH mode (k_src == v_src == NULL, page_ids non-NULL): the pages already hold the data
+ *    (filled earlier through another stream); they are appended to this stream's page table
+ *    without copying and their reference count is incremented.  This is both PIC chunk splicing
+ *    ("directly reusing the prefix-robust local segments") and shared-prefix
+ *    aliasing.  Requires the stream's current length to be a multiple of page_size, and
+ *    n_page_ids == ceil(n_tokens / page_size).  On a planning-only cache pages may be attached
+ *    without ever having been filled.
+ *
+ * Errors: INVALID (indices out of range, n_tokens < 1, page id out of range / not free in COPY
+ * mode / not in use in ATTACH mode on a device cache, wrong n_page_ids, one of k_src / v_src NULL),
+ * OOM (no free page), STATE (COPY on a planning-only cache), CUDA.
+ */
+segpa_status_t segpa_append_pages(segpa_cache_t *cache, int32_t layer, int32_t kv_head,
+                                  int64_t seq_id, const void *k_src, const void *v_src,
+                                  int64_t src_row_stride_elems, int64_t n_tokens,
+                                  const int32_t *page_ids, int32_t n_page_ids, void *cuda_stream);
+
+/* Drop a stream: its pages' reference counts are decremented; pages reaching zero return to the
+ * free list.  Errors: INVALID (no such stream). */
+segpa_status_t segpa_free_stream(segpa_cache_t *cache, int32_t layer, int32_t kv_head,
+                                 int64_t seq_id);
+
+/* Query a stream.  kv_len / n_pages may be NULL.  If page_ids_out != NULL, up to cap ids are
+ * written.  Errors: INVALID (no such stream). */
+segpa_status_t segpa_stream_info(const segpa_cache_t *cache, int32_t layer, int32_t kv_head,
+                                 int64_t seq_id, int64_t *kv_len, int32_t *n_pages,
+                                 int32_t *page_ids_out, int32_t cap);
+
+/* Pool occupancy: pages in use (refcount > 0) and free. Either pointer may be NULL. */
+segpa_status_t segpa_pool_stats(const segpa_cache_t *cache, int64_t *pages_in_use,
+                                int64_t *pages_free);
+
+/* ------------------------------------------------------------------------------------------- */
+/* Segment descriptor builder + tile scheduler (Alg. 2 lines 1-14).           */
+/* ------------------------------------------------------------------------------------------- */
+
+typedef struct {
+    int64_t seq_id;      /* request; the stream is (layer, kv_head, seq_id) */
+    int32_t kv_head;     /* h */
+    int32_t head_class;  /* p = P(l, h): SEGPA_GLOBAL or SEGPA_LOCAL */
+    int32_t window;      /* LOCAL: W = number of visible keys INCLUDING the query's own position
+                            (paper's w = W - 1; reading A1). >= 1.
+                            Ignored for GLOBAL. */
+    int32_t n_sink;      /* LOCAL: first n_sink tokens stay visible (S_sink).
+                            Must be 0 in this version (sinks on the GPU are NEXT #1). */
+    int64_t q_row_start; /* first row of this segment's queries in q / out */
+    int32_t q_len;       /* 1 <= q_len <= kv_len; query t has position kv_len - q_len + t
+                            (bottom-right aligned, the flash_attn_varlen convention) */
+    int32_t reserved;    /* 0 */
+} segpa_segment_req_t;
+
+/*
+ * Build one layer's metadata M_l and the tile schedule for n segments.
+ *
+ * Per segment: visible positions are [0, kv_len) for GLOBAL and
+ * [max(0, kv_len - q_len - W + 1), kv_len) for LOCAL (Alg. 2 lines 6-10); the pages covering
+ * them are translated to physical ids (line 12); pages outside the visible range are replaced by
+ * the always-zero page, so evicted pages are never read ("true eviction").  Query
+ * rows are cut into tiles of floor(128 / G) tokens x G query heads (GQA packing: the G heads of a
+ * KV head share every K/V page load); each tile gets exactly the KV block range it attends to,
+ * so no work is issued for fully masked blocks.  Long tiles are split along KV when the grid
+ * would otherwise be unbalanced, and all work items are ordered longest-first.
+ * The descriptors are uploaded with one async copy per array on cuda_stream.
+ *
+ * Queries of segment (seq_id, kv_head) are rows q_row_start .. q_row_start + q_len - 1, heads
+ * kv_head*G .. kv_head*G + G - 1 (contiguous GQA groups).  (row, head) pairs not covered by any
+ * segment are never written by attention_fwd.
+ *
+ * Errors: INVALID (n < 1, unknown stream, q_len < 1 or > kv_len, LOCAL with window < 1, bad
+ * class, negative q_row_start, two segments overlapping on (row, head)), UNSUPPORTED (n_sink != 0),
+ * OOM, CUDA.
+ */
+segpa_status_t segpa_build_segments(segpa_cache_t *cache, int32_t layer,
+                                    const segpa_segment_req_t *reqs, int32_t n,
+                                    segpa_segments_t **out, void *cuda_stream);
+
+segpa_status_t segpa_free_segments(segpa_cache_t *cache, segpa_segments_t *segs);
+
+typedef struct {
+    int32_t n_segments;
+    int32_t n_tiles;          /* (segment, token-range) tiles of <= 128 rows */
+    int32_t n_items;          /* work items after KV splitting */
+    int32_t n_split_tiles;    /* tiles cut into more than one item */
+    int32_t tile_tokens;      /* floor(128 / G) */
+    int32_t block_keys;       /* 128 */
+    int64_t kv_blocks;        /* sum over items of visited 128-key blocks */
+    int64_t attended_pairs;   /* (query, key, q head) triples actually attended */
+    int64_t q_rows;           /* max(q_row_start + q_len) */
+    int64_t visible_kv_tokens;/* sum over segments of tokens in visible pages (algorithmic K/V reads) */
+    int64_t workspace_bytes;  /* split-KV partials */
+} segpa_plan_stats_t;
+
+segpa_status_t segpa_segments_stats(const segpa_segments_t *segs, segpa_plan_stats_t *out);
+
+typedef struct {
+    int32_t segment;   /* index into reqs */
+    int32_t t0;        /* first token of the tile within the segment's q range */
+    int32_t n_tok;     /* tokens in the tile (rows = n_tok * G) */
+    int32_t kb_lo;     /* first visited 128-key block */
+    int32_t kb_hi;     /* one past the last visited block */
+    int32_t split;     /* -1: writes the output directly; >= 0: index of this item's partial */
+    int32_t n_splits;  /* number of items this tile was cut into */
+    int32_t tile;      /* tile id (items of one tile share it) */
+} segpa_item_t;
+
+/* Copy up to cap work items (in schedule order) to host memory; *n_out = total count. */
+segpa_status_t segpa_segments_items(const segpa_segments_t *segs, segpa_item_t *items_out,
+                                    int32_t cap, int32_t *n_out);
+
+/* Per-segment translated page list as uploaded (length *n_out; zero page = num_pages). */
+segpa_status_t segpa_segments_pages(const segpa_segments_t *segs, int32_t segment,
+                                    int32_t *first_page_index, int32_t *page_ids_out, int32_t cap,
+                                    int32_t *n_out);
+
+/* ------------------------------------------------------------------------------------------- */
+/* Fused attention (Alg. 2 lines 15-16).                                      */
+/* ------------------------------------------------------------------------------------------- */
+
+/*
+ * out[row][head][:] = softmax_j( softmax_scale * q[row][head] . K[j] ) V[j]  over the visible keys
+ * of the covering segment; lse[head][row] = ln sum_j exp(softmax_scale * q . K[j]) (natural log of
+ * the scaled scores).  bf16 x bf16 products accumulate in fp32 on the tensor cores; softmax runs
+ * in fp32; probabilities are rounded to bf16 before the PV product; out is rounded to bf16 (RNE).
+ * MergeHeads (Alg. 2 line 16) is the output layout itself.
+ *
+ *   q, out : device bf16, row r / head h / element d at  base + r*row_stride + h*D + d
+ *   lse    : device fp32 [Hq][lse_stride], lse_stride >= T; may be NULL
+ *   T      : number of rows in q / out (>= the plan's q_rows)
+ *
+ * Asynchronous on cuda_stream; deterministic (no floating-point atomics; split-KV partials are
+ * merged in a fixed order).  Errors: INVALID, STATE (planning-only cache, or segments built by
+ * another cache), CUDA (also reports an earlier asynchronous failure).
+ */
+segpa_status_t segpa_attention_fwd(segpa_cache_t *cache, const segpa_segments_t *segs,
+                                   const void *q, int64_t q_row_stride_elems, float softmax_scale,
+                                   void *out, int64_t out_row_stride_elems, float *lse,
+                                   int64_t lse_stride, int64_t T, void *cuda_stream);
+
+/*
+ * Same computation with HOST buffers: q is copied to the device, attention runs, out and lse are
+ * copied back, and the call returns after the copies complete (synchronous).  q/out are dense
+ * [T][Hq][D] bf16, lse [Hq][T] fp32 (may be NULL).  Staging buffers are owned by the cache and
+ * reused.  This is the end-to-end path bench.py times.
+ */
+segpa_status_t segpa_attention_fwd_host(segpa_cache_t *cache, const segpa_segments_t *segs,
+                                        const void *q_host, float softmax_scale, void *out_host,
+                                        float *lse_host, int64_t T, void *cuda_stream);
+
+/* Number of kernel launches the last attention_fwd on this cache issued (1, or 2 with split-KV). */
+int32_t segpa_last_launch_count(const segpa_cache_t *cache);
+
+/* ------------------------------------------------------------------------------------------- */
+
+/* Frees the pool (unless caller-owned), all streams and all segment objects. NULL is OK. */
+segpa_status_t segpa_destroy(segpa_cache_t *cache);
+
+/* Message for the most recent error on this thread (never NULL). */
+const char *segpa_last_error(void);
+
+int32_t segpa_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SEGPA_H_ */

@@ -1,0 +1,429 @@
+// Fused variable-length attention over per-head page lists (Alg. 2 line 15) for
+// sm_100a: cp.async.bulk (TMA) page gather -> shared memory, tcgen05.mma with TMEM accumulators
+// for S = Q K^T and O += P V, fp32 online softmax, bf16 output + fp32 LSE.  See DESIGN.md.
+//
+// One persistent CTA per SM, warp-specialised:
+//   warp 0        loader: one bulk copy per physical page into a ring of K/V stages
+//   warp 1        MMA issuer (one elected thread)
+//   warps 4..7    softmax / correction / epilogue warpgroup of tile 0 (thread = query row)
+//   warps 8..11   the same for tile 1 (NT = 2: two 128-row tiles of adjacent tokens share every
+//                 K/V stage and ping-pong on the tensor pipe)
+// A tile row r is (token t0 + r / G, query head kv_head*G + r % G): the G heads of a KV head share
+// each K/V page load (GQA packing).
+//
+// TMEM (512 columns): S_t at [128 t, 128 t + 128) (P_t, bf16, aliases its first 64 columns),
+// O_t at [256 + 128 t, +D).
+#include "segpa_internal.h"
+#include "sm100_ptx.cuh"
+
+#include <climits>
+#include <cstdlib>
+
+namespace segpa {
+using namespace ptx;
+
+namespace {
+
+constexpr int kLoaderWarp = 0;
+constexpr int kMmaWarp = 1;
+constexpr int kFirstSoftmaxWarp = 4;
+constexpr float kRescaleThreshold = 8.0f;  // log2 units: O is rescaled only when the max grows by > 2^8
+
+template <int D, int NT>
+struct Cfg {
+    static constexpr int kThreads = 128 + 128 * NT;
+    static constexpr int kTileBytes = kTileRows * D * 2;      // Q tile, K block or V block
+    static constexpr int kStages = (D == 128) ? 4 : 8;   // > 114 KB of smem either way: one CTA per SM (it owns all of TMEM)
+    static constexpr int kSmemQ = NT * kTileBytes;
+    static constexpr int kSmemKV = kStages * kTileBytes;
+    static constexpr int kSmemBytes = kSmemQ + kSmemKV + 1024 /*align slack*/;
+    static constexpr int kHalves = D / 64;
+    static constexpr uint32_t kSBO = kHalves * kAtomBytes;
+};
+
+struct Bars {
+    uint64_t kv_full[8];
+    uint64_t kv_empty[8];
+    uint64_t q_full[2];
+    uint64_t s_full[2];
+    uint64_t p_full[2];
+    uint64_t o_final[2];
+    uint32_t tmem_base;
+};
+
+struct TileRange {
+    int n_rows;   // valid rows (0 = tile unused in this item)
+    int tok0;     // first token of the tile inside the segment's q range
+    int lo, hi;   // KV blocks [lo, hi) this tile takes part in
+};
+
+__device__ __forceinline__ int item_for(int k, int cta, int n_cta) {
+    // cost-sorted item list dealt in boustrophedon order: round k goes left-to-right when even
+    return k * n_cta + ((k & 1) ? (n_cta - 1 - cta) : cta);
+}
+
+__device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev& sg, int tile, int TT, int G) {
+    TileRange r;
+    const int tok_lo = it.t0 + tile * TT;
+    const int tok_hi = min(it.t0 + it.n_tok, tok_lo + TT);
+    r.tok0 = tok_lo;
+    r.n_rows = max(0, tok_hi - tok_lo) * G;
+    if (r.n_rows == 0) { r.lo = r.hi = 0; return r; }
+    const int i0 = sg.kv_len - sg.q_len + tok_lo, i1 = sg.kv_len - sg.q_len + tok_hi - 1;
+    r.lo = max(it.kb_lo, max(0, i0 - sg.window + 1) / kBlockKeys);
+    r.hi = min(it.kb_hi, i1 / kBlockKeys + 1);
+    if (r.hi < r.lo) r.hi = r.lo;
+    return r;
+}
+
+}  // namespace
+
+template <int D, int NT>
+__global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(const FwdParams p) {
+    using C = Cfg<D, NT>;
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ Bars bars;
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
+    const uint32_t sQ = smem_u32(smem);
+    const uint32_t sKV = sQ + C::kSmemQ;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int cta = blockIdx.x, n_cta = gridDim.x;
+    const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
+    const int rows_per_slot = kTileRows * p.tiles_per_item;
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < C::kStages; ++s) {
+            mbar_init(smem_u32(&bars.kv_full[s]), 1);
+            mbar_init(smem_u32(&bars.kv_empty[s]), 1);
+        }
+        for (int t = 0; t < 2; ++t) {
+            mbar_init(smem_u32(&bars.q_full[t]), 128);
+            mbar_init(smem_u32(&bars.s_full[t]), 1);
+            mbar_init(smem_u32(&bars.p_full[t]), 128);
+            mbar_init(smem_u32(&bars.o_final[t]), 1);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 2) {
+        tmem_alloc(smem_u32(&bars.tmem_base), 512);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = bars.tmem_base;
+
+    if (warp == kLoaderWarp) {
+        // ------------------------------------------------------------------ loader
+        uint32_t fill = 0;  // stage fills so far
+        for (int k = 0;; ++k) {
+            const int ii = item_for(k, cta, n_cta);
+            if (k * n_cta >= p.n_items) break;
+            if (ii >= p.n_items) continue;
+            const ItemDev it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            int jlo = INT_MAX, jhi = 0;
+            for (int t = 0; t < NT; ++t) {
+                const TileRange tr = tile_range(it, sg, t, TT, G);
+                if (tr.n_rows > 0 && tr.hi > tr.lo) { jlo = min(jlo, tr.lo); jhi = max(jhi, tr.hi); }
+            }
+            for (int j = jlo; j < jhi; ++j) {
+                int page = 0;
+                if (lane < ppb) page = p.pages[sg.page_off + (long long)(j * ppb - sg.first_page) + lane];
+                for (int kv = 0; kv < 2; ++kv) {
+                    const uint32_t st = fill % C::kStages, ph = (fill / C::kStages) & 1;
+                    if (lane == 0) {
+                        mbar_wait(smem_u32(&bars.kv_empty[st]), ph ^ 1);
+                        mbar_arrive_expect_tx(smem_u32(&bars.kv_full[st]), C::kTileBytes);
+                    }
+                    __syncwarp();
+                    if (lane < ppb) {
+                        const uint8_t* src = (kv == 0 ? p.k_pool : p.v_pool) + (size_t)page * p.page_bytes;
+                        bulk_g2s(sKV + st * C::kTileBytes + lane * p.page_bytes, src, p.page_bytes, smem_u32(&bars.kv_full[st]));
+                    }
+                    ++fill;
+                }
+            }
+        }
+    } else if (warp == kMmaWarp) {
+        // ------------------------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            const uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
+            const uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
+            uint32_t rd = 0;                       // stage reads so far
+            uint32_t n_q[2] = {0, 0}, n_p[2] = {0, 0};
+            for (int k = 0;; ++k) {
+                const int ii = item_for(k, cta, n_cta);
+                if (k * n_cta >= p.n_items) break;
+                if (ii >= p.n_items) continue;
+                const ItemDev it = p.items[ii];
+                const SegDev sg = p.segs[it.seg];
+                TileRange tr[2];
+                int jlo = INT_MAX, jhi = 0;
+                for (int t = 0; t < NT; ++t) {
+                    tr[t] = tile_range(it, sg, t, TT, G);
+                    if (tr[t].n_rows > 0 && tr[t].hi > tr[t].lo) { jlo = min(jlo, tr[t].lo); jhi = max(jhi, tr[t].hi); }
+                }
+                for (int t = 0; t < NT; ++t)
+                    if (tr[t].n_rows > 0) {
+                        mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
+                        ++n_q[t];
+                    }
+                tc_fence_after();
+                // step j: for each tile, PV(j-1) then QK(j).  K(j) and V(j-1) are the stages in use.
+                uint32_t st_v = 0;
+                for (int j = jlo; j <= jhi; ++j) {
+                    const bool have_k = j < jhi, have_v = j > jlo;
+                    uint32_t st_k = 0;
+                    if (have_v) {
+                        st_v = rd % C::kStages;
+                        mbar_wait(smem_u32(&bars.kv_full[st_v]), (rd / C::kStages) & 1);
+                        ++rd;
+                    }
+                    if (have_k) {
+                        st_k = rd % C::kStages;
+                        mbar_wait(smem_u32(&bars.kv_full[st_k]), (rd / C::kStages) & 1);
+                        ++rd;
+                    }
+                    tc_fence_after();
+                    for (int t = 0; t < NT; ++t) {
+                        if (tr[t].n_rows == 0) continue;
+                        const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
+                        if (have_v && j - 1 >= tr[t].lo && j - 1 < tr[t].hi) {
+                            mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
+                            ++n_p[t];
+                            tc_fence_after();
+                            const uint32_t vb = sKV + st_v * C::kTileBytes;
+#pragma unroll
+                            for (int kk = 0; kk < kBlockKeys / 16; ++kk) {
+                                const uint64_t bd = make_desc_sw128(vb + kk * 2 * C::kSBO, kAtomBytes, C::kSBO);
+                                mma_ts(tO, tS + kk * 8, bd, idesc_pv, (j - 1 > tr[t].lo || kk > 0) ? 1u : 0u);
+                            }
+                            if (j == tr[t].hi) tc_commit(smem_u32(&bars.o_final[t]));
+                        }
+                        if (have_k && j >= tr[t].lo && j < tr[t].hi) {
+                            const uint32_t qb = sQ + t * C::kTileBytes, kb = sKV + st_k * C::kTileBytes;
+#pragma unroll
+                            for (int kk = 0; kk < D / 16; ++kk) {
+                                const uint32_t o = (kk / 4) * kAtomBytes + (kk % 4) * 32;
+                                mma_ss(tS, make_desc_sw128(qb + o, 16, C::kSBO), make_desc_sw128(kb + o, 16, C::kSBO),
+                                       idesc_qk, kk > 0 ? 1u : 0u);
+                            }
+                            tc_commit(smem_u32(&bars.s_full[t]));
+                        }
+                    }
+                    if (have_v) tc_commit(smem_u32(&bars.kv_empty[st_v]));
+                    if (have_k) tc_commit(smem_u32(&bars.kv_empty[st_k]));
+                    // stage order in the ring is K(j), V(j): V(j-1) was read before K(j)
+                }
+            }
+        }
+    } else if (warp >= kFirstSoftmaxWarp) {
+        // ------------------------------------------------------------------ softmax warpgroups
+        const int tile = (warp - kFirstSoftmaxWarp) >> 2;
+        const int wq = warp & 3;                       // TMEM lane quadrant this warp may access
+        const int r = wq * 32 + lane;                  // row inside the tile
+        const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
+        const uint32_t tS = tmem + lane_base + tile * 128;
+        const uint32_t tO = tmem + lane_base + 256 + tile * 128;
+        const float sl2 = p.scale * 1.4426950408889634f;
+        uint32_t n_s = 0, n_o = 0;
+        for (int k = 0;; ++k) {
+            const int ii = item_for(k, cta, n_cta);
+            if (k * n_cta >= p.n_items) break;
+            if (ii >= p.n_items) continue;
+            const ItemDev it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            const TileRange tr = tile_range(it, sg, tile, TT, G);
+            if (tr.n_rows == 0) continue;
+
+            // ---- Q tile -> shared memory (K-major SW128 image), zero rows past the end
+            {
+                const uint32_t qb = sQ + tile * C::kTileBytes;
+                const int cpr = D / 8;                       // 16-byte chunks per row
+                const int rows_per_it = 32 / cpr;            // rows covered by one warp instruction
+                for (int rr = wq * 32; rr < wq * 32 + 32; rr += rows_per_it) {
+                    const int row_t = rr + lane / cpr, c = lane % cpr;
+                    uint4 v = make_uint4(0, 0, 0, 0);
+                    if (row_t < tr.n_rows) {
+                        const int t = tr.tok0 + row_t / G, head = sg.kv_head * G + row_t % G;
+                        v = *reinterpret_cast<const uint4*>(p.q + (sg.q_row_start + t) * p.q_row_stride + (long long)head * D + c * 8);
+                    }
+                    const uint32_t off = (uint32_t)((row_t >> 3) * C::kHalves * kAtomBytes + (c >> 3) * kAtomBytes +
+                                                    (row_t & 7) * 128 + (((c & 7) ^ (row_t & 7)) << 4));
+                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(qb + off), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+                }
+                fence_proxy_async_smem();
+                tc_fence_before();       // orders this thread's earlier TMEM reads (previous epilogue)
+                mbar_arrive(smem_u32(&bars.q_full[tile]));
+            }
+
+            const int rc = min(r, tr.n_rows - 1);            // rows past the end mirror the last valid row
+            const int tok = tr.tok0 + rc / G;
+            const int pos = sg.kv_len - sg.q_len + tok;      // query position i
+            const int key_lo = max(0, pos - sg.window + 1);  // visible keys [key_lo, pos]
+            float m_used = -INFINITY, l = 0.f;
+
+            for (int j = tr.lo; j < tr.hi; ++j) {
+                mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
+                ++n_s;
+                tc_fence_after();
+                const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;   // valid columns [cmin, cmax]
+                const bool need_mask = __any_sync(0xffffffffu, cmin > 0 || cmax < kBlockKeys - 1);
+                // pass 1: row max
+                float mx = -INFINITY;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    uint32_t v[32];
+                    tmem_ld32(tS + c * 32, v);
+                    tmem_wait_ld();
+                    if (need_mask) {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) {
+                            const int col = c * 32 + e;
+                            if (col >= cmin && col <= cmax) mx = fmaxf(mx, __uint_as_float(v[e]));
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) mx = fmaxf(mx, __uint_as_float(v[e]));
+                    }
+                }
+                const float mx2 = mx * sl2;
+                // lazy rescale (warp-uniform decision: tcgen05.ld/st are warp-collective)
+                const bool grow = mx2 > m_used + kRescaleThreshold;
+                if (__any_sync(0xffffffffu, grow)) {
+                    float corr = 1.f;
+                    if (grow) {
+                        corr = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - mx2);
+                        m_used = mx2;
+                        l *= corr;
+                    }
+                    if (j > tr.lo) {
+#pragma unroll
+                        for (int c = 0; c < D / 32; ++c) {
+                            uint32_t v[32];
+                            tmem_ld32(tO + c * 32, v);
+                            tmem_wait_ld();
+#pragma unroll
+                            for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * corr);
+                            tmem_st32(tO + c * 32, v);
+                        }
+                    }
+                }
+                const float mref = (m_used == -INFINITY) ? 0.f : m_used;
+                // pass 2: p = 2^(s*scale*log2e - m), row sum, bf16 P -> TMEM (aliases S columns [0, 64))
+                float rs = 0.f;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    uint32_t v[32];
+                    tmem_ld32(tS + c * 32, v);
+                    tmem_wait_ld();
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int e = 0; e < 32; e += 2) {
+                        float p0 = fast_exp2(fmaf(__uint_as_float(v[e]), sl2, -mref));
+                        float p1 = fast_exp2(fmaf(__uint_as_float(v[e + 1]), sl2, -mref));
+                        if (need_mask) {
+                            const int col = c * 32 + e;
+                            if (col < cmin || col > cmax) p0 = 0.f;
+                            if (col + 1 < cmin || col + 1 > cmax) p1 = 0.f;
+                        }
+                        rs += p0 + p1;
+                        pk[e >> 1] = pack_bf16x2(p0, p1);
+                    }
+                    tmem_st16(tS + c * 16, pk);
+                }
+                l += rs;
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(smem_u32(&bars.p_full[tile]));
+            }
+
+            // ---- epilogue
+            if (tr.hi > tr.lo) {
+                mbar_wait(smem_u32(&bars.o_final[tile]), n_o & 1);
+                ++n_o;
+                tc_fence_after();
+            }
+            const bool valid = r < tr.n_rows;
+            const int head = sg.kv_head * G + rc % G;
+            const long long row = sg.q_row_start + tok;
+            if (it.partial_slot >= 0) {
+                const size_t base = (size_t)it.partial_slot * rows_per_slot + (size_t)(tr.tok0 - it.t0) * G + r;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t v[32];
+                    if (tr.hi > tr.lo) { tmem_ld32(tO + c * 32, v); tmem_wait_ld(); }
+                    else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) v[e] = 0u;
+                    }
+                    if (valid) {
+                        float4* dst = reinterpret_cast<float4*>(p.ws_o + base * D + c * 32);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e)
+                            dst[e] = make_float4(__uint_as_float(v[4 * e]), __uint_as_float(v[4 * e + 1]),
+                                                 __uint_as_float(v[4 * e + 2]), __uint_as_float(v[4 * e + 3]));
+                    }
+                }
+                if (valid) { p.ws_ml[base * 2] = m_used; p.ws_ml[base * 2 + 1] = l; }
+            } else {
+                const float inv = 1.f / l;
+                uint16_t* orow = p.out + row * p.out_row_stride + (long long)head * D;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t v[32];
+                    tmem_ld32(tO + c * 32, v);
+                    tmem_wait_ld();
+                    if (valid) {
+                        uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            uint4 o;
+                            o.x = pack_bf16x2(__uint_as_float(v[8 * e + 0]) * inv, __uint_as_float(v[8 * e + 1]) * inv);
+                            o.y = pack_bf16x2(__uint_as_float(v[8 * e + 2]) * inv, __uint_as_float(v[8 * e + 3]) * inv);
+                            o.z = pack_bf16x2(__uint_as_float(v[8 * e + 4]) * inv, __uint_as_float(v[8 * e + 5]) * inv);
+                            o.w = pack_bf16x2(__uint_as_float(v[8 * e + 6]) * inv, __uint_as_float(v[8 * e + 7]) * inv);
+                            dst[e] = o;
+                        }
+                    }
+                }
+                if (valid && p.lse) p.lse[(long long)head * p.lse_stride + row] = (m_used + log2f(l)) * 0.6931471805599453f;
+            }
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tmem, 512);
+}
+
+// ---------------------------------------------------------------------------------------------
+int attention_tc_tiles_per_item() {
+    // SEGPA_TC_TILES=1|2 (bring-up knob; read at every build_segments call)
+    const char* e = getenv("SEGPA_TC_TILES");
+    const int t = e ? atoi(e) : 1;
+    return (t == 2) ? 2 : 1;
+}
+
+template <int D, int NT>
+static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
+    using C = Cfg<D, NT>;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<D, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const int grid = p.n_items < p.num_sms ? p.n_items : p.num_sms;
+    attention_tc_kernel<D, NT><<<grid, C::kThreads, C::kSmemBytes, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st) {
+    if (p.n_items == 0) return cudaSuccess;
+    if (p.tiles_per_item == 2) return p.D == 128 ? launch_one<128, 2>(p, st) : launch_one<64, 2>(p, st);
+    return p.D == 128 ? launch_one<128, 1>(p, st) : launch_one<64, 1>(p, st);
+}
+
+}  // namespace segpa

@@ -1,0 +1,680 @@
+// Host runtime of libsegpa.so: per-head paged KV pool, page tables, segment descriptor builder,
+// tile scheduler and the extern "C" entry points declared in include/segpa.h.
+// Operation semantics follow PAPER.md Sec. 4.3 / Algorithm 2; see DESIGN.md.
+#include "../../include/segpa.h"
+#include "segpa_internal.h"
+
+#include <algorithm>
+#include <climits>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+using namespace segpa;
+
+namespace {
+
+thread_local std::string g_err = "";
+
+segpa_status_t fail(segpa_status_t st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return st;
+}
+
+struct StreamKey {
+    int32_t layer, kv_head;
+    int64_t seq;
+    bool operator==(const StreamKey& o) const { return layer == o.layer && kv_head == o.kv_head && seq == o.seq; }
+};
+struct StreamKeyHash {
+    size_t operator()(const StreamKey& k) const {
+        uint64_t h = (uint64_t)k.seq * 0x9E3779B97F4A7C15ull;
+        h ^= ((uint64_t)(uint32_t)k.layer << 32 | (uint32_t)k.kv_head) + 0x7F4A7C15u + (h << 6) + (h >> 2);
+        return (size_t)h;
+    }
+};
+struct StreamRec {
+    std::vector<int32_t> pages;
+    int64_t kv_len = 0;
+};
+
+struct DeviceGuard {
+    int prev = -1;
+    bool active = false;
+    explicit DeviceGuard(int dev) {
+        if (dev >= 0 && cudaGetDevice(&prev) == cudaSuccess && prev != dev) {
+            cudaSetDevice(dev);
+            active = true;
+        }
+    }
+    ~DeviceGuard() { if (active) cudaSetDevice(prev); }
+};
+
+}  // namespace
+
+struct segpa_segments {
+    segpa_cache* cache = nullptr;
+    int32_t layer = 0;
+    std::vector<segpa_segment_req_t> reqs;
+    std::vector<SegDev> segs;
+    std::vector<ItemDev> items;
+    std::vector<segpa_item_t> items_pub;
+    std::vector<int32_t> pages;
+    std::vector<CombDev> combs;
+    segpa_plan_stats_t stats{};
+    int tiles_per_item = 1;
+    // device
+    uint8_t* d_blob = nullptr;
+    void* h_blob = nullptr;   // pinned staging for the upload
+    size_t blob_bytes = 0;
+    size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0;
+    int* d_counter = nullptr;
+    float* d_ws_o = nullptr;
+    float* d_ws_ml = nullptr;
+};
+
+struct segpa_cache {
+    segpa_cache_desc_t desc{};
+    int G = 1;
+    int page_bytes = 0;
+    bool planning_only = false;
+    bool own_pool = true;
+    uint8_t* k_pool = nullptr;
+    uint8_t* v_pool = nullptr;
+    std::vector<int32_t> refcnt;
+    std::vector<int32_t> free_list;  // may hold stale entries (refcnt != 0): skipped on pop
+    int64_t n_free = 0;
+    std::unordered_map<StreamKey, StreamRec, StreamKeyHash> streams;
+    std::vector<segpa_segments*> seg_objs;
+    int num_sms = 148;
+    int kernel_kind = 1;  // 0 = SIMT bring-up kernel (SEGPA_KERNEL=simt), 1 = tcgen05
+    int last_launches = 0;
+    // host-buffer entry point staging
+    uint16_t* st_q = nullptr;
+    uint16_t* st_out = nullptr;
+    float* st_lse = nullptr;
+    size_t st_q_bytes = 0, st_lse_bytes = 0;
+};
+
+namespace {
+
+int32_t pop_free_page(segpa_cache* c) {
+    while (!c->free_list.empty()) {
+        int32_t id = c->free_list.back();
+        c->free_list.pop_back();
+        if (c->refcnt[id] == 0) return id;
+    }
+    return -1;
+}
+
+void release_page(segpa_cache* c, int32_t id) {
+    if (--c->refcnt[id] == 0) {
+        c->free_list.push_back(id);
+        ++c->n_free;
+    }
+}
+
+void free_segments_obj(segpa_segments* s) {
+    if (!s) return;
+    if (s->d_blob) cudaFree(s->d_blob);
+    if (s->h_blob) cudaFreeHost(s->h_blob);
+    if (s->d_counter) cudaFree(s->d_counter);
+    if (s->d_ws_o) cudaFree(s->d_ws_o);
+    if (s->d_ws_ml) cudaFree(s->d_ws_ml);
+    delete s;
+}
+
+inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// attended keys of the query at position i (Alg. 2 policy; PAPER.md:219 with W = w + 1)
+inline int64_t visible_count(int64_t i, int head_class, int64_t W) {
+    return head_class == SEGPA_GLOBAL ? i + 1 : std::min<int64_t>(i + 1, W);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* segpa_last_error(void) { return g_err.c_str(); }
+int32_t segpa_version(void) { return SEGPA_VERSION; }
+
+int64_t segpa_pool_bytes(const segpa_cache_desc_t* d) {
+    if (!d || d->num_pages < 1 || d->page_size < 1 || d->head_dim < 1) return 0;
+    return (d->num_pages + 1) * (int64_t)d->page_size * d->head_dim * 2;
+}
+
+segpa_status_t segpa_create_cache(const segpa_cache_desc_t* d, segpa_cache_t** out) {
+    if (!d || !out) return fail(SEGPA_ERR_INVALID, "create_cache: null argument");
+    *out = nullptr;
+    if (d->num_layers < 1 || d->num_q_heads < 1 || d->num_kv_heads < 1 || d->num_pages < 1)
+        return fail(SEGPA_ERR_INVALID, "create_cache: counts must be >= 1");
+    if (d->num_q_heads % d->num_kv_heads != 0)
+        return fail(SEGPA_ERR_INVALID, "create_cache: num_q_heads %d not a multiple of num_kv_heads %d",
+                    d->num_q_heads, d->num_kv_heads);
+    if (d->head_dim != 64 && d->head_dim != 128)
+        return fail(SEGPA_ERR_UNSUPPORTED, "create_cache: head_dim %d (supported: 64, 128)", d->head_dim);
+    if (d->page_size != 16 && d->page_size != 32)
+        return fail(SEGPA_ERR_UNSUPPORTED, "create_cache: page_size %d (supported: 16, 32)", d->page_size);
+    if (d->num_q_heads / d->num_kv_heads > 16)
+        return fail(SEGPA_ERR_UNSUPPORTED, "create_cache: GQA group %d > 16", d->num_q_heads / d->num_kv_heads);
+    if (d->num_pages >= INT32_MAX - 1) return fail(SEGPA_ERR_INVALID, "create_cache: num_pages too large");
+    if ((d->k_pool == nullptr) != (d->v_pool == nullptr))
+        return fail(SEGPA_ERR_INVALID, "create_cache: give both k_pool and v_pool or neither");
+    if (d->device < -1) return fail(SEGPA_ERR_INVALID, "create_cache: bad device %d", d->device);
+
+    segpa_cache* c = new (std::nothrow) segpa_cache();
+    if (!c) return fail(SEGPA_ERR_OOM, "create_cache: host allocation failed");
+    c->desc = *d;
+    c->G = d->num_q_heads / d->num_kv_heads;
+    c->page_bytes = d->page_size * d->head_dim * 2;
+    c->planning_only = (d->device == -1);
+    const char* kk = getenv("SEGPA_KERNEL");
+    c->kernel_kind = (kk && strcmp(kk, "simt") == 0) ? 0 : 1;
+    try {
+        c->refcnt.assign((size_t)d->num_pages, 0);
+        c->free_list.resize((size_t)d->num_pages);
+        for (int64_t i = 0; i < d->num_pages; ++i) c->free_list[(size_t)i] = (int32_t)(d->num_pages - 1 - i);
+    } catch (const std::bad_alloc&) {
+        delete c;
+        return fail(SEGPA_ERR_OOM, "create_cache: host allocation failed");
+    }
+    c->n_free = d->num_pages;
+
+    if (!c->planning_only) {
+        int ndev = 0;
+        cudaError_t e = cudaGetDeviceCount(&ndev);
+        if (e != cudaSuccess || d->device >= ndev) {
+            delete c;
+            return fail(SEGPA_ERR_CUDA, "create_cache: no CUDA device %d (%s); there is no CPU fallback",
+                        d->device, e == cudaSuccess ? "ordinal out of range" : cudaGetErrorString(e));
+        }
+        cudaDeviceProp prop{};
+        cudaGetDeviceProperties(&prop, d->device);
+        if (prop.major != 10) {
+            delete c;
+            return fail(SEGPA_ERR_UNSUPPORTED, "create_cache: device %d is sm_%d%d; this library is built for sm_100a",
+                        d->device, prop.major, prop.minor);
+        }
+        c->num_sms = prop.multiProcessorCount;
+        DeviceGuard g(d->device);
+        const size_t bytes = (size_t)segpa_pool_bytes(d);
+        if (d->k_pool) {
+            c->own_pool = false;
+            c->k_pool = (uint8_t*)d->k_pool;
+            c->v_pool = (uint8_t*)d->v_pool;
+        } else {
+            if (cudaMalloc(&c->k_pool, bytes) != cudaSuccess || cudaMalloc(&c->v_pool, bytes) != cudaSuccess) {
+                cudaGetLastError();
+                if (c->k_pool) cudaFree(c->k_pool);
+                delete c;
+                return fail(SEGPA_ERR_OOM, "create_cache: cudaMalloc of 2 x %zu bytes failed", bytes);
+            }
+        }
+        if (cudaMemset(c->k_pool, 0, bytes) != cudaSuccess || cudaMemset(c->v_pool, 0, bytes) != cudaSuccess) {
+            cudaError_t e2 = cudaGetLastError();
+            if (c->own_pool) { cudaFree(c->k_pool); cudaFree(c->v_pool); }
+            delete c;
+            return fail(SEGPA_ERR_CUDA, "create_cache: memset failed: %s", cudaGetErrorString(e2));
+        }
+    }
+    *out = c;
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_destroy(segpa_cache_t* c) {
+    if (!c) return SEGPA_OK;
+    DeviceGuard g(c->desc.device);
+    if (!c->planning_only) cudaDeviceSynchronize();
+    for (auto* s : c->seg_objs) free_segments_obj(s);
+    if (c->st_q) cudaFree(c->st_q);
+    if (c->st_out) cudaFree(c->st_out);
+    if (c->st_lse) cudaFree(c->st_lse);
+    if (c->own_pool && c->k_pool) { cudaFree(c->k_pool); cudaFree(c->v_pool); }
+    delete c;
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_append_pages(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                  const void* k_src, const void* v_src, int64_t src_row_stride_elems,
+                                  int64_t n_tokens, const int32_t* page_ids, int32_t n_page_ids,
+                                  void* cuda_stream) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "append_pages: null cache");
+    if (layer < 0 || layer >= c->desc.num_layers) return fail(SEGPA_ERR_INVALID, "append_pages: layer %d out of range", layer);
+    if (kv_head < 0 || kv_head >= c->desc.num_kv_heads) return fail(SEGPA_ERR_INVALID, "append_pages: kv_head %d out of range", kv_head);
+    if (n_tokens < 1) return fail(SEGPA_ERR_INVALID, "append_pages: n_tokens %lld < 1", (long long)n_tokens);
+    if ((k_src == nullptr) != (v_src == nullptr)) return fail(SEGPA_ERR_INVALID, "append_pages: give both k_src and v_src, or neither (attach)");
+    if (n_page_ids < 0 || (n_page_ids > 0 && !page_ids)) return fail(SEGPA_ERR_INVALID, "append_pages: bad page_ids");
+    const bool attach = (k_src == nullptr);
+    const int P = c->desc.page_size, D = c->desc.head_dim;
+    if (!attach && c->planning_only) return fail(SEGPA_ERR_STATE, "append_pages: copy mode on a planning-only cache");
+    if (!attach && src_row_stride_elems < D) return fail(SEGPA_ERR_INVALID, "append_pages: src_row_stride_elems %lld < head_dim", (long long)src_row_stride_elems);
+
+    StreamKey key{layer, kv_head, seq_id};
+    auto it = c->streams.find(key);
+    const int64_t cur_len = (it == c->streams.end()) ? 0 : it->second.kv_len;
+    const int64_t cur_pages = cdiv(cur_len, P);
+    const int64_t new_len = cur_len + n_tokens;
+    if (new_len > (int64_t)INT32_MAX - 2 * kBlockKeys) return fail(SEGPA_ERR_INVALID, "append_pages: stream too long");
+    const int64_t need = cdiv(new_len, P) - cur_pages;
+
+    std::vector<int32_t> newp;
+    if (attach) {
+        if (!page_ids) return fail(SEGPA_ERR_INVALID, "append_pages: attach needs page_ids");
+        if (cur_len % P != 0) return fail(SEGPA_ERR_INVALID, "append_pages: attach needs the stream length (%lld) to be a multiple of page_size", (long long)cur_len);
+        if (n_page_ids != need) return fail(SEGPA_ERR_INVALID, "append_pages: attach needs %lld page ids, got %d", (long long)need, n_page_ids);
+        for (int32_t i = 0; i < n_page_ids; ++i) {
+            if (page_ids[i] < 0 || page_ids[i] >= c->desc.num_pages) return fail(SEGPA_ERR_INVALID, "append_pages: page id %d out of range", page_ids[i]);
+            if (!c->planning_only && c->refcnt[page_ids[i]] == 0) return fail(SEGPA_ERR_INVALID, "append_pages: attach of page %d which holds no data", page_ids[i]);
+        }
+        newp.assign(page_ids, page_ids + n_page_ids);
+    } else if (page_ids) {
+        if (n_page_ids != need) return fail(SEGPA_ERR_INVALID, "append_pages: need %lld page ids, got %d", (long long)need, n_page_ids);
+        for (int32_t i = 0; i < n_page_ids; ++i) {
+            if (page_ids[i] < 0 || page_ids[i] >= c->desc.num_pages) return fail(SEGPA_ERR_INVALID, "append_pages: page id %d out of range", page_ids[i]);
+            if (c->refcnt[page_ids[i]] != 0) return fail(SEGPA_ERR_INVALID, "append_pages: page %d is not free", page_ids[i]);
+        }
+        newp.assign(page_ids, page_ids + n_page_ids);
+        std::vector<int32_t> tmp(newp);
+        std::sort(tmp.begin(), tmp.end());
+        if (std::adjacent_find(tmp.begin(), tmp.end()) != tmp.end()) return fail(SEGPA_ERR_INVALID, "append_pages: duplicate page id");
+    } else {
+        if (need > c->n_free) return fail(SEGPA_ERR_OOM, "append_pages: pool exhausted (%lld pages needed, %lld free)", (long long)need, (long long)c->n_free);
+    }
+
+    // device part first (nothing is applied on error)
+    std::vector<int32_t> touched;
+    if (!attach) {
+        if (page_ids == nullptr) {
+            // peek pages without committing: pop now, push back on failure
+            for (int64_t i = 0; i < need; ++i) newp.push_back(pop_free_page(c));
+        }
+        if (cur_len % P != 0) touched.push_back(it->second.pages.back());
+        touched.insert(touched.end(), newp.begin(), newp.end());
+        DeviceGuard g(c->desc.device);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        int* d_ids = nullptr;
+        cudaError_t e = cudaMallocAsync((void**)&d_ids, touched.size() * sizeof(int), st);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_ids, touched.data(), touched.size() * sizeof(int), cudaMemcpyHostToDevice, st);
+        if (e == cudaSuccess)
+            e = launch_scatter_pages(c->k_pool, c->v_pool, (const uint16_t*)k_src, (const uint16_t*)v_src,
+                                     src_row_stride_elems, d_ids, (int)(cur_len % P), n_tokens,
+                                     (int)touched.size(), D, P, st);
+        if (d_ids) cudaFreeAsync(d_ids, st);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            if (page_ids == nullptr)
+                for (auto id : newp) c->free_list.push_back(id);
+            return fail(SEGPA_ERR_CUDA, "append_pages: %s", cudaGetErrorString(e));
+        }
+    }
+    // commit
+    StreamRec& rec = c->streams[key];
+    for (auto id : newp) {
+        if (c->refcnt[id] == 0) --c->n_free;
+        ++c->refcnt[id];
+        rec.pages.push_back(id);
+    }
+    rec.kv_len = new_len;
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_free_stream(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "free_stream: null cache");
+    auto it = c->streams.find(StreamKey{layer, kv_head, seq_id});
+    if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "free_stream: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
+    for (auto id : it->second.pages) release_page(c, id);
+    c->streams.erase(it);
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_stream_info(const segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                 int64_t* kv_len, int32_t* n_pages, int32_t* page_ids_out, int32_t cap) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "stream_info: null cache");
+    auto it = c->streams.find(StreamKey{layer, kv_head, seq_id});
+    if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "stream_info: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
+    if (kv_len) *kv_len = it->second.kv_len;
+    if (n_pages) *n_pages = (int32_t)it->second.pages.size();
+    if (page_ids_out)
+        for (int32_t i = 0; i < cap && i < (int32_t)it->second.pages.size(); ++i) page_ids_out[i] = it->second.pages[i];
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_pool_stats(const segpa_cache_t* c, int64_t* in_use, int64_t* n_free) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "pool_stats: null cache");
+    if (in_use) *in_use = c->desc.num_pages - c->n_free;
+    if (n_free) *n_free = c->n_free;
+    return SEGPA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Alg. 2 lines 1-14 + the tile scheduler
+// ---------------------------------------------------------------------------------------------
+segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa_segment_req_t* reqs,
+                                    int32_t n, segpa_segments_t** out, void* cuda_stream) {
+    if (!c || !reqs || !out) return fail(SEGPA_ERR_INVALID, "build_segments: null argument");
+    *out = nullptr;
+    if (n < 1) return fail(SEGPA_ERR_INVALID, "build_segments: n %d < 1", n);
+    if (layer < 0 || layer >= c->desc.num_layers) return fail(SEGPA_ERR_INVALID, "build_segments: layer %d out of range", layer);
+    const int P = c->desc.page_size, G = c->G, D = c->desc.head_dim;
+    const int ppb = kBlockKeys / P;
+    const int32_t zero_page = (int32_t)c->desc.num_pages;
+    const int tiles_per_item = (c->kernel_kind == 1) ? attention_tc_tiles_per_item() : 1;
+    const int TT = kTileRows / G;               // tokens per 128-row tile (GQA packing)
+    const int item_tok = TT * tiles_per_item;
+
+    segpa_segments* S = new (std::nothrow) segpa_segments();
+    if (!S) return fail(SEGPA_ERR_OOM, "build_segments: host allocation failed");
+    S->cache = c;
+    S->layer = layer;
+    S->tiles_per_item = tiles_per_item;
+    struct TileTmp { int seg, t0, n_tok, kb_lo, kb_hi; };
+    std::vector<TileTmp> tiles;
+    int64_t q_rows = 0, pairs = 0, vis_tokens = 0;
+    try {
+        S->reqs.assign(reqs, reqs + n);
+        // validation + per-segment metadata
+        struct Iv { int32_t kv_head; int64_t lo, hi; };
+        std::vector<Iv> ivs;
+        for (int32_t s = 0; s < n; ++s) {
+            const segpa_segment_req_t& r = reqs[s];
+            if (r.kv_head < 0 || r.kv_head >= c->desc.num_kv_heads) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: kv_head %d out of range", s, r.kv_head); }
+            auto it = c->streams.find(StreamKey{layer, r.kv_head, r.seq_id});
+            if (it == c->streams.end()) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: no stream (layer %d, kv_head %d, seq %lld)", s, layer, r.kv_head, (long long)r.seq_id); }
+            const StreamRec& rec = it->second;
+            if (r.head_class != SEGPA_GLOBAL && r.head_class != SEGPA_LOCAL) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: bad head_class %d", s, r.head_class); }
+            if (r.q_len < 1 || r.q_len > rec.kv_len) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: q_len %d not in [1, kv_len=%lld]", s, r.q_len, (long long)rec.kv_len); }
+            if (r.head_class == SEGPA_LOCAL && r.window < 1) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: LOCAL window %d < 1", s, r.window); }
+            if (r.q_row_start < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: negative q_row_start", s); }
+            if (r.n_sink < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: negative n_sink", s); }
+            if (r.n_sink != 0 && r.head_class == SEGPA_LOCAL) { delete S; return fail(SEGPA_ERR_UNSUPPORTED, "build_segments: segment %d: n_sink %d (sink tokens are not implemented on the GPU yet)", s, r.n_sink); }
+            ivs.push_back(Iv{r.kv_head, r.q_row_start, r.q_row_start + r.q_len});
+
+            const int64_t kv_len = rec.kv_len;
+            const int64_t W = (r.head_class == SEGPA_GLOBAL) ? (int64_t)INT32_MAX / 2 : r.window;
+            // Alg. 2 lines 6-10: visible positions of the whole segment
+            const int64_t vis_lo = std::max<int64_t>(0, kv_len - r.q_len - W + 1);
+            const int64_t seg_kb_lo = vis_lo / kBlockKeys;
+            const int64_t seg_kb_hi = (kv_len - 1) / kBlockKeys + 1;
+            const int64_t first_vis_page = vis_lo / P;
+            const int64_t n_stream_pages = cdiv(kv_len, P);
+            SegDev sd{};
+            sd.q_row_start = r.q_row_start;
+            sd.page_off = (long long)S->pages.size();
+            sd.q_len = r.q_len;
+            sd.kv_len = (int)kv_len;
+            sd.head_class = r.head_class;
+            sd.window = (int)W;
+            sd.n_sink = 0;
+            sd.kv_head = r.kv_head;
+            sd.first_page = (int)(seg_kb_lo * ppb);
+            sd.n_pages_listed = (int)((seg_kb_hi - seg_kb_lo) * ppb);
+            // Alg. 2 line 12: Translate(T_page, U_h); invisible / absent pages -> the zero page
+            for (int64_t pg = sd.first_page; pg < sd.first_page + sd.n_pages_listed; ++pg)
+                S->pages.push_back((pg >= first_vis_page && pg < n_stream_pages) ? rec.pages[(size_t)pg] : zero_page);
+            S->segs.push_back(sd);
+            vis_tokens += kv_len - first_vis_page * P;
+            q_rows = std::max<int64_t>(q_rows, r.q_row_start + r.q_len);
+            for (int64_t t = 0; t < r.q_len; ++t) pairs += visible_count(kv_len - r.q_len + t, r.head_class, W);
+            // tiles: exactly the KV blocks the tile's rows attend to
+            for (int64_t t0 = 0; t0 < r.q_len; t0 += item_tok) {
+                const int64_t n_tok = std::min<int64_t>(item_tok, r.q_len - t0);
+                const int64_t i0 = kv_len - r.q_len + t0, i1 = i0 + n_tok - 1;
+                const int64_t lo = std::max<int64_t>(0, i0 - W + 1);
+                tiles.push_back(TileTmp{s, (int)t0, (int)n_tok, (int)(lo / kBlockKeys), (int)(i1 / kBlockKeys + 1)});
+            }
+        }
+        // overlap check on (row, head): same kv_head (hence same q heads) and intersecting rows
+        std::sort(ivs.begin(), ivs.end(), [](const Iv& a, const Iv& b) { return a.kv_head != b.kv_head ? a.kv_head < b.kv_head : a.lo < b.lo; });
+        for (size_t i = 1; i < ivs.size(); ++i)
+            if (ivs[i].kv_head == ivs[i - 1].kv_head && ivs[i].lo < ivs[i - 1].hi) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: two segments of kv_head %d overlap on rows [%lld, %lld)", ivs[i].kv_head, (long long)ivs[i].lo, (long long)std::min(ivs[i].hi, ivs[i - 1].hi)); }
+
+        // scheduler: split long tiles along KV when the grid would be unbalanced, then order
+        // longest-first; CTAs pull items from a shared cursor (greedy LPT).
+        int64_t total_cost = 0;
+        for (auto& t : tiles) total_cost += t.kb_hi - t.kb_lo;
+        const int64_t chunk = std::max<int64_t>(8, cdiv(total_cost, (int64_t)c->num_sms * 4));
+        int n_split_tiles = 0, n_slots = 0;
+        for (size_t ti = 0; ti < tiles.size(); ++ti) {
+            const TileTmp& t = tiles[ti];
+            const int cost = t.kb_hi - t.kb_lo;
+            int parts = 1;
+            if (cost > chunk + chunk / 2) parts = (int)cdiv(cost, chunk);
+            if (parts > 1) {
+                ++n_split_tiles;
+                S->combs.push_back(CombDev{t.seg, t.t0, t.n_tok, n_slots, parts, 0, 0, 0});
+            }
+            for (int p = 0; p < parts; ++p) {
+                const int lo = t.kb_lo + (int)((int64_t)cost * p / parts);
+                const int hi = t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
+                const int slot = parts > 1 ? n_slots++ : -1;
+                S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, 0, 0});
+                S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti});
+            }
+        }
+        std::vector<int> order(S->items.size());
+        for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+            return (S->items[a].kb_hi - S->items[a].kb_lo) > (S->items[b].kb_hi - S->items[b].kb_lo);
+        });
+        std::vector<ItemDev> it2(order.size());
+        std::vector<segpa_item_t> ip2(order.size());
+        int64_t kv_blocks = 0;
+        for (size_t i = 0; i < order.size(); ++i) {
+            it2[i] = S->items[order[i]];
+            ip2[i] = S->items_pub[order[i]];
+            kv_blocks += it2[i].kb_hi - it2[i].kb_lo;
+        }
+        S->items.swap(it2);
+        S->items_pub.swap(ip2);
+
+        segpa_plan_stats_t& stt = S->stats;
+        stt.n_segments = n;
+        stt.n_tiles = (int32_t)tiles.size();
+        stt.n_items = (int32_t)S->items.size();
+        stt.n_split_tiles = n_split_tiles;
+        stt.tile_tokens = TT;
+        stt.block_keys = kBlockKeys;
+        stt.kv_blocks = kv_blocks;
+        stt.attended_pairs = pairs * G;
+        stt.q_rows = q_rows;
+        stt.visible_kv_tokens = vis_tokens;
+        stt.workspace_bytes = (int64_t)n_slots * kTileRows * tiles_per_item * (D + 2) * 4;
+    } catch (const std::bad_alloc&) {
+        delete S;
+        return fail(SEGPA_ERR_OOM, "build_segments: host allocation failed");
+    }
+
+    if (!c->planning_only) {
+        DeviceGuard g(c->desc.device);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+        S->off_segs = 0;
+        S->off_items = al(S->off_segs + S->segs.size() * sizeof(SegDev));
+        S->off_pages = al(S->off_items + S->items.size() * sizeof(ItemDev));
+        S->off_combs = al(S->off_pages + S->pages.size() * sizeof(int32_t));
+        S->blob_bytes = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
+        cudaError_t e = cudaMallocHost(&S->h_blob, S->blob_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&S->d_blob, S->blob_bytes);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&S->d_counter, 256);
+        if (e == cudaSuccess && S->stats.workspace_bytes > 0) {
+            const size_t slots = (size_t)S->stats.workspace_bytes / ((size_t)kTileRows * tiles_per_item * (D + 2) * 4);
+            e = cudaMalloc((void**)&S->d_ws_o, slots * kTileRows * tiles_per_item * D * 4);
+            if (e == cudaSuccess) e = cudaMalloc((void**)&S->d_ws_ml, slots * kTileRows * tiles_per_item * 2 * 4);
+        }
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            free_segments_obj(S);
+            return fail(e == cudaErrorMemoryAllocation ? SEGPA_ERR_OOM : SEGPA_ERR_CUDA, "build_segments: %s", cudaGetErrorString(e));
+        }
+        uint8_t* hb = (uint8_t*)S->h_blob;
+        memcpy(hb + S->off_segs, S->segs.data(), S->segs.size() * sizeof(SegDev));
+        memcpy(hb + S->off_items, S->items.data(), S->items.size() * sizeof(ItemDev));
+        memcpy(hb + S->off_pages, S->pages.data(), S->pages.size() * sizeof(int32_t));
+        if (!S->combs.empty()) memcpy(hb + S->off_combs, S->combs.data(), S->combs.size() * sizeof(CombDev));
+        e = cudaMemcpyAsync(S->d_blob, S->h_blob, S->blob_bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            free_segments_obj(S);
+            return fail(SEGPA_ERR_CUDA, "build_segments: upload failed: %s", cudaGetErrorString(e));
+        }
+    }
+    c->seg_objs.push_back(S);
+    *out = S;
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_free_segments(segpa_cache_t* c, segpa_segments_t* s) {
+    if (!c || !s) return fail(SEGPA_ERR_INVALID, "free_segments: null argument");
+    auto it = std::find(c->seg_objs.begin(), c->seg_objs.end(), s);
+    if (it == c->seg_objs.end()) return fail(SEGPA_ERR_STATE, "free_segments: not owned by this cache");
+    c->seg_objs.erase(it);
+    DeviceGuard g(c->desc.device);
+    if (!c->planning_only) cudaDeviceSynchronize();  // the upload / a running fwd may still use it
+    free_segments_obj(s);
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_segments_stats(const segpa_segments_t* s, segpa_plan_stats_t* out) {
+    if (!s || !out) return fail(SEGPA_ERR_INVALID, "segments_stats: null argument");
+    *out = s->stats;
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_segments_items(const segpa_segments_t* s, segpa_item_t* items_out, int32_t cap, int32_t* n_out) {
+    if (!s) return fail(SEGPA_ERR_INVALID, "segments_items: null argument");
+    if (n_out) *n_out = (int32_t)s->items_pub.size();
+    if (items_out)
+        for (int32_t i = 0; i < cap && i < (int32_t)s->items_pub.size(); ++i) items_out[i] = s->items_pub[(size_t)i];
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_segments_pages(const segpa_segments_t* s, int32_t segment, int32_t* first_page_index,
+                                    int32_t* page_ids_out, int32_t cap, int32_t* n_out) {
+    if (!s || segment < 0 || segment >= (int32_t)s->segs.size()) return fail(SEGPA_ERR_INVALID, "segments_pages: bad argument");
+    const SegDev& sd = s->segs[(size_t)segment];
+    if (first_page_index) *first_page_index = sd.first_page;
+    if (n_out) *n_out = sd.n_pages_listed;
+    if (page_ids_out)
+        for (int32_t i = 0; i < cap && i < sd.n_pages_listed; ++i) page_ids_out[i] = s->pages[(size_t)sd.page_off + i];
+    return SEGPA_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Alg. 2 lines 15-16
+// ---------------------------------------------------------------------------------------------
+segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, const void* q,
+                                   int64_t q_row_stride, float scale, void* out, int64_t out_row_stride,
+                                   float* lse, int64_t lse_stride, int64_t T, void* cuda_stream) {
+    if (!c || !s || !q || !out) return fail(SEGPA_ERR_INVALID, "attention_fwd: null argument");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "attention_fwd: planning-only cache has no device; there is no CPU fallback");
+    if (s->cache != c) return fail(SEGPA_ERR_STATE, "attention_fwd: segments were built by another cache");
+    if (std::find(c->seg_objs.begin(), c->seg_objs.end(), s) == c->seg_objs.end()) return fail(SEGPA_ERR_STATE, "attention_fwd: stale segments object");
+    const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
+    if (T < s->stats.q_rows) return fail(SEGPA_ERR_INVALID, "attention_fwd: T %lld < rows used by the plan %lld", (long long)T, (long long)s->stats.q_rows);
+    if (q_row_stride < (int64_t)Hq * D || out_row_stride < (int64_t)Hq * D) return fail(SEGPA_ERR_INVALID, "attention_fwd: row stride smaller than Hq*D");
+    if ((q_row_stride % 8) || (out_row_stride % 8) || ((uintptr_t)q % 16) || ((uintptr_t)out % 16)) return fail(SEGPA_ERR_INVALID, "attention_fwd: q/out must be 16-byte aligned with row strides multiple of 8 elements");
+    if (lse && lse_stride < T) return fail(SEGPA_ERR_INVALID, "attention_fwd: lse_stride < T");
+    if (!(scale > 0.f) || !(scale < 1e30f)) return fail(SEGPA_ERR_INVALID, "attention_fwd: softmax_scale must be positive and finite");
+
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(SEGPA_ERR_CUDA, "attention_fwd: earlier asynchronous failure: %s", cudaGetErrorString(e));
+
+    FwdParams p{};
+    p.segs = (const SegDev*)(s->d_blob + s->off_segs);
+    p.items = (const ItemDev*)(s->d_blob + s->off_items);
+    p.pages = (const int*)(s->d_blob + s->off_pages);
+    p.combs = (const CombDev*)(s->d_blob + s->off_combs);
+    p.n_items = (int)s->items.size();
+    p.n_combs = (int)s->combs.size();
+    p.counter = s->d_counter;
+    p.k_pool = c->k_pool;
+    p.v_pool = c->v_pool;
+    p.q = (const uint16_t*)q;
+    p.out = (uint16_t*)out;
+    p.lse = lse;
+    p.ws_o = s->d_ws_o;
+    p.ws_ml = s->d_ws_ml;
+    p.q_row_stride = q_row_stride;
+    p.out_row_stride = out_row_stride;
+    p.lse_stride = lse_stride;
+    p.scale = scale;
+    p.Hq = Hq;
+    p.Hkv = c->desc.num_kv_heads;
+    p.G = c->G;
+    p.D = D;
+    p.P = c->desc.page_size;
+    p.tile_tokens = kTileRows / c->G;
+    p.tiles_per_item = s->tiles_per_item;
+    p.page_bytes = c->page_bytes;
+    p.num_sms = c->num_sms;
+
+    e = cudaMemsetAsync(s->d_counter, 0, 256, st);
+    int launches = 0;
+    if (e == cudaSuccess) {
+        e = (c->kernel_kind == 0) ? launch_attention_simt(p, st) : launch_attention_tc(p, st);
+        ++launches;
+    }
+    if (e == cudaSuccess && p.n_combs > 0) {
+        e = launch_combine(p, st);
+        ++launches;
+    }
+    c->last_launches = launches;
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(SEGPA_ERR_CUDA, "attention_fwd: launch failed: %s", cudaGetErrorString(e));
+    }
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t* s, const void* q_host,
+                                        float scale, void* out_host, float* lse_host, int64_t T,
+                                        void* cuda_stream) {
+    if (!c || !s || !q_host || !out_host) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: null argument");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "attention_fwd_host: planning-only cache has no device; there is no CPU fallback");
+    if (T < 1) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: T < 1");
+    const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
+    const size_t qb = (size_t)T * Hq * D * 2, lb = (size_t)T * Hq * 4;
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (qb > c->st_q_bytes) {
+        if (c->st_q) { cudaStreamSynchronize(st); cudaFree(c->st_q); cudaFree(c->st_out); c->st_q = c->st_out = nullptr; c->st_q_bytes = 0; }
+        if (cudaMalloc((void**)&c->st_q, qb) != cudaSuccess || cudaMalloc((void**)&c->st_out, qb) != cudaSuccess) {
+            cudaGetLastError();
+            if (c->st_q) cudaFree(c->st_q);
+            c->st_q = c->st_out = nullptr;
+            return fail(SEGPA_ERR_OOM, "attention_fwd_host: staging allocation of 2 x %zu bytes failed", qb);
+        }
+        c->st_q_bytes = qb;
+    }
+    if (lb > c->st_lse_bytes) {
+        if (c->st_lse) { cudaStreamSynchronize(st); cudaFree(c->st_lse); c->st_lse = nullptr; c->st_lse_bytes = 0; }
+        if (cudaMalloc((void**)&c->st_lse, lb) != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_OOM, "attention_fwd_host: staging allocation failed"); }
+        c->st_lse_bytes = lb;
+    }
+    cudaError_t e = cudaMemcpyAsync(c->st_q, q_host, qb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_fwd_host: H2D failed: %s", cudaGetErrorString(e)); }
+    segpa_status_t rc = segpa_attention_fwd(c, s, c->st_q, (int64_t)Hq * D, scale, c->st_out, (int64_t)Hq * D,
+                                            c->st_lse, T, T, cuda_stream);
+    if (rc != SEGPA_OK) return rc;
+    e = cudaMemcpyAsync(out_host, c->st_out, qb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && lse_host) e = cudaMemcpyAsync(lse_host, c->st_lse, lb, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_fwd_host: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
+int32_t segpa_last_launch_count(const segpa_cache_t* c) { return c ? c->last_launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,100 @@
+// Internal structures shared by the host runtime and the CUDA kernels of libsegpa.so.
+// Not part of the ABI (include/segpa.h is).  Nothing here is used by oracle/.
+#pragma once
+
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace segpa {
+
+constexpr int kBlockKeys = 128;   // KV block (keys per MMA tile column block)
+constexpr int kTileRows = 128;    // query rows per tile (UMMA M)
+constexpr int kAtomBytes = 1024;  // one swizzle-128B atom: 8 rows x 128 B
+
+// ---------------------------------------------------------------------------------------------
+// Page image.  A physical page holds P tokens x D bf16 of ONE KV head,
+// stored as the exact shared-memory image tcgen05.mma consumes, so one cp.async.bulk moves it:
+//   for g in [0, P/8)          group of 8 tokens
+//     for h in [0, D/64)       64-element (128-byte) half of the head dim
+//       atom: 8 rows x 128 B; the 16-byte chunk c of row r is stored at chunk (c ^ r)   (SW128)
+// byte offset of (slot s, element d):
+//   (s/8)*(D/64)*1024 + (d/64)*1024 + (s%8)*128 + ((((d%64)/8) ^ (s%8)) * 16) + (d%8)*2
+// The same image serves K (K-major B operand of S = Q K^T; SBO = (D/64)*1024) and V (MN-major B
+// operand of O = P V; SBO = (D/64)*1024, LBO = 1024).
+// ---------------------------------------------------------------------------------------------
+__host__ __device__ inline uint32_t page_elem_offset_bytes(int D, int slot, int d) {
+    const int halves = D >> 6;
+    const int r = slot & 7;
+    return (uint32_t)((slot >> 3) * halves * kAtomBytes + (d >> 6) * kAtomBytes + r * 128 +
+                      ((((d & 63) >> 3) ^ r) << 4) + ((d & 7) << 1));
+}
+
+struct SegDev {
+    long long q_row_start;
+    long long page_off;     // index into the page-id array of this segment's first listed page
+    int q_len;
+    int kv_len;
+    int head_class;         // 0 GLOBAL, 1 LOCAL
+    int window;             // W (keys incl. self); large for GLOBAL
+    int n_sink;
+    int kv_head;
+    int first_page;         // absolute page index (position / P) of page_off
+    int n_pages_listed;
+};
+
+struct ItemDev {
+    int seg;
+    int t0;                 // first token of the item inside the segment's query range
+    int n_tok;              // tokens (rows = n_tok * G), <= tiles_per_item * tile_tokens
+    int kb_lo;              // visited KV blocks [kb_lo, kb_hi)
+    int kb_hi;
+    int partial_slot;       // -1: final result written to out/lse; else split-KV partial slot
+    int pad0, pad1;
+};
+
+struct CombDev {
+    int seg;
+    int t0;
+    int n_tok;
+    int first_slot;
+    int n_splits;
+    int pad0, pad1, pad2;
+};
+
+struct FwdParams {
+    const SegDev* segs;
+    const ItemDev* items;
+    const int* pages;            // translated physical page ids (zero page = num_pages)
+    const CombDev* combs;
+    int n_items;
+    int n_combs;
+    int* counter;                // dynamic scheduler cursor (zeroed before launch)
+    const uint8_t* k_pool;
+    const uint8_t* v_pool;
+    const uint16_t* q;
+    uint16_t* out;
+    float* lse;                  // may be null
+    float* ws_o;                 // split-KV partial O  [slot][rows_per_item][D]  (unnormalised)
+    float* ws_ml;                // split-KV partial (m, l) [slot][rows_per_item][2], m in log2 units
+    long long q_row_stride;      // elements
+    long long out_row_stride;
+    long long lse_stride;
+    float scale;
+    int Hq, Hkv, G, D, P;
+    int tile_tokens;             // floor(128 / G)
+    int tiles_per_item;
+    int page_bytes;
+    int num_sms;
+};
+
+// kernel launchers (each returns the CUDA error of its launch)
+cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const uint16_t* k_src,
+                                 const uint16_t* v_src, long long src_stride, const int* page_ids_dev,
+                                 int first_slot, long long n_tokens, int n_pages, int D, int P,
+                                 cudaStream_t st);
+cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st);
+cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st);
+cudaError_t launch_combine(const FwdParams& p, cudaStream_t st);
+int attention_tc_tiles_per_item();
+
+}  // namespace segpa

@@ -1,0 +1,163 @@
+// Small kernels of libsegpa.so: page scatter (append), split-KV combine, and the SIMT bring-up
+// attention kernel (selected with SEGPA_KERNEL=simt; the product kernel is segpa_attn_tc.cu).
+#include "segpa_internal.h"
+
+#include <cuda_bf16.h>
+
+namespace segpa {
+
+// ---------------------------------------------------------------------------------------------
+// a1: write K/V rows into the per-head page images.
+// One thread per (slot, 16-byte chunk); slots past the last new token of the last page are zeroed.
+// ---------------------------------------------------------------------------------------------
+__global__ void scatter_pages_kernel(uint8_t* __restrict__ k_pool, uint8_t* __restrict__ v_pool,
+                                     const uint16_t* __restrict__ k_src, const uint16_t* __restrict__ v_src,
+                                     long long src_stride, const int* __restrict__ page_ids,
+                                     int first_slot, long long n_tokens, int n_pages, int D, int P) {
+    const int cpr = D >> 3;  // 16-byte chunks per row
+    const long long total_slots = (long long)n_pages * P - first_slot;
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= total_slots * cpr) return;
+    const long long n = idx / cpr;
+    const int c = (int)(idx % cpr);
+    const long long gs = first_slot + n;
+    const int page = page_ids[gs / P];
+    const int slot = (int)(gs % P);
+    const size_t dst = (size_t)page * ((size_t)P * D * 2) + page_elem_offset_bytes(D, slot, c * 8);
+    uint4 kv = make_uint4(0, 0, 0, 0), vv = make_uint4(0, 0, 0, 0);
+    if (n < n_tokens) {
+        kv = *reinterpret_cast<const uint4*>(k_src + n * src_stride + c * 8);
+        vv = *reinterpret_cast<const uint4*>(v_src + n * src_stride + c * 8);
+    }
+    *reinterpret_cast<uint4*>(k_pool + dst) = kv;
+    *reinterpret_cast<uint4*>(v_pool + dst) = vv;
+}
+
+cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const uint16_t* k_src,
+                                 const uint16_t* v_src, long long src_stride, const int* page_ids_dev,
+                                 int first_slot, long long n_tokens, int n_pages, int D, int P,
+                                 cudaStream_t st) {
+    const long long total = ((long long)n_pages * P - first_slot) * (D >> 3);
+    if (total <= 0) return cudaSuccess;
+    const int threads = 256;
+    const long long blocks = (total + threads - 1) / threads;
+    scatter_pages_kernel<<<(unsigned)blocks, threads, 0, st>>>(k_pool, v_pool, k_src, v_src, src_stride,
+                                                               page_ids_dev, first_slot, n_tokens, n_pages, D, P);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// a7: split-KV combine.  Partials hold unnormalised O, running max m (log2 units) and sum l;
+// merged in ascending split order (deterministic).  Exactness of the merge: PAPER.md:302.
+// One warp per row.
+// ---------------------------------------------------------------------------------------------
+__global__ void combine_kernel(FwdParams p) {
+    const int rows_per_slot = kTileRows * p.tiles_per_item;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    for (int ci = blockIdx.x; ci < p.n_combs; ci += gridDim.x) {
+        const CombDev c = p.combs[ci];
+        const SegDev sg = p.segs[c.seg];
+        const int rows = c.n_tok * p.G;
+        for (int r = warp; r < rows; r += nw) {
+            float M = -INFINITY;
+            for (int s = 0; s < c.n_splits; ++s)
+                M = fmaxf(M, p.ws_ml[((size_t)(c.first_slot + s) * rows_per_slot + r) * 2]);
+            float L = 0.f;
+            float acc[4] = {0.f, 0.f, 0.f, 0.f};
+            for (int s = 0; s < c.n_splits; ++s) {
+                const size_t base = (size_t)(c.first_slot + s) * rows_per_slot + r;
+                const float ms = p.ws_ml[base * 2], ls = p.ws_ml[base * 2 + 1];
+                const float w = (ms == -INFINITY) ? 0.f : exp2f(ms - M);
+                L += w * ls;
+                for (int k = 0; k < p.D / 32; ++k) acc[k] += w * p.ws_o[base * p.D + lane + 32 * k];
+            }
+            const int t = c.t0 + r / p.G, head = sg.kv_head * p.G + r % p.G;
+            const long long row = sg.q_row_start + t;
+            const float inv = 1.f / L;
+            for (int k = 0; k < p.D / 32; ++k)
+                p.out[row * p.out_row_stride + (long long)head * p.D + lane + 32 * k] =
+                    __bfloat16_as_ushort(__float2bfloat16_rn(acc[k] * inv));
+            if (p.lse && lane == 0) p.lse[(long long)head * p.lse_stride + row] = (M + log2f(L)) * 0.6931471805599453f;
+        }
+    }
+}
+
+cudaError_t launch_combine(const FwdParams& p, cudaStream_t st) {
+    const int blocks = p.n_combs < 4 * p.num_sms ? p.n_combs : 4 * p.num_sms;
+    combine_kernel<<<blocks, 256, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// SIMT bring-up attention: same plan, same outputs, no tensor cores.  One warp per query row;
+// lanes split the head dim; keys visited one at a time.  Exists to validate the pool layout, the
+// builder and the scheduler independently of the tcgen05 kernel.
+// ---------------------------------------------------------------------------------------------
+__device__ inline float bf16_bits_to_float(uint32_t b) { return __uint_as_float(b << 16); }
+
+__global__ void attention_simt_kernel(FwdParams p) {
+    __shared__ int s_item;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
+    const int epl = p.D / 32;  // elements per lane (2 or 4)
+    const float sl2 = p.scale * 1.4426950408889634f;
+    const int rows_per_slot = kTileRows * p.tiles_per_item;
+    while (true) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_item = atomicAdd(p.counter, 1);
+        __syncthreads();
+        const int ii = s_item;
+        if (ii >= p.n_items) break;
+        const ItemDev it = p.items[ii];
+        const SegDev sg = p.segs[it.seg];
+        const int rows = it.n_tok * p.G;
+        for (int r = warp; r < rows; r += nw) {
+            const int t = it.t0 + r / p.G, head = sg.kv_head * p.G + r % p.G;
+            const long long row = sg.q_row_start + t;
+            const int i = sg.kv_len - sg.q_len + t;
+            float qv[4], acc[4] = {0.f, 0.f, 0.f, 0.f};
+            for (int k = 0; k < epl; ++k)
+                qv[k] = bf16_bits_to_float(p.q[row * p.q_row_stride + (long long)head * p.D + lane * epl + k]);
+            float m = -INFINITY, l = 0.f;
+            int jlo = max(it.kb_lo * kBlockKeys, i - sg.window + 1);
+            int jhi = min(it.kb_hi * kBlockKeys - 1, i);
+            for (int j = jlo; j <= jhi; ++j) {
+                const int pg = j / p.P, slot = j % p.P;
+                const int page = p.pages[sg.page_off + (pg - sg.first_page)];
+                const size_t off = (size_t)page * p.page_bytes;
+                float dot = 0.f;
+                float vv[4];
+                for (int k = 0; k < epl; ++k) {
+                    const uint32_t eo = page_elem_offset_bytes(p.D, slot, lane * epl + k);
+                    dot += qv[k] * bf16_bits_to_float(*reinterpret_cast<const uint16_t*>(p.k_pool + off + eo));
+                    vv[k] = bf16_bits_to_float(*reinterpret_cast<const uint16_t*>(p.v_pool + off + eo));
+                }
+                for (int o = 16; o > 0; o >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, o);
+                const float s2 = dot * sl2;
+                const float mn = fmaxf(m, s2);
+                const float corr = exp2f(m - mn);   // m = -inf first time: exp2(-inf) = 0
+                const float pj = exp2f(s2 - mn);
+                l = l * corr + pj;
+                for (int k = 0; k < epl; ++k) acc[k] = acc[k] * corr + pj * vv[k];
+                m = mn;
+            }
+            if (it.partial_slot >= 0) {
+                const size_t base = (size_t)it.partial_slot * rows_per_slot + r;
+                for (int k = 0; k < epl; ++k) p.ws_o[base * p.D + lane * epl + k] = acc[k];
+                if (lane == 0) { p.ws_ml[base * 2] = m; p.ws_ml[base * 2 + 1] = l; }
+            } else {
+                const float inv = 1.f / l;
+                for (int k = 0; k < epl; ++k)
+                    p.out[row * p.out_row_stride + (long long)head * p.D + lane * epl + k] =
+                        __bfloat16_as_ushort(__float2bfloat16_rn(acc[k] * inv));
+                if (p.lse && lane == 0) p.lse[(long long)head * p.lse_stride + row] = (m + log2f(l)) * 0.6931471805599453f;
+            }
+        }
+    }
+}
+
+cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st) {
+    attention_simt_kernel<<<p.num_sms * 4, 256, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+}  // namespace segpa

@@ -1,0 +1,45 @@
+"""Feeds a workloads.Workload through the C ABI (segpa_create_cache / segpa_append_pages /
+segpa_build_segments).  Plumbing only; used by tests/, bench.py and __graft_entry__.smoke()."""
+from __future__ import annotations
+
+from typing import Dict, List, Optional, Tuple
+
+import numpy as np
+
+from . import binding as B
+from . import workloads as wl
+
+
+def create_cache(w: wl.Workload, device: int = 0) -> int:
+    return B.segpa_create_cache(num_layers=w.num_layers, num_q_heads=w.Hq, num_kv_heads=w.Hkv, head_dim=w.D,
+                                page_size=w.P, num_pages=w.num_pages, device=device)
+
+
+def append_workload(cache: int, w: wl.Workload, k_pool=None, v_pool=None, stream=None) -> None:
+    """Owners first (copy mode with the workload's page placement), then aliasing streams (attach the
+    shared prefix pages, copy the rest).  k_pool/v_pool: torch bf16 [num_pages][P][D] on the cache's
+    device, or None for a planning-only cache (attach everything)."""
+    owners = [s for s in w.streams if s.shared_from is None]
+    aliased = [s for s in w.streams if s.shared_from is not None]
+    for s in owners + aliased:
+        if k_pool is None:
+            B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, None, None, s.kv_len, page_ids=s.page_ids)
+            continue
+        pp = s.n_shared_prefix_pages
+        if pp > 0:
+            B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, None, None, pp * w.P, page_ids=s.page_ids[:pp])
+        n_rest = s.kv_len - pp * w.P
+        if n_rest > 0:
+            kr = wl.stream_rows(k_pool, s, w.P, lo_page=pp)
+            vr = wl.stream_rows(v_pool, s, w.P, lo_page=pp)
+            B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, kr, vr, n_rest, page_ids=s.page_ids[pp:],
+                                 stream=stream)
+
+
+def segment_reqs(w: wl.Workload, layer: int) -> List[tuple]:
+    return [(s.seq_id, s.kv_head, s.head_class, s.window, s.n_sink, s.q_row_start, s.q_len)
+            for s in w.layer_segments(layer)]
+
+
+def build_layer(cache: int, w: wl.Workload, layer: int, stream=None) -> int:
+    return B.segpa_build_segments(cache, layer, segment_reqs(w, layer), stream=stream)

@@ -1,0 +1,246 @@
+"""GPU parity: libsegpa.so (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances: BASELINE.json north_star (out max-abs 2e-2, mean-abs 2e-3, LSE 1e-3)."""
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+from paper_2606_06256_b200.workloads import GLOBAL, LOCAL
+from tests.gpu_helpers import GpuRun, LSE_SENTINEL, OUT_SENTINEL, compare, sample_rows
+
+pytestmark = pytest.mark.gpu
+
+# (kernel, tiles per item): the product kernel is tc; simt is the bring-up kernel kept as a cross-check
+VARIANTS = [("tc", 1), ("tc", 2), ("simt", 1)]
+
+
+def _run_full(w, kernel, tiles, label):
+    g = GpuRun(w, kernel, tiles)
+    try:
+        msgs = []
+        for layer in range(w.num_layers):
+            q, out, lse = g.layer(layer)
+            msgs.append(compare(w, layer, g.k_pool, g.v_pool, q, out, lse, label="%s[%s,%d] L%d" % (label, kernel, tiles, layer)))
+        return msgs
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("kernel,tiles", VARIANTS)
+def test_cfg1_tiny(kernel, tiles):
+    print(_run_full(wl.config1(), kernel, tiles, "cfg1"))
+
+
+RAGGED = [
+    # Hq, Hkv, D, P, requests
+    (8, 2, 64, 16, [{"kv_len": 700, "heads": {0: (GLOBAL, 0, 0, 700), 1: (LOCAL, 100, 0, 300)}}]),
+    (4, 4, 128, 16, [{"kv_len": 391, "heads": {0: (GLOBAL, 0, 0, 391), 1: (LOCAL, 1, 0, 391), 2: (LOCAL, 129, 0, 5), 3: (GLOBAL, 0, 0, 1)}}]),
+    (28, 4, 128, 32, [{"kv_len": 1000, "heads": {0: (GLOBAL, 0, 0, 1000), 1: (LOCAL, 257, 0, 1000), 2: (LOCAL, 4096, 0, 77), 3: (GLOBAL, 0, 0, 19)}}]),
+    (64, 8, 128, 16, [{"kv_len": 2049, "heads": {h: ((GLOBAL, 0, 0, 500) if h == 0 else (LOCAL, 300 + 37 * h, 0, 129)) for h in range(8)}}]),
+    (8, 2, 128, 16, [{"kv_len": 17, "heads": {0: (GLOBAL, 0, 0, 17), 1: (LOCAL, 5, 0, 17)}},
+                     {"kv_len": 1, "heads": {0: (GLOBAL, 0, 0, 1), 1: (LOCAL, 5, 0, 1)}},
+                     {"kv_len": 3000, "heads": {0: (GLOBAL, 0, 0, 1), 1: (LOCAL, 640, 0, 1)}},
+                     {"kv_len": 515, "heads": {0: (LOCAL, 128, 0, 515), 1: (GLOBAL, 0, 0, 130)}}]),
+    (32, 8, 128, 16, [{"kv_len": 129, "heads": {h: (LOCAL if h % 2 else GLOBAL, 64, 0, 129) for h in range(8)}}]),
+]
+
+
+@pytest.mark.parametrize("kernel,tiles", VARIANTS)
+@pytest.mark.parametrize("case", range(len(RAGGED)))
+def test_ragged_small(case, kernel, tiles):
+    Hq, Hkv, D, P, reqs = RAGGED[case]
+    w = wl.make_workload("ragged%d" % case, Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=900 + case)
+    print(_run_full(w, kernel, tiles, "ragged%d" % case))
+
+
+@pytest.mark.parametrize("kernel,tiles", VARIANTS)
+def test_decode_split_kv(kernel, tiles):
+    """Decode-shaped: few rows, long KV -> the scheduler splits along KV and the combine kernel merges."""
+    reqs = [{"kv_len": 20000 + 333 * r, "heads": {0: (GLOBAL, 0, 0, 1), 1: (LOCAL, 2048, 0, 1)}} for r in range(3)]
+    reqs.append({"kv_len": 9000, "heads": {0: (GLOBAL, 0, 0, 40), 1: (GLOBAL, 0, 0, 3)}})
+    w = wl.make_workload("decode", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=77)
+    g = GpuRun(w, kernel, tiles)
+    try:
+        q, out, lse = g.layer(0)
+        st = B.segpa_segments_stats(g.segs[0])
+        assert st["n_split_tiles"] > 0 and B.segpa_last_launch_count(g.cache) == 2
+        print(compare(w, 0, g.k_pool, g.v_pool, q, out, lse, label="decode[%s,%d]" % (kernel, tiles)), st)
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("tiles", [1, 2])
+def test_determinism_and_page_permutation(tiles):
+    """Run-to-run bit determinism, and bit-identical results under a different page placement of the
+    same logical streams (same arithmetic order)."""
+    reqs = [{"kv_len": 1500, "heads": {0: (GLOBAL, 0, 0, 1500), 1: (LOCAL, 300, 0, 700)}},
+            {"kv_len": 26000, "heads": {0: (GLOBAL, 0, 0, 2), 1: (LOCAL, 999, 0, 2)}}]
+    wa = wl.make_workload("perm_a", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=1)
+    wb = wl.make_workload("perm_b", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=2)
+    dev = torch.device("cuda:0")
+    ka, va = wl.pool_values(wa, dev)
+    kb, vb = torch.zeros_like(ka), torch.zeros_like(va)
+    for sa, sb in zip(wa.streams, wb.streams):
+        ia = torch.from_numpy(sa.page_ids.astype(np.int64)).to(dev)
+        ib = torch.from_numpy(sb.page_ids.astype(np.int64)).to(dev)
+        kb[ib] = ka[ia]
+        vb[ib] = va[ia]
+    ga, gb = GpuRun(wa, "tc", tiles, ka, va), GpuRun(wb, "tc", tiles, kb, vb)
+    try:
+        q, o1, l1 = ga.layer(0)
+        _, o2, l2 = ga.layer(0, q)
+        assert torch.equal(o1, o2) and torch.equal(l1, l2)
+        _, o3, l3 = gb.layer(0, q)
+        assert torch.equal(o1, o3) and torch.equal(l1, l3)
+    finally:
+        ga.close()
+        gb.close()
+
+
+def test_window_one_is_exact():
+    """W = 1 returns V at the query's own position bit-exactly (BASELINE north_star invariant)."""
+    w = wl.make_workload("w1", Hq=8, Hkv=2, D=128, P=16, seed=5,
+                         requests=[{"kv_len": 777, "heads": {0: (LOCAL, 1, 0, 777), 1: (LOCAL, 1, 0, 100)}}])
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        sm = w.stream_map()
+        for s in w.segments:
+            st = sm[(0, s.kv_head, 0)]
+            rows = wl.stream_rows(g.v_pool, st, w.P)[st.kv_len - s.q_len:]           # V at own positions
+            for gi in range(w.G):
+                got = out[s.q_row_start:s.q_row_start + s.q_len, s.kv_head * w.G + gi]
+                assert torch.equal(got, rows)
+    finally:
+        g.close()
+
+
+def test_poison_outside_visible_pages():
+    """Non-visible pages are never read (PAPER.md:366 'true eviction'): poison unused pool pages and the
+    evicted prefix pages of a LOCAL head; the output must not change.  Tokens inside a visible page must
+    be finite (masked probabilities multiply them) -- see DESIGN.md."""
+    reqs = [{"kv_len": 5000, "heads": {0: (LOCAL, 512, 0, 64), 1: (GLOBAL, 0, 0, 64)}}]
+    w = wl.make_workload("poison", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=9)
+    dev = torch.device("cuda:0")
+    k, v = wl.pool_values(w, dev)
+    g = GpuRun(w, "tc", 2, k, v)
+    q, o1, l1 = g.layer(0)
+    g.close()
+    k2, v2 = k.clone(), v.clone()
+    used = set()
+    for s in w.streams:
+        used.update(int(x) for x in s.page_ids)
+    unused = torch.tensor([p for p in range(w.num_pages) if p not in used], device=dev)
+    k2[unused] = float("nan")
+    v2[unused] = float("inf")
+    st = w.stream_map()[(0, 0, 0)]
+    first_vis_page = (5000 - 64 - 512 + 1) // 16
+    ev = torch.from_numpy(st.page_ids[:first_vis_page].astype(np.int64)).to(dev)
+    k2[ev] = float("nan")
+    v2[ev] = 1e30
+    g2 = GpuRun(w, "tc", 2, k2, v2)
+    try:
+        _, o2, l2 = g2.layer(0, q)
+        assert torch.equal(o1, o2) and torch.equal(l1, l2)
+    finally:
+        g2.close()
+
+
+def test_host_buffer_entry_point_matches_device_path():
+    w = wl.config1()
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        qh = q.cpu().pin_memory()
+        oh = torch.empty_like(qh).pin_memory()
+        lh = torch.empty((w.Hq, w.T[0]), dtype=torch.float32).pin_memory()
+        B.segpa_attention_fwd_host(g.cache, g.segs[0], qh, w.scale, oh, lh)
+        cov = torch.from_numpy(np.ascontiguousarray(np.repeat(np.ones((w.T[0], w.Hq), bool)[..., None], w.D, 2)))
+        assert torch.equal(oh[cov], out.cpu()[cov]) and torch.equal(lh, lse.cpu())
+    finally:
+        g.close()
+
+
+def test_no_dense_allocation():
+    """'No dense [B,H,L,D] tensor and no additive mask is built': device memory taken by
+    build_segments + attention_fwd stays far below one [L, L] mask."""
+    w = wl.make_workload("mem", Hq=8, Hkv=2, D=128, P=16, seed=3,
+                         requests=[{"kv_len": 16384, "heads": {0: (GLOBAL, 0, 0, 16384), 1: (LOCAL, 1024, 0, 16384)}}])
+    g = GpuRun(w, "tc", 2)
+    try:
+        torch.cuda.synchronize()
+        free0, _ = torch.cuda.mem_get_info()
+        q = wl.q_values(w, 0, g.dev)
+        out = torch.empty_like(q)
+        g.segs[0] = H.build_layer(g.cache, w, 0)
+        B.segpa_attention_fwd(g.cache, g.segs[0], q, w.scale, out, None)
+        torch.cuda.synchronize()
+        free1, _ = torch.cuda.mem_get_info()
+        extra = free0 - free1 - 2 * q.numel() * 2
+        assert extra < 16 * 2 ** 20, extra          # an [L, L] bool mask alone would be 256 MiB
+    finally:
+        g.close()
+
+
+# ----------------------------------------------------------------------------- full-size configs
+@pytest.mark.parametrize("tiles", [1, 2])
+def test_cfg2_sampled(tiles):
+    w = wl.config2()
+    g = GpuRun(w, "tc", tiles)
+    try:
+        q, out, lse = g.layer(0)
+        rows = sample_rows(w, 0, n_random=256, seed=2)
+        print(len(rows), compare(w, 0, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg2[tc,%d]" % tiles))
+    finally:
+        g.close()
+
+
+def test_cfg3_sampled():
+    w = wl.config3()
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        rows = sample_rows(w, 0, n_random=64, seed=3)
+        rows = rows[:: max(1, len(rows) // 300)]
+        print(len(rows), compare(w, 0, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg3"))
+    finally:
+        g.close()
+
+
+def test_cfg4_sampled():
+    w = wl.config4()
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        rows = sample_rows(w, 0, n_random=512, seed=4)
+        rows = rows[:: max(1, len(rows) // 1500)]
+        print(len(rows), compare(w, 0, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg4"))
+        st = B.segpa_segments_stats(g.segs[0])
+        print(st)
+    finally:
+        g.close()
+
+
+def test_cfg4_decode_only_sampled():
+    w = wl.config4(decode_only=True)
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        print(compare(w, 0, g.k_pool, g.v_pool, q, out, lse, label="cfg4d"), B.segpa_segments_stats(g.segs[0]))
+    finally:
+        g.close()
+
+
+def test_cfg5_two_layers_sampled():
+    w = wl.config5(num_layers=2)
+    g = GpuRun(w, "tc", 2)
+    try:
+        for layer in range(2):
+            q, out, lse = g.layer(layer)
+            rows = sample_rows(w, layer, n_random=64, seed=5)
+            rows = rows[:: max(1, len(rows) // 300)]
+            print(len(rows), compare(w, layer, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg5 L%d" % layer))
+    finally:
+        g.close()

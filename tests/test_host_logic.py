@@ -1,0 +1,210 @@
+"""CPU tests of libsegpa.so's host logic on a planning-only cache (device = -1): exports, pool
+bookkeeping, visible-page selection (Alg. 2 lines 6-12), tile schedule, error behaviour."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+from paper_2606_06256_b200.workloads import GLOBAL, LOCAL
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def plan_cache(Hq=8, Hkv=2, D=128, P=16, num_pages=4096, layers=1):
+    return B.segpa_create_cache(num_layers=layers, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=D, page_size=P,
+                                num_pages=num_pages, device=-1)
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "segpa.h")).read()
+    declared = sorted(set(re.findall(r"\b(segpa_[a-z_]+)\s*\(", hdr)))
+    assert set(declared) == set(B.EXPORTS), (declared, B.EXPORTS)
+    L = ctypes.CDLL(B.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert B.segpa_version() == 1
+
+
+def test_no_cpu_fallback_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(B.SegpaError) as e:
+        B.segpa_create_cache(num_layers=1, num_q_heads=8, num_kv_heads=2, head_dim=128, page_size=16, num_pages=8, device=0)
+    assert e.value.status == B.ERR_CUDA
+    c = plan_cache()
+    B.segpa_append_pages(c, 0, 0, 0, None, None, 16, page_ids=[0])
+    segs = B.segpa_build_segments(c, 0, [(0, 0, GLOBAL, 0, 0, 0, 1)])
+    rc = B.lib().segpa_attention_fwd(c, segs, ctypes.c_void_p(16), 1024, ctypes.c_float(1.0), ctypes.c_void_p(16), 1024,
+                                     None, 0, 1, None)
+    assert rc == B.ERR_STATE
+    B.segpa_destroy(c)
+
+
+def test_create_cache_rejections():
+    def mk(**kw):
+        d = dict(num_layers=1, num_q_heads=8, num_kv_heads=2, head_dim=128, page_size=16, num_pages=8, device=-1)
+        d.update(kw)
+        return B.segpa_create_cache(**d)
+    for kw, st in [(dict(num_q_heads=7), B.ERR_INVALID), (dict(head_dim=96), B.ERR_UNSUPPORTED),
+                   (dict(page_size=8), B.ERR_UNSUPPORTED), (dict(num_pages=0), B.ERR_INVALID),
+                   (dict(num_q_heads=34, num_kv_heads=2), B.ERR_UNSUPPORTED), (dict(num_layers=0), B.ERR_INVALID)]:
+        with pytest.raises(B.SegpaError) as e:
+            mk(**kw)
+        assert e.value.status == st, kw
+
+
+def test_pool_bookkeeping_attach_and_refcounts():
+    c = plan_cache(num_pages=64)
+    B.segpa_append_pages(c, 0, 0, 1, None, None, 40, page_ids=[5, 9, 2])          # 40 tokens -> 3 pages
+    kv, ids = B.segpa_stream_info(c, 0, 0, 1)
+    assert kv == 40 and list(ids) == [5, 9, 2]
+    assert B.segpa_pool_stats(c) == (3, 61)
+    # alias the first two pages from another request, then extend
+    B.segpa_append_pages(c, 0, 0, 2, None, None, 32, page_ids=[5, 9])
+    B.segpa_append_pages(c, 0, 0, 2, None, None, 16, page_ids=[7])
+    assert B.segpa_pool_stats(c) == (4, 60)
+    # attach requires a page-aligned stream: stream 1 has 40 tokens
+    with pytest.raises(B.SegpaError) as e:
+        B.segpa_append_pages(c, 0, 0, 1, None, None, 16, page_ids=[11])
+    assert e.value.status == B.ERR_INVALID
+    with pytest.raises(B.SegpaError):
+        B.segpa_append_pages(c, 0, 0, 3, None, None, 16, page_ids=[64])               # out of range
+    with pytest.raises(B.SegpaError):
+        B.segpa_append_pages(c, 0, 0, 3, None, None, 17, page_ids=[1])                # wrong page count
+    with pytest.raises(B.SegpaError):
+        B.segpa_append_pages(c, 0, 2, 3, None, None, 16, page_ids=[1])                # kv_head out of range
+    with pytest.raises(B.SegpaError):
+        B.segpa_append_pages(c, 1, 0, 3, None, None, 16, page_ids=[1])                # layer out of range
+    B.segpa_free_stream(c, 0, 0, 1)
+    assert B.segpa_pool_stats(c) == (3, 61)          # pages 5, 9 still referenced by stream 2; page 2 freed
+    B.segpa_free_stream(c, 0, 0, 2)
+    assert B.segpa_pool_stats(c) == (0, 64)
+    with pytest.raises(B.SegpaError):
+        B.segpa_free_stream(c, 0, 0, 2)
+    B.segpa_destroy(c)
+
+
+def _expected_pages(kv_len, q_len, cls, W, P, page_ids, zero):
+    """Independent restatement of Alg. 2 lines 6-12 for one segment."""
+    vis_lo = 0 if cls == GLOBAL else max(0, kv_len - q_len - W + 1)
+    kb_lo, kb_hi = vis_lo // 128, (kv_len - 1) // 128 + 1
+    ppb = 128 // P
+    out = []
+    for pg in range(kb_lo * ppb, kb_hi * ppb):
+        visible = any(vis_lo <= j < kv_len for j in range(pg * P, pg * P + P))
+        out.append(int(page_ids[pg]) if visible else zero)
+    return kb_lo * ppb, out
+
+
+@pytest.mark.parametrize("P", [16, 32])
+def test_visible_page_selection_and_tiles(P):
+    rng = np.random.default_rng(P)
+    for trial in range(40):
+        kv_len = int(rng.integers(1, 3000))
+        q_len = int(rng.integers(1, kv_len + 1))
+        cls = int(rng.integers(0, 2))
+        W = int(rng.choice([1, 2, P - 1, P, P + 1, 127, 128, 129, 700, 5000]))
+        G = int(rng.choice([1, 4, 7, 8]))
+        c = plan_cache(Hq=2 * G, Hkv=2, P=P, num_pages=1024)
+        npg = (kv_len + P - 1) // P
+        ids = rng.permutation(1024)[:npg].astype(np.int32)
+        B.segpa_append_pages(c, 0, 1, 42, None, None, kv_len, page_ids=ids)
+        for tiles in (1, 2):
+            os.environ["SEGPA_TC_TILES"] = str(tiles)
+            segs = B.segpa_build_segments(c, 0, [(42, 1, cls, W, 0, 10, q_len)])
+            first, got = B.segpa_segments_pages(segs, 0)
+            efirst, exp = _expected_pages(kv_len, q_len, cls, W, P, ids, 1024)
+            assert first == efirst and list(got) == exp, (kv_len, q_len, cls, W, P)
+            st = B.segpa_segments_stats(segs)
+            items = B.segpa_segments_items(segs)
+            TT = 128 // G
+            assert st["tile_tokens"] == TT and st["q_rows"] == 10 + q_len
+            # brute force: per item, the blocks holding at least one visible (row, key) pair
+            pairs = 0
+            seen_tok = np.zeros(q_len, dtype=int)
+            by_tile = {}
+            for it in items:
+                by_tile.setdefault(it["tile"], []).append(it)
+            for tile, parts in by_tile.items():
+                parts.sort(key=lambda x: x["kb_lo"])
+                t0, n_tok = parts[0]["t0"], parts[0]["n_tok"]
+                assert n_tok <= TT * tiles
+                seen_tok[t0:t0 + n_tok] += 1
+                need = set()
+                for t in range(t0, t0 + n_tok):
+                    i = kv_len - q_len + t
+                    lo = 0 if cls == GLOBAL else max(0, i - W + 1)
+                    need.update(range(lo // 128, i // 128 + 1))
+                    pairs += (i - lo + 1) * G
+                got_blocks = []
+                for pt in parts:
+                    assert pt["kb_hi"] > pt["kb_lo"]                # no empty item
+                    got_blocks += list(range(pt["kb_lo"], pt["kb_hi"]))
+                assert sorted(need) == got_blocks                    # exactly the attended blocks, once each
+                assert all(pt["n_splits"] == len(parts) for pt in parts)
+            assert np.all(seen_tok == 1)
+            assert st["attended_pairs"] == pairs
+            costs = [it["kb_hi"] - it["kb_lo"] for it in items]
+            assert costs == sorted(costs, reverse=True)              # longest first
+            assert st["kv_blocks"] == sum(costs)
+            B.segpa_free_segments(c, segs)
+        B.segpa_destroy(c)
+
+
+def test_split_kv_plan_for_decode():
+    os.environ["SEGPA_TC_TILES"] = "1"
+    c = plan_cache(num_pages=4096)
+    B.segpa_append_pages(c, 0, 0, 0, None, None, 30000, page_ids=np.arange(1875))
+    segs = B.segpa_build_segments(c, 0, [(0, 0, GLOBAL, 0, 0, 0, 1)])
+    st = B.segpa_segments_stats(segs)
+    assert st["n_tiles"] == 1 and st["n_split_tiles"] == 1 and st["n_items"] > 8
+    assert st["workspace_bytes"] == st["n_items"] * 128 * (128 + 2) * 4
+    B.segpa_destroy(c)
+
+
+def test_build_segments_rejections():
+    c = plan_cache(num_pages=256)
+    B.segpa_append_pages(c, 0, 0, 0, None, None, 100, page_ids=np.arange(7))
+    B.segpa_append_pages(c, 0, 1, 0, None, None, 100, page_ids=np.arange(7, 14))
+    bad = [
+        ([(0, 0, GLOBAL, 0, 0, 0, 101)], B.ERR_INVALID),                 # q_len > kv_len
+        ([(0, 0, GLOBAL, 0, 0, 0, 0)], B.ERR_INVALID),                   # q_len < 1
+        ([(0, 0, LOCAL, 0, 0, 0, 5)], B.ERR_INVALID),                    # LOCAL window < 1
+        ([(0, 0, 2, 4, 0, 0, 5)], B.ERR_INVALID),                        # bad class
+        ([(9, 0, GLOBAL, 0, 0, 0, 5)], B.ERR_INVALID),                   # unknown stream
+        ([(0, 2, GLOBAL, 0, 0, 0, 5)], B.ERR_INVALID),                   # kv_head out of range
+        ([(0, 0, GLOBAL, 0, 0, -1, 5)], B.ERR_INVALID),                  # negative row
+        ([(0, 0, GLOBAL, 0, 0, 0, 50), (0, 0, LOCAL, 8, 0, 49, 10)], B.ERR_INVALID),   # (row, head) overlap
+        ([(0, 0, LOCAL, 8, 4, 0, 5)], B.ERR_UNSUPPORTED),                # sinks: NEXT #1
+        ([], B.ERR_INVALID),
+    ]
+    for reqs, st in bad:
+        with pytest.raises(B.SegpaError) as e:
+            B.segpa_build_segments(c, 0, reqs)
+        assert e.value.status == st, reqs
+    # different kv heads may share rows; same head may use disjoint rows
+    segs = B.segpa_build_segments(c, 0, [(0, 0, GLOBAL, 0, 0, 0, 50), (0, 1, LOCAL, 8, 0, 0, 50), (0, 0, GLOBAL, 0, 0, 50, 10)])
+    assert B.segpa_segments_stats(segs)["n_segments"] == 3
+    with pytest.raises(B.SegpaError):
+        B.segpa_build_segments(c, 1, [(0, 0, GLOBAL, 0, 0, 0, 5)])       # layer out of range
+    B.segpa_destroy(c)
+
+
+def test_config_plans_match_closed_forms():
+    """Useful work of the five BASELINE configs as planned by the library == generator closed forms."""
+    os.environ["SEGPA_TC_TILES"] = "2"
+    for cfg in (1, 2, 3, 4):
+        w = wl.CONFIGS[cfg]()
+        c = B.segpa_create_cache(num_layers=1, num_q_heads=w.Hq, num_kv_heads=w.Hkv, head_dim=w.D, page_size=w.P,
+                                 num_pages=w.num_pages, device=-1)
+        H.append_workload(c, w)
+        segs = H.build_layer(c, w, 0)
+        st = B.segpa_segments_stats(segs)
+        assert st["attended_pairs"] * 4 * w.D == wl.useful_flops(w, 0)
+        used, free = B.segpa_pool_stats(c)
+        assert used == len({int(p) for s in w.streams for p in s.page_ids})
+        B.segpa_destroy(c)
