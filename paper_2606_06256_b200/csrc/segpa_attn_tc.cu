@@ -5,6 +5,8 @@
 // One persistent CTA per SM, warp-specialised:
 //   warp 0        loader: one bulk copy per physical page into a ring of K/V stages
 //   warp 1        MMA issuer (one elected thread)
+//   warps 2, 3    Q loaders (cp.async into the swizzled Q image of tile 0 / tile 1), running one
+//                 item ahead: a Q buffer is refilled as soon as its last QK^T has completed
 //   warps 4..7    softmax / correction / epilogue warpgroup of tile 0 (thread = query row)
 //   warps 8..11   the same for tile 1 (NT = 2: two 128-row tiles of adjacent tokens share every
 //                 K/V stage and ping-pong on the tensor pipe)
@@ -27,6 +29,8 @@ namespace {
 constexpr int kLoaderWarp = 0;
 constexpr int kMmaWarp = 1;
 constexpr int kFirstSoftmaxWarp = 4;
+constexpr int kRegsLow = 64;     // warps 0..3 (loader, MMA issuer, Q loaders)
+constexpr int kRegsHigh = 216;   // softmax warps: 128 * 64 + 256 * 216 = 63488 <= 65536
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: O is rescaled only when the max grows by > 2^8
 
 template <int D, int NT>
@@ -45,6 +49,7 @@ struct Bars {
     uint64_t kv_full[8];
     uint64_t kv_empty[8];
     uint64_t q_full[2];
+    uint64_t q_empty[2];
     uint64_t s_full[2];
     uint64_t p_full[2];
     uint64_t o_final[2];
@@ -97,7 +102,8 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
             mbar_init(smem_u32(&bars.kv_empty[s]), 1);
         }
         for (int t = 0; t < 2; ++t) {
-            mbar_init(smem_u32(&bars.q_full[t]), 128);
+            mbar_init(smem_u32(&bars.q_full[t]), 32);
+            mbar_init(smem_u32(&bars.q_empty[t]), 1);
             mbar_init(smem_u32(&bars.s_full[t]), 1);
             mbar_init(smem_u32(&bars.p_full[t]), 128);
             mbar_init(smem_u32(&bars.o_final[t]), 1);
@@ -112,9 +118,12 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = bars.tmem_base;
+    // register budget (setmaxnreg inside each role branch so ptxas sees the limit per role): the softmax
+    // warpgroups hold a whole 128-column score row per thread; warps 0-3 give registers up
 
     if (warp == kLoaderWarp) {
         // ------------------------------------------------------------------ loader
+        reg_dec<kRegsLow>();
         uint32_t fill = 0;  // stage fills so far
         for (int k = 0;; ++k) {
             const int ii = item_for(k, cta, n_cta);
@@ -147,6 +156,7 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
         }
     } else if (warp == kMmaWarp) {
         // ------------------------------------------------------------------ MMA issuer
+        reg_dec<kRegsLow>();
         if (lane == 0) {
             const uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
             const uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
@@ -165,11 +175,12 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                     if (tr[t].n_rows > 0 && tr[t].hi > tr[t].lo) { jlo = min(jlo, tr[t].lo); jhi = max(jhi, tr[t].hi); }
                 }
                 for (int t = 0; t < NT; ++t)
-                    if (tr[t].n_rows > 0) {
+                    if (tr[t].n_rows > 0 && tr[t].hi <= tr[t].lo) {
+                        // tile present but no block of its own in this (split) item: hand Q straight back
                         mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
                         ++n_q[t];
+                        tc_commit(smem_u32(&bars.q_empty[t]));
                     }
-                tc_fence_after();
                 // step j: for each tile, PV(j-1) then QK(j).  K(j) and V(j-1) are the stages in use.
                 uint32_t st_v = 0;
                 for (int j = jlo; j <= jhi; ++j) {
@@ -202,6 +213,11 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                             if (j == tr[t].hi) tc_commit(smem_u32(&bars.o_final[t]));
                         }
                         if (have_k && j >= tr[t].lo && j < tr[t].hi) {
+                            if (j == tr[t].lo) {
+                                mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
+                                ++n_q[t];
+                                tc_fence_after();
+                            }
                             const uint32_t qb = sQ + t * C::kTileBytes, kb = sKV + st_k * C::kTileBytes;
 #pragma unroll
                             for (int kk = 0; kk < D / 16; ++kk) {
@@ -210,6 +226,7 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                                        idesc_qk, kk > 0 ? 1u : 0u);
                             }
                             tc_commit(smem_u32(&bars.s_full[t]));
+                            if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
                         }
                     }
                     if (have_v) tc_commit(smem_u32(&bars.kv_empty[st_v]));
@@ -218,8 +235,46 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                 }
             }
         }
+    } else if (warp == 2 || warp == 3) {
+        // ------------------------------------------------------------------ Q loaders
+        reg_dec<kRegsLow>();
+        const int tile = warp - 2;
+        if (tile < NT) {
+            const uint32_t qb = sQ + tile * C::kTileBytes;
+            constexpr int cpr = D / 8;                   // 16-byte chunks per row
+            constexpr int rows_per_it = 32 / cpr;        // rows covered by one warp instruction
+            uint32_t n_fill = 0;
+            for (int k = 0;; ++k) {
+                const int ii = item_for(k, cta, n_cta);
+                if (k * n_cta >= p.n_items) break;
+                if (ii >= p.n_items) continue;
+                const ItemDev it = p.items[ii];
+                const SegDev sg = p.segs[it.seg];
+                const TileRange tr = tile_range(it, sg, tile, TT, G);
+                if (tr.n_rows == 0) continue;
+                mbar_wait(smem_u32(&bars.q_empty[tile]), (n_fill & 1) ^ 1);   // last QK^T on the old Q is done
+                ++n_fill;
+                for (int rr = 0; rr < kTileRows; rr += rows_per_it) {
+                    const int row_t = rr + lane / cpr, c = lane % cpr;
+                    const uint16_t* src = p.q;
+                    uint32_t bytes = 0;                  // rows past the end are zero-filled
+                    if (row_t < tr.n_rows) {
+                        const int t = tr.tok0 + row_t / G, head = sg.kv_head * G + row_t % G;
+                        src = p.q + (sg.q_row_start + t) * p.q_row_stride + (long long)head * D + c * 8;
+                        bytes = 16;
+                    }
+                    const uint32_t off = (uint32_t)((row_t >> 3) * C::kHalves * kAtomBytes + (c >> 3) * kAtomBytes +
+                                                    (row_t & 7) * 128 + (((c & 7) ^ (row_t & 7)) << 4));
+                    cp_async16(qb + off, src, bytes);
+                }
+                cp_async_wait_all();
+                fence_proxy_async_smem();
+                mbar_arrive(smem_u32(&bars.q_full[tile]));
+            }
+        }
     } else if (warp >= kFirstSoftmaxWarp) {
         // ------------------------------------------------------------------ softmax warpgroups
+        reg_inc<kRegsHigh>();
         const int tile = (warp - kFirstSoftmaxWarp) >> 2;
         const int wq = warp & 3;                       // TMEM lane quadrant this warp may access
         const int r = wq * 32 + lane;                  // row inside the tile
@@ -237,27 +292,6 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
             const TileRange tr = tile_range(it, sg, tile, TT, G);
             if (tr.n_rows == 0) continue;
 
-            // ---- Q tile -> shared memory (K-major SW128 image), zero rows past the end
-            {
-                const uint32_t qb = sQ + tile * C::kTileBytes;
-                const int cpr = D / 8;                       // 16-byte chunks per row
-                const int rows_per_it = 32 / cpr;            // rows covered by one warp instruction
-                for (int rr = wq * 32; rr < wq * 32 + 32; rr += rows_per_it) {
-                    const int row_t = rr + lane / cpr, c = lane % cpr;
-                    uint4 v = make_uint4(0, 0, 0, 0);
-                    if (row_t < tr.n_rows) {
-                        const int t = tr.tok0 + row_t / G, head = sg.kv_head * G + row_t % G;
-                        v = *reinterpret_cast<const uint4*>(p.q + (sg.q_row_start + t) * p.q_row_stride + (long long)head * D + c * 8);
-                    }
-                    const uint32_t off = (uint32_t)((row_t >> 3) * C::kHalves * kAtomBytes + (c >> 3) * kAtomBytes +
-                                                    (row_t & 7) * 128 + (((c & 7) ^ (row_t & 7)) << 4));
-                    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(qb + off), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
-                }
-                fence_proxy_async_smem();
-                tc_fence_before();       // orders this thread's earlier TMEM reads (previous epilogue)
-                mbar_arrive(smem_u32(&bars.q_full[tile]));
-            }
-
             const int rc = min(r, tr.n_rows - 1);            // rows past the end mirror the last valid row
             const int tok = tr.tok0 + rc / G;
             const int pos = sg.kv_len - sg.q_len + tok;      // query position i
@@ -270,24 +304,26 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                 tc_fence_after();
                 const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;   // valid columns [cmin, cmax]
                 const bool need_mask = __any_sync(0xffffffffu, cmin > 0 || cmax < kBlockKeys - 1);
-                // pass 1: row max
-                float mx = -INFINITY;
+                // the whole score row of this thread: 128 fp32 columns -> registers, one wait
+                uint32_t s[kBlockKeys];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    uint32_t v[32];
-                    tmem_ld32(tS + c * 32, v);
-                    tmem_wait_ld();
-                    if (need_mask) {
+                for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, s + c * 32);
+                tmem_wait_ld();
+                if (need_mask) {
+                    // boundary block (causal diagonal / window edge): element mask in registers
 #pragma unroll
-                        for (int e = 0; e < 32; ++e) {
-                            const int col = c * 32 + e;
-                            if (col >= cmin && col <= cmax) mx = fmaxf(mx, __uint_as_float(v[e]));
-                        }
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) mx = fmaxf(mx, __uint_as_float(v[e]));
-                    }
+                    for (int e = 0; e < kBlockKeys; ++e)
+                        if (e < cmin || e > cmax) s[e] = 0xff800000u;   // -inf
                 }
+                float mxa = -INFINITY, mxb = -INFINITY, mxc = -INFINITY, mxd = -INFINITY;
+#pragma unroll
+                for (int e = 0; e < kBlockKeys; e += 8) {
+                    mxa = max3(mxa, __uint_as_float(s[e + 0]), __uint_as_float(s[e + 1]));
+                    mxb = max3(mxb, __uint_as_float(s[e + 2]), __uint_as_float(s[e + 3]));
+                    mxc = max3(mxc, __uint_as_float(s[e + 4]), __uint_as_float(s[e + 5]));
+                    mxd = max3(mxd, __uint_as_float(s[e + 6]), __uint_as_float(s[e + 7]));
+                }
+                const float mx = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
                 const float mx2 = mx * sl2;
                 // lazy rescale (warp-uniform decision: tcgen05.ld/st are warp-collective)
                 const bool grow = mx2 > m_used + kRescaleThreshold;
@@ -299,41 +335,36 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                         l *= corr;
                     }
                     if (j > tr.lo) {
-#pragma unroll
-                        for (int c = 0; c < D / 32; ++c) {
-                            uint32_t v[32];
-                            tmem_ld32(tO + c * 32, v);
+#pragma unroll 1
+                        for (int c = 0; c < D / 16; ++c) {
+                            uint32_t v[16];
+                            tmem_ld16(tO + c * 16, v);
                             tmem_wait_ld();
 #pragma unroll
-                            for (int e = 0; e < 32; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * corr);
-                            tmem_st32(tO + c * 32, v);
+                            for (int e = 0; e < 16; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * corr);
+                            tmem_st16(tO + c * 16, v);
                         }
                     }
                 }
                 const float mref = (m_used == -INFINITY) ? 0.f : m_used;
-                // pass 2: p = 2^(s*scale*log2e - m), row sum, bf16 P -> TMEM (aliases S columns [0, 64))
-                float rs = 0.f;
+                // p = 2^(s*scale*log2e - m) (masked columns: 2^-inf = 0), row sum, bf16 P -> TMEM (aliases S[0, 64))
+                float rs0 = 0.f, rs1 = 0.f, rs2 = 0.f, rs3 = 0.f;
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    uint32_t v[32];
-                    tmem_ld32(tS + c * 32, v);
-                    tmem_wait_ld();
                     uint32_t pk[16];
 #pragma unroll
-                    for (int e = 0; e < 32; e += 2) {
-                        float p0 = fast_exp2(fmaf(__uint_as_float(v[e]), sl2, -mref));
-                        float p1 = fast_exp2(fmaf(__uint_as_float(v[e + 1]), sl2, -mref));
-                        if (need_mask) {
-                            const int col = c * 32 + e;
-                            if (col < cmin || col > cmax) p0 = 0.f;
-                            if (col + 1 < cmin || col + 1 > cmax) p1 = 0.f;
-                        }
-                        rs += p0 + p1;
-                        pk[e >> 1] = pack_bf16x2(p0, p1);
+                    for (int e = 0; e < 32; e += 4) {
+                        const float p0 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 0]), sl2, -mref));
+                        const float p1 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 1]), sl2, -mref));
+                        const float p2 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 2]), sl2, -mref));
+                        const float p3 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 3]), sl2, -mref));
+                        rs0 += p0; rs1 += p1; rs2 += p2; rs3 += p3;
+                        pk[(e >> 1) + 0] = pack_bf16x2(p0, p1);
+                        pk[(e >> 1) + 1] = pack_bf16x2(p2, p3);
                     }
                     tmem_st16(tS + c * 16, pk);
                 }
-                l += rs;
+                l += (rs0 + rs1) + (rs2 + rs3);
                 tmem_wait_st();
                 tc_fence_before();
                 mbar_arrive(smem_u32(&bars.p_full[tile]));
