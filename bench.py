@@ -364,7 +364,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="2")
-    ap.add_argument("--tiles", type=int, default=1)
+    ap.add_argument("--tiles", type=int, default=2)
     ap.add_argument("--cpu-rows", type=int, default=384, help="rows in the cpu_baseline oracle sample")
     ap.add_argument("--ref-rows", type=int, default=128, help="rows per step of the --impl reference oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -156,83 +156,99 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
         }
     } else if (warp == kMmaWarp) {
         // ------------------------------------------------------------------ MMA issuer
+        // The whole warp walks the schedule and waits on the barriers (warp-uniform control flow);
+        // one elected lane issues the tcgen05 instructions.
         reg_dec<kRegsLow>();
-        if (lane == 0) {
-            const uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
-            const uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
-            uint32_t rd = 0;                       // stage reads so far
-            uint32_t n_q[2] = {0, 0}, n_p[2] = {0, 0};
-            for (int k = 0;; ++k) {
-                const int ii = item_for(k, cta, n_cta);
-                if (k * n_cta >= p.n_items) break;
-                if (ii >= p.n_items) continue;
-                const ItemDev it = p.items[ii];
-                const SegDev sg = p.segs[it.seg];
-                TileRange tr[2];
-                int jlo = INT_MAX, jhi = 0;
-                for (int t = 0; t < NT; ++t) {
-                    tr[t] = tile_range(it, sg, t, TT, G);
-                    if (tr[t].n_rows > 0 && tr[t].hi > tr[t].lo) { jlo = min(jlo, tr[t].lo); jhi = max(jhi, tr[t].hi); }
+        constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
+        constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
+        // descriptors differ from a base only in the start-address field: add (bytes >> 4)
+        const uint64_t dq0 = make_desc_sw128(sQ, 16, C::kSBO);
+        const uint64_t dk0 = make_desc_sw128(sKV, 16, C::kSBO);
+        const uint64_t dv0 = make_desc_sw128(sKV, kAtomBytes, C::kSBO);
+        uint32_t rd = 0;                       // stage reads so far
+        uint32_t n_q[2] = {0, 0}, n_p[2] = {0, 0};
+        for (int k = 0;; ++k) {
+            const int ii = item_for(k, cta, n_cta);
+            if (k * n_cta >= p.n_items) break;
+            if (ii >= p.n_items) continue;
+            const ItemDev it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            TileRange tr[2];
+            int jlo = INT_MAX, jhi = 0;
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+                tr[t] = tile_range(it, sg, t, TT, G);
+                if (tr[t].n_rows > 0 && tr[t].hi > tr[t].lo) { jlo = min(jlo, tr[t].lo); jhi = max(jhi, tr[t].hi); }
+            }
+#pragma unroll
+            for (int t = 0; t < NT; ++t)
+                if (tr[t].n_rows > 0 && tr[t].hi <= tr[t].lo) {
+                    // tile present but no block of its own in this (split) item: hand Q straight back
+                    mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
+                    ++n_q[t];
+                    if (elect_one()) tc_commit(smem_u32(&bars.q_empty[t]));
+                    __syncwarp();
                 }
-                for (int t = 0; t < NT; ++t)
-                    if (tr[t].n_rows > 0 && tr[t].hi <= tr[t].lo) {
-                        // tile present but no block of its own in this (split) item: hand Q straight back
+            // step j: for each tile, PV(j-1) then QK(j).  K(j) and V(j-1) are the stages in use.
+            uint32_t st_v = 0;
+            for (int j = jlo; j <= jhi; ++j) {
+                const bool have_k = j < jhi, have_v = j > jlo;
+                uint32_t st_k = 0;
+                if (have_v) {
+                    st_v = rd % C::kStages;
+                    mbar_wait(smem_u32(&bars.kv_full[st_v]), (rd / C::kStages) & 1);
+                    ++rd;
+                }
+                if (have_k) {
+                    st_k = rd % C::kStages;
+                    mbar_wait(smem_u32(&bars.kv_full[st_k]), (rd / C::kStages) & 1);
+                    ++rd;
+                }
+#pragma unroll
+                for (int t = 0; t < NT; ++t) {
+                    if (tr[t].n_rows == 0) continue;
+                    const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
+                    const bool do_pv = have_v && j - 1 >= tr[t].lo && j - 1 < tr[t].hi;
+                    const bool do_qk = have_k && j >= tr[t].lo && j < tr[t].hi;
+                    if (do_pv) {
+                        mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
+                        ++n_p[t];
+                    }
+                    if (do_qk && j == tr[t].lo) {
                         mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
                         ++n_q[t];
-                        tc_commit(smem_u32(&bars.q_empty[t]));
-                    }
-                // step j: for each tile, PV(j-1) then QK(j).  K(j) and V(j-1) are the stages in use.
-                uint32_t st_v = 0;
-                for (int j = jlo; j <= jhi; ++j) {
-                    const bool have_k = j < jhi, have_v = j > jlo;
-                    uint32_t st_k = 0;
-                    if (have_v) {
-                        st_v = rd % C::kStages;
-                        mbar_wait(smem_u32(&bars.kv_full[st_v]), (rd / C::kStages) & 1);
-                        ++rd;
-                    }
-                    if (have_k) {
-                        st_k = rd % C::kStages;
-                        mbar_wait(smem_u32(&bars.kv_full[st_k]), (rd / C::kStages) & 1);
-                        ++rd;
                     }
                     tc_fence_after();
-                    for (int t = 0; t < NT; ++t) {
-                        if (tr[t].n_rows == 0) continue;
-                        const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
-                        if (have_v && j - 1 >= tr[t].lo && j - 1 < tr[t].hi) {
-                            mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
-                            ++n_p[t];
-                            tc_fence_after();
-                            const uint32_t vb = sKV + st_v * C::kTileBytes;
+                    if (elect_one()) {
+                        if (do_pv) {
+                            const uint64_t dv = dv0 + (uint64_t)((st_v * C::kTileBytes) >> 4);
+                            const uint32_t acc0 = (j - 1 > tr[t].lo) ? 1u : 0u;
 #pragma unroll
-                            for (int kk = 0; kk < kBlockKeys / 16; ++kk) {
-                                const uint64_t bd = make_desc_sw128(vb + kk * 2 * C::kSBO, kAtomBytes, C::kSBO);
-                                mma_ts(tO, tS + kk * 8, bd, idesc_pv, (j - 1 > tr[t].lo || kk > 0) ? 1u : 0u);
-                            }
+                            for (int kk = 0; kk < kBlockKeys / 16; ++kk)
+                                mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
                             if (j == tr[t].hi) tc_commit(smem_u32(&bars.o_final[t]));
                         }
-                        if (have_k && j >= tr[t].lo && j < tr[t].hi) {
-                            if (j == tr[t].lo) {
-                                mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
-                                ++n_q[t];
-                                tc_fence_after();
-                            }
-                            const uint32_t qb = sQ + t * C::kTileBytes, kb = sKV + st_k * C::kTileBytes;
+                        if (do_qk) {
+                            const uint64_t dq = dq0 + (uint64_t)((t * C::kTileBytes) >> 4);
+                            const uint64_t dk = dk0 + (uint64_t)((st_k * C::kTileBytes) >> 4);
 #pragma unroll
                             for (int kk = 0; kk < D / 16; ++kk) {
-                                const uint32_t o = (kk / 4) * kAtomBytes + (kk % 4) * 32;
-                                mma_ss(tS, make_desc_sw128(qb + o, 16, C::kSBO), make_desc_sw128(kb + o, 16, C::kSBO),
-                                       idesc_qk, kk > 0 ? 1u : 0u);
+                                constexpr int dummy = 0; (void)dummy;
+                                const uint32_t o = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                                mma_ss(tS, dq + o, dk + o, idesc_qk, kk > 0 ? 1u : 0u);
                             }
                             tc_commit(smem_u32(&bars.s_full[t]));
                             if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
                         }
                     }
+                    __syncwarp();
+                }
+                if (elect_one()) {
                     if (have_v) tc_commit(smem_u32(&bars.kv_empty[st_v]));
                     if (have_k) tc_commit(smem_u32(&bars.kv_empty[st_k]));
-                    // stage order in the ring is K(j), V(j): V(j-1) was read before K(j)
                 }
+                __syncwarp();
+                // stage order in the ring is K(j), V(j): V(j-1) was read before K(j)
             }
         }
     } else if (warp == 2 || warp == 3) {
@@ -433,8 +449,8 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
 int attention_tc_tiles_per_item() {
     // SEGPA_TC_TILES=1|2 (bring-up knob; read at every build_segments call)
     const char* e = getenv("SEGPA_TC_TILES");
-    const int t = e ? atoi(e) : 1;
-    return (t == 2) ? 2 : 1;
+    const int t = e ? atoi(e) : 2;
+    return (t == 1) ? 1 : 2;
 }
 
 template <int D, int NT>
