@@ -84,7 +84,7 @@ __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev&
 }  // namespace
 
 template <int D, int NT>
-__global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(const FwdParams p) {
+__global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(const __grid_constant__ FwdParams p) {
     using C = Cfg<D, NT>;
     extern __shared__ uint8_t smem_raw[];
     __shared__ Bars bars;
@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
             mbar_init(smem_u32(&bars.kv_empty[s]), 1);
         }
         for (int t = 0; t < 2; ++t) {
-            mbar_init(smem_u32(&bars.q_full[t]), 32);
+            mbar_init(smem_u32(&bars.q_full[t]), 1);
             mbar_init(smem_u32(&bars.q_empty[t]), 1);
             mbar_init(smem_u32(&bars.s_full[t]), 1);
             mbar_init(smem_u32(&bars.p_full[t]), 128);
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
         constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
         constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
         // descriptors differ from a base only in the start-address field: add (bytes >> 4)
-        const uint64_t dq0 = make_desc_sw128(sQ, 16, C::kSBO);
+        const uint64_t dq0 = make_desc_sw128(sQ, 16, kAtomBytes);
         const uint64_t dk0 = make_desc_sw128(sKV, 16, C::kSBO);
         const uint64_t dv0 = make_desc_sw128(sKV, kAtomBytes, C::kSBO);
         uint32_t rd = 0;                       // stage reads so far
@@ -233,9 +233,9 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                             const uint64_t dk = dk0 + (uint64_t)((st_k * C::kTileBytes) >> 4);
 #pragma unroll
                             for (int kk = 0; kk < D / 16; ++kk) {
-                                constexpr int dummy = 0; (void)dummy;
-                                const uint32_t o = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
-                                mma_ss(tS, dq + o, dk + o, idesc_qk, kk > 0 ? 1u : 0u);
+                                const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
+                                const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                                mma_ss(tS, dq + oq, dk + ok, idesc_qk, kk > 0 ? 1u : 0u);
                             }
                             tc_commit(smem_u32(&bars.s_full[t]));
                             if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
@@ -252,14 +252,17 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
             }
         }
     } else if (warp == 2 || warp == 3) {
-        // ------------------------------------------------------------------ Q loaders
+        // ------------------------------------------------------------------ Q loaders (TMA)
+        // Q tile image: [D/64 halves][128 rows][128 B], SWIZZLE_128B; row r = (token, group head) as the
+        // TMA box {64 elements, G heads, tile_tokens tokens} lays it out.  Rows >= G*tile_tokens are never
+        // written (their scores are garbage and never stored); tokens past T are zero-filled by TMA.
         reg_dec<kRegsLow>();
         const int tile = warp - 2;
         if (tile < NT) {
             const uint32_t qb = sQ + tile * C::kTileBytes;
-            constexpr int cpr = D / 8;                   // 16-byte chunks per row
-            constexpr int rows_per_it = 32 / cpr;        // rows covered by one warp instruction
+            const uint32_t box_bytes = (uint32_t)(64 * 2 * G * TT);
             uint32_t n_fill = 0;
+            if (lane == 0) prefetch_tmap(&p.q_map);
             for (int k = 0;; ++k) {
                 const int ii = item_for(k, cta, n_cta);
                 if (k * n_cta >= p.n_items) break;
@@ -270,22 +273,14 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                 if (tr.n_rows == 0) continue;
                 mbar_wait(smem_u32(&bars.q_empty[tile]), (n_fill & 1) ^ 1);   // last QK^T on the old Q is done
                 ++n_fill;
-                for (int rr = 0; rr < kTileRows; rr += rows_per_it) {
-                    const int row_t = rr + lane / cpr, c = lane % cpr;
-                    const uint16_t* src = p.q;
-                    uint32_t bytes = 0;                  // rows past the end are zero-filled
-                    if (row_t < tr.n_rows) {
-                        const int t = tr.tok0 + row_t / G, head = sg.kv_head * G + row_t % G;
-                        src = p.q + (sg.q_row_start + t) * p.q_row_stride + (long long)head * D + c * 8;
-                        bytes = 16;
-                    }
-                    const uint32_t off = (uint32_t)((row_t >> 3) * C::kHalves * kAtomBytes + (c >> 3) * kAtomBytes +
-                                                    (row_t & 7) * 128 + (((c & 7) ^ (row_t & 7)) << 4));
-                    cp_async16(qb + off, src, bytes);
+                if (elect_one()) {
+                    mbar_arrive_expect_tx(smem_u32(&bars.q_full[tile]), box_bytes * C::kHalves);
+#pragma unroll
+                    for (int h = 0; h < C::kHalves; ++h)
+                        tma_load_3d(qb + h * (kTileRows * 128), &p.q_map, h * 64, sg.kv_head * G, (int)(sg.q_row_start + tr.tok0),
+                                    smem_u32(&bars.q_full[tile]));
                 }
-                cp_async_wait_all();
-                fence_proxy_async_smem();
-                mbar_arrive(smem_u32(&bars.q_full[tile]));
+                __syncwarp();
             }
         }
     } else if (warp >= kFirstSoftmaxWarp) {

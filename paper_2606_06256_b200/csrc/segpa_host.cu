@@ -4,6 +4,8 @@
 #include "../../include/segpa.h"
 #include "segpa_internal.h"
 
+#include <cuda.h>   // CUtensorMap types only; the encoder is fetched with cudaGetDriverEntryPoint (no -lcuda)
+
 #include <algorithm>
 #include <climits>
 #include <cstdarg>
@@ -135,6 +137,36 @@ void free_segments_obj(segpa_segments* s) {
 }
 
 inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+// TMA descriptor of Q [T][Hq][D] bf16 (row stride given): box {64 elements, G heads, tile_tokens tokens},
+// SWIZZLE_128B, out-of-range tokens zero-filled.  One box = one 64-element half of a 128-row Q tile.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+const char* encode_q_map(TensorMap* out, const void* q, int64_t T, int Hq, int D, int G, int tile_tokens,
+                         int64_t row_stride_elems) {
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qr) != cudaSuccess || !f ||
+            qr != cudaDriverEntryPointSuccess) {
+            cudaGetLastError();
+            return "cuTensorMapEncodeTiled is not available from the driver";
+        }
+        fn = (EncodeTiledFn)f;
+    }
+    static_assert(sizeof(CUtensorMap) == sizeof(TensorMap), "tensor map size");
+    const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)T};
+    const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)row_stride_elems * 2};
+    const cuuint32_t box[3] = {64u, (cuuint32_t)G, (cuuint32_t)tile_tokens};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    CUresult r = fn((CUtensorMap*)out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? nullptr : "cuTensorMapEncodeTiled failed";
+}
 
 // attended keys of the query at position i (Alg. 2 policy; PAPER.md:219 with W = w + 1)
 inline int64_t visible_count(int64_t i, int head_class, int64_t W) {
@@ -619,6 +651,10 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     p.tiles_per_item = s->tiles_per_item;
     p.page_bytes = c->page_bytes;
     p.num_sms = c->num_sms;
+    if (c->kernel_kind == 1) {
+        const char* why = encode_q_map(&p.q_map, q, T, Hq, D, c->G, p.tile_tokens, q_row_stride);
+        if (why) return fail(SEGPA_ERR_CUDA, "attention_fwd: %s", why);
+    }
 
     e = cudaMemsetAsync(s->d_counter, 0, 256, st);
     int launches = 0;

@@ -61,7 +61,13 @@ struct CombDev {
     int pad0, pad1, pad2;
 };
 
+// 128-byte TMA descriptor (CUtensorMap) of Q viewed as [T][Hq][D]; encoded per attention_fwd call.
+struct alignas(64) TensorMap {
+    unsigned long long opaque[16];
+};
+
 struct FwdParams {
+    TensorMap q_map;             // box {64 elements, G heads, tile_tokens tokens}, SWIZZLE_128B
     const SegDev* segs;
     const ItemDev* items;
     const int* pages;            // translated physical page ids (zero page = num_pages)
