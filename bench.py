@@ -183,38 +183,27 @@ def run_ours(args):
     qs = [wl.q_values(w, l, dev) for l in range(w.num_layers)]
     outs = [torch.empty_like(q) for q in qs]
     lses = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32, device=dev) for l in range(w.num_layers)]
-    # the batch's K/V rows, resident in HBM (what the QKV projections would have produced)
-    owners = [s for s in w.streams if s.shared_from is None]
-    aliased = [s for s in w.streams if s.shared_from is not None]
-    order = owners + aliased
-    rows = {}
-    for s in order:
-        pp = s.n_shared_prefix_pages
-        if s.kv_len - pp * w.P > 0:
-            rows[id(s)] = (wl.stream_rows(k_pool, s, w.P, pp), wl.stream_rows(v_pool, s, w.P, pp))
+    # the batch's K/V rows, resident in HBM (what the QKV projections would have produced); the
+    # marshalled request array is prepared once (the same batch is stored every step)
+    append_reqs = H.append_requests(w, k_pool, v_pool)
+    batch = B.AppendBatch(append_reqs)
+    rows = [(r[3], r[4]) for r in append_reqs if r[3] is not None]
     cache = H.create_cache(w, local_rank)
     stream = torch.cuda.current_stream()
     flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
     useful = sum(wl.useful_flops(w, l) for l in range(w.num_layers))
     seg_objs = []
-    appended = [False]
     launches = [0]
+    seg_batches = [B.SegmentBatch(H.segment_reqs(w, l)) for l in range(w.num_layers)]
 
     def append_all():
-        n = 0
-        if appended[0]:
-            for s in reversed(order):
-                B.segpa_free_stream(cache, s.layer, s.kv_head, s.seq_id)
-        for s in order:
-            pp = s.n_shared_prefix_pages
-            if pp > 0:
-                B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, None, None, pp * w.P, page_ids=s.page_ids[:pp])
-            if id(s) in rows:
-                kr, vr = rows[id(s)]
-                B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, kr, vr, kr.shape[0], page_ids=s.page_ids[pp:], stream=stream)
-                n += 1
-        appended[0] = True
-        return n
+        """a1: drop the previous batch's streams and segment objects, store this batch (one scatter launch)"""
+        for s in seg_objs:
+            B.segpa_free_segments(cache, s)
+        seg_objs.clear()
+        B.segpa_clear_streams(cache)
+        B.segpa_append_pages_batch(cache, batch, stream=stream)
+        return 1
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
@@ -225,7 +214,7 @@ def run_ours(args):
         e0.record(stream)
         n = append_all()
         for l in range(w.num_layers):
-            segs = H.build_layer(cache, w, l, stream=stream)
+            segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
             seg_objs.append(segs)
             a, b = ev(), ev()
             a.record(stream)
@@ -240,9 +229,6 @@ def run_ours(args):
 
     def free_segs():
         torch.cuda.synchronize()
-        for s in seg_objs:
-            B.segpa_free_segments(cache, s)
-        seg_objs.clear()
 
     for _ in range(args.warmup):
         step(False)
@@ -278,20 +264,20 @@ def run_ours(args):
     fwd_mean = float(np.mean(fwd_ms))
 
     # ---- e2e through the host-buffer entry point: H2D of the step's K/V rows and Q, D2H of out + LSE
-    h_rows = {k: (a.cpu().pin_memory(), b.cpu().pin_memory()) for k, (a, b) in rows.items()}
+    h_rows = [(a.cpu().pin_memory(), b.cpu().pin_memory()) for a, b in rows]
     h_q = [q.cpu().pin_memory() for q in qs]
     h_out = [torch.empty_like(q).pin_memory() for q in h_q]
     h_lse = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32).pin_memory() for l in range(w.num_layers)]
-    h2d = sum(a.numel() * 2 * 2 for a, _ in h_rows.values()) + sum(q.numel() * 2 for q in h_q)
+    h2d = sum(a.numel() * 2 * 2 for a, _ in h_rows) + sum(q.numel() * 2 for q in h_q)
     d2h = sum(o.numel() * 2 for o in h_out) + sum(x.numel() * 4 for x in h_lse)
 
     def e2e_step():
-        for k, (a, b) in h_rows.items():
-            rows[k][0].copy_(a, non_blocking=True)
-            rows[k][1].copy_(b, non_blocking=True)
+        for (dk, dv), (a, b) in zip(rows, h_rows):
+            dk.copy_(a, non_blocking=True)
+            dv.copy_(b, non_blocking=True)
         append_all()
         for l in range(w.num_layers):
-            segs = H.build_layer(cache, w, l, stream=stream)
+            segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
             seg_objs.append(segs)
             B.segpa_attention_fwd_host(cache, segs, h_q[l], w.scale, h_out[l], h_lse[l], stream=stream)
         torch.cuda.synchronize()
@@ -311,12 +297,13 @@ def run_ours(args):
     e2e_val = world * useful / e2e_s / 1e12
 
     # ---- plan statistics / algorithmic bytes for the roofline
-    segs0 = H.build_layer(cache, w, 0)
-    st0 = B.segpa_segments_stats(segs0)
+    st0 = None
     alg_bytes = 0
     for l in range(w.num_layers):
-        sg = segs0 if l == 0 else H.build_layer(cache, w, l)
+        sg = H.build_layer(cache, w, l)
         st = B.segpa_segments_stats(sg)
+        B.segpa_free_segments(cache, sg)
+        st0 = st0 or st
         cov_rows = sum(s.q_len * w.G for s in w.layer_segments(l))
         alg_bytes += st["visible_kv_tokens"] * w.D * 2 * 2 + cov_rows * w.D * 2 * 2 + cov_rows * 4
     torch.cuda.synchronize()
@@ -337,7 +324,7 @@ def run_ours(args):
             "data": "synthetic",
             "config": {"workload": w.name, "Hq": w.Hq, "Hkv": w.Hkv, "D": w.D, "page_size": w.P, "layers": w.num_layers,
                        "q_rows": int(sum(w.T)), "segments": len(w.segments), "l2_flush_between_steps": True,
-                       "step": "append_pages + build_segments + attention_fwd per layer", "tiles_per_item": int(os.environ["SEGPA_TC_TILES"]),
+                       "step": "append_pages_batch + (build_segments + attention_fwd) per layer", "tiles_per_item": int(os.environ["SEGPA_TC_TILES"]),
                        "replicas": world},
             "fwd_ms_per_step": fwd_mean, "us_per_layer": 1e3 * fwd_mean / w.num_layers,
             "pct_of_bf16_peak": 100.0 * (useful / (fwd_mean * 1e-3) / 1e12) / peaks["bf16_tflops"],

@@ -114,6 +114,34 @@ segpa_status_t segpa_append_pages(segpa_cache_t *cache, int32_t layer, int32_t k
                                   int64_t src_row_stride_elems, int64_t n_tokens,
                                   const int32_t *page_ids, int32_t n_page_ids, void *cuda_stream);
 
+/*
+ * Batched form of segpa_append_pages: the n requests are applied in order (a later request may
+ * attach pages an earlier one of the same batch fills, or extend the same stream) with ONE
+ * descriptor upload and ONE scatter-kernel launch on cuda_stream for all COPY-mode requests.
+ * This is how a layer's batch of new K/V rows is stored (a1 of the hot path).  All-or-nothing: on
+ * error no stream, page table or reference count has changed.  Field meaning and errors are those
+ * of segpa_append_pages; the message names the failing request index.
+ */
+typedef struct {
+    int32_t layer;
+    int32_t kv_head;
+    int64_t seq_id;
+    const void *k_src;            /* device bf16 rows, or NULL (with v_src NULL) = ATTACH */
+    const void *v_src;
+    int64_t src_row_stride_elems;
+    int64_t n_tokens;
+    const int32_t *page_ids;      /* host; NULL = allocator chooses (COPY mode only) */
+    int32_t n_page_ids;
+    int32_t reserved;             /* 0 */
+} segpa_append_req_t;
+
+segpa_status_t segpa_append_pages_batch(segpa_cache_t *cache, const segpa_append_req_t *reqs, int32_t n,
+                                        void *cuda_stream);
+
+/* Drop every stream of the cache (all pages return to the free list).  Segment objects built
+ * earlier keep their translated page lists and must not be used afterwards. */
+segpa_status_t segpa_clear_streams(segpa_cache_t *cache);
+
 /* Drop a stream: its pages' reference counts are decremented; pages reaching zero return to the
  * free list.  Errors: INVALID (no such stream). */
 segpa_status_t segpa_free_stream(segpa_cache_t *cache, int32_t layer, int32_t kv_head,
@@ -173,6 +201,9 @@ segpa_status_t segpa_build_segments(segpa_cache_t *cache, int32_t layer,
                                     const segpa_segment_req_t *reqs, int32_t n,
                                     segpa_segments_t **out, void *cuda_stream);
 
+/* Release a segments object.  Does not synchronise the device: its buffers are recycled by later
+ * build_segments calls only after the work that last used them (upload, attention_fwd) has
+ * completed (tracked with an event on the stream it was last used on). */
 segpa_status_t segpa_free_segments(segpa_cache_t *cache, segpa_segments_t *segs);
 
 typedef struct {

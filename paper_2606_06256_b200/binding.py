@@ -18,7 +18,8 @@ GLOBAL, LOCAL = 0, 1
 _STATUS = {0: "OK", 1: "INVALID", 2: "OOM", 3: "CUDA", 4: "UNSUPPORTED", 5: "STATE"}
 
 EXPORTS = [
-    "segpa_pool_bytes", "segpa_create_cache", "segpa_append_pages", "segpa_free_stream",
+    "segpa_pool_bytes", "segpa_create_cache", "segpa_append_pages", "segpa_append_pages_batch",
+    "segpa_clear_streams", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
     "segpa_attention_fwd_host", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
@@ -42,6 +43,12 @@ class SegmentReq(C.Structure):
     _fields_ = [("seq_id", C.c_int64), ("kv_head", C.c_int32), ("head_class", C.c_int32),
                 ("window", C.c_int32), ("n_sink", C.c_int32), ("q_row_start", C.c_int64),
                 ("q_len", C.c_int32), ("reserved", C.c_int32)]
+
+
+class AppendReq(C.Structure):
+    _fields_ = [("layer", C.c_int32), ("kv_head", C.c_int32), ("seq_id", C.c_int64), ("k_src", C.c_void_p),
+                ("v_src", C.c_void_p), ("src_row_stride_elems", C.c_int64), ("n_tokens", C.c_int64),
+                ("page_ids", C.c_void_p), ("n_page_ids", C.c_int32), ("reserved", C.c_int32)]
 
 
 class PlanStats(C.Structure):
@@ -74,6 +81,8 @@ def lib():
         L.segpa_create_cache.argtypes = [C.POINTER(CacheDesc), C.POINTER(C.c_void_p)]
         L.segpa_append_pages.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_void_p, C.c_void_p,
                                          C.c_int64, C.c_int64, C.c_void_p, C.c_int32, C.c_void_p]
+        L.segpa_append_pages_batch.argtypes = [C.c_void_p, C.POINTER(AppendReq), C.c_int32, C.c_void_p]
+        L.segpa_clear_streams.argtypes = [C.c_void_p]
         L.segpa_free_stream.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64]
         L.segpa_stream_info.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_int64),
                                         C.POINTER(C.c_int32), C.c_void_p, C.c_int32]
@@ -139,6 +148,43 @@ def segpa_append_pages(cache: int, layer: int, kv_head: int, seq_id: int, k_src,
                                     _stream_ptr(stream)))
 
 
+class AppendBatch:
+    """Marshalled argument array of segpa_append_pages_batch; can be prepared once and passed again
+    (the tensors and page-id arrays it refers to are kept alive here)."""
+
+    def __init__(self, reqs: Sequence[tuple]):
+        """reqs: tuples (layer, kv_head, seq_id, k_src, v_src, n_tokens, page_ids) with k_src / v_src torch
+        bf16 device tensors [n_tokens][D] or None (attach), page_ids an int sequence or None."""
+        self.n = len(reqs)
+        self.arr = (AppendReq * max(1, self.n))()
+        self._keep = []
+        for i, (layer, kvh, seq, k_src, v_src, n_tokens, page_ids) in enumerate(reqs):
+            kp = vp = None
+            stride = 0
+            if k_src is not None:
+                assert k_src.is_cuda and v_src.is_cuda and k_src.stride(-1) == 1 and v_src.stride(-1) == 1
+                assert k_src.stride(0) == v_src.stride(0)
+                kp, vp, stride = k_src.data_ptr(), v_src.data_ptr(), k_src.stride(0)
+                self._keep.append((k_src, v_src))
+            ip, n_ids = None, 0
+            if page_ids is not None:
+                ids = np.ascontiguousarray(page_ids, dtype=np.int32)
+                self._keep.append(ids)
+                ip, n_ids = ids.ctypes.data, len(ids)
+            self.arr[i] = AppendReq(int(layer), int(kvh), int(seq), kp, vp, int(stride), int(n_tokens), ip, n_ids, 0)
+
+
+def segpa_append_pages_batch(cache: int, batch, stream=None) -> None:
+    """batch: an AppendBatch, or the list of tuples AppendBatch takes."""
+    if not isinstance(batch, AppendBatch):
+        batch = AppendBatch(batch)
+    _check(lib().segpa_append_pages_batch(cache, batch.arr, batch.n, _stream_ptr(stream)))
+
+
+def segpa_clear_streams(cache: int) -> None:
+    _check(lib().segpa_clear_streams(cache))
+
+
 def segpa_free_stream(cache: int, layer: int, kv_head: int, seq_id: int) -> None:
     _check(lib().segpa_free_stream(cache, layer, kv_head, seq_id))
 
@@ -158,13 +204,23 @@ def segpa_pool_stats(cache: int):
     return a.value, b.value
 
 
-def segpa_build_segments(cache: int, layer: int, reqs: Sequence[tuple], stream=None) -> int:
-    """reqs: tuples (seq_id, kv_head, head_class, window, n_sink, q_row_start, q_len)."""
-    arr = (SegmentReq * max(1, len(reqs)))()
-    for i, (seq, kvh, cls, W, ns, qs, ql) in enumerate(reqs):
-        arr[i] = SegmentReq(int(seq), int(kvh), int(cls), int(W), int(ns), int(qs), int(ql), 0)
+class SegmentBatch:
+    """Marshalled segpa_segment_req_t array; can be prepared once and passed again."""
+
+    def __init__(self, reqs: Sequence[tuple]):
+        """reqs: tuples (seq_id, kv_head, head_class, window, n_sink, q_row_start, q_len)."""
+        self.n = len(reqs)
+        self.arr = (SegmentReq * max(1, self.n))()
+        for i, (seq, kvh, cls, W, ns, qs, ql) in enumerate(reqs):
+            self.arr[i] = SegmentReq(int(seq), int(kvh), int(cls), int(W), int(ns), int(qs), int(ql), 0)
+
+
+def segpa_build_segments(cache: int, layer: int, reqs, stream=None) -> int:
+    """reqs: a SegmentBatch, or the list of tuples SegmentBatch takes."""
+    if not isinstance(reqs, SegmentBatch):
+        reqs = SegmentBatch(reqs)
     out = C.c_void_p()
-    _check(lib().segpa_build_segments(cache, layer, arr, len(reqs), C.byref(out), _stream_ptr(stream)))
+    _check(lib().segpa_build_segments(cache, layer, reqs.arr, reqs.n, C.byref(out), _stream_ptr(stream)))
     return out.value
 
 

@@ -64,6 +64,79 @@ struct DeviceGuard {
 
 }  // namespace
 
+namespace {
+
+// Pinned host + device buffer pair reused by successive uploads.  `ev` marks the completion of the
+// last work that used the pair; it is waited for (on the host) before the pair is overwritten.
+struct Staging {
+    void* h = nullptr;
+    void* d = nullptr;
+    size_t cap = 0;
+    cudaEvent_t ev = nullptr;
+    bool pending = false;
+};
+
+cudaError_t staging_acquire(Staging& s, size_t bytes) {
+    cudaError_t e = cudaSuccess;
+    if (!s.ev) {
+        e = cudaEventCreateWithFlags(&s.ev, cudaEventDisableTiming);
+        if (e != cudaSuccess) return e;
+    }
+    if (s.pending) {
+        e = cudaEventSynchronize(s.ev);
+        s.pending = false;
+        if (e != cudaSuccess) return e;
+    }
+    if (bytes > s.cap) {
+        if (s.h) cudaFreeHost(s.h);
+        if (s.d) cudaFree(s.d);
+        s.h = s.d = nullptr;
+        s.cap = 0;
+        const size_t cap = std::max<size_t>(bytes + bytes / 2, 64 << 10);
+        e = cudaMallocHost(&s.h, cap);
+        if (e == cudaSuccess) e = cudaMalloc(&s.d, cap);
+        if (e != cudaSuccess) {
+            if (s.h) cudaFreeHost(s.h);
+            s.h = nullptr;
+            return e;
+        }
+        s.cap = cap;
+    }
+    return cudaSuccess;
+}
+
+void staging_release(Staging& s, cudaStream_t st) {
+    if (s.ev && cudaEventRecord(s.ev, st) == cudaSuccess) s.pending = true;
+}
+
+void staging_free(Staging& s) {
+    if (s.h) cudaFreeHost(s.h);
+    if (s.d) cudaFree(s.d);
+    if (s.ev) cudaEventDestroy(s.ev);
+    s = Staging();
+}
+
+// Device-side storage of one segments object (descriptor blob, scheduler cursor, split-KV
+// workspace); recycled through the cache's free list instead of cudaMalloc / cudaFree per build.
+struct SegBuf {
+    Staging blob;
+    int* counter = nullptr;
+    float* ws_o = nullptr;
+    float* ws_ml = nullptr;
+    size_t ws_rows = 0;   // capacity in partial rows
+};
+
+void segbuf_free(SegBuf* b) {
+    if (!b) return;
+    staging_free(b->blob);
+    if (b->counter) cudaFree(b->counter);
+    if (b->ws_o) cudaFree(b->ws_o);
+    if (b->ws_ml) cudaFree(b->ws_ml);
+    delete b;
+}
+
+}  // namespace
+
 struct segpa_segments {
     segpa_cache* cache = nullptr;
     int32_t layer = 0;
@@ -76,13 +149,9 @@ struct segpa_segments {
     segpa_plan_stats_t stats{};
     int tiles_per_item = 1;
     // device
-    uint8_t* d_blob = nullptr;
-    void* h_blob = nullptr;   // pinned staging for the upload
-    size_t blob_bytes = 0;
+    SegBuf* buf = nullptr;
+    mutable cudaStream_t last_stream = nullptr;   // stream of the last upload / attention_fwd
     size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0;
-    int* d_counter = nullptr;
-    float* d_ws_o = nullptr;
-    float* d_ws_ml = nullptr;
 };
 
 struct segpa_cache {
@@ -98,6 +167,11 @@ struct segpa_cache {
     int64_t n_free = 0;
     std::unordered_map<StreamKey, StreamRec, StreamKeyHash> streams;
     std::vector<segpa_segments*> seg_objs;
+    std::vector<SegBuf*> free_bufs;
+    std::vector<uint32_t> dup_mark;  // append_pages: duplicate detection stamps
+    uint32_t dup_stamp = 0;
+    Staging append_stage[2];         // alternating, so staging a batch does not wait for the previous one
+    int append_turn = 0;
     int num_sms = 148;
     int kernel_kind = 1;  // 0 = SIMT bring-up kernel (SEGPA_KERNEL=simt), 1 = tcgen05
     int last_launches = 0;
@@ -126,13 +200,13 @@ void release_page(segpa_cache* c, int32_t id) {
     }
 }
 
-void free_segments_obj(segpa_segments* s) {
+// returns the object's device storage to the cache's free list (no device synchronisation)
+void free_segments_obj(segpa_cache* c, segpa_segments* s) {
     if (!s) return;
-    if (s->d_blob) cudaFree(s->d_blob);
-    if (s->h_blob) cudaFreeHost(s->h_blob);
-    if (s->d_counter) cudaFree(s->d_counter);
-    if (s->d_ws_o) cudaFree(s->d_ws_o);
-    if (s->d_ws_ml) cudaFree(s->d_ws_ml);
+    if (s->buf) {
+        staging_release(s->buf->blob, s->last_stream);
+        c->free_bufs.push_back(s->buf);
+    }
     delete s;
 }
 
@@ -267,7 +341,10 @@ segpa_status_t segpa_destroy(segpa_cache_t* c) {
     if (!c) return SEGPA_OK;
     DeviceGuard g(c->desc.device);
     if (!c->planning_only) cudaDeviceSynchronize();
-    for (auto* s : c->seg_objs) free_segments_obj(s);
+    for (auto* s : c->seg_objs) free_segments_obj(c, s);
+    for (auto* b : c->free_bufs) segbuf_free(b);
+    staging_free(c->append_stage[0]);
+    staging_free(c->append_stage[1]);
     if (c->st_q) cudaFree(c->st_q);
     if (c->st_out) cudaFree(c->st_out);
     if (c->st_lse) cudaFree(c->st_lse);
@@ -276,87 +353,161 @@ segpa_status_t segpa_destroy(segpa_cache_t* c) {
     return SEGPA_OK;
 }
 
+segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req_t* reqs, int32_t n,
+                                        void* cuda_stream) {
+    if (!c || !reqs) return fail(SEGPA_ERR_INVALID, "append_pages: null argument");
+    if (n < 1) return fail(SEGPA_ERR_INVALID, "append_pages: batch size %d < 1", n);
+    const int P = c->desc.page_size, D = c->desc.head_dim;
+
+    // Requests are applied to the host state in order; `undo` lets a later failure restore it exactly.
+    struct Undo { StreamKey key; bool created; int64_t old_len; size_t n_new; };
+    std::vector<Undo> undo;
+    std::vector<ScatterJob> jobs;
+    std::vector<int32_t> touched;     // page ids the scatter kernel indexes, job after job
+    long long total_chunks = 0;
+    auto rollback = [&]() {
+        for (size_t u = undo.size(); u-- > 0;) {
+            auto it = c->streams.find(undo[u].key);
+            StreamRec& rec = it->second;
+            for (size_t k = 0; k < undo[u].n_new; ++k) {
+                release_page(c, rec.pages.back());
+                rec.pages.pop_back();
+            }
+            rec.kv_len = undo[u].old_len;
+            if (undo[u].created) c->streams.erase(it);
+        }
+    };
+#define APPEND_FAIL(code, ...) do { rollback(); return fail(code, __VA_ARGS__); } while (0)
+
+    try {
+        for (int32_t i = 0; i < n; ++i) {
+            const segpa_append_req_t& r = reqs[i];
+            if (r.layer < 0 || r.layer >= c->desc.num_layers) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: layer %d out of range", i, r.layer);
+            if (r.kv_head < 0 || r.kv_head >= c->desc.num_kv_heads) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: kv_head %d out of range", i, r.kv_head);
+            if (r.n_tokens < 1) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: n_tokens %lld < 1", i, (long long)r.n_tokens);
+            if ((r.k_src == nullptr) != (r.v_src == nullptr)) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: give both k_src and v_src, or neither (attach)", i);
+            if (r.n_page_ids < 0 || (r.n_page_ids > 0 && !r.page_ids)) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: bad page_ids", i);
+            const bool attach = (r.k_src == nullptr);
+            if (!attach && c->planning_only) APPEND_FAIL(SEGPA_ERR_STATE, "append_pages[%d]: copy mode on a planning-only cache", i);
+            if (!attach && r.src_row_stride_elems < D) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: src_row_stride_elems %lld < head_dim", i, (long long)r.src_row_stride_elems);
+            if (!attach && ((r.src_row_stride_elems % 8) || ((uintptr_t)r.k_src % 16) || ((uintptr_t)r.v_src % 16)))
+                APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: k_src / v_src must be 16-byte aligned with a row stride multiple of 8 elements", i);
+
+            const StreamKey key{r.layer, r.kv_head, r.seq_id};
+            auto it = c->streams.find(key);
+            const bool created = (it == c->streams.end());
+            const int64_t cur_len = created ? 0 : it->second.kv_len;
+            const int64_t cur_pages = cdiv(cur_len, P);
+            const int64_t new_len = cur_len + r.n_tokens;
+            if (new_len > (int64_t)INT32_MAX - 2 * kBlockKeys) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: stream too long", i);
+            const int64_t need = cdiv(new_len, P) - cur_pages;
+
+            if (attach) {
+                if (!r.page_ids) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs page_ids", i);
+                if (cur_len % P != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs the stream length (%lld) to be a multiple of page_size", i, (long long)cur_len);
+                if (r.n_page_ids != need) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs %lld page ids, got %d", i, (long long)need, r.n_page_ids);
+                for (int32_t k = 0; k < r.n_page_ids; ++k) {
+                    if (r.page_ids[k] < 0 || r.page_ids[k] >= c->desc.num_pages) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page id %d out of range", i, r.page_ids[k]);
+                    if (!c->planning_only && c->refcnt[r.page_ids[k]] == 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach of page %d which holds no data", i, r.page_ids[k]);
+                }
+            } else if (r.page_ids) {
+                if (r.n_page_ids != need) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: need %lld page ids, got %d", i, (long long)need, r.n_page_ids);
+                for (int32_t k = 0; k < r.n_page_ids; ++k) {
+                    if (r.page_ids[k] < 0 || r.page_ids[k] >= c->desc.num_pages) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page id %d out of range", i, r.page_ids[k]);
+                    if (c->refcnt[r.page_ids[k]] != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page %d is not free", i, r.page_ids[k]);
+                }
+                // duplicates inside one request: stamp array, O(n)
+                if (c->dup_mark.size() != c->refcnt.size()) c->dup_mark.assign(c->refcnt.size(), 0);
+                const uint32_t stamp = ++c->dup_stamp;
+                for (int32_t k = 0; k < r.n_page_ids; ++k) {
+                    if (c->dup_mark[r.page_ids[k]] == stamp) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: duplicate page id %d", i, r.page_ids[k]);
+                    c->dup_mark[r.page_ids[k]] = stamp;
+                }
+            } else {
+                if (need > c->n_free) APPEND_FAIL(SEGPA_ERR_OOM, "append_pages[%d]: pool exhausted (%lld pages needed, %lld free)", i, (long long)need, (long long)c->n_free);
+            }
+
+            // the request is valid: apply it
+            StreamRec& rec = c->streams[key];
+            undo.push_back(Undo{key, created, cur_len, (size_t)need});
+            if (!attach) {
+                ScatterJob jb{};
+                jb.k_src = (const uint16_t*)r.k_src;
+                jb.v_src = (const uint16_t*)r.v_src;
+                jb.src_stride = r.src_row_stride_elems;
+                jb.n_tokens = r.n_tokens;
+                jb.chunk_begin = total_chunks;
+                jb.page_off = (long long)touched.size();
+                jb.first_slot = (int)(cur_len % P);
+                jb.n_pages = (int)need + (cur_len % P != 0 ? 1 : 0);
+                if (cur_len % P != 0) touched.push_back(rec.pages.back());
+                total_chunks += ((long long)jb.n_pages * P - jb.first_slot) * (D >> 3);
+                jobs.push_back(jb);
+            }
+            for (int64_t k = 0; k < need; ++k) {
+                const int32_t id = r.page_ids ? r.page_ids[k] : pop_free_page(c);
+                if (c->refcnt[id] == 0) --c->n_free;
+                ++c->refcnt[id];
+                rec.pages.push_back(id);
+                if (!attach) touched.push_back(id);
+            }
+            rec.kv_len = new_len;
+        }
+    } catch (const std::bad_alloc&) {
+        APPEND_FAIL(SEGPA_ERR_OOM, "append_pages: host allocation failed");
+    }
+
+    // device part: one descriptor upload + one scatter launch for the whole batch
+    if (!jobs.empty()) {
+        DeviceGuard g(c->desc.device);
+        cudaStream_t st = (cudaStream_t)cuda_stream;
+        Staging& sg = c->append_stage[c->append_turn];
+        c->append_turn ^= 1;
+        const size_t jobs_bytes = (jobs.size() * sizeof(ScatterJob) + 255) & ~(size_t)255;
+        const size_t bytes = jobs_bytes + touched.size() * sizeof(int32_t);
+        cudaError_t e = staging_acquire(sg, bytes);
+        if (e == cudaSuccess) {
+            memcpy(sg.h, jobs.data(), jobs.size() * sizeof(ScatterJob));
+            memcpy((uint8_t*)sg.h + jobs_bytes, touched.data(), touched.size() * sizeof(int32_t));
+            e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+        }
+        if (e == cudaSuccess)
+            e = launch_scatter_pages(c->k_pool, c->v_pool, (const ScatterJob*)sg.d, (int)jobs.size(),
+                                     (const int*)((const uint8_t*)sg.d + jobs_bytes), total_chunks, D, P, st);
+        if (e == cudaSuccess) staging_release(sg, st);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            APPEND_FAIL(SEGPA_ERR_CUDA, "append_pages: %s", cudaGetErrorString(e));
+        }
+    }
+#undef APPEND_FAIL
+    return SEGPA_OK;
+}
+
 segpa_status_t segpa_append_pages(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id,
                                   const void* k_src, const void* v_src, int64_t src_row_stride_elems,
                                   int64_t n_tokens, const int32_t* page_ids, int32_t n_page_ids,
                                   void* cuda_stream) {
-    if (!c) return fail(SEGPA_ERR_INVALID, "append_pages: null cache");
-    if (layer < 0 || layer >= c->desc.num_layers) return fail(SEGPA_ERR_INVALID, "append_pages: layer %d out of range", layer);
-    if (kv_head < 0 || kv_head >= c->desc.num_kv_heads) return fail(SEGPA_ERR_INVALID, "append_pages: kv_head %d out of range", kv_head);
-    if (n_tokens < 1) return fail(SEGPA_ERR_INVALID, "append_pages: n_tokens %lld < 1", (long long)n_tokens);
-    if ((k_src == nullptr) != (v_src == nullptr)) return fail(SEGPA_ERR_INVALID, "append_pages: give both k_src and v_src, or neither (attach)");
-    if (n_page_ids < 0 || (n_page_ids > 0 && !page_ids)) return fail(SEGPA_ERR_INVALID, "append_pages: bad page_ids");
-    const bool attach = (k_src == nullptr);
-    const int P = c->desc.page_size, D = c->desc.head_dim;
-    if (!attach && c->planning_only) return fail(SEGPA_ERR_STATE, "append_pages: copy mode on a planning-only cache");
-    if (!attach && src_row_stride_elems < D) return fail(SEGPA_ERR_INVALID, "append_pages: src_row_stride_elems %lld < head_dim", (long long)src_row_stride_elems);
+    segpa_append_req_t r{};
+    r.layer = layer;
+    r.kv_head = kv_head;
+    r.seq_id = seq_id;
+    r.k_src = k_src;
+    r.v_src = v_src;
+    r.src_row_stride_elems = src_row_stride_elems;
+    r.n_tokens = n_tokens;
+    r.page_ids = page_ids;
+    r.n_page_ids = n_page_ids;
+    return segpa_append_pages_batch(c, &r, 1, cuda_stream);
+}
 
-    StreamKey key{layer, kv_head, seq_id};
-    auto it = c->streams.find(key);
-    const int64_t cur_len = (it == c->streams.end()) ? 0 : it->second.kv_len;
-    const int64_t cur_pages = cdiv(cur_len, P);
-    const int64_t new_len = cur_len + n_tokens;
-    if (new_len > (int64_t)INT32_MAX - 2 * kBlockKeys) return fail(SEGPA_ERR_INVALID, "append_pages: stream too long");
-    const int64_t need = cdiv(new_len, P) - cur_pages;
-
-    std::vector<int32_t> newp;
-    if (attach) {
-        if (!page_ids) return fail(SEGPA_ERR_INVALID, "append_pages: attach needs page_ids");
-        if (cur_len % P != 0) return fail(SEGPA_ERR_INVALID, "append_pages: attach needs the stream length (%lld) to be a multiple of page_size", (long long)cur_len);
-        if (n_page_ids != need) return fail(SEGPA_ERR_INVALID, "append_pages: attach needs %lld page ids, got %d", (long long)need, n_page_ids);
-        for (int32_t i = 0; i < n_page_ids; ++i) {
-            if (page_ids[i] < 0 || page_ids[i] >= c->desc.num_pages) return fail(SEGPA_ERR_INVALID, "append_pages: page id %d out of range", page_ids[i]);
-            if (!c->planning_only && c->refcnt[page_ids[i]] == 0) return fail(SEGPA_ERR_INVALID, "append_pages: attach of page %d which holds no data", page_ids[i]);
-        }
-        newp.assign(page_ids, page_ids + n_page_ids);
-    } else if (page_ids) {
-        if (n_page_ids != need) return fail(SEGPA_ERR_INVALID, "append_pages: need %lld page ids, got %d", (long long)need, n_page_ids);
-        for (int32_t i = 0; i < n_page_ids; ++i) {
-            if (page_ids[i] < 0 || page_ids[i] >= c->desc.num_pages) return fail(SEGPA_ERR_INVALID, "append_pages: page id %d out of range", page_ids[i]);
-            if (c->refcnt[page_ids[i]] != 0) return fail(SEGPA_ERR_INVALID, "append_pages: page %d is not free", page_ids[i]);
-        }
-        newp.assign(page_ids, page_ids + n_page_ids);
-        std::vector<int32_t> tmp(newp);
-        std::sort(tmp.begin(), tmp.end());
-        if (std::adjacent_find(tmp.begin(), tmp.end()) != tmp.end()) return fail(SEGPA_ERR_INVALID, "append_pages: duplicate page id");
-    } else {
-        if (need > c->n_free) return fail(SEGPA_ERR_OOM, "append_pages: pool exhausted (%lld pages needed, %lld free)", (long long)need, (long long)c->n_free);
-    }
-
-    // device part first (nothing is applied on error)
-    std::vector<int32_t> touched;
-    if (!attach) {
-        if (page_ids == nullptr) {
-            // peek pages without committing: pop now, push back on failure
-            for (int64_t i = 0; i < need; ++i) newp.push_back(pop_free_page(c));
-        }
-        if (cur_len % P != 0) touched.push_back(it->second.pages.back());
-        touched.insert(touched.end(), newp.begin(), newp.end());
-        DeviceGuard g(c->desc.device);
-        cudaStream_t st = (cudaStream_t)cuda_stream;
-        int* d_ids = nullptr;
-        cudaError_t e = cudaMallocAsync((void**)&d_ids, touched.size() * sizeof(int), st);
-        if (e == cudaSuccess) e = cudaMemcpyAsync(d_ids, touched.data(), touched.size() * sizeof(int), cudaMemcpyHostToDevice, st);
-        if (e == cudaSuccess)
-            e = launch_scatter_pages(c->k_pool, c->v_pool, (const uint16_t*)k_src, (const uint16_t*)v_src,
-                                     src_row_stride_elems, d_ids, (int)(cur_len % P), n_tokens,
-                                     (int)touched.size(), D, P, st);
-        if (d_ids) cudaFreeAsync(d_ids, st);
-        if (e != cudaSuccess) {
-            cudaGetLastError();
-            if (page_ids == nullptr)
-                for (auto id : newp) c->free_list.push_back(id);
-            return fail(SEGPA_ERR_CUDA, "append_pages: %s", cudaGetErrorString(e));
-        }
-    }
-    // commit
-    StreamRec& rec = c->streams[key];
-    for (auto id : newp) {
-        if (c->refcnt[id] == 0) --c->n_free;
-        ++c->refcnt[id];
-        rec.pages.push_back(id);
-    }
-    rec.kv_len = new_len;
+segpa_status_t segpa_clear_streams(segpa_cache_t* c) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "clear_streams: null cache");
+    c->streams.clear();
+    std::fill(c->refcnt.begin(), c->refcnt.end(), 0);
+    c->free_list.resize((size_t)c->desc.num_pages);
+    for (int64_t i = 0; i < c->desc.num_pages; ++i) c->free_list[(size_t)i] = (int32_t)(c->desc.num_pages - 1 - i);
+    c->n_free = c->desc.num_pages;
     return SEGPA_OK;
 }
 
@@ -534,29 +685,44 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         S->off_items = al(S->off_segs + S->segs.size() * sizeof(SegDev));
         S->off_pages = al(S->off_items + S->items.size() * sizeof(ItemDev));
         S->off_combs = al(S->off_pages + S->pages.size() * sizeof(int32_t));
-        S->blob_bytes = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
-        cudaError_t e = cudaMallocHost(&S->h_blob, S->blob_bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&S->d_blob, S->blob_bytes);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&S->d_counter, 256);
-        if (e == cudaSuccess && S->stats.workspace_bytes > 0) {
-            const size_t slots = (size_t)S->stats.workspace_bytes / ((size_t)kTileRows * tiles_per_item * (D + 2) * 4);
-            e = cudaMalloc((void**)&S->d_ws_o, slots * kTileRows * tiles_per_item * D * 4);
-            if (e == cudaSuccess) e = cudaMalloc((void**)&S->d_ws_ml, slots * kTileRows * tiles_per_item * 2 * 4);
+        const size_t blob_bytes = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
+        // device storage: recycled from the cache's free list (no cudaMalloc / cudaMallocHost in steady state)
+        SegBuf* B = nullptr;
+        if (!c->free_bufs.empty()) {
+            B = c->free_bufs.back();
+            c->free_bufs.pop_back();
+        } else {
+            B = new (std::nothrow) SegBuf();
+            if (!B) { delete S; return fail(SEGPA_ERR_OOM, "build_segments: host allocation failed"); }
+        }
+        S->buf = B;
+        S->last_stream = st;
+        cudaError_t e = staging_acquire(B->blob, blob_bytes);
+        if (e == cudaSuccess && !B->counter) e = cudaMalloc((void**)&B->counter, 256);
+        const size_t ws_rows = (size_t)S->stats.workspace_bytes / ((size_t)(D + 2) * 4);
+        if (e == cudaSuccess && ws_rows > B->ws_rows) {
+            if (B->ws_o) cudaFree(B->ws_o);
+            if (B->ws_ml) cudaFree(B->ws_ml);
+            B->ws_o = B->ws_ml = nullptr;
+            B->ws_rows = 0;
+            e = cudaMalloc((void**)&B->ws_o, ws_rows * D * 4);
+            if (e == cudaSuccess) e = cudaMalloc((void**)&B->ws_ml, ws_rows * 2 * 4);
+            if (e == cudaSuccess) B->ws_rows = ws_rows;
         }
         if (e != cudaSuccess) {
             cudaGetLastError();
-            free_segments_obj(S);
+            free_segments_obj(c, S);
             return fail(e == cudaErrorMemoryAllocation ? SEGPA_ERR_OOM : SEGPA_ERR_CUDA, "build_segments: %s", cudaGetErrorString(e));
         }
-        uint8_t* hb = (uint8_t*)S->h_blob;
+        uint8_t* hb = (uint8_t*)B->blob.h;
         memcpy(hb + S->off_segs, S->segs.data(), S->segs.size() * sizeof(SegDev));
         memcpy(hb + S->off_items, S->items.data(), S->items.size() * sizeof(ItemDev));
         memcpy(hb + S->off_pages, S->pages.data(), S->pages.size() * sizeof(int32_t));
         if (!S->combs.empty()) memcpy(hb + S->off_combs, S->combs.data(), S->combs.size() * sizeof(CombDev));
-        e = cudaMemcpyAsync(S->d_blob, S->h_blob, S->blob_bytes, cudaMemcpyHostToDevice, st);
+        e = cudaMemcpyAsync(B->blob.d, B->blob.h, blob_bytes, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) {
             cudaGetLastError();
-            free_segments_obj(S);
+            free_segments_obj(c, S);
             return fail(SEGPA_ERR_CUDA, "build_segments: upload failed: %s", cudaGetErrorString(e));
         }
     }
@@ -571,8 +737,7 @@ segpa_status_t segpa_free_segments(segpa_cache_t* c, segpa_segments_t* s) {
     if (it == c->seg_objs.end()) return fail(SEGPA_ERR_STATE, "free_segments: not owned by this cache");
     c->seg_objs.erase(it);
     DeviceGuard g(c->desc.device);
-    if (!c->planning_only) cudaDeviceSynchronize();  // the upload / a running fwd may still use it
-    free_segments_obj(s);
+    free_segments_obj(c, s);
     return SEGPA_OK;
 }
 
@@ -624,20 +789,22 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     if (e != cudaSuccess) return fail(SEGPA_ERR_CUDA, "attention_fwd: earlier asynchronous failure: %s", cudaGetErrorString(e));
 
     FwdParams p{};
-    p.segs = (const SegDev*)(s->d_blob + s->off_segs);
-    p.items = (const ItemDev*)(s->d_blob + s->off_items);
-    p.pages = (const int*)(s->d_blob + s->off_pages);
-    p.combs = (const CombDev*)(s->d_blob + s->off_combs);
+    const uint8_t* d_blob = (const uint8_t*)s->buf->blob.d;
+    s->last_stream = st;
+    p.segs = (const SegDev*)(d_blob + s->off_segs);
+    p.items = (const ItemDev*)(d_blob + s->off_items);
+    p.pages = (const int*)(d_blob + s->off_pages);
+    p.combs = (const CombDev*)(d_blob + s->off_combs);
     p.n_items = (int)s->items.size();
     p.n_combs = (int)s->combs.size();
-    p.counter = s->d_counter;
+    p.counter = s->buf->counter;
     p.k_pool = c->k_pool;
     p.v_pool = c->v_pool;
     p.q = (const uint16_t*)q;
     p.out = (uint16_t*)out;
     p.lse = lse;
-    p.ws_o = s->d_ws_o;
-    p.ws_ml = s->d_ws_ml;
+    p.ws_o = s->buf->ws_o;
+    p.ws_ml = s->buf->ws_ml;
     p.q_row_stride = q_row_stride;
     p.out_row_stride = out_row_stride;
     p.lse_stride = lse_stride;
@@ -656,7 +823,7 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
         if (why) return fail(SEGPA_ERR_CUDA, "attention_fwd: %s", why);
     }
 
-    e = cudaMemsetAsync(s->d_counter, 0, 256, st);
+    if (c->kernel_kind == 0) e = cudaMemsetAsync(s->buf->counter, 0, 256, st);   // only the SIMT kernel pulls from a cursor
     int launches = 0;
     if (e == cudaSuccess) {
         e = (c->kernel_kind == 0) ? launch_attention_simt(p, st) : launch_attention_tc(p, st);

@@ -93,11 +93,21 @@ struct FwdParams {
     int num_sms;
 };
 
+// one COPY-mode append of a batch (a1): rows [n_tokens][D] -> the page images listed at page_off
+struct ScatterJob {
+    const uint16_t* k_src;
+    const uint16_t* v_src;
+    long long src_stride;        // elements
+    long long n_tokens;
+    long long chunk_begin;       // first 16-byte chunk of this job in the batch-wide chunk index
+    long long page_off;          // index of this job's first touched page id in the batch's id array
+    int first_slot;              // slot of the first new token inside the first touched page
+    int n_pages;                 // touched pages (the partial last page of the stream + new pages)
+};
+
 // kernel launchers (each returns the CUDA error of its launch)
-cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const uint16_t* k_src,
-                                 const uint16_t* v_src, long long src_stride, const int* page_ids_dev,
-                                 int first_slot, long long n_tokens, int n_pages, int D, int P,
-                                 cudaStream_t st);
+cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const ScatterJob* jobs_dev, int n_jobs,
+                                 const int* page_ids_dev, long long total_chunks, int D, int P, cudaStream_t st);
 cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st);
 cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st);
 cudaError_t launch_combine(const FwdParams& p, cudaStream_t st);

@@ -8,41 +8,47 @@ namespace segpa {
 
 // ---------------------------------------------------------------------------------------------
 // a1: write K/V rows into the per-head page images.
-// One thread per (slot, 16-byte chunk); slots past the last new token of the last page are zeroed.
+// One launch serves a whole batch of streams: one thread per (slot, 16-byte chunk); the job a chunk
+// belongs to is found by binary search over the jobs' chunk prefix.  Slots past the last new token of
+// a job's last page are zeroed (masked probabilities multiply them, so they must stay finite).
 // ---------------------------------------------------------------------------------------------
 __global__ void scatter_pages_kernel(uint8_t* __restrict__ k_pool, uint8_t* __restrict__ v_pool,
-                                     const uint16_t* __restrict__ k_src, const uint16_t* __restrict__ v_src,
-                                     long long src_stride, const int* __restrict__ page_ids,
-                                     int first_slot, long long n_tokens, int n_pages, int D, int P) {
+                                     const ScatterJob* __restrict__ jobs, int n_jobs,
+                                     const int* __restrict__ page_ids, long long total_chunks, int D, int P) {
     const int cpr = D >> 3;  // 16-byte chunks per row
-    const long long total_slots = (long long)n_pages * P - first_slot;
-    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (idx >= total_slots * cpr) return;
-    const long long n = idx / cpr;
-    const int c = (int)(idx % cpr);
-    const long long gs = first_slot + n;
-    const int page = page_ids[gs / P];
-    const int slot = (int)(gs % P);
-    const size_t dst = (size_t)page * ((size_t)P * D * 2) + page_elem_offset_bytes(D, slot, c * 8);
-    uint4 kv = make_uint4(0, 0, 0, 0), vv = make_uint4(0, 0, 0, 0);
-    if (n < n_tokens) {
-        kv = *reinterpret_cast<const uint4*>(k_src + n * src_stride + c * 8);
-        vv = *reinterpret_cast<const uint4*>(v_src + n * src_stride + c * 8);
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total_chunks;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int lo = 0, hi = n_jobs - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (jobs[mid].chunk_begin <= idx) lo = mid; else hi = mid - 1;
+        }
+        const ScatterJob jb = jobs[lo];
+        const long long local = idx - jb.chunk_begin;
+        const long long n = local / cpr;
+        const int c = (int)(local % cpr);
+        const long long gs = jb.first_slot + n;
+        const int page = page_ids[jb.page_off + gs / P];
+        const int slot = (int)(gs % P);
+        const size_t dst = (size_t)page * ((size_t)P * D * 2) + page_elem_offset_bytes(D, slot, c * 8);
+        uint4 kv = make_uint4(0, 0, 0, 0), vv = make_uint4(0, 0, 0, 0);
+        if (n < jb.n_tokens) {
+            kv = *reinterpret_cast<const uint4*>(jb.k_src + n * jb.src_stride + c * 8);
+            vv = *reinterpret_cast<const uint4*>(jb.v_src + n * jb.src_stride + c * 8);
+        }
+        *reinterpret_cast<uint4*>(k_pool + dst) = kv;
+        *reinterpret_cast<uint4*>(v_pool + dst) = vv;
     }
-    *reinterpret_cast<uint4*>(k_pool + dst) = kv;
-    *reinterpret_cast<uint4*>(v_pool + dst) = vv;
 }
 
-cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const uint16_t* k_src,
-                                 const uint16_t* v_src, long long src_stride, const int* page_ids_dev,
-                                 int first_slot, long long n_tokens, int n_pages, int D, int P,
-                                 cudaStream_t st) {
-    const long long total = ((long long)n_pages * P - first_slot) * (D >> 3);
-    if (total <= 0) return cudaSuccess;
+cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const ScatterJob* jobs_dev, int n_jobs,
+                                 const int* page_ids_dev, long long total_chunks, int D, int P, cudaStream_t st) {
+    if (total_chunks <= 0 || n_jobs <= 0) return cudaSuccess;
     const int threads = 256;
-    const long long blocks = (total + threads - 1) / threads;
-    scatter_pages_kernel<<<(unsigned)blocks, threads, 0, st>>>(k_pool, v_pool, k_src, v_src, src_stride,
-                                                               page_ids_dev, first_slot, n_tokens, n_pages, D, P);
+    long long blocks = (total_chunks + threads - 1) / threads;
+    if (blocks > 148 * 64) blocks = 148 * 64;   // grid-stride beyond 64 CTAs per SM
+    scatter_pages_kernel<<<(unsigned)blocks, threads, 0, st>>>(k_pool, v_pool, jobs_dev, n_jobs, page_ids_dev,
+                                                               total_chunks, D, P);
     return cudaGetLastError();
 }
 

@@ -15,25 +15,38 @@ def create_cache(w: wl.Workload, device: int = 0) -> int:
                                 page_size=w.P, num_pages=w.num_pages, device=device)
 
 
-def append_workload(cache: int, w: wl.Workload, k_pool=None, v_pool=None, stream=None) -> None:
-    """Owners first (copy mode with the workload's page placement), then aliasing streams (attach the
-    shared prefix pages, copy the rest).  k_pool/v_pool: torch bf16 [num_pages][P][D] on the cache's
-    device, or None for a planning-only cache (attach everything)."""
+def append_requests(w: wl.Workload, k_pool=None, v_pool=None) -> List[tuple]:
+    """The workload's appends as segpa_append_pages_batch request tuples: owners first (copy mode with
+    the workload's page placement), then aliasing streams (attach the shared prefix pages, copy the rest).
+    k_pool / v_pool: torch bf16 [num_pages][P][D] on the cache's device, or None for a planning-only
+    cache (attach everything)."""
     owners = [s for s in w.streams if s.shared_from is None]
     aliased = [s for s in w.streams if s.shared_from is not None]
+    reqs = []
     for s in owners + aliased:
         if k_pool is None:
-            B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, None, None, s.kv_len, page_ids=s.page_ids)
+            reqs.append((s.layer, s.kv_head, s.seq_id, None, None, s.kv_len, s.page_ids))
             continue
         pp = s.n_shared_prefix_pages
         if pp > 0:
-            B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, None, None, pp * w.P, page_ids=s.page_ids[:pp])
+            reqs.append((s.layer, s.kv_head, s.seq_id, None, None, pp * w.P, s.page_ids[:pp]))
         n_rest = s.kv_len - pp * w.P
         if n_rest > 0:
             kr = wl.stream_rows(k_pool, s, w.P, lo_page=pp)
             vr = wl.stream_rows(v_pool, s, w.P, lo_page=pp)
-            B.segpa_append_pages(cache, s.layer, s.kv_head, s.seq_id, kr, vr, n_rest, page_ids=s.page_ids[pp:],
-                                 stream=stream)
+            reqs.append((s.layer, s.kv_head, s.seq_id, kr, vr, n_rest, s.page_ids[pp:]))
+    return reqs
+
+
+def append_workload(cache: int, w: wl.Workload, k_pool=None, v_pool=None, stream=None, batched: bool = True) -> None:
+    """Stores the whole workload: one segpa_append_pages_batch call, or (batched=False) one
+    segpa_append_pages call per request."""
+    reqs = append_requests(w, k_pool, v_pool)
+    if batched:
+        B.segpa_append_pages_batch(cache, reqs, stream=stream)
+        return
+    for (layer, kvh, seq, kr, vr, n, ids) in reqs:
+        B.segpa_append_pages(cache, layer, kvh, seq, kr, vr, n, page_ids=ids, stream=stream)
 
 
 def segment_reqs(w: wl.Workload, layer: int) -> List[tuple]:

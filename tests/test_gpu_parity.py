@@ -148,6 +148,40 @@ def test_poison_outside_visible_pages():
         g2.close()
 
 
+def test_batched_append_matches_per_stream_append():
+    """segpa_append_pages_batch (one scatter launch) and one segpa_append_pages per stream fill the pool
+    identically: attention over either is bit-identical; also exercises appending in two pieces
+    (partial last page refilled) and segment-buffer recycling without device synchronisation."""
+    reqs = [{"kv_len": 1000 + 37 * r, "heads": {0: (GLOBAL, 0, 0, 200), 1: (LOCAL, 300, 0, 64)}} for r in range(5)]
+    w = wl.make_workload("batch", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=11)
+    dev = torch.device("cuda:0")
+    k, v = wl.pool_values(w, dev)
+    q = wl.q_values(w, 0, dev)
+    outs = []
+    for mode in ("batched", "single", "pieces"):
+        cache = H.create_cache(w, 0)
+        if mode == "pieces":
+            ar = H.append_requests(w, k, v)
+            first = [(l, h, s_, kr[:333], vr[:333], 333, ids[:21]) for (l, h, s_, kr, vr, n, ids) in ar]
+            rest = [(l, h, s_, kr[333:], vr[333:], n - 333, ids[21:]) for (l, h, s_, kr, vr, n, ids) in ar]
+            B.segpa_append_pages_batch(cache, first)
+            B.segpa_append_pages_batch(cache, rest)
+        else:
+            H.append_workload(cache, w, k, v, batched=(mode == "batched"))
+        for rep in range(3):          # rebuild + free: buffers are recycled through the cache's free list
+            segs = H.build_layer(cache, w, 0)
+            out = torch.full_like(q, OUT_SENTINEL)
+            lse = torch.full((w.Hq, w.T[0]), LSE_SENTINEL, dtype=torch.float32, device=dev)
+            B.segpa_attention_fwd(cache, segs, q, w.scale, out, lse)
+            B.segpa_free_segments(cache, segs)
+        torch.cuda.synchronize()
+        outs.append((out, lse))
+        B.segpa_destroy(cache)
+    for o, l in outs[1:]:
+        assert torch.equal(o, outs[0][0]) and torch.equal(l, outs[0][1])
+    print(compare(w, 0, k, v, q, outs[0][0], outs[0][1], label="batched append"))
+
+
 def test_host_buffer_entry_point_matches_device_path():
     w = wl.config1()
     g = GpuRun(w, "tc", 2)

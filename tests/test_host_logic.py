@@ -88,6 +88,32 @@ def test_pool_bookkeeping_attach_and_refcounts():
     B.segpa_destroy(c)
 
 
+def test_batched_append_is_ordered_and_all_or_nothing():
+    c = plan_cache(num_pages=64)
+    # a later request of the batch aliases pages an earlier one introduces, and a stream is extended twice
+    B.segpa_append_pages_batch(c, [(0, 0, 1, None, None, 32, [5, 9]),
+                                   (0, 0, 2, None, None, 32, [5, 9]),
+                                   (0, 0, 2, None, None, 16, [7]),
+                                   (0, 1, 1, None, None, 48, [1, 2, 3])])
+    assert B.segpa_stream_info(c, 0, 0, 2)[0] == 48 and list(B.segpa_stream_info(c, 0, 0, 2)[1]) == [5, 9, 7]
+    assert B.segpa_pool_stats(c) == (6, 58)
+    # the third request is invalid (page id out of range): nothing of the batch may stick
+    with pytest.raises(B.SegpaError) as e:
+        B.segpa_append_pages_batch(c, [(0, 0, 3, None, None, 16, [20]),
+                                       (0, 0, 1, None, None, 16, [21]),
+                                       (0, 0, 4, None, None, 16, [64])])
+    assert e.value.status == B.ERR_INVALID and "[2]" in str(e.value)
+    assert B.segpa_pool_stats(c) == (6, 58)
+    assert B.segpa_stream_info(c, 0, 0, 1)[0] == 32
+    with pytest.raises(B.SegpaError):
+        B.segpa_stream_info(c, 0, 0, 3)
+    B.segpa_clear_streams(c)
+    assert B.segpa_pool_stats(c) == (0, 64)
+    with pytest.raises(B.SegpaError):
+        B.segpa_stream_info(c, 0, 0, 1)
+    B.segpa_destroy(c)
+
+
 def _expected_pages(kv_len, q_len, cls, W, P, page_ids, zero):
     """Independent restatement of Alg. 2 lines 6-12 for one segment."""
     vis_lo = 0 if cls == GLOBAL else max(0, kv_len - q_len - W + 1)
