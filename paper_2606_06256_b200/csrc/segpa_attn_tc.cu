@@ -1,15 +1,21 @@
 // Fused variable-length attention over per-head page lists (Alg. 2 line 15) for
-// sm_100a: cp.async.bulk (TMA) page gather -> shared memory, tcgen05.mma with TMEM accumulators
-// for S = Q K^T and O += P V, fp32 online softmax, bf16 output + fp32 LSE.  See DESIGN.md.
+// sm_100a: cp.async.bulk (TMA) page gather -> shared memory, TMA tensor-map loads of Q, tcgen05.mma
+// with TMEM accumulators for S = Q K^T and O += P V, fp32 online softmax, bf16 output + fp32 LSE.
+// See DESIGN.md section 5.2.
 //
-// One persistent CTA per SM, warp-specialised:
-//   warp 0        loader: one bulk copy per physical page into a ring of K/V stages
-//   warp 1        MMA issuer (one elected thread)
-//   warps 2, 3    Q loaders (cp.async into the swizzled Q image of tile 0 / tile 1), running one
-//                 item ahead: a Q buffer is refilled as soon as its last QK^T has completed
-//   warps 4..7    softmax / correction / epilogue warpgroup of tile 0 (thread = query row)
-//   warps 8..11   the same for tile 1 (NT = 2: two 128-row tiles of adjacent tokens share every
-//                 K/V stage and ping-pong on the tensor pipe)
+// One persistent CTA per SM, 16 warps, warp-specialised:
+//   warp 0        K/V loader: one bulk copy per physical page into a ring of K/V stages
+//   warp 1        MMA issuer (whole warp walks the schedule, one elected lane issues)
+//   warp 2        Q loader: two TMA boxes per 128-row tile, next item's Q prefetched into L2
+//   warp 3        TMEM allocation, otherwise idle
+//   warps 4..7    softmax warpgroup of tile 0 (thread = query row)
+//   warps 8..11   softmax warpgroup of tile 1 (NT = 2: two 128-row tiles of adjacent tokens share
+//                 every K/V stage and ping-pong on the tensor pipe)
+//   warps 12..15  epilogue warpgroup: O / l -> bf16, LSE, split-KV partials, for both tiles
+// The MMA schedule is one continuous sequence of steps across work items: step (item, block j) issues
+// for each tile PV of the PREVIOUS step's block (possibly the last block of the previous item) and
+// QK^T of block j, so the tensor pipe does not drain at item boundaries; the epilogue of item i runs
+// beside the first blocks of item i+1.
 // A tile row r is (token t0 + r / G, query head kv_head*G + r % G): the G heads of a KV head share
 // each K/V page load (GQA packing).
 //
@@ -28,14 +34,32 @@ namespace {
 
 constexpr int kLoaderWarp = 0;
 constexpr int kMmaWarp = 1;
+constexpr int kQWarp = 2;
 constexpr int kFirstSoftmaxWarp = 4;
-constexpr int kRegsLow = 64;     // warps 0..3 (loader, MMA issuer, Q loaders)
-constexpr int kRegsHigh = 216;   // softmax warps: 128 * 64 + 256 * 216 = 63488 <= 65536
+constexpr int kFirstEpilogueWarp = 12;
+constexpr int kThreads = 512;
+// register budgets (setmaxnreg): 128 * 48 + 256 * 200 + 128 * 64 = 65536
+constexpr int kRegsLow = 48;
+constexpr int kRegsSoftmax = 200;
+constexpr int kRegsEpilogue = 64;
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: O is rescaled only when the max grows by > 2^8
+
+// Pipeline trace (debug builds with -DSEGPA_TRACE only): lane 0 of every warp of CTA 0 logs
+// (tag, arg, SM clock) records that _work scripts turn into a timeline.
+#ifdef SEGPA_TRACE
+#define TRACE(tag, arg)                                                                                          \
+    do {                                                                                                         \
+        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && trace_n < kTraceCap)                                   \
+            p.trace[(threadIdx.x >> 5) * kTraceCap + trace_n++] =                                                \
+                ((unsigned long long)(tag) << 56) | ((unsigned long long)((arg) & 0xffff) << 40) |               \
+                ((unsigned long long)clock64() & 0xffffffffffull);                                               \
+    } while (0)
+#else
+#define TRACE(tag, arg) do { } while (0)
+#endif
 
 template <int D, int NT>
 struct Cfg {
-    static constexpr int kThreads = 128 + 128 * NT;
     static constexpr int kTileBytes = kTileRows * D * 2;      // Q tile, K block or V block
     static constexpr int kStages = (D == 128) ? 4 : 8;   // > 114 KB of smem either way: one CTA per SM (it owns all of TMEM)
     static constexpr int kSmemQ = NT * kTileBytes;
@@ -52,7 +76,10 @@ struct Bars {
     uint64_t q_empty[2];
     uint64_t s_full[2];
     uint64_t p_full[2];
-    uint64_t o_final[2];
+    uint64_t o_final[2];    // MMA -> epilogue: last PV of the item's tile has completed
+    uint64_t o_free[2];     // epilogue -> MMA: O_t has been read out, the next item may overwrite it
+    uint64_t stat_full[2];  // softmax -> epilogue: (m, l) of the finished tile are in smem
+    uint64_t stat_free[2];  // epilogue -> softmax
     uint32_t tmem_base;
 };
 
@@ -84,10 +111,11 @@ __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev&
 }  // namespace
 
 template <int D, int NT>
-__global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(const __grid_constant__ FwdParams p) {
+__global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_constant__ FwdParams p) {
     using C = Cfg<D, NT>;
     extern __shared__ uint8_t smem_raw[];
     __shared__ Bars bars;
+    __shared__ float2 stats[2][kTileRows];   // (m in log2 units, l) of a finished tile, softmax -> epilogue
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
     const uint32_t sQ = smem_u32(smem);
     const uint32_t sKV = sQ + C::kSmemQ;
@@ -95,6 +123,9 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
     const int cta = blockIdx.x, n_cta = gridDim.x;
     const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
     const int rows_per_slot = kTileRows * p.tiles_per_item;
+#ifdef SEGPA_TRACE
+    int trace_n = 0;
+#endif
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < C::kStages; ++s) {
@@ -107,10 +138,13 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
             mbar_init(smem_u32(&bars.s_full[t]), 1);
             mbar_init(smem_u32(&bars.p_full[t]), 128);
             mbar_init(smem_u32(&bars.o_final[t]), 1);
+            mbar_init(smem_u32(&bars.o_free[t]), 128);
+            mbar_init(smem_u32(&bars.stat_full[t]), 128);
+            mbar_init(smem_u32(&bars.stat_free[t]), 128);
         }
         fence_mbar_init();
     }
-    if (warp == 2) {
+    if (warp == 3) {
         tmem_alloc(smem_u32(&bars.tmem_base), 512);
         tmem_relinquish();
     }
@@ -118,11 +152,9 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = bars.tmem_base;
-    // register budget (setmaxnreg inside each role branch so ptxas sees the limit per role): the softmax
-    // warpgroups hold a whole 128-column score row per thread; warps 0-3 give registers up
 
     if (warp == kLoaderWarp) {
-        // ------------------------------------------------------------------ loader
+        // ------------------------------------------------------------------ K/V loader
         reg_dec<kRegsLow>();
         uint32_t fill = 0;  // stage fills so far
         for (int k = 0;; ++k) {
@@ -141,10 +173,12 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                 if (lane < ppb) page = p.pages[sg.page_off + (long long)(j * ppb - sg.first_page) + lane];
                 for (int kv = 0; kv < 2; ++kv) {
                     const uint32_t st = fill % C::kStages, ph = (fill / C::kStages) & 1;
+                    TRACE(1, j * 2 + kv);
                     if (lane == 0) {
                         mbar_wait(smem_u32(&bars.kv_empty[st]), ph ^ 1);
                         mbar_arrive_expect_tx(smem_u32(&bars.kv_full[st]), C::kTileBytes);
                     }
+                    TRACE(2, j * 2 + kv);
                     __syncwarp();
                     if (lane < ppb) {
                         const uint8_t* src = (kv == 0 ? p.k_pool : p.v_pool) + (size_t)page * p.page_bytes;
@@ -166,14 +200,89 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
         const uint64_t dk0 = make_desc_sw128(sKV, 16, C::kSBO);
         const uint64_t dv0 = make_desc_sw128(sKV, kAtomBytes, C::kSBO);
         uint32_t rd = 0;                       // stage reads so far
-        uint32_t n_q[2] = {0, 0}, n_p[2] = {0, 0};
+        uint32_t n_q[2] = {0, 0}, n_p[2] = {0, 0}, n_of[2] = {0, 0};
+        // the block whose PV is still to be issued, per tile (it may belong to the previous item)
+        bool pv_valid[2] = {false, false}, pv_first[2] = {false, false}, pv_last[2] = {false, false};
+        TileRange tr[2];
+        tr[1].n_rows = 0; tr[1].lo = tr[1].hi = 0; tr[1].tok0 = 0;
+
+        // One step of the continuous schedule: per tile, PV of the pending block, then QK^T of block j.
+        // Ring order is K(j), V(j); V of the pending block was filled before K(j).
+        auto step = [&](const bool have_k, const int j) {
+            const bool have_v = pv_valid[0] || pv_valid[1];
+            uint32_t st_v = 0, st_k = 0;
+            TRACE(10, j);
+            if (have_v) {
+                st_v = rd % C::kStages;
+                mbar_wait(smem_u32(&bars.kv_full[st_v]), (rd / C::kStages) & 1);
+                ++rd;
+            }
+            if (have_k) {
+                st_k = rd % C::kStages;
+                mbar_wait(smem_u32(&bars.kv_full[st_k]), (rd / C::kStages) & 1);
+                ++rd;
+            }
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+                const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
+                const bool do_pv = pv_valid[t];
+                const bool do_qk = have_k && tr[t].n_rows > 0 && j >= tr[t].lo && j < tr[t].hi;
+                TRACE(11 + t * 4, j);
+                if (do_pv) {
+                    mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
+                    ++n_p[t];
+                    if (pv_first[t]) {   // first PV of an item overwrites O_t: the epilogue must have read it out
+                        mbar_wait(smem_u32(&bars.o_free[t]), (n_of[t] & 1) ^ 1);
+                        ++n_of[t];
+                    }
+                }
+                if (do_qk && j == tr[t].lo) {
+                    mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
+                    ++n_q[t];
+                }
+                tc_fence_after();
+                TRACE(12 + t * 4, j);
+                if (elect_one()) {
+                    if (do_pv) {
+                        const uint64_t dv = dv0 + (uint64_t)((st_v * C::kTileBytes) >> 4);
+                        const uint32_t acc0 = pv_first[t] ? 0u : 1u;
+#pragma unroll
+                        for (int kk = 0; kk < kBlockKeys / 16; ++kk)
+                            mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
+                        if (pv_last[t]) tc_commit(smem_u32(&bars.o_final[t]));
+                    }
+                    if (do_qk) {
+                        const uint64_t dq = dq0 + (uint64_t)((t * C::kTileBytes) >> 4);
+                        const uint64_t dk = dk0 + (uint64_t)((st_k * C::kTileBytes) >> 4);
+#pragma unroll
+                        for (int kk = 0; kk < D / 16; ++kk) {
+                            const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
+                            const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                            mma_ss(tS, dq + oq, dk + ok, idesc_qk, kk > 0 ? 1u : 0u);
+                        }
+                        tc_commit(smem_u32(&bars.s_full[t]));
+                        if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
+                    }
+                }
+                __syncwarp();
+                TRACE(13 + t * 4, j);
+                pv_valid[t] = do_qk;
+                pv_first[t] = do_qk && j == tr[t].lo;
+                pv_last[t] = do_qk && j + 1 == tr[t].hi;
+            }
+            if (elect_one()) {
+                if (have_v) tc_commit(smem_u32(&bars.kv_empty[st_v]));
+                if (have_k) tc_commit(smem_u32(&bars.kv_empty[st_k]));
+            }
+            __syncwarp();
+        };
+
         for (int k = 0;; ++k) {
             const int ii = item_for(k, cta, n_cta);
             if (k * n_cta >= p.n_items) break;
             if (ii >= p.n_items) continue;
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
-            TileRange tr[2];
             int jlo = INT_MAX, jhi = 0;
 #pragma unroll
             for (int t = 0; t < NT; ++t) {
@@ -189,80 +298,71 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                     if (elect_one()) tc_commit(smem_u32(&bars.q_empty[t]));
                     __syncwarp();
                 }
-            // step j: for each tile, PV(j-1) then QK(j).  K(j) and V(j-1) are the stages in use.
-            uint32_t st_v = 0;
-            for (int j = jlo; j <= jhi; ++j) {
-                const bool have_k = j < jhi, have_v = j > jlo;
-                uint32_t st_k = 0;
-                if (have_v) {
-                    st_v = rd % C::kStages;
-                    mbar_wait(smem_u32(&bars.kv_full[st_v]), (rd / C::kStages) & 1);
-                    ++rd;
-                }
-                if (have_k) {
-                    st_k = rd % C::kStages;
-                    mbar_wait(smem_u32(&bars.kv_full[st_k]), (rd / C::kStages) & 1);
-                    ++rd;
-                }
-#pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                    if (tr[t].n_rows == 0) continue;
-                    const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
-                    const bool do_pv = have_v && j - 1 >= tr[t].lo && j - 1 < tr[t].hi;
-                    const bool do_qk = have_k && j >= tr[t].lo && j < tr[t].hi;
-                    if (do_pv) {
-                        mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
-                        ++n_p[t];
-                    }
-                    if (do_qk && j == tr[t].lo) {
-                        mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
-                        ++n_q[t];
-                    }
-                    tc_fence_after();
-                    if (elect_one()) {
-                        if (do_pv) {
-                            const uint64_t dv = dv0 + (uint64_t)((st_v * C::kTileBytes) >> 4);
-                            const uint32_t acc0 = (j - 1 > tr[t].lo) ? 1u : 0u;
-#pragma unroll
-                            for (int kk = 0; kk < kBlockKeys / 16; ++kk)
-                                mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
-                            if (j == tr[t].hi) tc_commit(smem_u32(&bars.o_final[t]));
-                        }
-                        if (do_qk) {
-                            const uint64_t dq = dq0 + (uint64_t)((t * C::kTileBytes) >> 4);
-                            const uint64_t dk = dk0 + (uint64_t)((st_k * C::kTileBytes) >> 4);
-#pragma unroll
-                            for (int kk = 0; kk < D / 16; ++kk) {
-                                const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
-                                const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
-                                mma_ss(tS, dq + oq, dk + ok, idesc_qk, kk > 0 ? 1u : 0u);
-                            }
-                            tc_commit(smem_u32(&bars.s_full[t]));
-                            if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
-                        }
-                    }
-                    __syncwarp();
-                }
-                if (elect_one()) {
-                    if (have_v) tc_commit(smem_u32(&bars.kv_empty[st_v]));
-                    if (have_k) tc_commit(smem_u32(&bars.kv_empty[st_k]));
-                }
-                __syncwarp();
-                // stage order in the ring is K(j), V(j): V(j-1) was read before K(j)
-            }
+            for (int j = jlo; j < jhi; ++j) step(true, j);
         }
-    } else if (warp == 2 || warp == 3) {
-        // ------------------------------------------------------------------ Q loaders (TMA)
+        step(false, 0);   // PV of the very last block
+    } else if (warp == kQWarp) {
+        // ------------------------------------------------------------------ Q loader (TMA)
         // Q tile image: [D/64 halves][128 rows][128 B], SWIZZLE_128B; row r = (token, group head) as the
         // TMA box {64 elements, G heads, tile_tokens tokens} lays it out.  Rows >= G*tile_tokens are never
         // written (their scores are garbage and never stored); tokens past T are zero-filled by TMA.
         reg_dec<kRegsLow>();
-        const int tile = warp - 2;
+        const uint32_t box_bytes = (uint32_t)(64 * 2 * G * TT);
+        uint32_t n_fill[2] = {0, 0};
+        if (lane == 0) prefetch_tmap(&p.q_map);
+        for (int k = 0;; ++k) {
+            const int ii = item_for(k, cta, n_cta);
+            if (k * n_cta >= p.n_items) break;
+            if (ii >= p.n_items) continue;
+            const ItemDev it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            // pull the next item's Q tiles towards L2 while this one is computed
+            const int in = item_for(k + 1, cta, n_cta);
+            if ((k + 1) * n_cta < p.n_items && in < p.n_items && elect_one()) {
+                const ItemDev itn = p.items[in];
+                const SegDev sgn = p.segs[itn.seg];
+#pragma unroll
+                for (int t = 0; t < NT; ++t) {
+                    const TileRange trn = tile_range(itn, sgn, t, TT, G);
+                    if (trn.n_rows == 0) continue;
+#pragma unroll
+                    for (int h = 0; h < C::kHalves; ++h)
+                        tma_prefetch_3d(&p.q_map, h * 64, sgn.kv_head * G, (int)(sgn.q_row_start + trn.tok0));
+                }
+            }
+            __syncwarp();
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+                const TileRange tr = tile_range(it, sg, t, TT, G);
+                if (tr.n_rows == 0) continue;
+                TRACE(40, t);
+                mbar_wait(smem_u32(&bars.q_empty[t]), (n_fill[t] & 1) ^ 1);   // last QK^T on the old Q is done
+                ++n_fill[t];
+                TRACE(41, t);
+                if (elect_one()) {
+                    mbar_arrive_expect_tx(smem_u32(&bars.q_full[t]), box_bytes * C::kHalves);
+#pragma unroll
+                    for (int h = 0; h < C::kHalves; ++h)
+                        tma_load_3d(sQ + t * C::kTileBytes + h * (kTileRows * 128), &p.q_map, h * 64, sg.kv_head * G,
+                                    (int)(sg.q_row_start + tr.tok0), smem_u32(&bars.q_full[t]));
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp == 3) {
+        reg_dec<kRegsLow>();
+    } else if (warp < kFirstEpilogueWarp) {
+        // ------------------------------------------------------------------ softmax warpgroups
+        reg_inc<kRegsSoftmax>();
+        const int tile = (warp - kFirstSoftmaxWarp) >> 2;
         if (tile < NT) {
-            const uint32_t qb = sQ + tile * C::kTileBytes;
-            const uint32_t box_bytes = (uint32_t)(64 * 2 * G * TT);
-            uint32_t n_fill = 0;
-            if (lane == 0) prefetch_tmap(&p.q_map);
+            const int wq = warp & 3;                       // TMEM lane quadrant this warp may access
+            const int r = wq * 32 + lane;                  // row inside the tile
+            const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
+            const uint32_t tS = tmem + lane_base + tile * 128;
+            const uint32_t tO = tmem + lane_base + 256 + tile * 128;
+            const float sl2 = p.scale * 1.4426950408889634f;
+            uint32_t n_s = 0, n_st = 0;
             for (int k = 0;; ++k) {
                 const int ii = item_for(k, cta, n_cta);
                 if (k * n_cta >= p.n_items) break;
@@ -271,173 +371,188 @@ __global__ void __launch_bounds__(Cfg<D, NT>::kThreads, 1) attention_tc_kernel(c
                 const SegDev sg = p.segs[it.seg];
                 const TileRange tr = tile_range(it, sg, tile, TT, G);
                 if (tr.n_rows == 0) continue;
-                mbar_wait(smem_u32(&bars.q_empty[tile]), (n_fill & 1) ^ 1);   // last QK^T on the old Q is done
-                ++n_fill;
-                if (elect_one()) {
-                    mbar_arrive_expect_tx(smem_u32(&bars.q_full[tile]), box_bytes * C::kHalves);
+
+                const int rc = min(r, tr.n_rows - 1);            // rows past the end mirror the last valid row
+                const int tok = tr.tok0 + rc / G;
+                const int pos = sg.kv_len - sg.q_len + tok;      // query position i
+                const int key_lo = max(0, pos - sg.window + 1);  // visible keys [key_lo, pos]
+                const bool warp_has_rows = wq * 32 < tr.n_rows;  // decode-shaped tiles: most warps hold no row
+                float m_used = -INFINITY, l = 0.f;
+
+                for (int j = tr.lo; j < tr.hi; ++j) {
+                    TRACE(20, j);
+                    mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
+                    ++n_s;
+                    tc_fence_after();
+                    TRACE(21, j);
+                    if (warp_has_rows) {
+                        const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;   // valid columns [cmin, cmax]
+                        const bool need_mask = __any_sync(0xffffffffu, cmin > 0 || cmax < kBlockKeys - 1);
+                        // the whole score row of this thread: 128 fp32 columns -> registers, one wait
+                        uint32_t s[kBlockKeys];
 #pragma unroll
-                    for (int h = 0; h < C::kHalves; ++h)
-                        tma_load_3d(qb + h * (kTileRows * 128), &p.q_map, h * 64, sg.kv_head * G, (int)(sg.q_row_start + tr.tok0),
-                                    smem_u32(&bars.q_full[tile]));
+                        for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, s + c * 32);
+                        tmem_wait_ld();
+                        TRACE(22, j);
+                        if (need_mask) {
+                            // boundary block (causal diagonal / window edge): element mask in registers
+#pragma unroll
+                            for (int e = 0; e < kBlockKeys; ++e)
+                                if (e < cmin || e > cmax) s[e] = 0xff800000u;   // -inf
+                        }
+                        float mxa = -INFINITY, mxb = -INFINITY, mxc = -INFINITY, mxd = -INFINITY;
+#pragma unroll
+                        for (int e = 0; e < kBlockKeys; e += 8) {
+                            mxa = max3(mxa, __uint_as_float(s[e + 0]), __uint_as_float(s[e + 1]));
+                            mxb = max3(mxb, __uint_as_float(s[e + 2]), __uint_as_float(s[e + 3]));
+                            mxc = max3(mxc, __uint_as_float(s[e + 4]), __uint_as_float(s[e + 5]));
+                            mxd = max3(mxd, __uint_as_float(s[e + 6]), __uint_as_float(s[e + 7]));
+                        }
+                        const float mx = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
+                        const float mx2 = mx * sl2;
+                        // lazy rescale (warp-uniform decision: tcgen05.ld/st are warp-collective)
+                        const bool grow = mx2 > m_used + kRescaleThreshold;
+                        if (__any_sync(0xffffffffu, grow)) {
+                            float corr = 1.f;
+                            if (grow) {
+                                corr = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - mx2);
+                                m_used = mx2;
+                                l *= corr;
+                            }
+                            if (j > tr.lo) {
+#pragma unroll 1
+                                for (int c = 0; c < D / 16; ++c) {
+                                    uint32_t v[16];
+                                    tmem_ld16(tO + c * 16, v);
+                                    tmem_wait_ld();
+#pragma unroll
+                                    for (int e = 0; e < 16; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * corr);
+                                    tmem_st16(tO + c * 16, v);
+                                }
+                            }
+                        }
+                        TRACE(23, j);
+                        const float mref = (m_used == -INFINITY) ? 0.f : m_used;
+                        // p = 2^(s*scale*log2e - m) (masked columns: 2^-inf = 0), row sum, bf16 P -> TMEM (aliases S[0, 64))
+                        float rs0 = 0.f, rs1 = 0.f, rs2 = 0.f, rs3 = 0.f;
+#pragma unroll
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t pk[16];
+#pragma unroll
+                            for (int e = 0; e < 32; e += 4) {
+                                const float p0 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 0]), sl2, -mref));
+                                const float p1 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 1]), sl2, -mref));
+                                const float p2 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 2]), sl2, -mref));
+                                const float p3 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 3]), sl2, -mref));
+                                rs0 += p0; rs1 += p1; rs2 += p2; rs3 += p3;
+                                pk[(e >> 1) + 0] = pack_bf16x2(p0, p1);
+                                pk[(e >> 1) + 1] = pack_bf16x2(p2, p3);
+                            }
+                            tmem_st16(tS + c * 16, pk);
+                        }
+                        l += (rs0 + rs1) + (rs2 + rs3);
+                        tmem_wait_st();
+                    }
+                    tc_fence_before();
+                    mbar_arrive(smem_u32(&bars.p_full[tile]));
+                    TRACE(24, j);
                 }
-                __syncwarp();
+                // hand (m, l) to the epilogue warpgroup and go straight on to the next item
+                mbar_wait(smem_u32(&bars.stat_free[tile]), (n_st & 1) ^ 1);
+                ++n_st;
+                stats[tile][r] = make_float2(m_used, l);
+                mbar_arrive(smem_u32(&bars.stat_full[tile]));   // release: orders the store before the arrive
             }
         }
-    } else if (warp >= kFirstSoftmaxWarp) {
-        // ------------------------------------------------------------------ softmax warpgroups
-        reg_inc<kRegsHigh>();
-        const int tile = (warp - kFirstSoftmaxWarp) >> 2;
-        const int wq = warp & 3;                       // TMEM lane quadrant this warp may access
-        const int r = wq * 32 + lane;                  // row inside the tile
+    } else {
+        // ------------------------------------------------------------------ epilogue warpgroup
+        reg_dec<kRegsEpilogue>();
+        const int wq = warp & 3;
+        const int r = wq * 32 + lane;
         const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
-        const uint32_t tS = tmem + lane_base + tile * 128;
-        const uint32_t tO = tmem + lane_base + 256 + tile * 128;
-        const float sl2 = p.scale * 1.4426950408889634f;
-        uint32_t n_s = 0, n_o = 0;
+        uint32_t n_o[2] = {0, 0}, n_st[2] = {0, 0};
         for (int k = 0;; ++k) {
             const int ii = item_for(k, cta, n_cta);
             if (k * n_cta >= p.n_items) break;
             if (ii >= p.n_items) continue;
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
-            const TileRange tr = tile_range(it, sg, tile, TT, G);
-            if (tr.n_rows == 0) continue;
-
-            const int rc = min(r, tr.n_rows - 1);            // rows past the end mirror the last valid row
-            const int tok = tr.tok0 + rc / G;
-            const int pos = sg.kv_len - sg.q_len + tok;      // query position i
-            const int key_lo = max(0, pos - sg.window + 1);  // visible keys [key_lo, pos]
-            float m_used = -INFINITY, l = 0.f;
-
-            for (int j = tr.lo; j < tr.hi; ++j) {
-                mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
-                ++n_s;
-                tc_fence_after();
-                const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;   // valid columns [cmin, cmax]
-                const bool need_mask = __any_sync(0xffffffffu, cmin > 0 || cmax < kBlockKeys - 1);
-                // the whole score row of this thread: 128 fp32 columns -> registers, one wait
-                uint32_t s[kBlockKeys];
-#pragma unroll
-                for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, s + c * 32);
-                tmem_wait_ld();
-                if (need_mask) {
-                    // boundary block (causal diagonal / window edge): element mask in registers
-#pragma unroll
-                    for (int e = 0; e < kBlockKeys; ++e)
-                        if (e < cmin || e > cmax) s[e] = 0xff800000u;   // -inf
-                }
-                float mxa = -INFINITY, mxb = -INFINITY, mxc = -INFINITY, mxd = -INFINITY;
-#pragma unroll
-                for (int e = 0; e < kBlockKeys; e += 8) {
-                    mxa = max3(mxa, __uint_as_float(s[e + 0]), __uint_as_float(s[e + 1]));
-                    mxb = max3(mxb, __uint_as_float(s[e + 2]), __uint_as_float(s[e + 3]));
-                    mxc = max3(mxc, __uint_as_float(s[e + 4]), __uint_as_float(s[e + 5]));
-                    mxd = max3(mxd, __uint_as_float(s[e + 6]), __uint_as_float(s[e + 7]));
-                }
-                const float mx = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
-                const float mx2 = mx * sl2;
-                // lazy rescale (warp-uniform decision: tcgen05.ld/st are warp-collective)
-                const bool grow = mx2 > m_used + kRescaleThreshold;
-                if (__any_sync(0xffffffffu, grow)) {
-                    float corr = 1.f;
-                    if (grow) {
-                        corr = (m_used == -INFINITY) ? 0.f : fast_exp2(m_used - mx2);
-                        m_used = mx2;
-                        l *= corr;
-                    }
-                    if (j > tr.lo) {
 #pragma unroll 1
-                        for (int c = 0; c < D / 16; ++c) {
-                            uint32_t v[16];
-                            tmem_ld16(tO + c * 16, v);
-                            tmem_wait_ld();
+            for (int tile = 0; tile < NT; ++tile) {
+                const TileRange tr = tile_range(it, sg, tile, TT, G);
+                if (tr.n_rows == 0) continue;
+                const uint32_t tO = tmem + lane_base + 256 + tile * 128;
+                const bool has_blocks = tr.hi > tr.lo;
+                const int rc = min(r, tr.n_rows - 1);
+                const int tok = tr.tok0 + rc / G;
+                const bool valid = r < tr.n_rows;
+                const int head = sg.kv_head * G + rc % G;
+                const long long row = sg.q_row_start + tok;
+                TRACE(30, tile);
+                mbar_wait(smem_u32(&bars.stat_full[tile]), n_st[tile] & 1);
+                ++n_st[tile];
+                const float2 ml = stats[tile][r];
+                mbar_arrive(smem_u32(&bars.stat_free[tile]));
+                if (has_blocks) {
+                    mbar_wait(smem_u32(&bars.o_final[tile]), n_o[tile] & 1);
+                    ++n_o[tile];
+                    tc_fence_after();
+                }
+                TRACE(31, tile);
+                if (it.partial_slot >= 0) {
+                    const size_t base = (size_t)it.partial_slot * rows_per_slot + (size_t)(tr.tok0 - it.t0) * G + r;
+#pragma unroll 1
+                    for (int c = 0; c < D / 16; ++c) {
+                        uint32_t v[16];
+                        if (has_blocks) { tmem_ld16(tO + c * 16, v); tmem_wait_ld(); }
+                        else {
 #pragma unroll
-                            for (int e = 0; e < 16; ++e) v[e] = __float_as_uint(__uint_as_float(v[e]) * corr);
-                            tmem_st16(tO + c * 16, v);
+                            for (int e = 0; e < 16; ++e) v[e] = 0u;
+                        }
+                        if (valid) {
+                            float4* dst = reinterpret_cast<float4*>(p.ws_o + base * D + c * 16);
+#pragma unroll
+                            for (int e = 0; e < 4; ++e)
+                                dst[e] = make_float4(__uint_as_float(v[4 * e]), __uint_as_float(v[4 * e + 1]),
+                                                     __uint_as_float(v[4 * e + 2]), __uint_as_float(v[4 * e + 3]));
                         }
                     }
-                }
-                const float mref = (m_used == -INFINITY) ? 0.f : m_used;
-                // p = 2^(s*scale*log2e - m) (masked columns: 2^-inf = 0), row sum, bf16 P -> TMEM (aliases S[0, 64))
-                float rs0 = 0.f, rs1 = 0.f, rs2 = 0.f, rs3 = 0.f;
+                    if (valid) { p.ws_ml[base * 2] = ml.x; p.ws_ml[base * 2 + 1] = ml.y; }
+                } else {
+                    const float inv = 1.f / ml.y;
+                    uint16_t* orow = p.out + row * p.out_row_stride + (long long)head * D;
+#pragma unroll 2
+                    for (int c = 0; c < D / 16; ++c) {
+                        uint32_t v[16];
+                        tmem_ld16(tO + c * 16, v);
+                        tmem_wait_ld();
+                        if (valid) {
+                            uint4* dst = reinterpret_cast<uint4*>(orow + c * 16);
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    uint32_t pk[16];
-#pragma unroll
-                    for (int e = 0; e < 32; e += 4) {
-                        const float p0 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 0]), sl2, -mref));
-                        const float p1 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 1]), sl2, -mref));
-                        const float p2 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 2]), sl2, -mref));
-                        const float p3 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 3]), sl2, -mref));
-                        rs0 += p0; rs1 += p1; rs2 += p2; rs3 += p3;
-                        pk[(e >> 1) + 0] = pack_bf16x2(p0, p1);
-                        pk[(e >> 1) + 1] = pack_bf16x2(p2, p3);
-                    }
-                    tmem_st16(tS + c * 16, pk);
-                }
-                l += (rs0 + rs1) + (rs2 + rs3);
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(smem_u32(&bars.p_full[tile]));
-            }
-
-            // ---- epilogue
-            if (tr.hi > tr.lo) {
-                mbar_wait(smem_u32(&bars.o_final[tile]), n_o & 1);
-                ++n_o;
-                tc_fence_after();
-            }
-            const bool valid = r < tr.n_rows;
-            const int head = sg.kv_head * G + rc % G;
-            const long long row = sg.q_row_start + tok;
-            if (it.partial_slot >= 0) {
-                const size_t base = (size_t)it.partial_slot * rows_per_slot + (size_t)(tr.tok0 - it.t0) * G + r;
-#pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t v[32];
-                    if (tr.hi > tr.lo) { tmem_ld32(tO + c * 32, v); tmem_wait_ld(); }
-                    else {
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) v[e] = 0u;
-                    }
-                    if (valid) {
-                        float4* dst = reinterpret_cast<float4*>(p.ws_o + base * D + c * 32);
-#pragma unroll
-                        for (int e = 0; e < 8; ++e)
-                            dst[e] = make_float4(__uint_as_float(v[4 * e]), __uint_as_float(v[4 * e + 1]),
-                                                 __uint_as_float(v[4 * e + 2]), __uint_as_float(v[4 * e + 3]));
-                    }
-                }
-                if (valid) { p.ws_ml[base * 2] = m_used; p.ws_ml[base * 2 + 1] = l; }
-            } else {
-                const float inv = 1.f / l;
-                uint16_t* orow = p.out + row * p.out_row_stride + (long long)head * D;
-#pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t v[32];
-                    tmem_ld32(tO + c * 32, v);
-                    tmem_wait_ld();
-                    if (valid) {
-                        uint4* dst = reinterpret_cast<uint4*>(orow + c * 32);
-#pragma unroll
-                        for (int e = 0; e < 4; ++e) {
-                            uint4 o;
-                            o.x = pack_bf16x2(__uint_as_float(v[8 * e + 0]) * inv, __uint_as_float(v[8 * e + 1]) * inv);
-                            o.y = pack_bf16x2(__uint_as_float(v[8 * e + 2]) * inv, __uint_as_float(v[8 * e + 3]) * inv);
-                            o.z = pack_bf16x2(__uint_as_float(v[8 * e + 4]) * inv, __uint_as_float(v[8 * e + 5]) * inv);
-                            o.w = pack_bf16x2(__uint_as_float(v[8 * e + 6]) * inv, __uint_as_float(v[8 * e + 7]) * inv);
-                            dst[e] = o;
+                            for (int e = 0; e < 2; ++e) {
+                                uint4 o;
+                                o.x = pack_bf16x2(__uint_as_float(v[8 * e + 0]) * inv, __uint_as_float(v[8 * e + 1]) * inv);
+                                o.y = pack_bf16x2(__uint_as_float(v[8 * e + 2]) * inv, __uint_as_float(v[8 * e + 3]) * inv);
+                                o.z = pack_bf16x2(__uint_as_float(v[8 * e + 4]) * inv, __uint_as_float(v[8 * e + 5]) * inv);
+                                o.w = pack_bf16x2(__uint_as_float(v[8 * e + 6]) * inv, __uint_as_float(v[8 * e + 7]) * inv);
+                                dst[e] = o;
+                            }
                         }
                     }
+                    if (valid && p.lse) p.lse[(long long)head * p.lse_stride + row] = (ml.x + log2f(ml.y)) * 0.6931471805599453f;
                 }
-                if (valid && p.lse) p.lse[(long long)head * p.lse_stride + row] = (m_used + log2f(l)) * 0.6931471805599453f;
+                if (has_blocks) {
+                    tc_fence_before();
+                    mbar_arrive(smem_u32(&bars.o_free[tile]));   // O_t may be overwritten by the next item
+                }
+                TRACE(32, tile);
             }
         }
     }
 
     tc_fence_before();
     __syncthreads();
-    if (warp == 2) tmem_dealloc(tmem, 512);
+    if (warp == 3) tmem_dealloc(tmem, 512);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -458,7 +573,7 @@ static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
         configured = true;
     }
     const int grid = p.n_items < p.num_sms ? p.n_items : p.num_sms;
-    attention_tc_kernel<D, NT><<<grid, C::kThreads, C::kSmemBytes, st>>>(p);
+    attention_tc_kernel<D, NT><<<grid, kThreads, C::kSmemBytes, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -823,6 +823,12 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
         if (why) return fail(SEGPA_ERR_CUDA, "attention_fwd: %s", why);
     }
 
+#ifdef SEGPA_TRACE
+    static unsigned long long* d_trace = nullptr;
+    if (!d_trace) cudaMalloc((void**)&d_trace, 16 * kTraceCap * 8);
+    cudaMemsetAsync(d_trace, 0, 16 * kTraceCap * 8, st);
+    p.trace = d_trace;
+#endif
     if (c->kernel_kind == 0) e = cudaMemsetAsync(s->buf->counter, 0, 256, st);   // only the SIMT kernel pulls from a cursor
     int launches = 0;
     if (e == cudaSuccess) {
@@ -833,6 +839,14 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
         e = launch_combine(p, st);
         ++launches;
     }
+#ifdef SEGPA_TRACE
+    if (const char* tf = getenv("SEGPA_TRACE_FILE")) {
+        std::vector<unsigned long long> h(16 * kTraceCap);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(h.data(), d_trace, h.size() * 8, cudaMemcpyDeviceToHost);
+        if (FILE* f = fopen(tf, "wb")) { fwrite(h.data(), 8, h.size(), f); fclose(f); }
+    }
+#endif
     c->last_launches = launches;
     if (e != cudaSuccess) {
         cudaGetLastError();

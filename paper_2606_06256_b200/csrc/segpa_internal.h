@@ -91,7 +91,13 @@ struct FwdParams {
     int tiles_per_item;
     int page_bytes;
     int num_sms;
+#ifdef SEGPA_TRACE
+    unsigned long long* trace;   // [16 warps][kTraceCap] (tag << 56 | arg << 40 | clock) of CTA 0; debug builds only
+#endif
 };
+#ifdef SEGPA_TRACE
+constexpr int kTraceCap = 8192;
+#endif
 
 // one COPY-mode append of a batch (a1): rows [n_tokens][D] -> the page images listed at page_off
 struct ScatterJob {
