@@ -186,7 +186,8 @@ typedef struct {
  * rows are cut into tiles of floor(128 / G) tokens x G query heads (GQA packing: the G heads of a
  * KV head share every K/V page load); each tile gets exactly the KV block range it attends to,
  * so no work is issued for fully masked blocks.  Long tiles are split along KV when the grid
- * would otherwise be unbalanced, and all work items are ordered longest-first.
+ * would otherwise be unbalanced; work items are then assigned longest-first to the least-loaded CTA of
+ * the persistent grid (LPT), each CTA running its items in descending cost order.
  * The descriptors are uploaded with one async copy per array on cuda_stream.
  *
  * Queries of segment (seq_id, kv_head) are rows q_row_start .. q_row_start + q_len - 1, heads
@@ -231,9 +232,12 @@ typedef struct {
     int32_t split;     /* -1: writes the output directly; >= 0: index of this item's partial */
     int32_t n_splits;  /* number of items this tile was cut into */
     int32_t tile;      /* tile id (items of one tile share it) */
+    int32_t cta;       /* CTA of the persistent grid the item is assigned to */
+    int32_t reserved;
 } segpa_item_t;
 
-/* Copy up to cap work items (in schedule order) to host memory; *n_out = total count. */
+/* Copy up to cap work items (in schedule order: CTA by CTA, each CTA's items by descending cost) to
+ * host memory; *n_out = total count. */
 segpa_status_t segpa_segments_items(const segpa_segments_t *segs, segpa_item_t *items_out,
                                     int32_t cap, int32_t *n_out);
 

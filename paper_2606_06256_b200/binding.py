@@ -60,7 +60,8 @@ class PlanStats(C.Structure):
 
 class Item(C.Structure):
     _fields_ = [("segment", C.c_int32), ("t0", C.c_int32), ("n_tok", C.c_int32), ("kb_lo", C.c_int32),
-                ("kb_hi", C.c_int32), ("split", C.c_int32), ("n_splits", C.c_int32), ("tile", C.c_int32)]
+                ("kb_hi", C.c_int32), ("split", C.c_int32), ("n_splits", C.c_int32), ("tile", C.c_int32),
+                ("cta", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib = None

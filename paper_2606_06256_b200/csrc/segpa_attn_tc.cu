@@ -38,10 +38,15 @@ constexpr int kQWarp = 2;
 constexpr int kFirstSoftmaxWarp = 4;
 constexpr int kFirstEpilogueWarp = 12;
 constexpr int kThreads = 512;
-// register budgets (setmaxnreg): 128 * 48 + 256 * 200 + 128 * 64 = 65536
-constexpr int kRegsLow = 48;
-constexpr int kRegsSoftmax = 200;
-constexpr int kRegsEpilogue = 64;
+constexpr int kHalfKeys = 64;
+// register budgets (setmaxnreg): 128 * 72 + 256 * 192 + 128 * 56 = 65536
+constexpr int kRegsLow = 72;
+constexpr int kRegsSoftmax = 192;
+constexpr int kRegsEpilogue = 56;
+#ifndef SEGPA_POLY_MASK
+#define SEGPA_POLY_MASK 0x00
+#endif
+constexpr unsigned kPolyMask = SEGPA_POLY_MASK;   // bit q: pair q of every 8 pairs takes the polynomial exp2
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: O is rescaled only when the max grows by > 2^8
 
 // Pipeline trace (debug builds with -DSEGPA_TRACE only): lane 0 of every warp of CTA 0 logs
@@ -84,15 +89,11 @@ struct Bars {
 };
 
 struct TileRange {
-    int n_rows;   // valid rows (0 = tile unused in this item)
-    int tok0;     // first token of the tile inside the segment's q range
-    int lo, hi;   // KV blocks [lo, hi) this tile takes part in
+    int n_rows;       // valid rows (0 = tile unused in this item)
+    int tok0;         // first token of the tile inside the segment's q range
+    int lo64, hi64;   // 64-key halves [lo64, hi64) that hold keys visible to some row of the tile
+    int lo, hi;       // the 128-key blocks [lo, hi) covering them
 };
-
-__device__ __forceinline__ int item_for(int k, int cta, int n_cta) {
-    // cost-sorted item list dealt in boustrophedon order: round k goes left-to-right when even
-    return k * n_cta + ((k & 1) ? (n_cta - 1 - cta) : cta);
-}
 
 __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev& sg, int tile, int TT, int G) {
     TileRange r;
@@ -100,12 +101,20 @@ __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev&
     const int tok_hi = min(it.t0 + it.n_tok, tok_lo + TT);
     r.tok0 = tok_lo;
     r.n_rows = max(0, tok_hi - tok_lo) * G;
-    if (r.n_rows == 0) { r.lo = r.hi = 0; return r; }
+    r.lo64 = r.hi64 = r.lo = r.hi = 0;
+    if (r.n_rows == 0) return r;
     const int i0 = sg.kv_len - sg.q_len + tok_lo, i1 = sg.kv_len - sg.q_len + tok_hi - 1;
-    r.lo = max(it.kb_lo, max(0, i0 - sg.window + 1) / kBlockKeys);
-    r.hi = min(it.kb_hi, i1 / kBlockKeys + 1);
-    if (r.hi < r.lo) r.hi = r.lo;
+    r.lo64 = max(it.kb_lo * 2, max(0, i0 - sg.window + 1) / kHalfKeys);
+    r.hi64 = min(it.kb_hi * 2, i1 / kHalfKeys + 1);
+    if (r.hi64 < r.lo64) r.hi64 = r.lo64;
+    r.lo = r.lo64 >> 1;
+    r.hi = (r.hi64 == r.lo64) ? r.lo : ((r.hi64 + 1) >> 1);
     return r;
+}
+
+// halves (bit 0 = keys [0, 64), bit 1 = keys [64, 128)) of block j inside the tile's range
+__device__ __forceinline__ int half_mask(const TileRange& r, int j) {
+    return ((2 * j >= r.lo64 && 2 * j < r.hi64) ? 1 : 0) | ((2 * j + 1 >= r.lo64 && 2 * j + 1 < r.hi64) ? 2 : 0);
 }
 
 }  // namespace
@@ -120,7 +129,8 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
     const uint32_t sQ = smem_u32(smem);
     const uint32_t sKV = sQ + C::kSmemQ;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int cta = blockIdx.x, n_cta = gridDim.x;
+    // this CTA's work items: a contiguous, cost-descending slice of the list (host-side LPT assignment)
+    const int i_lo = p.cta_off[blockIdx.x], i_hi = p.cta_off[blockIdx.x + 1];
     const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
     const int rows_per_slot = kTileRows * p.tiles_per_item;
 #ifdef SEGPA_TRACE
@@ -157,10 +167,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         // ------------------------------------------------------------------ K/V loader
         reg_dec<kRegsLow>();
         uint32_t fill = 0;  // stage fills so far
-        for (int k = 0;; ++k) {
-            const int ii = item_for(k, cta, n_cta);
-            if (k * n_cta >= p.n_items) break;
-            if (ii >= p.n_items) continue;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
             int jlo = INT_MAX, jhi = 0;
@@ -194,6 +201,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         // one elected lane issues the tcgen05 instructions.
         reg_dec<kRegsLow>();
         constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, 0, 0);
+        constexpr uint32_t idesc_qk64 = make_idesc_bf16(128, kHalfKeys, 0, 0);   // edge blocks: one 64-key half only
         constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, 0, 1);
         // descriptors differ from a base only in the start-address field: add (bytes >> 4)
         const uint64_t dq0 = make_desc_sw128(sQ, 16, kAtomBytes);
@@ -203,6 +211,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         uint32_t n_q[2] = {0, 0}, n_p[2] = {0, 0}, n_of[2] = {0, 0};
         // the block whose PV is still to be issued, per tile (it may belong to the previous item)
         bool pv_valid[2] = {false, false}, pv_first[2] = {false, false}, pv_last[2] = {false, false};
+        int pv_mask[2] = {0, 0};   // halves of the pending block that hold visible keys
         TileRange tr[2];
         tr[1].n_rows = 0; tr[1].lo = tr[1].hi = 0; tr[1].tok0 = 0;
 
@@ -226,7 +235,8 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             for (int t = 0; t < NT; ++t) {
                 const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
                 const bool do_pv = pv_valid[t];
-                const bool do_qk = have_k && tr[t].n_rows > 0 && j >= tr[t].lo && j < tr[t].hi;
+                const int am = (have_k && tr[t].n_rows > 0) ? half_mask(tr[t], j) : 0;
+                const bool do_qk = am != 0;
                 TRACE(11 + t * 4, j);
                 if (do_pv) {
                     mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
@@ -246,19 +256,37 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                     if (do_pv) {
                         const uint64_t dv = dv0 + (uint64_t)((st_v * C::kTileBytes) >> 4);
                         const uint32_t acc0 = pv_first[t] ? 0u : 1u;
+                        if (pv_mask[t] == 3) {
 #pragma unroll
-                        for (int kk = 0; kk < kBlockKeys / 16; ++kk)
-                            mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
+                            for (int kk = 0; kk < kBlockKeys / 16; ++kk)
+                                mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
+                        } else {   // edge block: the other half has no visible key (its P is zero anyway)
+                            const int k0 = (pv_mask[t] == 2) ? 4 : 0;
+#pragma unroll
+                            for (int kk = 0; kk < kHalfKeys / 16; ++kk)
+                                mma_ts(tO, tS + (k0 + kk) * 8, dv + (uint64_t)(((k0 + kk) * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
+                        }
                         if (pv_last[t]) tc_commit(smem_u32(&bars.o_final[t]));
                     }
                     if (do_qk) {
                         const uint64_t dq = dq0 + (uint64_t)((t * C::kTileBytes) >> 4);
                         const uint64_t dk = dk0 + (uint64_t)((st_k * C::kTileBytes) >> 4);
+                        if (am == 3) {
 #pragma unroll
-                        for (int kk = 0; kk < D / 16; ++kk) {
-                            const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
-                            const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
-                            mma_ss(tS, dq + oq, dk + ok, idesc_qk, kk > 0 ? 1u : 0u);
+                            for (int kk = 0; kk < D / 16; ++kk) {
+                                const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
+                                const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                                mma_ss(tS, dq + oq, dk + ok, idesc_qk, kk > 0 ? 1u : 0u);
+                            }
+                        } else {
+                            const int hb = (am == 2) ? 1 : 0;
+                            const uint64_t dkh = dk + (uint64_t)((hb * 8 * C::kSBO) >> 4);
+#pragma unroll
+                            for (int kk = 0; kk < D / 16; ++kk) {
+                                const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
+                                const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                                mma_ss(tS + hb * kHalfKeys, dq + oq, dkh + ok, idesc_qk64, kk > 0 ? 1u : 0u);
+                            }
                         }
                         tc_commit(smem_u32(&bars.s_full[t]));
                         if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
@@ -267,6 +295,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 __syncwarp();
                 TRACE(13 + t * 4, j);
                 pv_valid[t] = do_qk;
+                pv_mask[t] = am;
                 pv_first[t] = do_qk && j == tr[t].lo;
                 pv_last[t] = do_qk && j + 1 == tr[t].hi;
             }
@@ -277,10 +306,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             __syncwarp();
         };
 
-        for (int k = 0;; ++k) {
-            const int ii = item_for(k, cta, n_cta);
-            if (k * n_cta >= p.n_items) break;
-            if (ii >= p.n_items) continue;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
             int jlo = INT_MAX, jhi = 0;
@@ -310,15 +336,12 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         const uint32_t box_bytes = (uint32_t)(64 * 2 * G * TT);
         uint32_t n_fill[2] = {0, 0};
         if (lane == 0) prefetch_tmap(&p.q_map);
-        for (int k = 0;; ++k) {
-            const int ii = item_for(k, cta, n_cta);
-            if (k * n_cta >= p.n_items) break;
-            if (ii >= p.n_items) continue;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
             // pull the next item's Q tiles towards L2 while this one is computed
-            const int in = item_for(k + 1, cta, n_cta);
-            if ((k + 1) * n_cta < p.n_items && in < p.n_items && elect_one()) {
+            const int in = ii + 1;
+            if (in < i_hi && elect_one()) {
                 const ItemDev itn = p.items[in];
                 const SegDev sgn = p.segs[itn.seg];
 #pragma unroll
@@ -363,10 +386,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             const uint32_t tO = tmem + lane_base + 256 + tile * 128;
             const float sl2 = p.scale * 1.4426950408889634f;
             uint32_t n_s = 0, n_st = 0;
-            for (int k = 0;; ++k) {
-                const int ii = item_for(k, cta, n_cta);
-                if (k * n_cta >= p.n_items) break;
-                if (ii >= p.n_items) continue;
+            for (int ii = i_lo; ii < i_hi; ++ii) {
                 const ItemDev it = p.items[ii];
                 const SegDev sg = p.segs[it.seg];
                 const TileRange tr = tile_range(it, sg, tile, TT, G);
@@ -394,11 +414,22 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, s + c * 32);
                         tmem_wait_ld();
                         TRACE(22, j);
+                        bool dead[4] = {false, false, false, false};   // 32-column chunk masked for every row of the warp
                         if (need_mask) {
-                            // boundary block (causal diagonal / window edge): element mask in registers
+                            // boundary block (causal diagonal / window edge).  Per 32-column chunk, warp-uniformly:
+                            // all visible -> untouched; all masked -> no exp at all; ragged -> element mask in registers
+                            const int mn_cmin = __reduce_min_sync(0xffffffffu, cmin), mx_cmin = __reduce_max_sync(0xffffffffu, cmin);
+                            const int mn_cmax = __reduce_min_sync(0xffffffffu, cmax), mx_cmax = __reduce_max_sync(0xffffffffu, cmax);
 #pragma unroll
-                            for (int e = 0; e < kBlockKeys; ++e)
-                                if (e < cmin || e > cmax) s[e] = 0xff800000u;   // -inf
+                            for (int c = 0; c < 4; ++c) {
+                                const int c0 = 32 * c, c1 = 32 * c + 31;
+                                dead[c] = c1 < mn_cmin || c0 > mx_cmax;
+                                if (!(c0 >= mx_cmin && c1 <= mn_cmax)) {
+#pragma unroll
+                                    for (int e = 0; e < 32; ++e)
+                                        if (c0 + e < cmin || c0 + e > cmax) s[c0 + e] = 0xff800000u;   // -inf
+                                }
+                            }
                         }
                         float mxa = -INFINITY, mxb = -INFINITY, mxc = -INFINITY, mxd = -INFINITY;
 #pragma unroll
@@ -434,22 +465,40 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         TRACE(23, j);
                         const float mref = (m_used == -INFINITY) ? 0.f : m_used;
                         // p = 2^(s*scale*log2e - m) (masked columns: 2^-inf = 0), row sum, bf16 P -> TMEM (aliases S[0, 64))
-                        float rs0 = 0.f, rs1 = 0.f, rs2 = 0.f, rs3 = 0.f;
+                        // exp2 is split between the MUFU pipe and the FMA pipe (exp2_poly2): the two are
+                        // co-limiters of this loop, kPolyMask picks the pairs (of every 8) that go to the FMA pipe
+                        const uint64_t sl2x2 = pack2(sl2, sl2), nmx2 = pack2(-mref, -mref);
+                        uint64_t rsa = pack2(0.f, 0.f), rsb = pack2(0.f, 0.f);
 #pragma unroll
                         for (int c = 0; c < 4; ++c) {
                             uint32_t pk[16];
+                            if (dead[c]) {
 #pragma unroll
-                            for (int e = 0; e < 32; e += 4) {
-                                const float p0 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 0]), sl2, -mref));
-                                const float p1 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 1]), sl2, -mref));
-                                const float p2 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 2]), sl2, -mref));
-                                const float p3 = fast_exp2(fmaf(__uint_as_float(s[c * 32 + e + 3]), sl2, -mref));
-                                rs0 += p0; rs1 += p1; rs2 += p2; rs3 += p3;
-                                pk[(e >> 1) + 0] = pack_bf16x2(p0, p1);
-                                pk[(e >> 1) + 1] = pack_bf16x2(p2, p3);
+                                for (int q = 0; q < 16; ++q) pk[q] = 0u;
+                                tmem_st16(tS + c * 16, pk);
+                                continue;
+                            }
+#pragma unroll
+                            for (int q = 0; q < 16; ++q) {
+                                const int e = c * 32 + 2 * q;
+                                const uint64_t x = ffma2(pack2(__uint_as_float(s[e]), __uint_as_float(s[e + 1])), sl2x2, nmx2);
+                                float p0, p1;
+                                if ((kPolyMask >> (q & 7)) & 1) {
+                                    exp2_poly2(x, p0, p1);
+                                } else {
+                                    float x0, x1;
+                                    unpack2(x, x0, x1);
+                                    p0 = fast_exp2(x0);
+                                    p1 = fast_exp2(x1);
+                                }
+                                if (q & 1) rsb = fadd2(rsb, pack2(p0, p1)); else rsa = fadd2(rsa, pack2(p0, p1));
+                                pk[q] = pack_bf16x2(p0, p1);
                             }
                             tmem_st16(tS + c * 16, pk);
                         }
+                        float rs0, rs1, rs2, rs3;
+                        unpack2(rsa, rs0, rs1);
+                        unpack2(rsb, rs2, rs3);
                         l += (rs0 + rs1) + (rs2 + rs3);
                         tmem_wait_st();
                     }
@@ -471,10 +520,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         const int r = wq * 32 + lane;
         const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
         uint32_t n_o[2] = {0, 0}, n_st[2] = {0, 0};
-        for (int k = 0;; ++k) {
-            const int ii = item_for(k, cta, n_cta);
-            if (k * n_cta >= p.n_items) break;
-            if (ii >= p.n_items) continue;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
 #pragma unroll 1
@@ -572,8 +618,7 @@ static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
         if (e != cudaSuccess) return e;
         configured = true;
     }
-    const int grid = p.n_items < p.num_sms ? p.n_items : p.num_sms;
-    attention_tc_kernel<D, NT><<<grid, kThreads, C::kSmemBytes, st>>>(p);
+    attention_tc_kernel<D, NT><<<p.n_cta, kThreads, C::kSmemBytes, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -13,6 +13,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <queue>
 #include <string>
 #include <unordered_map>
 #include <vector>
@@ -146,12 +147,13 @@ struct segpa_segments {
     std::vector<segpa_item_t> items_pub;
     std::vector<int32_t> pages;
     std::vector<CombDev> combs;
+    std::vector<int32_t> cta_off;   // items of CTA q: [cta_off[q], cta_off[q+1])
     segpa_plan_stats_t stats{};
     int tiles_per_item = 1;
     // device
     SegBuf* buf = nullptr;
     mutable cudaStream_t last_stream = nullptr;   // stream of the last upload / attention_fwd
-    size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0;
+    size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0, off_cta = 0;
 };
 
 struct segpa_cache {
@@ -641,21 +643,46 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 const int hi = t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
                 const int slot = parts > 1 ? n_slots++ : -1;
                 S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, 0, 0});
-                S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti});
+                S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti, 0, 0});
             }
         }
+        // LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid; a CTA's
+        // items stay in descending order.  Cost = visited blocks + a fixed per-item term (pipeline refill,
+        // Q load, epilogue: about 0.6 block-times measured), in thirds of a block.
+        const int n_cta = (int)std::min<size_t>(S->items.size(), (size_t)c->num_sms);
         std::vector<int> order(S->items.size());
         for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
             return (S->items[a].kb_hi - S->items[a].kb_lo) > (S->items[b].kb_hi - S->items[b].kb_lo);
         });
-        std::vector<ItemDev> it2(order.size());
-        std::vector<segpa_item_t> ip2(order.size());
+        std::vector<std::vector<int>> per_cta((size_t)n_cta);
+        {
+            typedef std::pair<int64_t, int> Load;   // (load, cta): min-heap, ties to the lower CTA index
+            std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+            for (int q = 0; q < n_cta; ++q) heap.push(Load(0, q));
+            for (int idx : order) {
+                Load ld = heap.top();
+                heap.pop();
+                per_cta[(size_t)ld.second].push_back(idx);
+                ld.first += 3 * (int64_t)(S->items[idx].kb_hi - S->items[idx].kb_lo) + 2;
+                heap.push(ld);
+            }
+        }
+        std::vector<ItemDev> it2;
+        std::vector<segpa_item_t> ip2;
+        it2.reserve(order.size());
+        ip2.reserve(order.size());
+        S->cta_off.assign((size_t)n_cta + 1, 0);
         int64_t kv_blocks = 0;
-        for (size_t i = 0; i < order.size(); ++i) {
-            it2[i] = S->items[order[i]];
-            ip2[i] = S->items_pub[order[i]];
-            kv_blocks += it2[i].kb_hi - it2[i].kb_lo;
+        for (int q = 0; q < n_cta; ++q) {
+            for (int idx : per_cta[(size_t)q]) {
+                it2.push_back(S->items[idx]);
+                segpa_item_t pub = S->items_pub[idx];
+                pub.cta = q;
+                ip2.push_back(pub);
+                kv_blocks += S->items[idx].kb_hi - S->items[idx].kb_lo;
+            }
+            S->cta_off[(size_t)q + 1] = (int32_t)it2.size();
         }
         S->items.swap(it2);
         S->items_pub.swap(ip2);
@@ -685,7 +712,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         S->off_items = al(S->off_segs + S->segs.size() * sizeof(SegDev));
         S->off_pages = al(S->off_items + S->items.size() * sizeof(ItemDev));
         S->off_combs = al(S->off_pages + S->pages.size() * sizeof(int32_t));
-        const size_t blob_bytes = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
+        S->off_cta = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
+        const size_t blob_bytes = al(S->off_cta + S->cta_off.size() * sizeof(int32_t));
         // device storage: recycled from the cache's free list (no cudaMalloc / cudaMallocHost in steady state)
         SegBuf* B = nullptr;
         if (!c->free_bufs.empty()) {
@@ -719,6 +747,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         memcpy(hb + S->off_items, S->items.data(), S->items.size() * sizeof(ItemDev));
         memcpy(hb + S->off_pages, S->pages.data(), S->pages.size() * sizeof(int32_t));
         if (!S->combs.empty()) memcpy(hb + S->off_combs, S->combs.data(), S->combs.size() * sizeof(CombDev));
+        memcpy(hb + S->off_cta, S->cta_off.data(), S->cta_off.size() * sizeof(int32_t));
         e = cudaMemcpyAsync(B->blob.d, B->blob.h, blob_bytes, cudaMemcpyHostToDevice, st);
         if (e != cudaSuccess) {
             cudaGetLastError();
@@ -795,6 +824,8 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     p.items = (const ItemDev*)(d_blob + s->off_items);
     p.pages = (const int*)(d_blob + s->off_pages);
     p.combs = (const CombDev*)(d_blob + s->off_combs);
+    p.cta_off = (const int*)(d_blob + s->off_cta);
+    p.n_cta = (int)s->cta_off.size() - 1;
     p.n_items = (int)s->items.size();
     p.n_combs = (int)s->combs.size();
     p.counter = s->buf->counter;

@@ -72,6 +72,8 @@ struct FwdParams {
     const ItemDev* items;
     const int* pages;            // translated physical page ids (zero page = num_pages)
     const CombDev* combs;
+    const int* cta_off;          // [n_cta + 1]: CTA c of the attention kernel owns items [cta_off[c], cta_off[c+1])
+    int n_cta;
     int n_items;
     int n_combs;
     int* counter;                // dynamic scheduler cursor (zeroed before launch)

@@ -198,6 +198,51 @@ __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.al
 template <int N>
 __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 
+// ------------------------------------------------------------------------------- packed fp32x2 (FFMA2 / FADD2)
+__device__ __forceinline__ uint64_t pack2(float lo, float hi) {
+    uint64_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(uint64_t v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t ffma2(uint64_t a, uint64_t b, uint64_t c) {
+    uint64_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ uint64_t fsub2(uint64_t a, uint64_t b) {
+    uint64_t d;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// 2^x for a pair on the FMA pipe (no MUFU): round-to-nearest split x = j + f, f in [-0.5, 0.5], degree-3
+// minimax polynomial for 2^f (max relative error 7.5e-5, well below the bf16 rounding of P), exponent
+// added as an integer.  x is clamped to >= -126 (2^-126 stands in for 0; -inf inputs become ~1e-38).
+__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1) {
+    float x0, x1;
+    unpack2(x, x0, x1);
+    x = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
+    const uint64_t magic = pack2(12582912.f, 12582912.f);                    // 1.5 * 2^23
+    const uint64_t t = fadd2(x, magic);                                      // low mantissa bits = round(x)
+    const uint64_t f = fsub2(x, fsub2(t, magic));
+    uint64_t p = ffma2(f, pack2(0.0551716610789299f, 0.0551716610789299f), pack2(0.2426111251115799f, 0.2426111251115799f));
+    p = ffma2(p, f, pack2(0.6932609677314758f, 0.6932609677314758f));
+    p = ffma2(p, f, pack2(0.9999280571937561f, 0.9999280571937561f));
+    float t0, t1, q0, q1;
+    unpack2(t, t0, t1);
+    unpack2(p, q0, q1);
+    p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
+    p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
+}
+
 __device__ __forceinline__ float max3(float a, float b, float c) {
     float d;
     asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));

@@ -175,8 +175,17 @@ def test_visible_page_selection_and_tiles(P):
             assert np.all(seen_tok == 1)
             assert st["attended_pairs"] == pairs
             costs = [it["kb_hi"] - it["kb_lo"] for it in items]
-            assert costs == sorted(costs, reverse=True)              # longest first
             assert st["kv_blocks"] == sum(costs)
+            # LPT schedule: items listed CTA by CTA, longest first inside a CTA, loads balanced to within one item
+            ctas = [it["cta"] for it in items]
+            assert ctas == sorted(ctas) and ctas[0] == 0 and ctas[-1] == min(len(items), 148) - 1
+            loads = {}
+            for it, cst in zip(items, costs):
+                loads.setdefault(it["cta"], []).append(cst)
+            for q, cs in loads.items():
+                assert cs == sorted(cs, reverse=True)
+            tot = [sum(3 * x + 2 for x in cs) for cs in loads.values()]
+            assert max(tot) - min(tot) <= 3 * max(costs) + 2
             B.segpa_free_segments(c, segs)
         B.segpa_destroy(c)
 
