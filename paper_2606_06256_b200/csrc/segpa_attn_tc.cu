@@ -80,7 +80,7 @@ struct Bars {
     uint64_t q_full[2];
     uint64_t q_empty[2];
     uint64_t s_full[2];
-    uint64_t p_full[2];
+    uint64_t p_full[2][2];     // [tile][half]: P columns of keys [0,64) / [64,128) are in TMEM (PV starts on the first half)
     uint64_t o_final[2];    // MMA -> epilogue: last PV of the item's tile has completed
     uint64_t o_free[2];     // epilogue -> MMA: O_t has been read out, the next item may overwrite it
     uint64_t stat_full[2];  // softmax -> epilogue: (m, l) of the finished tile are in smem
@@ -146,7 +146,8 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             mbar_init(smem_u32(&bars.q_full[t]), 1);
             mbar_init(smem_u32(&bars.q_empty[t]), 1);
             mbar_init(smem_u32(&bars.s_full[t]), 1);
-            mbar_init(smem_u32(&bars.p_full[t]), 128);
+            mbar_init(smem_u32(&bars.p_full[t][0]), 128);
+            mbar_init(smem_u32(&bars.p_full[t][1]), 128);
             mbar_init(smem_u32(&bars.o_final[t]), 1);
             mbar_init(smem_u32(&bars.o_free[t]), 128);
             mbar_init(smem_u32(&bars.stat_full[t]), 128);
@@ -238,13 +239,25 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const int am = (have_k && tr[t].n_rows > 0) ? half_mask(tr[t], j) : 0;
                 const bool do_qk = am != 0;
                 TRACE(11 + t * 4, j);
+                const uint64_t dv = dv0 + (uint64_t)((st_v * C::kTileBytes) >> 4);
+                const uint32_t acc0 = pv_first[t] ? 0u : 1u;
                 if (do_pv) {
-                    mbar_wait(smem_u32(&bars.p_full[t]), n_p[t] & 1);
-                    ++n_p[t];
+                    // PV starts as soon as the first 64 keys of P are in TMEM; the softmax warpgroup is still
+                    // working on the other 64
+                    mbar_wait(smem_u32(&bars.p_full[t][0]), n_p[t] & 1);
                     if (pv_first[t]) {   // first PV of an item overwrites O_t: the epilogue must have read it out
                         mbar_wait(smem_u32(&bars.o_free[t]), (n_of[t] & 1) ^ 1);
                         ++n_of[t];
                     }
+                    tc_fence_after();
+                    if ((pv_mask[t] & 1) && elect_one()) {
+#pragma unroll
+                        for (int kk = 0; kk < kHalfKeys / 16; ++kk)
+                            mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
+                    }
+                    __syncwarp();
+                    mbar_wait(smem_u32(&bars.p_full[t][1]), n_p[t] & 1);
+                    ++n_p[t];
                 }
                 if (do_qk && j == tr[t].lo) {
                     mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
@@ -254,17 +267,11 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 TRACE(12 + t * 4, j);
                 if (elect_one()) {
                     if (do_pv) {
-                        const uint64_t dv = dv0 + (uint64_t)((st_v * C::kTileBytes) >> 4);
-                        const uint32_t acc0 = pv_first[t] ? 0u : 1u;
-                        if (pv_mask[t] == 3) {
+                        if (pv_mask[t] & 2) {   // (a half without visible keys is skipped: its P is zero anyway)
+                            const uint32_t acc1 = (pv_mask[t] & 1) ? 1u : acc0;
 #pragma unroll
-                            for (int kk = 0; kk < kBlockKeys / 16; ++kk)
-                                mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
-                        } else {   // edge block: the other half has no visible key (its P is zero anyway)
-                            const int k0 = (pv_mask[t] == 2) ? 4 : 0;
-#pragma unroll
-                            for (int kk = 0; kk < kHalfKeys / 16; ++kk)
-                                mma_ts(tO, tS + (k0 + kk) * 8, dv + (uint64_t)(((k0 + kk) * 2 * C::kSBO) >> 4), idesc_pv, kk > 0 ? 1u : acc0);
+                            for (int kk = kHalfKeys / 16; kk < kBlockKeys / 16; ++kk)
+                                mma_ts(tO, tS + kk * 8, dv + (uint64_t)((kk * 2 * C::kSBO) >> 4), idesc_pv, kk > kHalfKeys / 16 ? 1u : acc1);
                         }
                         if (pv_last[t]) tc_commit(smem_u32(&bars.o_final[t]));
                     }
@@ -476,6 +483,11 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
 #pragma unroll
                                 for (int q = 0; q < 16; ++q) pk[q] = 0u;
                                 tmem_st16(tS + c * 16, pk);
+                                if (c == 1) {
+                                    tmem_wait_st();
+                                    tc_fence_before();
+                                    mbar_arrive(smem_u32(&bars.p_full[tile][0]));
+                                }
                                 continue;
                             }
 #pragma unroll
@@ -495,15 +507,22 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                                 pk[q] = pack_bf16x2(p0, p1);
                             }
                             tmem_st16(tS + c * 16, pk);
+                            if (c == 1) {   // keys [0, 64) done: let their PV start
+                                tmem_wait_st();
+                                tc_fence_before();
+                                mbar_arrive(smem_u32(&bars.p_full[tile][0]));
+                            }
                         }
                         float rs0, rs1, rs2, rs3;
                         unpack2(rsa, rs0, rs1);
                         unpack2(rsb, rs2, rs3);
                         l += (rs0 + rs1) + (rs2 + rs3);
                         tmem_wait_st();
+                    } else {
+                        mbar_arrive(smem_u32(&bars.p_full[tile][0]));
                     }
                     tc_fence_before();
-                    mbar_arrive(smem_u32(&bars.p_full[tile]));
+                    mbar_arrive(smem_u32(&bars.p_full[tile][1]));
                     TRACE(24, j);
                 }
                 // hand (m, l) to the epilogue warpgroup and go straight on to the next item
