@@ -44,6 +44,20 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(workload: str):
+    """DRAM bytes (read + write) of one attention launch from the committed ncu --set full capture of this
+    workload (profiles/r1_traffic.csv), or None when none was taken."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    try:
+        for line in open(p).read().splitlines()[1:]:
+            f = line.rsplit(",", 1)
+            if f[0].split(",")[0] == workload:
+                return int(f[1])
+    except Exception:
+        pass
+    return None
+
+
 def get_workload(name: str):
     from paper_2606_06256_b200 import workloads as wl
     if name == "4d":
@@ -313,7 +327,7 @@ def run_ours(args):
     else:
         roof = {"bound": "tensor", "achieved": useful / (fwd_mean * 1e-3) / 1e12, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s"}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
+    roof["traffic"] = ncu_traffic(w.name)
     roof["kernel"] = "attention_tc_kernel (segpa_attention_fwd), avg of %d launches-groups timed with CUDA events" % args.steps
     roof["peak_source"] = peaks_src + (", burst figure" if not decode_shaped else "")
     roof["algorithmic_bytes"] = alg_bytes
