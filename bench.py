@@ -170,6 +170,47 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------------
+# context only: the same shapes as dense attention with an explicit mask ("Dense+mask")
+# ---------------------------------------------------------------------------------------------
+def dense_mask_ms(w, k_pool, v_pool, q, layer: int = 0, reps: int = 3):
+    """Time of torch SDPA with a boolean attn_mask over gathered dense [1, H, L, D] K/V for one layer of `w`:
+    per request, one call per group of KV heads sharing (class, window, q_len).  The gather is not timed.
+    Library code, used as context for the paper's mask-penalty statement, not as a baseline to beat."""
+    import torch
+    import torch.nn.functional as F
+    from paper_2606_06256_b200 import workloads as wl
+    sm = w.stream_map()
+    groups = {}
+    for s in w.layer_segments(layer):
+        groups.setdefault((s.seq_id, s.head_class, s.window if s.head_class == wl.LOCAL else 0, s.q_row_start, s.q_len), []).append(s.kv_head)
+    calls = []
+    for (seq, cls, W, q0, ql), heads in groups.items():
+        L = sm[(layer, heads[0], seq)].kv_len
+        kd = torch.stack([wl.stream_rows(k_pool, sm[(layer, h, seq)], w.P) for h in heads])      # [n_kvh, L, D]
+        vd = torch.stack([wl.stream_rows(v_pool, sm[(layer, h, seq)], w.P) for h in heads])
+        kd = kd.repeat_interleave(w.G, dim=0).unsqueeze(0)
+        vd = vd.repeat_interleave(w.G, dim=0).unsqueeze(0)
+        qh = torch.cat([torch.arange(h * w.G, (h + 1) * w.G) for h in heads]).to(q.device)
+        qd = q[q0:q0 + ql][:, qh].permute(1, 0, 2).unsqueeze(0).contiguous()                      # [1, Hg, ql, D]
+        i = torch.arange(L - ql, L, device=q.device).unsqueeze(1)
+        j = torch.arange(L, device=q.device).unsqueeze(0)
+        mask = (j <= i) if cls == wl.GLOBAL else ((j <= i) & (j > i - W))
+        calls.append((qd, kd, vd, mask))
+    def run():
+        for qd, kd, vd, mask in calls:
+            F.scaled_dot_product_attention(qd, kd, vd, attn_mask=mask, scale=w.scale)
+    run()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        run()
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1) / reps, len(calls)
+
+
+# ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -348,6 +389,14 @@ def run_ours(args):
                     "ms_per_step": 1e3 * e2e_s},
             "gpu_launches": int(launches[0]), "wall_s_timed_region": wall}
 
+    if rank == 0 and world == 1 and (args.dense_mask == "on" or (args.dense_mask == "auto" and args.config == "2")):
+        try:
+            dm, ncalls = dense_mask_ms(w, k_pool, v_pool, qs[0])
+            line["dense_mask_context"] = {"ms_per_layer": dm, "x_slower_than_segpa_fwd": dm / (fwd_mean / w.num_layers),
+                                          "how": "torch SDPA, boolean attn_mask, dense gathered K/V, %d calls (one per request x head class), layer 0" % ncalls,
+                                          "note": "context for the paper's 4.9-7.6x mask penalty (PAPER.md:19; its shapes are unknown), not a like-for-like number"}
+        except Exception as ex:  # library path, context only
+            line["dense_mask_context"] = {"error": repr(ex)[:200]}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         tf, dt, cores, pairs, desc = oracle_sample(w, args.cpu_rows, seed=0, k_pool=k_pool.cpu(), v_pool=v_pool.cpu(), q=qs[0].cpu())
         line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc + "; %.1f s" % dt}
@@ -366,9 +415,11 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="2")
     ap.add_argument("--tiles", type=int, default=2)
-    ap.add_argument("--cpu-rows", type=int, default=384, help="rows in the cpu_baseline oracle sample")
-    ap.add_argument("--ref-rows", type=int, default=128, help="rows per step of the --impl reference oracle sample")
+    ap.add_argument("--cpu-rows", type=int, default=20000, help="rows in the cpu_baseline oracle sample")
+    ap.add_argument("--ref-rows", type=int, default=2048, help="rows per step of the --impl reference oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--dense-mask", default="auto", choices=["auto", "on", "off"],
+                    help="also time dense attention with an explicit mask (context; auto = only for --config 2)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

@@ -47,6 +47,18 @@ RAGGED = [
 ]
 
 
+RAGGED += [
+    # G = 16 (largest supported group): 8 tokens per tile; D = 64 with 32-token pages
+    (32, 2, 64, 32, [{"kv_len": 777, "heads": {0: (GLOBAL, 0, 0, 777), 1: (LOCAL, 65, 0, 400)}}]),
+    # G = 1 (MHA): 128 tokens per tile, windows around the 64-key half and 128-key block edges
+    (4, 4, 128, 16, [{"kv_len": 1300, "heads": {0: (LOCAL, 64, 0, 1300), 1: (LOCAL, 63, 0, 1300), 2: (LOCAL, 128, 0, 515), 3: (LOCAL, 193, 0, 1300)}}]),
+    # many tiny segments: more segments than CTAs, one- and two-row tiles, kv_len around one page
+    (8, 2, 128, 16, [{"kv_len": 1 + (7 * r) % 40, "heads": {0: (GLOBAL, 0, 0, 1 + r % 2), 1: (LOCAL, 1 + r % 5, 0, 1)}} for r in range(170)]),
+    # the item's second tile holds a single token
+    (8, 2, 128, 16, [{"kv_len": 4000, "heads": {0: (GLOBAL, 0, 0, 33), 1: (LOCAL, 700, 0, 33)}}]),
+]
+
+
 @pytest.mark.parametrize("kernel,tiles", VARIANTS)
 @pytest.mark.parametrize("case", range(len(RAGGED)))
 def test_ragged_small(case, kernel, tiles):
