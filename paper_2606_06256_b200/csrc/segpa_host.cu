@@ -244,9 +244,14 @@ const char* encode_q_map(TensorMap* out, const void* q, int64_t T, int Hq, int D
     return r == CUDA_SUCCESS ? nullptr : "cuTensorMapEncodeTiled failed";
 }
 
-// attended keys of the query at position i (Alg. 2 policy; PAPER.md:219 with W = w + 1)
-inline int64_t visible_count(int64_t i, int head_class, int64_t W) {
-    return head_class == SEGPA_GLOBAL ? i + 1 : std::min<int64_t>(i + 1, W);
+// attended (query, key) pairs of the queries at positions [i0, i1]: sum of min(i + 1, W) (Alg. 2 policy;
+// PAPER.md:219 with W = w + 1; GLOBAL passes a W larger than any position)
+inline int64_t visible_pairs(int64_t i0, int64_t i1, int64_t W) {
+    auto tri = [](int64_t a, int64_t b) { return a > b ? (int64_t)0 : (a + b) * (b - a + 1) / 2; };   // a + ... + b
+    const int64_t knee = W - 1;                       // positions <= knee see i + 1 keys, later ones see W
+    const int64_t ramp = tri(i0 + 1, std::min(i1, knee) + 1);
+    const int64_t flat = i1 > knee ? (i1 - std::max(i0, knee + 1) + 1) * W : 0;
+    return ramp + flat;
 }
 
 }  // namespace
@@ -567,6 +572,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
     int64_t q_rows = 0, pairs = 0, vis_tokens = 0;
     try {
         S->reqs.assign(reqs, reqs + n);
+        S->segs.reserve((size_t)n);
         // validation + per-segment metadata
         struct Iv { int32_t kv_head; int64_t lo, hi; };
         std::vector<Iv> ivs;
@@ -604,12 +610,17 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             sd.first_page = (int)(seg_kb_lo * ppb);
             sd.n_pages_listed = (int)((seg_kb_hi - seg_kb_lo) * ppb);
             // Alg. 2 line 12: Translate(T_page, U_h); invisible / absent pages -> the zero page
-            for (int64_t pg = sd.first_page; pg < sd.first_page + sd.n_pages_listed; ++pg)
-                S->pages.push_back((pg >= first_vis_page && pg < n_stream_pages) ? rec.pages[(size_t)pg] : zero_page);
+            {
+                const int64_t lst_lo = sd.first_page, lst_hi = sd.first_page + sd.n_pages_listed;
+                const int64_t vis_a = std::max(lst_lo, first_vis_page), vis_b = std::min(lst_hi, n_stream_pages);
+                S->pages.insert(S->pages.end(), (size_t)(vis_a - lst_lo), zero_page);
+                S->pages.insert(S->pages.end(), rec.pages.begin() + vis_a, rec.pages.begin() + vis_b);
+                S->pages.insert(S->pages.end(), (size_t)(lst_hi - vis_b), zero_page);
+            }
             S->segs.push_back(sd);
             vis_tokens += kv_len - first_vis_page * P;
             q_rows = std::max<int64_t>(q_rows, r.q_row_start + r.q_len);
-            for (int64_t t = 0; t < r.q_len; ++t) pairs += visible_count(kv_len - r.q_len + t, r.head_class, W);
+            pairs += visible_pairs(kv_len - r.q_len, kv_len - 1, W);
             // tiles: exactly the KV blocks the tile's rows attend to
             for (int64_t t0 = 0; t0 < r.q_len; t0 += item_tok) {
                 const int64_t n_tok = std::min<int64_t>(item_tok, r.q_len - t0);
