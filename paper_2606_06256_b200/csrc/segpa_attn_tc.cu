@@ -26,6 +26,7 @@
 
 #include <climits>
 #include <cstdlib>
+#include <type_traits>
 
 namespace segpa {
 using namespace ptx;
@@ -92,16 +93,23 @@ struct TileRange {
     int n_rows;       // valid rows (0 = tile unused in this item)
     int tok0;         // first token of the tile inside the segment's q range
     int lo64, hi64;   // 64-key halves [lo64, hi64) that hold keys visible to some row of the tile
-    int lo, hi;       // the 128-key blocks [lo, hi) covering them
+    int lo, hi;       // first block of the tile and one past its last block
+    int step;         // 1; or 2 for a strided item (the two tiles hold the SAME rows and take alternate blocks)
 };
 
+// A strided item (ItemDev::flags & 1, decode-shaped: all its rows fit one tile) runs its KV range as two
+// independent chains: tile t takes the blocks kb_lo + t, kb_lo + t + 2, ... and writes its own split-KV
+// partial; the combine kernel merges them.  That keeps two QK^T -> softmax -> PV chains in flight where a
+// single tile would leave the second tile slot (and half of the latency hiding) unused.
 __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev& sg, int tile, int TT, int G) {
     TileRange r;
-    const int tok_lo = it.t0 + tile * TT;
+    const bool strided = (it.flags & 1) != 0;
+    const int tok_lo = it.t0 + (strided ? 0 : tile * TT);
     const int tok_hi = min(it.t0 + it.n_tok, tok_lo + TT);
     r.tok0 = tok_lo;
     r.n_rows = max(0, tok_hi - tok_lo) * G;
     r.lo64 = r.hi64 = r.lo = r.hi = 0;
+    r.step = 1;
     if (r.n_rows == 0) return r;
     const int i0 = sg.kv_len - sg.q_len + tok_lo, i1 = sg.kv_len - sg.q_len + tok_hi - 1;
     r.lo64 = max(it.kb_lo * 2, max(0, i0 - sg.window + 1) / kHalfKeys);
@@ -109,11 +117,19 @@ __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev&
     if (r.hi64 < r.lo64) r.hi64 = r.lo64;
     r.lo = r.lo64 >> 1;
     r.hi = (r.hi64 == r.lo64) ? r.lo : ((r.hi64 + 1) >> 1);
+    if (strided) {
+        r.step = 2;
+        const int first = r.lo + (((r.lo - it.kb_lo) & 1) != tile ? 1 : 0);       // first block of this parity
+        if (first >= r.hi) { r.hi64 = r.lo64; r.lo = r.hi = first; return r; }   // no block of its own
+        r.hi = first + ((r.hi - 1 - first) & ~1) + 1;
+        r.lo = first;
+    }
     return r;
 }
 
-// halves (bit 0 = keys [0, 64), bit 1 = keys [64, 128)) of block j inside the tile's range
+// halves (bit 0 = keys [0, 64), bit 1 = keys [64, 128)) of block j the tile attends to (0: not its block)
 __device__ __forceinline__ int half_mask(const TileRange& r, int j) {
+    if (j < r.lo || j >= r.hi || ((j - r.lo) & (r.step - 1))) return 0;
     return ((2 * j >= r.lo64 && 2 * j < r.hi64) ? 1 : 0) | ((2 * j + 1 >= r.lo64 && 2 * j + 1 < r.hi64) ? 2 : 0);
 }
 
@@ -176,9 +192,13 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const TileRange tr = tile_range(it, sg, t, TT, G);
                 if (tr.n_rows > 0 && tr.hi > tr.lo) { jlo = min(jlo, tr.lo); jhi = max(jhi, tr.hi); }
             }
+            // page ids are fetched one block ahead: the dependent global load of block j + 1 is in flight while
+            // block j's copies are issued (decode-shaped items consume a block every ~1500 cycles)
+            const int* pg = p.pages + sg.page_off - sg.first_page + lane;
+            int page_next = (lane < ppb && jlo < jhi) ? pg[(long long)jlo * ppb] : 0;
             for (int j = jlo; j < jhi; ++j) {
-                int page = 0;
-                if (lane < ppb) page = p.pages[sg.page_off + (long long)(j * ppb - sg.first_page) + lane];
+                const int page = page_next;
+                if (lane < ppb && j + 1 < jhi) page_next = pg[(long long)(j + 1) * ppb];
                 for (int kv = 0; kv < 2; ++kv) {
                     const uint32_t st = fill % C::kStages, ph = (fill / C::kStages) & 1;
                     TRACE(1, j * 2 + kv);
@@ -232,8 +252,9 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 mbar_wait(smem_u32(&bars.kv_full[st_k]), (rd / C::kStages) & 1);
                 ++rd;
             }
-#pragma unroll
-            for (int t = 0; t < NT; ++t) {
+            // per-tile part of the step (t is a compile-time constant so the per-tile state stays in registers)
+            auto tile_part = [&](auto tile_c) {
+                constexpr int t = decltype(tile_c)::value;
                 const uint32_t tS = tmem + t * 128, tO = tmem + 256 + t * 128;
                 const bool do_pv = pv_valid[t];
                 const int am = (have_k && tr[t].n_rows > 0) ? half_mask(tr[t], j) : 0;
@@ -305,6 +326,16 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 pv_mask[t] = am;
                 pv_first[t] = do_qk && j == tr[t].lo;
                 pv_last[t] = do_qk && j + 1 == tr[t].hi;
+            };
+            // A tile with no pending PV can have its QK^T issued at once; one with a pending PV first waits
+            // for its softmax warpgroup.  Serve the former first (strided items: the two tiles alternate blocks,
+            // so this is what lets the two chains overlap instead of waiting on each other).
+            if (NT == 2) {
+                const bool t1_first = pv_valid[0] && !pv_valid[1];
+                if (t1_first) { tile_part(std::integral_constant<int, 1>{}); tile_part(std::integral_constant<int, 0>{}); }
+                else { tile_part(std::integral_constant<int, 0>{}); tile_part(std::integral_constant<int, 1>{}); }
+            } else {
+                tile_part(std::integral_constant<int, 0>{});
             }
             if (elect_one()) {
                 if (have_v) tc_commit(smem_u32(&bars.kv_empty[st_v]));
@@ -406,7 +437,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const bool warp_has_rows = wq * 32 < tr.n_rows;  // decode-shaped tiles: most warps hold no row
                 float m_used = -INFINITY, l = 0.f;
 
-                for (int j = tr.lo; j < tr.hi; ++j) {
+                for (int j = tr.lo; j < tr.hi; j += tr.step) {
                     TRACE(20, j);
                     mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
                     ++n_s;
@@ -565,7 +596,8 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 }
                 TRACE(31, tile);
                 if (it.partial_slot >= 0) {
-                    const size_t base = (size_t)it.partial_slot * rows_per_slot + (size_t)(tr.tok0 - it.t0) * G + r;
+                    const size_t base = (size_t)it.partial_slot * rows_per_slot +
+                                        ((it.flags & 1) ? (size_t)tile * kTileRows : (size_t)(tr.tok0 - it.t0) * G) + r;
 #pragma unroll 1
                     for (int c = 0; c < D / 16; ++c) {
                         uint32_t v[16];

@@ -645,15 +645,18 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             const int cost = t.kb_hi - t.kb_lo;
             int parts = 1;
             if (cost > chunk + chunk / 2) parts = (int)cdiv(cost, chunk);
-            if (parts > 1) {
-                ++n_split_tiles;
-                S->combs.push_back(CombDev{t.seg, t.t0, t.n_tok, n_slots, parts, 0, 0, 0});
-            }
+            // Decode-shaped tile (all its rows fit the first of the item's two tile slots): run it STRIDED -- the
+            // two slots take alternate KV blocks of the same rows as two independent chains, each writing a
+            // partial that the combine kernel merges -- so the second slot is not left idle.
+            const bool strided = tiles_per_item == 2 && t.n_tok <= TT && cost >= 2 && c->kernel_kind == 1;
+            if (parts > 1) ++n_split_tiles;
+            if (parts > 1 || strided)
+                S->combs.push_back(CombDev{t.seg, t.t0, t.n_tok, n_slots, parts, strided ? 1 : 0, 0, 0});
             for (int p = 0; p < parts; ++p) {
                 const int lo = t.kb_lo + (int)((int64_t)cost * p / parts);
                 const int hi = t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
-                const int slot = parts > 1 ? n_slots++ : -1;
-                S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, 0, 0});
+                const int slot = (parts > 1 || strided) ? n_slots++ : -1;
+                S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, 0});
                 S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti, 0, 0});
             }
         }
@@ -675,7 +678,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 Load ld = heap.top();
                 heap.pop();
                 per_cta[(size_t)ld.second].push_back(idx);
-                ld.first += 3 * (int64_t)(S->items[idx].kb_hi - S->items[idx].kb_lo) + 2;
+                const int64_t blocks3 = 3 * (int64_t)(S->items[idx].kb_hi - S->items[idx].kb_lo);
+                ld.first += ((S->items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2;   // strided: two chains
                 heap.push(ld);
             }
         }
@@ -839,6 +843,8 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     p.n_cta = (int)s->cta_off.size() - 1;
     p.n_items = (int)s->items.size();
     p.n_combs = (int)s->combs.size();
+    p.comb_max_rows = 0;
+    for (const CombDev& cd : s->combs) p.comb_max_rows = std::max(p.comb_max_rows, cd.n_tok * c->G);
     p.counter = s->buf->counter;
     p.k_pool = c->k_pool;
     p.v_pool = c->v_pool;

@@ -49,7 +49,8 @@ struct ItemDev {
     int kb_lo;              // visited KV blocks [kb_lo, kb_hi)
     int kb_hi;
     int partial_slot;       // -1: final result written to out/lse; else split-KV partial slot
-    int pad0, pad1;
+    int flags;              // bit 0: strided (both tiles hold the same rows and take alternate KV blocks)
+    int pad1;
 };
 
 struct CombDev {
@@ -58,7 +59,8 @@ struct CombDev {
     int n_tok;
     int first_slot;
     int n_splits;
-    int pad0, pad1, pad2;
+    int flags;              // bit 0: strided items: every slot holds two partials of the same rows (at +0 and +128)
+    int pad1, pad2;
 };
 
 // 128-byte TMA descriptor (CUtensorMap) of Q viewed as [T][Hq][D]; encoded per attention_fwd call.
@@ -76,6 +78,7 @@ struct FwdParams {
     int n_cta;
     int n_items;
     int n_combs;
+    int comb_max_rows;           // most rows (tokens x G) any combine entry has
     int* counter;                // dynamic scheduler cursor (zeroed before launch)
     const uint8_t* k_pool;
     const uint8_t* v_pool;

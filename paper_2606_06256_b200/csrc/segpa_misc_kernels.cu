@@ -57,40 +57,80 @@ cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const Scatter
 // merged in ascending split order (deterministic).  Exactness of the merge: PAPER.md:302.
 // One warp per row.
 // ---------------------------------------------------------------------------------------------
-__global__ void combine_kernel(FwdParams p) {
+template <int D>
+__global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ FwdParams p) {
+    constexpr int EPL = D / 32;   // elements per lane
+    constexpr int NW = 8;         // warps per block: warp w merges partials w, w + 8, ... of the block's row
+    __shared__ float s_acc[NW][D];
+    __shared__ float s_l[NW];
     const int rows_per_slot = kTileRows * p.tiles_per_item;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nw = blockDim.x >> 5;
-    for (int ci = blockIdx.x; ci < p.n_combs; ci += gridDim.x) {
-        const CombDev c = p.combs[ci];
-        const SegDev sg = p.segs[c.seg];
-        const int rows = c.n_tok * p.G;
-        for (int r = warp; r < rows; r += nw) {
-            float M = -INFINITY;
-            for (int s = 0; s < c.n_splits; ++s)
-                M = fmaxf(M, p.ws_ml[((size_t)(c.first_slot + s) * rows_per_slot + r) * 2]);
-            float L = 0.f;
-            float acc[4] = {0.f, 0.f, 0.f, 0.f};
-            for (int s = 0; s < c.n_splits; ++s) {
-                const size_t base = (size_t)(c.first_slot + s) * rows_per_slot + r;
-                const float ms = p.ws_ml[base * 2], ls = p.ws_ml[base * 2 + 1];
-                const float w = (ms == -INFINITY) ? 0.f : exp2f(ms - M);
-                L += w * ls;
-                for (int k = 0; k < p.D / 32; ++k) acc[k] += w * p.ws_o[base * p.D + lane + 32 * k];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // block (x, y): comb x, rows y, y + gridDim.y, ...  One block per row: the chain of dependent loads of a
+    // row with many partials is cut eight ways; sums are formed in a fixed order (deterministic).
+    const CombDev c = p.combs[blockIdx.x];
+    const SegDev sg = p.segs[c.seg];
+    const int rows = c.n_tok * p.G;
+    // partials of row r: slot first_slot + s at row r; strided items hold a second one at row r + 128
+    const int per_slot = (c.flags & 1) ? 2 : 1;
+    const int n_part = c.n_splits * per_slot;
+    for (int r = blockIdx.y; r < rows; r += gridDim.y) {
+        auto part_row = [&](int s) {
+            return (size_t)(c.first_slot + s / per_slot) * rows_per_slot + (size_t)(s % per_slot) * kTileRows + r;
+        };
+        // global max M: every warp forms it (lanes over partials, loads independent)
+        float M = -INFINITY;
+        for (int s = lane; s < n_part; s += 32) M = fmaxf(M, p.ws_ml[part_row(s) * 2]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
+        // this warp's partials, ascending
+        float L = 0.f;
+        float acc[EPL];
+#pragma unroll
+        for (int k = 0; k < EPL; ++k) acc[k] = 0.f;
+        for (int s = warp; s < n_part; s += NW) {
+            const size_t base = part_row(s);
+            const float ms = p.ws_ml[base * 2], ls = p.ws_ml[base * 2 + 1];
+            float ov[EPL];
+#pragma unroll
+            for (int k = 0; k < EPL; ++k) ov[k] = p.ws_o[base * D + lane + 32 * k];
+            const float w = (ms == -INFINITY) ? 0.f : exp2f(ms - M);
+            L += w * ls;
+#pragma unroll
+            for (int k = 0; k < EPL; ++k) acc[k] += w * ov[k];
+        }
+#pragma unroll
+        for (int k = 0; k < EPL; ++k) s_acc[warp][lane + 32 * k] = acc[k];
+        if (lane == 0) s_l[warp] = L;
+        __syncthreads();
+        if (warp == 0) {
+            float Lt = 0.f;
+            float tot[EPL];
+#pragma unroll
+            for (int k = 0; k < EPL; ++k) tot[k] = 0.f;
+#pragma unroll
+            for (int w2 = 0; w2 < NW; ++w2) {     // fixed order
+                Lt += s_l[w2];
+#pragma unroll
+                for (int k = 0; k < EPL; ++k) tot[k] += s_acc[w2][lane + 32 * k];
             }
             const int t = c.t0 + r / p.G, head = sg.kv_head * p.G + r % p.G;
             const long long row = sg.q_row_start + t;
-            const float inv = 1.f / L;
-            for (int k = 0; k < p.D / 32; ++k)
-                p.out[row * p.out_row_stride + (long long)head * p.D + lane + 32 * k] =
-                    __bfloat16_as_ushort(__float2bfloat16_rn(acc[k] * inv));
-            if (p.lse && lane == 0) p.lse[(long long)head * p.lse_stride + row] = (M + log2f(L)) * 0.6931471805599453f;
+            const float inv = 1.f / Lt;
+#pragma unroll
+            for (int k = 0; k < EPL; ++k)
+                p.out[row * p.out_row_stride + (long long)head * D + lane + 32 * k] =
+                    __bfloat16_as_ushort(__float2bfloat16_rn(tot[k] * inv));
+            if (p.lse && lane == 0) p.lse[(long long)head * p.lse_stride + row] = (M + log2f(Lt)) * 0.6931471805599453f;
         }
+        __syncthreads();
     }
 }
 
 cudaError_t launch_combine(const FwdParams& p, cudaStream_t st) {
-    const int blocks = p.n_combs < 4 * p.num_sms ? p.n_combs : 4 * p.num_sms;
-    combine_kernel<<<blocks, 256, 0, st>>>(p);
+    if (p.n_combs == 0) return cudaSuccess;
+    const dim3 grid((unsigned)p.n_combs, (unsigned)(p.comb_max_rows < 1 ? 1 : (p.comb_max_rows > 256 ? 256 : p.comb_max_rows)));
+    if (p.D == 128) combine_kernel<128><<<grid, 256, 0, st>>>(p);
+    else combine_kernel<64><<<grid, 256, 0, st>>>(p);
     return cudaGetLastError();
 }
 
