@@ -138,6 +138,20 @@ typedef struct {
 segpa_status_t segpa_append_pages_batch(segpa_cache_t *cache, const segpa_append_req_t *reqs, int32_t n,
                                         void *cuda_stream);
 
+/*
+ * True eviction ("true eviction ... rather than zero-filling"): remove pages
+ * [first_page_index, first_page_index + n_pages) from a stream's page table.  Their reference counts
+ * are decremented (pages reaching zero return to the free list) and the entries become holes
+ * (reported as -1 by segpa_stream_info); the stream keeps its length.  This is how the middle of a
+ * LOCAL head's stream (between the sink tokens and the recent window) is dropped.  A later
+ * segpa_build_segments whose visible set (sink pages + window pages) touches a hole fails with
+ * INVALID; holes outside it are never read.
+ * Errors: INVALID (no such stream, range outside the page table, a page already evicted; the stream's
+ * partial last page cannot be evicted).
+ */
+segpa_status_t segpa_evict_pages(segpa_cache_t *cache, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                 int32_t first_page_index, int32_t n_pages);
+
 /* Drop every stream of the cache (all pages return to the free list).  Segment objects built
  * earlier keep their translated page lists and must not be used afterwards. */
 segpa_status_t segpa_clear_streams(segpa_cache_t *cache);
@@ -168,8 +182,8 @@ typedef struct {
     int32_t window;      /* LOCAL: W = number of visible keys INCLUDING the query's own position
                             (paper's w = W - 1; reading A1). >= 1.
                             Ignored for GLOBAL. */
-    int32_t n_sink;      /* LOCAL: first n_sink tokens stay visible (S_sink).
-                            Must be 0 in this version (sinks on the GPU are NEXT #1). */
+    int32_t n_sink;      /* LOCAL: the first n_sink tokens stay visible besides the window (S_sink,
+                            PAPER.md:219); >= 0.  Ignored for GLOBAL. */
     int64_t q_row_start; /* first row of this segment's queries in q / out */
     int32_t q_len;       /* 1 <= q_len <= kv_len; query t has position kv_len - q_len + t
                             (bottom-right aligned, the flash_attn_varlen convention) */
@@ -180,7 +194,8 @@ typedef struct {
  * Build one layer's metadata M_l and the tile schedule for n segments.
  *
  * Per segment: visible positions are [0, kv_len) for GLOBAL and
- * [max(0, kv_len - q_len - W + 1), kv_len) for LOCAL (Alg. 2 lines 6-10); the pages covering
+ * [0, n_sink) U [max(0, kv_len - q_len - W + 1), kv_len) for LOCAL (Alg. 2 lines 6-10: sink pages +
+ * recent pages; a work item of a segment with sinks visits two KV block ranges); the pages covering
  * them are translated to physical ids (line 12); pages outside the visible range are replaced by
  * the always-zero page, so evicted pages are never read ("true eviction").  Query
  * rows are cut into tiles of floor(128 / G) tokens x G query heads (GQA packing: the G heads of a
@@ -195,8 +210,8 @@ typedef struct {
  * segment are never written by attention_fwd.
  *
  * Errors: INVALID (n < 1, unknown stream, q_len < 1 or > kv_len, LOCAL with window < 1, bad
- * class, negative q_row_start, two segments overlapping on (row, head)), UNSUPPORTED (n_sink != 0),
- * OOM, CUDA.
+ * class, negative q_row_start or n_sink, two segments overlapping on (row, head), a visible page that was
+ * evicted), OOM, CUDA.
  */
 segpa_status_t segpa_build_segments(segpa_cache_t *cache, int32_t layer,
                                     const segpa_segment_req_t *reqs, int32_t n,

@@ -19,7 +19,7 @@ _STATUS = {0: "OK", 1: "INVALID", 2: "OOM", 3: "CUDA", 4: "UNSUPPORTED", 5: "STA
 
 EXPORTS = [
     "segpa_pool_bytes", "segpa_create_cache", "segpa_append_pages", "segpa_append_pages_batch",
-    "segpa_clear_streams", "segpa_free_stream",
+    "segpa_clear_streams", "segpa_evict_pages", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
     "segpa_attention_fwd_host", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
@@ -84,6 +84,7 @@ def lib():
                                          C.c_int64, C.c_int64, C.c_void_p, C.c_int32, C.c_void_p]
         L.segpa_append_pages_batch.argtypes = [C.c_void_p, C.POINTER(AppendReq), C.c_int32, C.c_void_p]
         L.segpa_clear_streams.argtypes = [C.c_void_p]
+        L.segpa_evict_pages.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int32, C.c_int32]
         L.segpa_free_stream.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64]
         L.segpa_stream_info.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_int64),
                                         C.POINTER(C.c_int32), C.c_void_p, C.c_int32]
@@ -180,6 +181,10 @@ def segpa_append_pages_batch(cache: int, batch, stream=None) -> None:
     if not isinstance(batch, AppendBatch):
         batch = AppendBatch(batch)
     _check(lib().segpa_append_pages_batch(cache, batch.arr, batch.n, _stream_ptr(stream)))
+
+
+def segpa_evict_pages(cache: int, layer: int, kv_head: int, seq_id: int, first_page_index: int, n_pages: int) -> None:
+    _check(lib().segpa_evict_pages(cache, layer, kv_head, seq_id, first_page_index, n_pages))
 
 
 def segpa_clear_streams(cache: int) -> None:

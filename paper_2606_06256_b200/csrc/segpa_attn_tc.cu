@@ -92,8 +92,10 @@ struct Bars {
 struct TileRange {
     int n_rows;       // valid rows (0 = tile unused in this item)
     int tok0;         // first token of the tile inside the segment's q range
-    int lo64, hi64;   // 64-key halves [lo64, hi64) that hold keys visible to some row of the tile
-    int lo, hi;       // first block of the tile and one past its last block
+    int sink64, sb;   // sink part: 64-key halves [0, sink64) in blocks [0, sb), visited before the window part
+                      // (0 when the segment has no sinks or the sink blocks touch the window blocks: merged)
+    int lo64, hi64;   // window part: 64-key halves [lo64, hi64) that hold keys visible to some row of the tile
+    int lo, hi;       // first block of the window part and one past its last block
     int step;         // 1; or 2 for a strided item (the two tiles hold the SAME rows and take alternate blocks)
 };
 
@@ -101,6 +103,10 @@ struct TileRange {
 // independent chains: tile t takes the blocks kb_lo + t, kb_lo + t + 2, ... and writes its own split-KV
 // partial; the combine kernel merges them.  That keeps two QK^T -> softmax -> PV chains in flight where a
 // single tile would leave the second tile slot (and half of the latency hiding) unused.
+// Sinks (LOCAL segments with n_sink > 0): the visible set is [0, n_sink) U [i - W + 1, i]; a tile
+// visits the sink blocks first and then its window blocks (two KV block ranges per item); when the two
+// ranges touch they are merged into one and the gap is masked per element.  In a strided item tile 0 takes
+// the sink blocks.
 __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev& sg, int tile, int TT, int G) {
     TileRange r;
     const bool strided = (it.flags & 1) != 0;
@@ -108,29 +114,62 @@ __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev&
     const int tok_hi = min(it.t0 + it.n_tok, tok_lo + TT);
     r.tok0 = tok_lo;
     r.n_rows = max(0, tok_hi - tok_lo) * G;
-    r.lo64 = r.hi64 = r.lo = r.hi = 0;
+    r.sink64 = r.sb = r.lo64 = r.hi64 = r.lo = r.hi = 0;
     r.step = 1;
     if (r.n_rows == 0) return r;
     const int i0 = sg.kv_len - sg.q_len + tok_lo, i1 = sg.kv_len - sg.q_len + tok_hi - 1;
     r.lo64 = max(it.kb_lo * 2, max(0, i0 - sg.window + 1) / kHalfKeys);
     r.hi64 = min(it.kb_hi * 2, i1 / kHalfKeys + 1);
     if (r.hi64 < r.lo64) r.hi64 = r.lo64;
+    if (sg.n_sink > 0 && it.kb_lo == 0) {
+        r.sink64 = (min(sg.n_sink, i1 + 1) + kHalfKeys - 1) / kHalfKeys;
+        r.sb = (r.sink64 + 1) >> 1;
+        if (r.hi64 > r.lo64 && r.sb >= (r.lo64 >> 1)) { r.lo64 = 0; r.sink64 = r.sb = 0; }   // ranges touch: merge
+        if (strided && tile != 0) r.sink64 = r.sb = 0;
+    }
     r.lo = r.lo64 >> 1;
     r.hi = (r.hi64 == r.lo64) ? r.lo : ((r.hi64 + 1) >> 1);
     if (strided) {
         r.step = 2;
         const int first = r.lo + (((r.lo - it.kb_lo) & 1) != tile ? 1 : 0);       // first block of this parity
-        if (first >= r.hi) { r.hi64 = r.lo64; r.lo = r.hi = first; return r; }   // no block of its own
+        if (first >= r.hi) { r.hi64 = r.lo64; r.lo = r.hi = first; return r; }   // no window block of its own
         r.hi = first + ((r.hi - 1 - first) & ~1) + 1;
         r.lo = first;
     }
     return r;
 }
 
+__device__ __forceinline__ bool has_blocks(const TileRange& r) { return r.sb > 0 || r.hi > r.lo; }
+__device__ __forceinline__ int first_block(const TileRange& r) { return r.sb > 0 ? 0 : r.lo; }
+__device__ __forceinline__ int last_block(const TileRange& r) { return r.hi > r.lo ? r.hi - 1 : r.sb - 1; }
+__device__ __forceinline__ int n_blocks(const TileRange& r) { return r.sb + (r.hi - r.lo + r.step - 1) / r.step; }
+// k-th block of the tile's sequence (sink blocks, then window blocks)
+__device__ __forceinline__ int block_at(const TileRange& r, int k) { return k < r.sb ? k : r.lo + (k - r.sb) * r.step; }
+
 // halves (bit 0 = keys [0, 64), bit 1 = keys [64, 128)) of block j the tile attends to (0: not its block)
 __device__ __forceinline__ int half_mask(const TileRange& r, int j) {
+    if (j < r.sb) return (2 * j < r.sink64 ? 1 : 0) | (2 * j + 1 < r.sink64 ? 2 : 0);
     if (j < r.lo || j >= r.hi || ((j - r.lo) & (r.step - 1))) return 0;
     return ((2 * j >= r.lo64 && 2 * j < r.hi64) ? 1 : 0) | ((2 * j + 1 >= r.lo64 && 2 * j + 1 < r.hi64) ? 2 : 0);
+}
+
+// The blocks the loader puts into the ring for an item: the union of its tiles' sequences, as sink blocks
+// [0, sb) followed by window blocks [lo, hi) (one range [0, hi) when they touch).
+struct ItemBlocks { int sb, lo, hi; };
+template <int NT>
+__device__ __forceinline__ ItemBlocks item_blocks(const ItemDev& it, const SegDev& sg, int TT, int G) {
+    ItemBlocks b;
+    b.sb = 0; b.lo = INT_MAX; b.hi = 0;
+#pragma unroll
+    for (int t = 0; t < NT; ++t) {
+        const TileRange tr = tile_range(it, sg, t, TT, G);
+        if (tr.n_rows == 0) continue;
+        b.sb = max(b.sb, tr.sb);
+        if (tr.hi > tr.lo) { b.lo = min(b.lo, tr.lo); b.hi = max(b.hi, tr.hi); }
+    }
+    if (b.hi <= b.lo) { b.lo = b.hi = b.sb; }
+    else if (b.sb >= b.lo) { b.lo = 0; b.sb = 0; }
+    return b;
 }
 
 }  // namespace
@@ -187,18 +226,17 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
-            int jlo = INT_MAX, jhi = 0;
-            for (int t = 0; t < NT; ++t) {
-                const TileRange tr = tile_range(it, sg, t, TT, G);
-                if (tr.n_rows > 0 && tr.hi > tr.lo) { jlo = min(jlo, tr.lo); jhi = max(jhi, tr.hi); }
-            }
-            // page ids are fetched one block ahead: the dependent global load of block j + 1 is in flight while
-            // block j's copies are issued (decode-shaped items consume a block every ~1500 cycles)
+            const ItemBlocks ib = item_blocks<NT>(it, sg, TT, G);
+            const int n_steps = ib.sb + ib.hi - ib.lo;
+            // page ids are fetched one block ahead: the dependent global load of the next block is in flight
+            // while this block's copies are issued (decode-shaped items consume a block every ~1500 cycles)
             const int* pg = p.pages + sg.page_off - sg.first_page + lane;
-            int page_next = (lane < ppb && jlo < jhi) ? pg[(long long)jlo * ppb] : 0;
-            for (int j = jlo; j < jhi; ++j) {
+            auto blk = [&](int x) { return x < ib.sb ? x : ib.lo + (x - ib.sb); };
+            int page_next = (lane < ppb && n_steps > 0) ? pg[(long long)blk(0) * ppb] : 0;
+            for (int x = 0; x < n_steps; ++x) {
+                const int j = blk(x);
                 const int page = page_next;
-                if (lane < ppb && j + 1 < jhi) page_next = pg[(long long)(j + 1) * ppb];
+                if (lane < ppb && x + 1 < n_steps) page_next = pg[(long long)blk(x + 1) * ppb];
                 for (int kv = 0; kv < 2; ++kv) {
                     const uint32_t st = fill % C::kStages, ph = (fill / C::kStages) & 1;
                     TRACE(1, j * 2 + kv);
@@ -280,7 +318,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                     mbar_wait(smem_u32(&bars.p_full[t][1]), n_p[t] & 1);
                     ++n_p[t];
                 }
-                if (do_qk && j == tr[t].lo) {
+                if (do_qk && j == first_block(tr[t])) {
                     mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
                     ++n_q[t];
                 }
@@ -317,15 +355,15 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                             }
                         }
                         tc_commit(smem_u32(&bars.s_full[t]));
-                        if (j + 1 == tr[t].hi) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
+                        if (j == last_block(tr[t])) tc_commit(smem_u32(&bars.q_empty[t]));   // Q_t may be refilled
                     }
                 }
                 __syncwarp();
                 TRACE(13 + t * 4, j);
                 pv_valid[t] = do_qk;
                 pv_mask[t] = am;
-                pv_first[t] = do_qk && j == tr[t].lo;
-                pv_last[t] = do_qk && j + 1 == tr[t].hi;
+                pv_first[t] = do_qk && j == first_block(tr[t]);
+                pv_last[t] = do_qk && j == last_block(tr[t]);
             };
             // A tile with no pending PV can have its QK^T issued at once; one with a pending PV first waits
             // for its softmax warpgroup.  Serve the former first (strided items: the two tiles alternate blocks,
@@ -344,27 +382,31 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             __syncwarp();
         };
 
-        for (int ii = i_lo; ii < i_hi; ++ii) {
-            const ItemDev it = p.items[ii];
-            const SegDev sg = p.segs[it.seg];
-            int jlo = INT_MAX, jhi = 0;
+        // (one pass more than there are items: the last one only flushes the PV of the very last block; `step`
+        // has a single call site on purpose -- it is large and every copy costs instruction-cache space)
+        for (int ii = i_lo; ii <= i_hi; ++ii) {
+            const bool flush = ii == i_hi;
+            ItemBlocks ib;
+            ib.sb = 0; ib.lo = 0; ib.hi = 1;
+            if (!flush) {
+                const ItemDev it = p.items[ii];
+                const SegDev sg = p.segs[it.seg];
+                ib = item_blocks<NT>(it, sg, TT, G);
 #pragma unroll
-            for (int t = 0; t < NT; ++t) {
-                tr[t] = tile_range(it, sg, t, TT, G);
-                if (tr[t].n_rows > 0 && tr[t].hi > tr[t].lo) { jlo = min(jlo, tr[t].lo); jhi = max(jhi, tr[t].hi); }
+                for (int t = 0; t < NT; ++t) tr[t] = tile_range(it, sg, t, TT, G);
+#pragma unroll
+                for (int t = 0; t < NT; ++t)
+                    if (tr[t].n_rows > 0 && !has_blocks(tr[t])) {
+                        // tile present but no block of its own in this (split) item: hand Q straight back
+                        mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
+                        ++n_q[t];
+                        if (elect_one()) tc_commit(smem_u32(&bars.q_empty[t]));
+                        __syncwarp();
+                    }
             }
-#pragma unroll
-            for (int t = 0; t < NT; ++t)
-                if (tr[t].n_rows > 0 && tr[t].hi <= tr[t].lo) {
-                    // tile present but no block of its own in this (split) item: hand Q straight back
-                    mbar_wait(smem_u32(&bars.q_full[t]), n_q[t] & 1);
-                    ++n_q[t];
-                    if (elect_one()) tc_commit(smem_u32(&bars.q_empty[t]));
-                    __syncwarp();
-                }
-            for (int j = jlo; j < jhi; ++j) step(true, j);
+            const int n_steps = ib.sb + ib.hi - ib.lo;
+            for (int x = 0; x < n_steps; ++x) step(!flush, x < ib.sb ? x : ib.lo + (x - ib.sb));
         }
-        step(false, 0);   // PV of the very last block
     } else if (warp == kQWarp) {
         // ------------------------------------------------------------------ Q loader (TMA)
         // Q tile image: [D/64 halves][128 rows][128 B], SWIZZLE_128B; row r = (token, group head) as the
@@ -437,15 +479,19 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const bool warp_has_rows = wq * 32 < tr.n_rows;  // decode-shaped tiles: most warps hold no row
                 float m_used = -INFINITY, l = 0.f;
 
-                for (int j = tr.lo; j < tr.hi; j += tr.step) {
+                const int nb = n_blocks(tr);
+                for (int kb = 0; kb < nb; ++kb) {
+                    const int j = block_at(tr, kb);
                     TRACE(20, j);
                     mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
                     ++n_s;
                     tc_fence_after();
                     TRACE(21, j);
                     if (warp_has_rows) {
-                        const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;   // valid columns [cmin, cmax]
-                        const bool need_mask = __any_sync(0xffffffffu, cmin > 0 || cmax < kBlockKeys - 1);
+                        // visible columns of this block: c <= cmax and (c >= cmin or c < csink)
+                        const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;
+                        const int csink = sg.n_sink - j * kBlockKeys;        // same for every row of the segment
+                        const bool need_mask = __any_sync(0xffffffffu, cmax < kBlockKeys - 1 || (cmin > 0 && csink < kBlockKeys));
                         // the whole score row of this thread: 128 fp32 columns -> registers, one wait
                         uint32_t s[kBlockKeys];
 #pragma unroll
@@ -454,18 +500,31 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         TRACE(22, j);
                         bool dead[4] = {false, false, false, false};   // 32-column chunk masked for every row of the warp
                         if (need_mask) {
-                            // boundary block (causal diagonal / window edge).  Per 32-column chunk, warp-uniformly:
+                            // boundary block (causal diagonal / window edge / sink edge).  Per 32-column chunk, warp-uniformly:
                             // all visible -> untouched; all masked -> no exp at all; ragged -> element mask in registers
                             const int mn_cmin = __reduce_min_sync(0xffffffffu, cmin), mx_cmin = __reduce_max_sync(0xffffffffu, cmin);
                             const int mn_cmax = __reduce_min_sync(0xffffffffu, cmax), mx_cmax = __reduce_max_sync(0xffffffffu, cmax);
+                            if (sg.n_sink == 0) {
 #pragma unroll
-                            for (int c = 0; c < 4; ++c) {
-                                const int c0 = 32 * c, c1 = 32 * c + 31;
-                                dead[c] = c1 < mn_cmin || c0 > mx_cmax;
-                                if (!(c0 >= mx_cmin && c1 <= mn_cmax)) {
+                                for (int c = 0; c < 4; ++c) {
+                                    const int c0 = 32 * c, c1 = 32 * c + 31;
+                                    dead[c] = c0 > mx_cmax || c1 < mn_cmin;
+                                    if (!(c1 <= mn_cmax && c0 >= mx_cmin)) {
 #pragma unroll
-                                    for (int e = 0; e < 32; ++e)
-                                        if (c0 + e < cmin || c0 + e > cmax) s[c0 + e] = 0xff800000u;   // -inf
+                                        for (int e = 0; e < 32; ++e)
+                                            if (c0 + e > cmax || c0 + e < cmin) s[c0 + e] = 0xff800000u;   // -inf
+                                    }
+                                }
+                            } else {   // with sinks the visible columns are two intervals: [0, csink) and [cmin, cmax]
+#pragma unroll
+                                for (int c = 0; c < 4; ++c) {
+                                    const int c0 = 32 * c, c1 = 32 * c + 31;
+                                    dead[c] = c0 > mx_cmax || (c1 < mn_cmin && c0 >= csink);
+                                    if (!(c1 <= mn_cmax && (c0 >= mx_cmin || c1 < csink))) {
+#pragma unroll
+                                        for (int e = 0; e < 32; ++e)
+                                            if (c0 + e > cmax || (c0 + e < cmin && c0 + e >= csink)) s[c0 + e] = 0xff800000u;
+                                    }
                                 }
                             }
                         }
@@ -488,7 +547,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                                 m_used = mx2;
                                 l *= corr;
                             }
-                            if (j > tr.lo) {
+                            if (kb > 0) {
 #pragma unroll 1
                                 for (int c = 0; c < D / 16; ++c) {
                                     uint32_t v[16];
@@ -578,7 +637,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const TileRange tr = tile_range(it, sg, tile, TT, G);
                 if (tr.n_rows == 0) continue;
                 const uint32_t tO = tmem + lane_base + 256 + tile * 128;
-                const bool has_blocks = tr.hi > tr.lo;
+                const bool has_blk = has_blocks(tr);
                 const int rc = min(r, tr.n_rows - 1);
                 const int tok = tr.tok0 + rc / G;
                 const bool valid = r < tr.n_rows;
@@ -589,7 +648,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 ++n_st[tile];
                 const float2 ml = stats[tile][r];
                 mbar_arrive(smem_u32(&bars.stat_free[tile]));
-                if (has_blocks) {
+                if (has_blk) {
                     mbar_wait(smem_u32(&bars.o_final[tile]), n_o[tile] & 1);
                     ++n_o[tile];
                     tc_fence_after();
@@ -601,7 +660,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
 #pragma unroll 1
                     for (int c = 0; c < D / 16; ++c) {
                         uint32_t v[16];
-                        if (has_blocks) { tmem_ld16(tO + c * 16, v); tmem_wait_ld(); }
+                        if (has_blk) { tmem_ld16(tO + c * 16, v); tmem_wait_ld(); }
                         else {
 #pragma unroll
                             for (int e = 0; e < 16; ++e) v[e] = 0u;
@@ -638,7 +697,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                     }
                     if (valid && p.lse) p.lse[(long long)head * p.lse_stride + row] = (ml.x + log2f(ml.y)) * 0.6931471805599453f;
                 }
-                if (has_blocks) {
+                if (has_blk) {
                     tc_fence_before();
                     mbar_arrive(smem_u32(&bars.o_free[tile]));   // O_t may be overwritten by the next item
                 }

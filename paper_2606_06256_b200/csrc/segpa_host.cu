@@ -447,7 +447,7 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 jb.page_off = (long long)touched.size();
                 jb.first_slot = (int)(cur_len % P);
                 jb.n_pages = (int)need + (cur_len % P != 0 ? 1 : 0);
-                if (cur_len % P != 0) touched.push_back(rec.pages.back());
+                if (cur_len % P != 0) touched.push_back(rec.pages.back());   // (a partial last page is never a hole: evict_pages refuses it)
                 total_chunks += ((long long)jb.n_pages * P - jb.first_slot) * (D >> 3);
                 jobs.push_back(jb);
             }
@@ -508,6 +508,26 @@ segpa_status_t segpa_append_pages(segpa_cache_t* c, int32_t layer, int32_t kv_he
     return segpa_append_pages_batch(c, &r, 1, cuda_stream);
 }
 
+segpa_status_t segpa_evict_pages(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                 int32_t first_page_index, int32_t n_pages) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "evict_pages: null cache");
+    auto it = c->streams.find(StreamKey{layer, kv_head, seq_id});
+    if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "evict_pages: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
+    StreamRec& rec = it->second;
+    const int P = c->desc.page_size;
+    if (first_page_index < 0 || n_pages < 1 || (int64_t)first_page_index + n_pages > (int64_t)rec.pages.size())
+        return fail(SEGPA_ERR_INVALID, "evict_pages: range [%d, %d) outside the stream's %zu pages", first_page_index, first_page_index + n_pages, rec.pages.size());
+    if (rec.kv_len % P != 0 && (size_t)first_page_index + n_pages == rec.pages.size())
+        return fail(SEGPA_ERR_INVALID, "evict_pages: the stream's partial last page cannot be evicted");
+    for (int32_t i = 0; i < n_pages; ++i)
+        if (rec.pages[(size_t)first_page_index + i] < 0) return fail(SEGPA_ERR_INVALID, "evict_pages: page index %d is already evicted", first_page_index + i);
+    for (int32_t i = 0; i < n_pages; ++i) {
+        release_page(c, rec.pages[(size_t)first_page_index + i]);
+        rec.pages[(size_t)first_page_index + i] = -1;
+    }
+    return SEGPA_OK;
+}
+
 segpa_status_t segpa_clear_streams(segpa_cache_t* c) {
     if (!c) return fail(SEGPA_ERR_INVALID, "clear_streams: null cache");
     c->streams.clear();
@@ -522,7 +542,8 @@ segpa_status_t segpa_free_stream(segpa_cache_t* c, int32_t layer, int32_t kv_hea
     if (!c) return fail(SEGPA_ERR_INVALID, "free_stream: null cache");
     auto it = c->streams.find(StreamKey{layer, kv_head, seq_id});
     if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "free_stream: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
-    for (auto id : it->second.pages) release_page(c, id);
+    for (auto id : it->second.pages)
+        if (id >= 0) release_page(c, id);
     c->streams.erase(it);
     return SEGPA_OK;
 }
@@ -567,7 +588,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
     S->cache = c;
     S->layer = layer;
     S->tiles_per_item = tiles_per_item;
-    struct TileTmp { int seg, t0, n_tok, kb_lo, kb_hi; };
+    struct TileTmp { int seg, t0, n_tok, kb_lo, kb_hi, cost; bool sink; };
     std::vector<TileTmp> tiles;
     int64_t q_rows = 0, pairs = 0, vis_tokens = 0;
     try {
@@ -587,14 +608,18 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             if (r.head_class == SEGPA_LOCAL && r.window < 1) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: LOCAL window %d < 1", s, r.window); }
             if (r.q_row_start < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: negative q_row_start", s); }
             if (r.n_sink < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: negative n_sink", s); }
-            if (r.n_sink != 0 && r.head_class == SEGPA_LOCAL) { delete S; return fail(SEGPA_ERR_UNSUPPORTED, "build_segments: segment %d: n_sink %d (sink tokens are not implemented on the GPU yet)", s, r.n_sink); }
             ivs.push_back(Iv{r.kv_head, r.q_row_start, r.q_row_start + r.q_len});
 
             const int64_t kv_len = rec.kv_len;
             const int64_t W = (r.head_class == SEGPA_GLOBAL) ? (int64_t)INT32_MAX / 2 : r.window;
             // Alg. 2 lines 6-10: visible positions of the whole segment
             const int64_t vis_lo = std::max<int64_t>(0, kv_len - r.q_len - W + 1);
-            const int64_t seg_kb_lo = vis_lo / kBlockKeys;
+            // S_sink: the first n_sink tokens stay visible to a LOCAL head; they matter only when
+            // some query's window starts after position 0 (the last query's does iff kv_len > W)
+            const int64_t ns = (r.head_class == SEGPA_LOCAL) ? std::min<int64_t>(r.n_sink, kv_len) : 0;
+            const bool has_sink = ns > 0 && kv_len > W;
+            const int64_t sink_pages = has_sink ? std::min(cdiv(std::min(ns, vis_lo), P), vis_lo / P) : 0;   // pages wholly before the window's first page
+            const int64_t seg_kb_lo = has_sink ? 0 : vis_lo / kBlockKeys;
             const int64_t seg_kb_hi = (kv_len - 1) / kBlockKeys + 1;
             const int64_t first_vis_page = vis_lo / P;
             const int64_t n_stream_pages = cdiv(kv_len, P);
@@ -605,28 +630,45 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             sd.kv_len = (int)kv_len;
             sd.head_class = r.head_class;
             sd.window = (int)W;
-            sd.n_sink = 0;
+            sd.n_sink = has_sink ? (int)ns : 0;
             sd.kv_head = r.kv_head;
             sd.first_page = (int)(seg_kb_lo * ppb);
             sd.n_pages_listed = (int)((seg_kb_hi - seg_kb_lo) * ppb);
-            // Alg. 2 line 12: Translate(T_page, U_h); invisible / absent pages -> the zero page
+            // Alg. 2 line 12: Translate(T_page, U_h): sink pages and recent-window pages (lines 9-10); invisible
+            // pages (the evicted middle) and absent ones -> the zero page, never read
             {
                 const int64_t lst_lo = sd.first_page, lst_hi = sd.first_page + sd.n_pages_listed;
                 const int64_t vis_a = std::max(lst_lo, first_vis_page), vis_b = std::min(lst_hi, n_stream_pages);
-                S->pages.insert(S->pages.end(), (size_t)(vis_a - lst_lo), zero_page);
+                for (int64_t pg = 0; pg < sink_pages; ++pg)
+                    if (rec.pages[(size_t)pg] < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: sink page %lld of the stream was evicted", s, (long long)pg); }
+                for (int64_t pg = vis_a; pg < vis_b; ++pg)
+                    if (rec.pages[(size_t)pg] < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: visible page %lld of the stream was evicted", s, (long long)pg); }
+                S->pages.insert(S->pages.end(), rec.pages.begin(), rec.pages.begin() + sink_pages);
+                S->pages.insert(S->pages.end(), (size_t)(vis_a - lst_lo - sink_pages), zero_page);
                 S->pages.insert(S->pages.end(), rec.pages.begin() + vis_a, rec.pages.begin() + vis_b);
                 S->pages.insert(S->pages.end(), (size_t)(lst_hi - vis_b), zero_page);
             }
             S->segs.push_back(sd);
-            vis_tokens += kv_len - first_vis_page * P;
+            vis_tokens += kv_len - first_vis_page * P + sink_pages * P;
             q_rows = std::max<int64_t>(q_rows, r.q_row_start + r.q_len);
             pairs += visible_pairs(kv_len - r.q_len, kv_len - 1, W);
+            if (has_sink)   // sink keys not already inside the window
+                for (int64_t i = kv_len - r.q_len; i < kv_len; ++i) pairs += std::max<int64_t>(0, std::min(ns, i - W + 1));
             // tiles: exactly the KV blocks the tile's rows attend to
             for (int64_t t0 = 0; t0 < r.q_len; t0 += item_tok) {
                 const int64_t n_tok = std::min<int64_t>(item_tok, r.q_len - t0);
                 const int64_t i0 = kv_len - r.q_len + t0, i1 = i0 + n_tok - 1;
                 const int64_t lo = std::max<int64_t>(0, i0 - W + 1);
-                tiles.push_back(TileTmp{s, (int)t0, (int)n_tok, (int)(lo / kBlockKeys), (int)(i1 / kBlockKeys + 1)});
+                TileTmp tt{s, (int)t0, (int)n_tok, (int)(lo / kBlockKeys), (int)(i1 / kBlockKeys + 1), 0, false};
+                tt.cost = tt.kb_hi - tt.kb_lo;
+                if (has_sink) {
+                    // two KV block ranges: sink blocks [0, sb) then the window blocks; one range when they touch
+                    const int sb = (int)cdiv(std::min(ns, i1 + 1), kBlockKeys);
+                    tt.cost = (sb >= tt.kb_lo) ? tt.kb_hi : sb + tt.kb_hi - tt.kb_lo;
+                    tt.kb_lo = 0;
+                    tt.sink = true;
+                }
+                tiles.push_back(tt);
             }
         }
         // overlap check on (row, head): same kv_head (hence same q heads) and intersecting rows
@@ -637,14 +679,14 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         // scheduler: split long tiles along KV when the grid would be unbalanced, then order
         // longest-first; CTAs pull items from a shared cursor (greedy LPT).
         int64_t total_cost = 0;
-        for (auto& t : tiles) total_cost += t.kb_hi - t.kb_lo;
+        for (auto& t : tiles) total_cost += t.cost;
         const int64_t chunk = std::max<int64_t>(8, cdiv(total_cost, (int64_t)c->num_sms * 4));
         int n_split_tiles = 0, n_slots = 0;
         for (size_t ti = 0; ti < tiles.size(); ++ti) {
             const TileTmp& t = tiles[ti];
-            const int cost = t.kb_hi - t.kb_lo;
+            const int cost = t.cost;
             int parts = 1;
-            if (cost > chunk + chunk / 2) parts = (int)cdiv(cost, chunk);
+            if (cost > chunk + chunk / 2 && !t.sink) parts = (int)cdiv(cost, chunk);   // (sink items are not cut along KV)
             // Decode-shaped tile (all its rows fit the first of the item's two tile slots): run it STRIDED -- the
             // two slots take alternate KV blocks of the same rows as two independent chains, each writing a
             // partial that the combine kernel merges -- so the second slot is not left idle.
@@ -653,10 +695,10 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             if (parts > 1 || strided)
                 S->combs.push_back(CombDev{t.seg, t.t0, t.n_tok, n_slots, parts, strided ? 1 : 0, 0, 0});
             for (int p = 0; p < parts; ++p) {
-                const int lo = t.kb_lo + (int)((int64_t)cost * p / parts);
-                const int hi = t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
+                const int lo = t.sink ? t.kb_lo : t.kb_lo + (int)((int64_t)cost * p / parts);
+                const int hi = t.sink ? t.kb_hi : t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
                 const int slot = (parts > 1 || strided) ? n_slots++ : -1;
-                S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, 0});
+                S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, t.sink ? t.cost : hi - lo});
                 S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti, 0, 0});
             }
         }
@@ -667,7 +709,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         std::vector<int> order(S->items.size());
         for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
         std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
-            return (S->items[a].kb_hi - S->items[a].kb_lo) > (S->items[b].kb_hi - S->items[b].kb_lo);
+            return S->items[a].cost > S->items[b].cost;
         });
         std::vector<std::vector<int>> per_cta((size_t)n_cta);
         {
@@ -678,7 +720,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 Load ld = heap.top();
                 heap.pop();
                 per_cta[(size_t)ld.second].push_back(idx);
-                const int64_t blocks3 = 3 * (int64_t)(S->items[idx].kb_hi - S->items[idx].kb_lo);
+                const int64_t blocks3 = 3 * (int64_t)S->items[idx].cost;
                 ld.first += ((S->items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2;   // strided: two chains
                 heap.push(ld);
             }
@@ -695,7 +737,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 segpa_item_t pub = S->items_pub[idx];
                 pub.cta = q;
                 ip2.push_back(pub);
-                kv_blocks += S->items[idx].kb_hi - S->items[idx].kb_lo;
+                kv_blocks += S->items[idx].cost;
             }
             S->cta_off[(size_t)q + 1] = (int32_t)it2.size();
         }

@@ -50,7 +50,7 @@ struct ItemDev {
     int kb_hi;
     int partial_slot;       // -1: final result written to out/lse; else split-KV partial slot
     int flags;              // bit 0: strided (both tiles hold the same rows and take alternate KV blocks)
-    int pad1;
+    int cost;               // KV blocks the item visits (scheduling only; < kb_hi - kb_lo for sink segments)
 };
 
 struct CombDev {

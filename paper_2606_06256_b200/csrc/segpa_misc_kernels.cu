@@ -166,7 +166,10 @@ __global__ void attention_simt_kernel(FwdParams p) {
             float m = -INFINITY, l = 0.f;
             int jlo = max(it.kb_lo * kBlockKeys, i - sg.window + 1);
             int jhi = min(it.kb_hi * kBlockKeys - 1, i);
-            for (int j = jlo; j <= jhi; ++j) {
+            // visible keys: sink tokens [0, n_sink) not already inside the window, then the window
+            const int n_sink_keys = (it.kb_lo == 0) ? min(sg.n_sink, jlo) : 0;
+            for (int jj = 0; jj < n_sink_keys + max(0, jhi - jlo + 1); ++jj) {
+                const int j = jj < n_sink_keys ? jj : jlo + (jj - n_sink_keys);
                 const int pg = j / p.P, slot = j % p.P;
                 const int page = p.pages[sg.page_off + (pg - sg.first_page)];
                 const size_t off = (size_t)page * p.page_bytes;

@@ -67,6 +67,55 @@ def test_ragged_small(case, kernel, tiles):
     print(_run_full(w, kernel, tiles, "ragged%d" % case))
 
 
+SINKS = [
+    # Hq, Hkv, D, P, requests with n_sink > 0 (W(i) = S_sink U [i - w, i])
+    # prefill: sinks of 4 (the paper's GQA setting), of one page, and spanning more than one 128-key block
+    (8, 2, 128, 16, [{"kv_len": 3000, "heads": {0: (LOCAL, 300, 4, 3000), 1: (LOCAL, 257, 200, 1500)}}]),
+    # sink block touching / overlapping the window (merged range, gap masked per element), W = 1
+    (8, 2, 128, 16, [{"kv_len": 700, "heads": {0: (LOCAL, 100, 128, 700), 1: (LOCAL, 1, 16, 700)}}]),
+    # decode with the paper's prefix-compression setting (W = 4096, sink = 128) and G = 7, P = 32
+    (28, 4, 128, 32, [{"kv_len": 20000 + 77 * r, "heads": {0: (LOCAL, 4096, 128, 1), 1: (LOCAL, 4096, 128, 3), 2: (GLOBAL, 0, 128, 1), 3: (LOCAL, 500, 4, 1)}} for r in range(3)]),
+    # n_sink larger than the stream, sinks inside the window from the start
+    (8, 2, 64, 16, [{"kv_len": 300, "heads": {0: (LOCAL, 64, 1000, 300), 1: (LOCAL, 200, 150, 10)}}]),
+]
+
+
+@pytest.mark.parametrize("kernel,tiles", VARIANTS)
+@pytest.mark.parametrize("case", range(len(SINKS)))
+def test_sinks(case, kernel, tiles):
+    Hq, Hkv, D, P, reqs = SINKS[case]
+    w = wl.make_workload("sinks%d" % case, Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=1200 + case)
+    print(_run_full(w, kernel, tiles, "sinks%d" % case))
+
+
+def test_true_eviction_between_sinks_and_window():
+    """the middle of a LOCAL head's stream is evicted, its physical pages are reused by another
+    stream holding NaN / 1e30; the head's result is unchanged and still matches the oracle."""
+    reqs = [{"kv_len": 9000, "heads": {0: (LOCAL, 1024, 128, 40), 1: (LOCAL, 2048, 4, 1)}}]
+    w = wl.make_workload("evict", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=31)
+    dev = torch.device("cuda:0")
+    k, v = wl.pool_values(w, dev)
+    g = GpuRun(w, "tc", 2, k, v)
+    try:
+        q, o1, l1 = g.layer(0)
+        print(compare(w, 0, k, v, q, o1, l1, label="evict: before"))
+        sm = w.stream_map()
+        junk_seq = 77
+        for h, (W, ns, ql) in {0: (1024, 128, 40), 1: (2048, 4, 1)}.items():
+            st = sm[(0, h, 0)]
+            lo, hi = (ns + 15) // 16, (9000 - ql - W + 1) // 16
+            B.segpa_evict_pages(g.cache, 0, h, 0, lo, hi - lo)
+            n_tok = (hi - lo) * 16
+            bad_k = torch.full((n_tok, 128), float("nan"), dtype=torch.bfloat16, device=dev)
+            bad_v = torch.full((n_tok, 128), 1e30, dtype=torch.bfloat16, device=dev)
+            B.segpa_append_pages(g.cache, 0, h, junk_seq, bad_k, bad_v, n_tok, page_ids=st.page_ids[lo:hi])
+        g.segs.pop(0)
+        _, o2, l2 = g.layer(0, q)
+        assert torch.equal(o1, o2) and torch.equal(l1, l2)
+    finally:
+        g.close()
+
+
 @pytest.mark.parametrize("kernel,tiles", VARIANTS)
 def test_decode_split_kv(kernel, tiles):
     """Decode-shaped: few rows, long KV -> the scheduler splits along KV and the combine kernel merges."""

@@ -214,7 +214,7 @@ def test_build_segments_rejections():
         ([(0, 2, GLOBAL, 0, 0, 0, 5)], B.ERR_INVALID),                   # kv_head out of range
         ([(0, 0, GLOBAL, 0, 0, -1, 5)], B.ERR_INVALID),                  # negative row
         ([(0, 0, GLOBAL, 0, 0, 0, 50), (0, 0, LOCAL, 8, 0, 49, 10)], B.ERR_INVALID),   # (row, head) overlap
-        ([(0, 0, LOCAL, 8, 4, 0, 5)], B.ERR_UNSUPPORTED),                # sinks: NEXT #1
+        ([(0, 0, LOCAL, 8, -1, 0, 5)], B.ERR_INVALID),                   # negative n_sink
         ([], B.ERR_INVALID),
     ]
     for reqs, st in bad:
@@ -226,6 +226,49 @@ def test_build_segments_rejections():
     assert B.segpa_segments_stats(segs)["n_segments"] == 3
     with pytest.raises(B.SegpaError):
         B.segpa_build_segments(c, 1, [(0, 0, GLOBAL, 0, 0, 0, 5)])       # layer out of range
+    B.segpa_destroy(c)
+
+
+def test_sinks_select_two_page_ranges_and_eviction_is_checked():
+    """LOCAL with sinks (Alg. 2 lines 9-10): sink pages + recent-window pages are translated, the
+    middle maps to the zero page and may be evicted; an evicted VISIBLE page is an error."""
+    P, n_pages_pool = 16, 512
+    c = plan_cache(P=P, num_pages=n_pages_pool)
+    kv_len, q_len, W, n_sink = 5000, 3, 700, 40
+    ids = np.arange(100, 100 + (kv_len + P - 1) // P)
+    B.segpa_append_pages(c, 0, 0, 0, None, None, kv_len, page_ids=ids)
+    segs = B.segpa_build_segments(c, 0, [(0, 0, LOCAL, W, n_sink, 0, q_len)])
+    first, pages = B.segpa_segments_pages(segs, 0)
+    assert first == 0
+    vis_lo = kv_len - q_len - W + 1
+    for pg, got in enumerate(pages):
+        in_sink = pg * P < n_sink
+        in_win = (pg + 1) * P > vis_lo and pg < len(ids)
+        assert got == (ids[pg] if (in_sink or in_win) else n_pages_pool), pg
+    st = B.segpa_segments_stats(segs)
+    want = sum(min(i + 1, W) + max(0, min(n_sink, i - W + 1)) for i in range(kv_len - q_len, kv_len)) * 4
+    assert st["attended_pairs"] == want
+    it = B.segpa_segments_items(segs)
+    assert len(it) == 1 and it[0]["kb_lo"] == 0 and st["kv_blocks"] == 1 + (kv_len - 1) // 128 + 1 - vis_lo // 128
+    # evict the middle: fine; evict into the window or the sinks: build fails
+    mid_lo, mid_hi = (n_sink + P - 1) // P, vis_lo // P
+    B.segpa_evict_pages(c, 0, 0, 0, mid_lo, mid_hi - mid_lo)
+    assert B.segpa_pool_stats(c)[0] == len(ids) - (mid_hi - mid_lo)
+    assert list(B.segpa_stream_info(c, 0, 0, 0)[1][mid_lo:mid_lo + 2]) == [-1, -1]
+    segs2 = B.segpa_build_segments(c, 0, [(0, 0, LOCAL, W, n_sink, 0, q_len)])
+    assert list(B.segpa_segments_pages(segs2, 0)[1]) == list(pages)
+    with pytest.raises(B.SegpaError):
+        B.segpa_evict_pages(c, 0, 0, 0, mid_lo, 1)                        # already evicted
+    with pytest.raises(B.SegpaError):
+        B.segpa_evict_pages(c, 0, 0, 0, len(ids) - 1, 1)                  # partial last page
+    B.segpa_evict_pages(c, 0, 0, 0, mid_hi, 1)                            # first window page
+    with pytest.raises(B.SegpaError) as e:
+        B.segpa_build_segments(c, 0, [(0, 0, LOCAL, W, n_sink, 0, q_len)])
+    assert e.value.status == B.ERR_INVALID
+    with pytest.raises(B.SegpaError):
+        B.segpa_build_segments(c, 0, [(0, 0, GLOBAL, 0, 0, 0, q_len)])    # a global head needs every page
+    B.segpa_free_stream(c, 0, 0, 0)
+    assert B.segpa_pool_stats(c) == (0, n_pages_pool)
     B.segpa_destroy(c)
 
 
