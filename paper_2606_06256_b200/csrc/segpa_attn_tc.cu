@@ -509,7 +509,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                                 for (int c = 0; c < 4; ++c) {
                                     const int c0 = 32 * c, c1 = 32 * c + 31;
                                     dead[c] = c0 > mx_cmax || c1 < mn_cmin;
-                                    if (!(c1 <= mn_cmax && c0 >= mx_cmin)) {
+                                    if (!dead[c] && !(c1 <= mn_cmax && c0 >= mx_cmin)) {
 #pragma unroll
                                         for (int e = 0; e < 32; ++e)
                                             if (c0 + e > cmax || c0 + e < cmin) s[c0 + e] = 0xff800000u;   // -inf
@@ -520,7 +520,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                                 for (int c = 0; c < 4; ++c) {
                                     const int c0 = 32 * c, c1 = 32 * c + 31;
                                     dead[c] = c0 > mx_cmax || (c1 < mn_cmin && c0 >= csink);
-                                    if (!(c1 <= mn_cmax && (c0 >= mx_cmin || c1 < csink))) {
+                                    if (!dead[c] && !(c1 <= mn_cmax && (c0 >= mx_cmin || c1 < csink))) {
 #pragma unroll
                                         for (int e = 0; e < 32; ++e)
                                             if (c0 + e > cmax || (c0 + e < cmin && c0 + e >= csink)) s[c0 + e] = 0xff800000u;
@@ -528,15 +528,20 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                                 }
                             }
                         }
-                        float mxa = -INFINITY, mxb = -INFINITY, mxc = -INFINITY, mxd = -INFINITY;
+                        // row max: one pair of chains per 32-column chunk, no branches; a dead chunk (left holding raw,
+                        // possibly stale scores) is dropped by a select.  max.f32 returns the non-NaN operand.
+                        float mc[4];
 #pragma unroll
-                        for (int e = 0; e < kBlockKeys; e += 8) {
-                            mxa = max3(mxa, __uint_as_float(s[e + 0]), __uint_as_float(s[e + 1]));
-                            mxb = max3(mxb, __uint_as_float(s[e + 2]), __uint_as_float(s[e + 3]));
-                            mxc = max3(mxc, __uint_as_float(s[e + 4]), __uint_as_float(s[e + 5]));
-                            mxd = max3(mxd, __uint_as_float(s[e + 6]), __uint_as_float(s[e + 7]));
+                        for (int c = 0; c < 4; ++c) {
+                            float ma = -INFINITY, mb = -INFINITY;
+#pragma unroll
+                            for (int e = 32 * c; e < 32 * c + 32; e += 4) {
+                                ma = max3(ma, __uint_as_float(s[e + 0]), __uint_as_float(s[e + 1]));
+                                mb = max3(mb, __uint_as_float(s[e + 2]), __uint_as_float(s[e + 3]));
+                            }
+                            mc[c] = dead[c] ? -INFINITY : fmaxf(ma, mb);
                         }
-                        const float mx = fmaxf(fmaxf(mxa, mxb), fmaxf(mxc, mxd));
+                        const float mx = fmaxf(fmaxf(mc[0], mc[1]), fmaxf(mc[2], mc[3]));
                         const float mx2 = mx * sl2;
                         // lazy rescale (warp-uniform decision: tcgen05.ld/st are warp-collective)
                         const bool grow = mx2 > m_used + kRescaleThreshold;
