@@ -6,8 +6,8 @@ input, all through the C ABI (include/segpa.h):
     segpa_append_pages   (a1: scatter the batch's K/V rows, resident in HBM, into per-head pages)
     segpa_build_segments (a2-a5: page selection, translation, descriptor packing, tile schedule, H2D)
     segpa_attention_fwd  (a6-a8: fused attention [+ split-KV combine]; heads merged by layout)
-Default workload: BASELINE.json configs[1] (Llama-3-8B-shaped layer).  `--config {1..5,4d}` selects
-another one for profiling.  Multi-GPU: the path does not shard (BASELINE north_star: one GPU, no
+Default workload: BASELINE.json configs[1] (Llama-3-8B-shaped layer).  `--config {1..5,4d,fig9-{decode,prefill}-{8,32,128}k}`
+selects another one.  Multi-GPU: the path does not shard (BASELINE north_star: one GPU, no
 collectives) -> N independent replicas, "scaling": "weak".
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C]
@@ -62,6 +62,9 @@ def get_workload(name: str):
     from paper_2606_06256_b200 import workloads as wl
     if name == "4d":
         return wl.config4(decode_only=True)
+    if name.startswith("fig9-"):      # fig9-decode-8k, fig9-prefill-32k, ...: the paper's micro-benchmark shape
+        _, mode, ctx = name.split("-")
+        return wl.fig9(int(ctx.rstrip("k")) * 1024, mode)
     return wl.CONFIGS[int(name)]()
 
 
@@ -362,7 +365,7 @@ def run_ours(args):
         cov_rows = sum(s.q_len * w.G for s in w.layer_segments(l))
         alg_bytes += st["visible_kv_tokens"] * w.D * 2 * 2 + cov_rows * w.D * 2 * 2 + cov_rows * 4
     torch.cuda.synchronize()
-    decode_shaped = args.config == "4d"
+    decode_shaped = args.config == "4d" or args.config.startswith("fig9-decode")
     if decode_shaped:
         roof = {"bound": "hbm", "achieved": alg_bytes / (fwd_mean * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
     else:

@@ -388,4 +388,21 @@ def config5(num_layers: int = 28) -> Workload:
     return w
 
 
+def fig9(L: int, mode: str, num_layers: int = 8) -> Workload:
+    """The paper's own kernel-isolated micro-benchmark shape (Fig. 9(e)-(h)): Qwen3-32B-shaped
+    layers, Hq 32 / Hkv 8 (GQA-4), D 128, bf16; half of the KV heads GLOBAL (full context), half LOCAL with a
+    320-token visible set (sink + recent: n_sink 4 + W 316); contexts 8K / 32K / 128K; one request.
+    mode "decode": q_len 1; mode "prefill": q_len = L (the paper does not state its prefill query length).
+    The paper runs 64 layers sequentially; here `num_layers` distinct layers are generated (enough that the
+    KV of consecutive launches never sits in L2 together) and the 64-layer figure is per-layer time x 64."""
+    assert mode in ("decode", "prefill")
+    seed = BASE_SEED + 9 + (0 if mode == "decode" else 1) + L
+    Hq, Hkv, D, P = 32, 8, 128, 16
+    q_len = 1 if mode == "decode" else L
+    heads = {h: ((GLOBAL, 0, 0, q_len) if h < 4 else (LOCAL, 316, 4, q_len)) for h in range(Hkv)}
+    w = make_workload("fig9_%s_%dk" % (mode, L // 1024), Hq=Hq, Hkv=Hkv, D=D, P=P, seed=seed, num_layers=num_layers,
+                      requests=[{"kv_len": L, "heads": heads}])
+    return w
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
