@@ -410,6 +410,66 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_rope(args):
+    """`--config rope`: the step before the hot path (RoPEAlign) on its own:
+    K of every stream of cfg3 (8 KV heads x 65536 tokens, D 128) rotated in place, one call per stream.
+    HBM-bound: algorithmic bytes = tokens x D x 2 B read + the same written."""
+    import torch
+    from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    w = wl.config3()
+    peaks, peaks_src = load_peaks()
+    k_pool, v_pool = wl.pool_values(w, dev)
+    cache = H.create_cache(w, 0)
+    H.append_workload(cache, w, k_pool, v_pool)
+    stream = torch.cuda.current_stream()
+    flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+    tokens = sum(s.kv_len for s in w.streams)
+    alg_bytes = tokens * w.D * 2 * 2
+
+    # the 12 reused chunks of every head, each moved by its own delta: one batched call, one launch
+    chunks = w.notes["chunks"]
+    reqs = []
+    for s in w.streams:
+        t0 = 0
+        for ci, n in enumerate(chunks):
+            reqs.append((s.layer, s.kv_head, s.seq_id, t0, n, 1000 + 4096 * ci))
+            t0 += n
+    tokens = sum(r[4] for r in reqs)
+    alg_bytes = tokens * w.D * 2 * 2
+
+    batch = B.RopeBatch(reqs)
+
+    def step():
+        B.segpa_rope_align_batch(cache, batch, 10000.0, stream=stream)
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    ms = []
+    for _ in range(args.steps):
+        flush_buf.fill_(1)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        step()
+        e1.record(stream)
+        e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    t = float(np.mean(ms))
+    gbs = alg_bytes / (t * 1e-3) / 1e9
+    B.segpa_destroy(cache)
+    print(json.dumps({"metric": "rope_align_gbs", "value": gbs, "unit": "GB/s (K bytes read + written)", "n_gpus": 1,
+                      "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": t, "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "bf16 in/out, fp32 rotation", "data": "synthetic",
+                      "config": {"workload": "rope_align over the reused chunks of cfg3_llama70b_64k (%d heads x %d chunks, %d tokens)" % (len(w.streams), len(chunks), tokens),
+                                 "l2_flush_between_steps": True},
+                      "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                   "frac": gbs / peaks["hbm_gbs"], "traffic": None, "algorithmic_bytes": alg_bytes,
+                                   "peak_source": peaks_src, "kernel": "rope_align_kernel, 1 launch per step (%d chunks)" % len(reqs)},
+                      "gpu_launches": args.steps}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -426,7 +486,9 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
-    if args.impl == "reference":
+    if args.config == "rope" and args.impl == "ours":
+        run_rope(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

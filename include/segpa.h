@@ -152,6 +152,47 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t *cache, const segpa_append
 segpa_status_t segpa_evict_pages(segpa_cache_t *cache, int32_t layer, int32_t kv_head, int64_t seq_id,
                                  int32_t first_page_index, int32_t n_pages);
 
+/*
+ * RoPE-based positional alignment of reused keys (Alg. 1 line 1 "RoPEAlign"):
+ *     K(p_on) = R(p_on) R(p_off)^-1 K(p_off) = R(delta_pos) K(p_off),   delta_pos = p_on - p_off,
+ * applied IN PLACE to the K rows of tokens [first_token, first_token + n_tokens) of a stream (a reused
+ * chunk moves as a unit, so one delta per call).  R(p) is the RoPE rotation: for pair index d in
+ * [0, D/2) the elements (d, d + D/2) of a key (the "rotate-half" pairing of the Llama / Qwen / Mistral
+ * families the paper evaluates; reading A20) are rotated by the angle p * rope_base^(-2d/D).
+ * The per-pair cos / sin are formed in double precision (on the device), the rotation runs in fp32 and
+ * the result is rounded to bf16 (RNE).  V is untouched.  Asynchronous on cuda_stream.
+ * Errors: INVALID (no such stream, range outside it, rope_base <= 1, a page of the range is shared
+ * with another stream (refcount > 1: rotating it would move the other stream's keys too) or evicted),
+ * STATE (planning-only cache), CUDA.
+ */
+segpa_status_t segpa_rope_align(segpa_cache_t *cache, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                int64_t first_token, int64_t n_tokens, int64_t delta_pos, double rope_base,
+                                void *cuda_stream);
+
+/* Batched form: every reused chunk of a batch (each with its own stream, token range and delta) in ONE
+ * descriptor upload and ONE kernel launch.  Ranges must not overlap.  All-or-nothing validation. */
+typedef struct {
+    int32_t layer;
+    int32_t kv_head;
+    int64_t seq_id;
+    int64_t first_token;
+    int64_t n_tokens;
+    int64_t delta_pos;
+} segpa_rope_req_t;
+
+segpa_status_t segpa_rope_align_batch(segpa_cache_t *cache, const segpa_rope_req_t *reqs, int32_t n,
+                                      double rope_base, void *cuda_stream);
+
+/*
+ * Copy the K and V rows of tokens [first_token, first_token + n_tokens) of a stream out of the paged pool
+ * into device bf16 buffers [n_tokens][D] (row stride given; either destination may be NULL).  The inverse of
+ * COPY-mode append: export of a head's KV (e.g. for transfer to another worker) and test read-back.
+ * Errors: INVALID (no such stream, range outside it or touching an evicted page, bad stride), STATE, CUDA.
+ */
+segpa_status_t segpa_gather_rows(segpa_cache_t *cache, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                 int64_t first_token, int64_t n_tokens, void *k_dst, void *v_dst,
+                                 int64_t dst_row_stride_elems, void *cuda_stream);
+
 /* Drop every stream of the cache (all pages return to the free list).  Segment objects built
  * earlier keep their translated page lists and must not be used afterwards. */
 segpa_status_t segpa_clear_streams(segpa_cache_t *cache);

@@ -5,3 +5,4 @@ import this package.  It shares no code with paper_2606_06256_b200/csrc and neve
 CUDA binding; the product path never imports it.
 """
 from .binding import OracleResult, build, num_threads, oracle_attention, set_num_threads  # noqa: F401
+from .rope_oracle import rope_align, rope_rotate  # noqa: F401

@@ -19,7 +19,7 @@ _STATUS = {0: "OK", 1: "INVALID", 2: "OOM", 3: "CUDA", 4: "UNSUPPORTED", 5: "STA
 
 EXPORTS = [
     "segpa_pool_bytes", "segpa_create_cache", "segpa_append_pages", "segpa_append_pages_batch",
-    "segpa_clear_streams", "segpa_evict_pages", "segpa_free_stream",
+    "segpa_clear_streams", "segpa_evict_pages", "segpa_rope_align", "segpa_rope_align_batch", "segpa_gather_rows", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
     "segpa_attention_fwd_host", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
@@ -49,6 +49,11 @@ class AppendReq(C.Structure):
     _fields_ = [("layer", C.c_int32), ("kv_head", C.c_int32), ("seq_id", C.c_int64), ("k_src", C.c_void_p),
                 ("v_src", C.c_void_p), ("src_row_stride_elems", C.c_int64), ("n_tokens", C.c_int64),
                 ("page_ids", C.c_void_p), ("n_page_ids", C.c_int32), ("reserved", C.c_int32)]
+
+
+class RopeReq(C.Structure):
+    _fields_ = [("layer", C.c_int32), ("kv_head", C.c_int32), ("seq_id", C.c_int64), ("first_token", C.c_int64),
+                ("n_tokens", C.c_int64), ("delta_pos", C.c_int64)]
 
 
 class PlanStats(C.Structure):
@@ -84,6 +89,11 @@ def lib():
                                          C.c_int64, C.c_int64, C.c_void_p, C.c_int32, C.c_void_p]
         L.segpa_append_pages_batch.argtypes = [C.c_void_p, C.POINTER(AppendReq), C.c_int32, C.c_void_p]
         L.segpa_clear_streams.argtypes = [C.c_void_p]
+        L.segpa_rope_align.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
+                                       C.c_double, C.c_void_p]
+        L.segpa_rope_align_batch.argtypes = [C.c_void_p, C.POINTER(RopeReq), C.c_int32, C.c_double, C.c_void_p]
+        L.segpa_gather_rows.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_void_p,
+                                        C.c_void_p, C.c_int64, C.c_void_p]
         L.segpa_evict_pages.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int32, C.c_int32]
         L.segpa_free_stream.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64]
         L.segpa_stream_info.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_int64),
@@ -185,6 +195,42 @@ def segpa_append_pages_batch(cache: int, batch, stream=None) -> None:
 
 def segpa_evict_pages(cache: int, layer: int, kv_head: int, seq_id: int, first_page_index: int, n_pages: int) -> None:
     _check(lib().segpa_evict_pages(cache, layer, kv_head, seq_id, first_page_index, n_pages))
+
+
+def segpa_rope_align(cache: int, layer: int, kv_head: int, seq_id: int, first_token: int, n_tokens: int,
+                     delta_pos: int, rope_base: float = 10000.0, stream=None) -> None:
+    _check(lib().segpa_rope_align(cache, layer, kv_head, seq_id, first_token, n_tokens, delta_pos, rope_base,
+                                  _stream_ptr(stream)))
+
+
+class RopeBatch:
+    """Marshalled segpa_rope_req_t array; can be prepared once and passed again."""
+
+    def __init__(self, reqs: Sequence[tuple]):
+        """reqs: tuples (layer, kv_head, seq_id, first_token, n_tokens, delta_pos)."""
+        self.n = len(reqs)
+        self.arr = (RopeReq * max(1, self.n))()
+        for i, r in enumerate(reqs):
+            self.arr[i] = RopeReq(*[int(x) for x in r])
+
+
+def segpa_rope_align_batch(cache: int, reqs, rope_base: float = 10000.0, stream=None) -> None:
+    """reqs: a RopeBatch, or the list of tuples RopeBatch takes."""
+    if not isinstance(reqs, RopeBatch):
+        reqs = RopeBatch(reqs)
+    _check(lib().segpa_rope_align_batch(cache, reqs.arr, reqs.n, rope_base, _stream_ptr(stream)))
+
+
+def segpa_gather_rows(cache: int, layer: int, kv_head: int, seq_id: int, first_token: int, n_tokens: int,
+                      k_dst=None, v_dst=None, stream=None) -> None:
+    """k_dst / v_dst: torch bf16 device tensors [n_tokens][D] (rows may be strided) or None."""
+    ref = k_dst if k_dst is not None else v_dst
+    assert ref is not None and ref.is_cuda and ref.stride(-1) == 1
+    if k_dst is not None and v_dst is not None:
+        assert k_dst.stride(0) == v_dst.stride(0)
+    _check(lib().segpa_gather_rows(cache, layer, kv_head, seq_id, first_token, n_tokens,
+                                   k_dst.data_ptr() if k_dst is not None else None,
+                                   v_dst.data_ptr() if v_dst is not None else None, ref.stride(0), _stream_ptr(stream)))
 
 
 def segpa_clear_streams(cache: int) -> None:

@@ -8,6 +8,7 @@
 
 #include <algorithm>
 #include <climits>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -525,6 +526,139 @@ segpa_status_t segpa_evict_pages(segpa_cache_t* c, int32_t layer, int32_t kv_hea
         release_page(c, rec.pages[(size_t)first_page_index + i]);
         rec.pages[(size_t)first_page_index + i] = -1;
     }
+    return SEGPA_OK;
+}
+
+namespace {
+
+// pages covering tokens [first_token, first_token + n) of a stream, uploaded through the append staging
+// buffers; *first_slot = slot of first_token inside the first page.  Returns nullptr and sets *why on error.
+const int* stage_token_range(segpa_cache* c, const StreamRec& rec, int64_t first_token, int64_t n, bool need_exclusive,
+                             cudaStream_t st, int* first_slot, Staging** used, const char** why, segpa_status_t* code) {
+    const int P = c->desc.page_size;
+    *code = SEGPA_ERR_INVALID;
+    if (first_token < 0 || n < 1 || first_token + n > rec.kv_len) { *why = "token range outside the stream"; return nullptr; }
+    const int64_t pg_lo = first_token / P, pg_hi = (first_token + n - 1) / P + 1;
+    for (int64_t pg = pg_lo; pg < pg_hi; ++pg) {
+        const int32_t id = rec.pages[(size_t)pg];
+        if (id < 0) { *why = "the range touches an evicted page"; return nullptr; }
+        if (need_exclusive && c->refcnt[id] > 1) { *why = "a page of the range is shared with another stream"; return nullptr; }
+    }
+    Staging& sg = c->append_stage[c->append_turn];
+    c->append_turn ^= 1;
+    const size_t bytes = (size_t)(pg_hi - pg_lo) * sizeof(int32_t);
+    cudaError_t e = staging_acquire(sg, bytes);
+    if (e == cudaSuccess) {
+        memcpy(sg.h, rec.pages.data() + pg_lo, bytes);
+        e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+    }
+    if (e != cudaSuccess) { cudaGetLastError(); *why = cudaGetErrorString(e); *code = SEGPA_ERR_CUDA; return nullptr; }
+    *first_slot = (int)(first_token % P);
+    *used = &sg;
+    return (const int*)sg.d;
+}
+
+}  // namespace
+
+segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* reqs, int32_t n, double rope_base,
+                                      void* cuda_stream) {
+    if (!c || !reqs) return fail(SEGPA_ERR_INVALID, "rope_align: null argument");
+    if (n < 1) return fail(SEGPA_ERR_INVALID, "rope_align: batch size %d < 1", n);
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "rope_align: planning-only cache has no device");
+    if (!(rope_base > 1.0)) return fail(SEGPA_ERR_INVALID, "rope_align: rope_base must be > 1");
+    const int D = c->desc.head_dim, P = c->desc.page_size;
+    std::vector<RopeJob> jobs;
+    std::vector<int32_t> ids;
+    long long total_chunks = 0;
+    // a token may be rotated once per batch: overlapping ranges would make the result order-dependent
+    struct Rng { StreamKey key; int64_t lo, hi; };
+    std::vector<Rng> seen;
+    try {
+        for (int32_t i = 0; i < n; ++i) {
+            const segpa_rope_req_t& r = reqs[i];
+            auto it = c->streams.find(StreamKey{r.layer, r.kv_head, r.seq_id});
+            if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: no stream (%d, %d, %lld)", i, r.layer, r.kv_head, (long long)r.seq_id);
+            const StreamRec& rec = it->second;
+            if (r.first_token < 0 || r.n_tokens < 1 || r.first_token + r.n_tokens > rec.kv_len)
+                return fail(SEGPA_ERR_INVALID, "rope_align[%d]: token range outside the stream", i);
+            for (const Rng& g : seen)
+                if (g.key == it->first && r.first_token < g.hi && g.lo < r.first_token + r.n_tokens)
+                    return fail(SEGPA_ERR_INVALID, "rope_align[%d]: token range overlaps an earlier request of the batch", i);
+            seen.push_back(Rng{it->first, r.first_token, r.first_token + r.n_tokens});
+            const int64_t pg_lo = r.first_token / P, pg_hi = (r.first_token + r.n_tokens - 1) / P + 1;
+            for (int64_t pg = pg_lo; pg < pg_hi; ++pg) {
+                const int32_t id = rec.pages[(size_t)pg];
+                if (id < 0) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: the range touches an evicted page", i);
+                if (c->refcnt[id] > 1) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: page %d is shared with another stream", i, id);
+            }
+            RopeJob jb{};
+            jb.chunk_begin = total_chunks;
+            jb.page_off = (long long)ids.size();
+            jb.n_tokens = r.n_tokens;
+            jb.delta_pos = r.delta_pos;   // R(p_on) R(p_off)^-1 = R(delta); the per-pair cos / sin are formed on the device in fp64
+            jb.first_slot = (int)(r.first_token % P);
+            ids.insert(ids.end(), rec.pages.begin() + pg_lo, rec.pages.begin() + pg_hi);
+            total_chunks += r.n_tokens * (D >> 4);
+            jobs.push_back(jb);
+        }
+    } catch (const std::bad_alloc&) {
+        return fail(SEGPA_ERR_OOM, "rope_align: host allocation failed");
+    }
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Staging& sg = c->append_stage[c->append_turn];
+    c->append_turn ^= 1;
+    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    const size_t off_tabs = al(jobs.size() * sizeof(RopeJob));
+    const size_t off_ids = al(off_tabs + jobs.size() * sizeof(RopeTable));   // (tables: device scratch, not uploaded)
+    const size_t bytes = off_ids + ids.size() * sizeof(int32_t);
+    cudaError_t e = staging_acquire(sg, bytes);
+    if (e == cudaSuccess) {
+        memcpy(sg.h, jobs.data(), jobs.size() * sizeof(RopeJob));
+        memcpy((uint8_t*)sg.h + off_ids, ids.data(), ids.size() * sizeof(int32_t));
+        e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+    }
+    if (e == cudaSuccess)
+        e = launch_rope_align(c->k_pool, (const RopeJob*)sg.d, (RopeTable*)((uint8_t*)sg.d + off_tabs), (int)jobs.size(),
+                              (const int*)((const uint8_t*)sg.d + off_ids), total_chunks, rope_base, D, P, st);
+    if (e == cudaSuccess) staging_release(sg, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "rope_align: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_rope_align(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id, int64_t first_token,
+                                int64_t n_tokens, int64_t delta_pos, double rope_base, void* cuda_stream) {
+    segpa_rope_req_t r{};
+    r.layer = layer;
+    r.kv_head = kv_head;
+    r.seq_id = seq_id;
+    r.first_token = first_token;
+    r.n_tokens = n_tokens;
+    r.delta_pos = delta_pos;
+    return segpa_rope_align_batch(c, &r, 1, rope_base, cuda_stream);
+}
+
+segpa_status_t segpa_gather_rows(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id, int64_t first_token,
+                                 int64_t n_tokens, void* k_dst, void* v_dst, int64_t dst_row_stride_elems, void* cuda_stream) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "gather_rows: null cache");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "gather_rows: planning-only cache has no device");
+    const int D = c->desc.head_dim;
+    if (dst_row_stride_elems < D || (dst_row_stride_elems % 8) || ((uintptr_t)k_dst % 16) || ((uintptr_t)v_dst % 16))
+        return fail(SEGPA_ERR_INVALID, "gather_rows: destinations must be 16-byte aligned with a row stride >= head_dim, multiple of 8 elements");
+    auto it = c->streams.find(StreamKey{layer, kv_head, seq_id});
+    if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "gather_rows: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int first_slot = 0;
+    Staging* used = nullptr;
+    const char* why = "";
+    segpa_status_t code = SEGPA_OK;
+    const int* ids = stage_token_range(c, it->second, first_token, n_tokens, false, st, &first_slot, &used, &why, &code);
+    if (!ids) return fail(code, "gather_rows: %s", why);
+    cudaError_t e = launch_gather_rows(c->k_pool, c->v_pool, ids, first_slot, n_tokens, (uint16_t*)k_dst, (uint16_t*)v_dst,
+                                       dst_row_stride_elems, D, c->desc.page_size, st);
+    staging_release(*used, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "gather_rows: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;
 }
 

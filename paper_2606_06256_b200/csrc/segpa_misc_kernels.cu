@@ -53,6 +53,113 @@ cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const Scatter
 }
 
 // ---------------------------------------------------------------------------------------------
+// RoPEAlign: K <- R(delta) K in place on the page images.  One thread per (token,
+// 16-byte chunk of the first half of the head dim): it holds the 8 pairs (d, d + D/2), d = 8c .. 8c+7.
+// HBM-bound: 2 * D * 2 bytes read + written per token.
+// ---------------------------------------------------------------------------------------------
+// cos / sin of delta * base^(-2d/D) per (job, pair d), in double precision (delta can be 10^5 and more:
+// fp32 argument reduction would cost ~1e-3 rad), rounded once to fp32
+__global__ void rope_table_kernel(const RopeJob* __restrict__ jobs, RopeTable* __restrict__ tabs, double rope_base, int D) {
+    const int d = threadIdx.x;
+    if (d >= D / 2) return;
+    const double ang = (double)jobs[blockIdx.x].delta_pos * pow(rope_base, -2.0 * d / D);
+    double sn, cs;
+    sincos(ang, &sn, &cs);
+    tabs[blockIdx.x].cs[d] = (float)cs;
+    tabs[blockIdx.x].sn[d] = (float)sn;
+}
+
+__global__ void rope_align_kernel(uint8_t* __restrict__ k_pool, const RopeJob* __restrict__ jobs,
+                                  const RopeTable* __restrict__ tabs, int n_jobs, const int* __restrict__ page_ids,
+                                  long long total_chunks, int D, int P) {
+    const int cph = D >> 4;  // 16-byte chunks per half row
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total_chunks;
+         idx += (long long)gridDim.x * blockDim.x) {
+        int lo = 0, hi = n_jobs - 1;
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (jobs[mid].chunk_begin <= idx) lo = mid; else hi = mid - 1;
+        }
+        const RopeJob jb = jobs[lo];
+        const float* cs_t = tabs[lo].cs;
+        const float* sn_t = tabs[lo].sn;
+        const long long local = idx - jb.chunk_begin;
+        const long long n = local / cph;
+        const int c = (int)(local % cph);
+        const long long gs = jb.first_slot + n;
+        const size_t page = (size_t)page_ids[jb.page_off + gs / P] * ((size_t)P * D * 2);
+        const int slot = (int)(gs % P);
+        uint4* pa = reinterpret_cast<uint4*>(k_pool + page + page_elem_offset_bytes(D, slot, c * 8));
+        uint4* pb = reinterpret_cast<uint4*>(k_pool + page + page_elem_offset_bytes(D, slot, c * 8 + D / 2));
+        uint4 a4 = *pa, b4 = *pb;
+        const float4 cs0 = *reinterpret_cast<const float4*>(cs_t + c * 8), cs1 = *reinterpret_cast<const float4*>(cs_t + c * 8 + 4);
+        const float4 sn0 = *reinterpret_cast<const float4*>(sn_t + c * 8), sn1 = *reinterpret_cast<const float4*>(sn_t + c * 8 + 4);
+        const float csv[8] = {cs0.x, cs0.y, cs0.z, cs0.w, cs1.x, cs1.y, cs1.z, cs1.w};
+        const float snv[8] = {sn0.x, sn0.y, sn0.z, sn0.w, sn1.x, sn1.y, sn1.z, sn1.w};
+        uint32_t* aw = reinterpret_cast<uint32_t*>(&a4);
+        uint32_t* bw = reinterpret_cast<uint32_t*>(&b4);
+#pragma unroll
+        for (int w = 0; w < 4; ++w) {
+            uint32_t ra = 0, rb = 0;
+#pragma unroll
+            for (int hlf = 0; hlf < 2; ++hlf) {
+                const float a = __uint_as_float(((aw[w] >> (16 * hlf)) & 0xffffu) << 16);
+                const float b = __uint_as_float(((bw[w] >> (16 * hlf)) & 0xffffu) << 16);
+                const float cs = csv[w * 2 + hlf], sn = snv[w * 2 + hlf];
+                const float na = a * cs - b * sn, nb = a * sn + b * cs;
+                ra |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(na)) << (16 * hlf);
+                rb |= (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(nb)) << (16 * hlf);
+            }
+            aw[w] = ra;
+            bw[w] = rb;
+        }
+        *pa = a4;
+        *pb = b4;
+    }
+}
+
+cudaError_t launch_rope_align(uint8_t* k_pool, const RopeJob* jobs_dev, RopeTable* tabs_dev, int n_jobs,
+                              const int* page_ids_dev, long long total_chunks, double rope_base, int D, int P, cudaStream_t st) {
+    if (total_chunks <= 0 || n_jobs <= 0) return cudaSuccess;
+    rope_table_kernel<<<n_jobs, 64, 0, st>>>(jobs_dev, tabs_dev, rope_base, D);
+    long long blocks = (total_chunks + 255) / 256;
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    rope_align_kernel<<<(unsigned)blocks, 256, 0, st>>>(k_pool, jobs_dev, tabs_dev, n_jobs, page_ids_dev, total_chunks, D, P);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Inverse of the scatter: page images -> rows [n][D] (export / read-back).  One thread per 16-byte chunk.
+// ---------------------------------------------------------------------------------------------
+__global__ void gather_rows_kernel(const uint8_t* __restrict__ k_pool, const uint8_t* __restrict__ v_pool,
+                                   const int* __restrict__ page_ids, int first_slot, long long n_tokens,
+                                   uint16_t* __restrict__ k_dst, uint16_t* __restrict__ v_dst, long long dst_stride,
+                                   int D, int P) {
+    const int cpr = D >> 3;
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n_tokens * cpr;
+         idx += (long long)gridDim.x * blockDim.x) {
+        const long long n = idx / cpr;
+        const int c = (int)(idx % cpr);
+        const long long gs = first_slot + n;
+        const size_t src = (size_t)page_ids[gs / P] * ((size_t)P * D * 2) + page_elem_offset_bytes(D, (int)(gs % P), c * 8);
+        if (k_dst) *reinterpret_cast<uint4*>(k_dst + n * dst_stride + c * 8) = *reinterpret_cast<const uint4*>(k_pool + src);
+        if (v_dst) *reinterpret_cast<uint4*>(v_dst + n * dst_stride + c * 8) = *reinterpret_cast<const uint4*>(v_pool + src);
+    }
+}
+
+cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, const int* page_ids_dev, int first_slot,
+                               long long n_tokens, uint16_t* k_dst, uint16_t* v_dst, long long dst_stride, int D, int P,
+                               cudaStream_t st) {
+    const long long total = n_tokens * (D >> 3);
+    if (total <= 0) return cudaSuccess;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    gather_rows_kernel<<<(unsigned)blocks, 256, 0, st>>>(k_pool, v_pool, page_ids_dev, first_slot, n_tokens, k_dst, v_dst,
+                                                         dst_stride, D, P);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
 // a7: split-KV combine.  Partials hold unnormalised O, running max m (log2 units) and sum l;
 // merged in ascending split order (deterministic).  Exactness of the merge: PAPER.md:302.
 // One warp per row.

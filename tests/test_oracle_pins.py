@@ -20,6 +20,7 @@ import numpy as np
 import pytest
 import torch
 
+import oracle
 from oracle import bruteforce
 from paper_2606_06256_b200 import workloads as wl
 from paper_2606_06256_b200.workloads import GLOBAL, LOCAL
@@ -366,3 +367,49 @@ def test_config_shapes():
     c5 = wl.config5()
     assert len(c5.segments) == 112 and sum(s.head_class == GLOBAL for s in c5.segments) == 16
     assert abs(wl.useful_flops(c5) / 1e12 - 74.08) < 0.01
+
+
+# ---------------------------------------------------------------------------------------------
+# RoPEAlign oracle pinned to things other than itself
+# ---------------------------------------------------------------------------------------------
+def _rope_inputs(n=37, D=16, seed=3):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal((n, D)), rng.integers(0, 5000, size=n), rng.integers(0, 70000, size=n)
+
+
+def test_rope_printed_constants_and_identity():
+    # D = 2: theta_0 = 1, one pair: (1, 0) at delta 1 -> (cos 1, sin 1); (0, 1) -> (-sin 1, cos 1)
+    out = oracle.rope_align(np.array([[1.0, 0.0], [0.0, 1.0]]), np.array([0, 0]), np.array([1, 1]))
+    assert np.allclose(out, [[0.5403023058681398, 0.8414709848078965], [-0.8414709848078965, 0.5403023058681398]], atol=1e-15)
+    k, p_off, _ = _rope_inputs()
+    assert np.allclose(oracle.rope_align(k, p_off, p_off), k, atol=1e-12)            # delta = 0
+
+
+def test_rope_composition_norm_and_pairing():
+    k, p_off, p_on = _rope_inputs()
+    D = k.shape[1]
+    a = oracle.rope_align(k, p_off, p_on)
+    # R(p_on) R(p_off)^-1 = R(p_on - p_off): one rotation by the difference gives the same rows
+    assert np.allclose(a, oracle.rope_rotate(k, p_on - p_off), atol=1e-9)
+    # each (d, d + D/2) pair keeps its norm; only those two elements mix
+    assert np.allclose(a[:, :D // 2] ** 2 + a[:, D // 2:] ** 2, k[:, :D // 2] ** 2 + k[:, D // 2:] ** 2, atol=1e-9)
+    k2 = k.copy()
+    k2[:, 3] += 1.0
+    diff = np.abs(oracle.rope_align(k2, p_off, p_on) - a) > 1e-12
+    assert diff[:, [3, 3 + D // 2]].any() and not np.delete(diff, [3, 3 + D // 2], axis=1).any()
+
+
+def test_rope_relative_position_property_and_complex_form():
+    k, p_off, p_on = _rope_inputs()
+    n, D = k.shape
+    rng = np.random.default_rng(5)
+    q = rng.standard_normal((n, D))
+    m = rng.integers(0, 70000, size=n)
+    # <R(m) q, K(p_on)> = <R(m - p_on + p_off) q, K(p_off)>: scores depend on relative position only
+    lhs = np.sum(oracle.rope_rotate(q, m) * oracle.rope_align(k, p_off, p_on), axis=1)
+    rhs = np.sum(oracle.rope_rotate(q, m - p_on + p_off) * k, axis=1)
+    assert np.allclose(lhs, rhs, atol=1e-8)
+    # library special case: the pair (a, b) as the complex number a + ib times e^{i delta theta_d}
+    theta = 10000.0 ** (-2.0 * np.arange(D // 2) / D)
+    z = (k[:, :D // 2] + 1j * k[:, D // 2:]) * np.exp(1j * np.outer(p_on - p_off, theta))
+    assert np.allclose(oracle.rope_align(k, p_off, p_on), np.concatenate([z.real, z.imag], axis=1), atol=1e-9)
