@@ -58,6 +58,16 @@ def ncu_traffic(workload: str):
     return None
 
 
+def max_over_ranks(x: float, dist, device) -> float:
+    """Replicas: the job's time is the slowest rank's (one all-reduce MAX; `dist` None = single process)."""
+    if dist is None:
+        return float(x)
+    import torch
+    t = torch.tensor([x], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def get_workload(name: str):
     from paper_2606_06256_b200 import workloads as wl
     if name == "4d":
@@ -313,10 +323,7 @@ def run_ours(args):
     clocks = sampler.stop()
     free_segs()
     total_ms = float(sum(step_ms))
-    if dist is not None:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dist, dev)
     ms_per_step = total_ms / args.steps
     value = world * useful / (ms_per_step * 1e-3) / 1e12
     fwd_mean = float(np.mean(fwd_ms))
@@ -348,10 +355,7 @@ def run_ours(args):
         e2e_step()
     e2e_s = (time.perf_counter() - t0) / n_e2e
     free_segs()
-    if dist is not None:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, dist, dev)
     e2e_val = world * useful / e2e_s / 1e12
 
     # ---- plan statistics / algorithmic bytes for the roofline
