@@ -821,10 +821,11 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             const int cost = t.cost;
             int parts = 1;
             if (cost > chunk + chunk / 2 && !t.sink) parts = (int)cdiv(cost, chunk);   // (sink items are not cut along KV)
-            // Decode-shaped tile (all its rows fit the first of the item's two tile slots): run it STRIDED -- the
+            // Decode-shaped segment (all its rows fit the first of the item's two tile slots; the short tail item of a
+            // long prefill segment does not count: it is not worth a combine pass): run it STRIDED -- the
             // two slots take alternate KV blocks of the same rows as two independent chains, each writing a
             // partial that the combine kernel merges -- so the second slot is not left idle.
-            const bool strided = tiles_per_item == 2 && t.n_tok <= TT && cost >= 2 && c->kernel_kind == 1;
+            const bool strided = tiles_per_item == 2 && S->reqs[(size_t)t.seg].q_len <= TT && cost >= 2 && c->kernel_kind == 1;
             if (parts > 1) ++n_split_tiles;
             if (parts > 1 || strided)
                 S->combs.push_back(CombDev{t.seg, t.t0, t.n_tok, n_slots, parts, strided ? 1 : 0, 0, 0});
