@@ -22,7 +22,7 @@ EXPORTS = [
     "segpa_clear_streams", "segpa_evict_pages", "segpa_rope_align", "segpa_rope_align_batch", "segpa_gather_rows", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
-    "segpa_attention_fwd_host", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
+    "segpa_attention_fwd_host", "segpa_merge", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
     "segpa_version",
 ]
 
@@ -110,6 +110,8 @@ def lib():
                                           C.c_int64, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
         L.segpa_attention_fwd_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
                                                C.c_void_p, C.c_int64, C.c_void_p]
+        L.segpa_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64,
+                                  C.c_int64, C.c_int64, C.c_void_p]
         L.segpa_destroy.argtypes = [C.c_void_p]
         _lib = L
     return _lib
@@ -327,6 +329,16 @@ def segpa_attention_fwd_host(cache: int, segs: int, q_host, softmax_scale: float
         lp = lse_host.data_ptr()
     _check(lib().segpa_attention_fwd_host(cache, segs, q_host.data_ptr(), softmax_scale, out_host.data_ptr(), lp, T,
                                           _stream_ptr(stream)))
+
+
+def segpa_merge(cache: int, out_a, lse_a, out_b, lse_b, out, lse, stream=None) -> None:
+    """out_*: torch bf16 device tensors [T][Hq][D] with the same row stride; lse_*: fp32 [Hq][T] with the same stride."""
+    for t in (out_a, out_b, out):
+        assert t.is_cuda and t.dim() == 3 and t.stride(2) == 1 and t.stride(1) == t.shape[2] and t.stride(0) == out.stride(0)
+    for t in (lse_a, lse_b, lse):
+        assert t.is_cuda and t.dim() == 2 and t.stride(1) == 1 and t.stride(0) == lse.stride(0)
+    _check(lib().segpa_merge(cache, out_a.data_ptr(), lse_a.data_ptr(), out_b.data_ptr(), lse_b.data_ptr(), out.data_ptr(),
+                             lse.data_ptr(), out.stride(0), lse.stride(0), out.shape[0], _stream_ptr(stream)))
 
 
 def segpa_last_launch_count(cache: int) -> int:

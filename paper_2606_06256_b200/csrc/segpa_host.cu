@@ -1117,6 +1117,19 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t
     return SEGPA_OK;
 }
 
+segpa_status_t segpa_merge(segpa_cache_t* c, const void* out_a, const float* lse_a, const void* out_b, const float* lse_b,
+                           void* out, float* lse, int64_t row_stride, int64_t lse_stride, int64_t T, void* cuda_stream) {
+    if (!c || !out_a || !lse_a || !out_b || !lse_b || !out || !lse) return fail(SEGPA_ERR_INVALID, "merge: null argument");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "merge: planning-only cache has no device");
+    const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
+    if (T < 1 || row_stride < (int64_t)Hq * D || lse_stride < T) return fail(SEGPA_ERR_INVALID, "merge: bad T / strides");
+    DeviceGuard g(c->desc.device);
+    cudaError_t e = launch_merge((const uint16_t*)out_a, lse_a, (const uint16_t*)out_b, lse_b, (uint16_t*)out, lse, row_stride,
+                                 lse_stride, T, Hq, D, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "merge: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
 int32_t segpa_last_launch_count(const segpa_cache_t* c) { return c ? c->last_launches : 0; }
 
 }  // extern "C"

@@ -137,6 +137,9 @@ cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, con
                                long long n_tokens, uint16_t* k_dst, uint16_t* v_dst, long long dst_stride, int D, int P,
                                cudaStream_t st);
 
+cudaError_t launch_merge(const uint16_t* out_a, const float* lse_a, const uint16_t* out_b, const float* lse_b, uint16_t* out,
+                         float* lse, long long row_stride, long long lse_stride, long long T, int Hq, int D, cudaStream_t st);
+
 // kernel launchers (each returns the CUDA error of its launch)
 cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const ScatterJob* jobs_dev, int n_jobs,
                                  const int* page_ids_dev, long long total_chunks, int D, int P, cudaStream_t st);

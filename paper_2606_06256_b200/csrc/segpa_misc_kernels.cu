@@ -242,6 +242,48 @@ cudaError_t launch_combine(const FwdParams& p, cudaStream_t st) {
 }
 
 // ---------------------------------------------------------------------------------------------
+// LSE merge of two results over disjoint key sets.  One warp per (row, head), lanes over D.
+// HBM-bound: 2 * D * 2 bytes read + D * 2 written per (row, head).
+// ---------------------------------------------------------------------------------------------
+__global__ void merge_kernel(const uint16_t* __restrict__ out_a, const float* __restrict__ lse_a,
+                             const uint16_t* __restrict__ out_b, const float* __restrict__ lse_b, uint16_t* out, float* lse,
+                             long long row_stride, long long lse_stride, long long T, int Hq, int D) {
+    const int lane = threadIdx.x & 31;
+    const long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long u = wid; u < T * Hq; u += nw) {
+        const long long row = u / Hq;
+        const int head = (int)(u % Hq);
+        const float la = lse_a[(long long)head * lse_stride + row], lb = lse_b[(long long)head * lse_stride + row];
+        const float m = fmaxf(la, lb);
+        float wa = 0.f, wb = 0.f, l = -INFINITY;
+        if (m != -INFINITY) {
+            const float ea = expf(la - m), eb = expf(lb - m);     // exp(-inf) = 0
+            wa = ea / (ea + eb);
+            wb = eb / (ea + eb);
+            l = m + logf(ea + eb);
+        }
+        const long long base = row * row_stride + (long long)head * D;
+        for (int d = lane; d < D; d += 32) {
+            // a side with weight 0 (lse = -inf) may hold anything, NaN included: it is not read into the sum
+            const float a = wa != 0.f ? __bfloat162float(__ushort_as_bfloat16(out_a[base + d])) : 0.f;
+            const float b = wb != 0.f ? __bfloat162float(__ushort_as_bfloat16(out_b[base + d])) : 0.f;
+            out[base + d] = __bfloat16_as_ushort(__float2bfloat16_rn(wa * a + wb * b));
+        }
+        if (lane == 0) lse[(long long)head * lse_stride + row] = l;
+    }
+}
+
+cudaError_t launch_merge(const uint16_t* out_a, const float* lse_a, const uint16_t* out_b, const float* lse_b, uint16_t* out,
+                         float* lse, long long row_stride, long long lse_stride, long long T, int Hq, int D, cudaStream_t st) {
+    const long long warps = T * Hq;
+    if (warps <= 0) return cudaSuccess;
+    long long blocks = (warps + 7) / 8;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    merge_kernel<<<(unsigned)blocks, 256, 0, st>>>(out_a, lse_a, out_b, lse_b, out, lse, row_stride, lse_stride, T, Hq, D);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
 // SIMT bring-up attention: same plan, same outputs, no tensor cores.  One warp per query row;
 // lanes split the head dim; keys visited one at a time.  Exists to validate the pool layout, the
 // builder and the scheduler independently of the tcgen05 kernel.

@@ -339,3 +339,43 @@ def test_cfg5_two_layers_sampled():
             print(len(rows), compare(w, layer, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg5 L%d" % layer))
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("j0", [1, 130, 1000, 2999])
+def test_lse_merge_of_split_key_sets(j0):
+    """results over two disjoint key sets merged with segpa_merge equal attention over the union
+    (checked against the oracle run on the whole stream, and against the kernel's own whole-stream result)."""
+    n = 3000
+    w = wl.make_workload("merge", Hq=8, Hkv=2, D=128, P=16, seed=41, pool_factor=4.0,
+                         requests=[{"kv_len": n, "heads": {0: (GLOBAL, 0, 0, 1), 1: (GLOBAL, 0, 0, 1)}}])
+    dev = torch.device("cuda:0")
+    k, v = wl.pool_values(w, dev)
+    g = GpuRun(w, "tc", 2, k, v)
+    try:
+        for h in (0, 1):
+            st = w.stream_map()[(0, h, 0)]
+            kr, vr = wl.stream_rows(k, st, w.P), wl.stream_rows(v, st, w.P)
+            B.segpa_append_pages(g.cache, 0, h, 100, kr[:j0].contiguous(), vr[:j0].contiguous(), j0)
+            B.segpa_append_pages(g.cache, 0, h, 200, kr[j0:].contiguous(), vr[j0:].contiguous(), n - j0)
+        q1 = wl.q_values(w, 0, dev)                                      # [1][Hq][D]
+        q3 = q1.repeat(3, 1, 1).contiguous()                              # the same query for whole / part a / part b
+        reqs = [(sid, h, GLOBAL, 0, 0, r, 1) for r, sid in enumerate((0, 100, 200)) for h in (0, 1)]
+        segs = B.segpa_build_segments(g.cache, 0, reqs)
+        out = torch.zeros_like(q3)
+        lse = torch.zeros((w.Hq, 3), dtype=torch.float32, device=dev)
+        B.segpa_attention_fwd(g.cache, segs, q3, w.scale, out, lse)
+        om = torch.zeros_like(q1)
+        lm = torch.zeros((w.Hq, 1), dtype=torch.float32, device=dev)
+        B.segpa_merge(g.cache, out[1:2], lse[:, 1:2].contiguous(), out[2:3], lse[:, 2:3].contiguous(), om, lm)
+        torch.cuda.synchronize()
+        print(compare(w, 0, k, v, q1, om, lm, label="merge j0=%d" % j0))
+        assert (om.float() - out[0:1].float()).abs().max() <= 2e-2 and (lm - lse[:, 0:1]).abs().max() <= 1e-3
+        # a side with no keys at all (lse = -inf, out anything) leaves the other side unchanged
+        junk = torch.full_like(q1, float("nan"))
+        ninf = torch.full_like(lm, float("-inf"))
+        o2, l2 = torch.zeros_like(q1), torch.zeros_like(lm)
+        B.segpa_merge(g.cache, out[0:1], lse[:, 0:1].contiguous(), junk, ninf, o2, l2)
+        torch.cuda.synchronize()
+        assert torch.equal(o2, out[0:1]) and torch.equal(l2, lse[:, 0:1])
+    finally:
+        g.close()
