@@ -837,28 +837,39 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti, 0, 0});
             }
         }
-        // LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid; a CTA's
-        // items stay in descending order.  Cost = visited blocks + a fixed per-item term (pipeline refill,
-        // Q load, epilogue: about 0.6 block-times measured), in thirds of a block.
-        const int n_cta = (int)std::min<size_t>(S->items.size(), (size_t)c->num_sms);
-        std::vector<int> order(S->items.size());
-        for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
-        std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
-            return S->items[a].cost > S->items[b].cost;
+        // LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid (min-heap on
+        // (load, cta)); a CTA's items stay in descending order.  Cost = visited blocks + a fixed per-item term
+        // (pipeline refill, Q load, epilogue: about 0.6 block-times measured), in thirds of a block.  Flat arrays
+        // only: the plan is built on the critical path of every layer.
+        const int n_items_all = (int)S->items.size();
+        const int n_cta = std::min(n_items_all, c->num_sms);
+        std::vector<int> order((size_t)n_items_all);
+        for (int i = 0; i < n_items_all; ++i) order[(size_t)i] = i;
+        std::sort(order.begin(), order.end(), [&](int a, int b) {
+            return S->items[a].cost != S->items[b].cost ? S->items[a].cost > S->items[b].cost : a < b;
         });
-        std::vector<std::vector<int>> per_cta((size_t)n_cta);
-        {
-            typedef std::pair<int64_t, int> Load;   // (load, cta): min-heap, ties to the lower CTA index
-            std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-            for (int q = 0; q < n_cta; ++q) heap.push(Load(0, q));
+        const int n_rounds = (n_items_all + n_cta - 1) / n_cta;
+        int cap = n_rounds + 8;      // slots per CTA (LPT can give a CTA a few more than the average count)
+        std::vector<int> slot, count;
+        for (;;) {
+            slot.assign((size_t)n_cta * cap, -1);
+            count.assign((size_t)n_cta, 0);
+            std::vector<int64_t> heap((size_t)n_cta);   // min-heap on the single key load * 1024 + cta
+            for (int q = 0; q < n_cta; ++q) heap[(size_t)q] = q;
+            auto gt = std::greater<int64_t>();
+            bool overflow = false;
             for (int idx : order) {
-                Load ld = heap.top();
-                heap.pop();
-                per_cta[(size_t)ld.second].push_back(idx);
+                std::pop_heap(heap.begin(), heap.end(), gt);
+                int64_t& top = heap.back();
+                const int q = (int)(top & 1023);
+                if (count[(size_t)q] == cap) { overflow = true; break; }
+                slot[(size_t)q * cap + count[(size_t)q]++] = idx;
                 const int64_t blocks3 = 3 * (int64_t)S->items[idx].cost;
-                ld.first += ((S->items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2;   // strided: two chains
-                heap.push(ld);
+                top += (((S->items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2) * 1024;   // strided: two chains
+                std::push_heap(heap.begin(), heap.end(), gt);
             }
+            if (!overflow) break;
+            cap *= 2;
         }
         std::vector<ItemDev> it2;
         std::vector<segpa_item_t> ip2;
@@ -867,7 +878,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         S->cta_off.assign((size_t)n_cta + 1, 0);
         int64_t kv_blocks = 0;
         for (int q = 0; q < n_cta; ++q) {
-            for (int idx : per_cta[(size_t)q]) {
+            for (int k2 = 0; k2 < count[(size_t)q]; ++k2) {
+                const int idx = slot[(size_t)q * cap + k2];
                 it2.push_back(S->items[idx]);
                 segpa_item_t pub = S->items_pub[idx];
                 pub.cta = q;
