@@ -349,6 +349,40 @@ segpa_status_t segpa_merge(segpa_cache_t *cache, const void *out_a, const float 
                            const float *lse_b, void *out, float *lse, int64_t row_stride_elems,
                            int64_t lse_stride, int64_t T, void *cuda_stream);
 
+/* ------------------------------------------------------------------------------------------- */
+/* Attention mass and salient-token selection (Alg. 1 line 19 SelectImportantTokens; */
+/* "computes attention mass over tokens and selects ... the smallest set of tokens whose cumulative */
+/* attention mass exceeds a threshold tau").  The step right after the fused attention. */
+/* ------------------------------------------------------------------------------------------- */
+
+/* Layout of the mass / selection arrays: segment s occupies entries [offsets[s], offsets[s] + kv_len_s)
+ * (offsets[s+1] - offsets[s] = kv_len_s rounded up to 128).  Writes min(cap, n + 1) offsets; *n_out = n. */
+segpa_status_t segpa_segments_mass_layout(const segpa_segments_t *segs, int64_t *offsets_out, int32_t cap,
+                                          int32_t *n_out);
+
+/*
+ * mass[offsets[s] + j] = sum over the query rows t and the G query heads g of segment s of p(t, g, j), where
+ * p(t, g, j) = exp(softmax_scale * q . K[j] - lse[g][t]) is the probability the fused attention gave key j
+ * (0 for keys the row does not see).  q, softmax_scale and lse are those of a completed segpa_attention_fwd
+ * with the same segments; the probabilities are recomputed on the tensor cores (S^T = K Q^T per 128-key block),
+ * they are never stored.  Entries of keys no query sees, and the padding up to the next multiple of 128, are 0.
+ * mass: device fp32 with at least offsets[n] entries.  Asynchronous on cuda_stream; deterministic.
+ * Errors: INVALID, STATE (planning-only cache, foreign or stale segments), OOM, CUDA.
+ */
+segpa_status_t segpa_attention_mass(segpa_cache_t *cache, const segpa_segments_t *segs, const void *q,
+                                    int64_t q_row_stride_elems, float softmax_scale, const float *lse,
+                                    int64_t lse_stride, int64_t T, float *mass, int64_t mass_len,
+                                    void *cuda_stream);
+
+/*
+ * Per segment, the smallest set of keys whose cumulative mass reaches tau * (the segment's total mass):
+ * selected[offsets[s] + j] = 1 / 0 (device uint8, same layout as mass), n_selected[s] = its size (device int32
+ * [n_segments]).  Keys are taken in order of decreasing mass; among keys of equal mass at the boundary the
+ * lowest positions are taken.  0 < tau <= 1.  Errors: INVALID, STATE, CUDA.
+ */
+segpa_status_t segpa_mass_select(segpa_cache_t *cache, const segpa_segments_t *segs, const float *mass, float tau,
+                                 uint8_t *selected, int32_t *n_selected, void *cuda_stream);
+
 /* Number of kernel launches the last attention_fwd on this cache issued (1, or 2 with split-KV). */
 int32_t segpa_last_launch_count(const segpa_cache_t *cache);
 

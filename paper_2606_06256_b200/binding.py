@@ -22,7 +22,8 @@ EXPORTS = [
     "segpa_clear_streams", "segpa_evict_pages", "segpa_rope_align", "segpa_rope_align_batch", "segpa_gather_rows", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
-    "segpa_attention_fwd_host", "segpa_merge", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
+    "segpa_attention_fwd_host", "segpa_merge", "segpa_segments_mass_layout", "segpa_attention_mass",
+    "segpa_mass_select", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
     "segpa_version",
 ]
 
@@ -112,6 +113,10 @@ def lib():
                                                C.c_void_p, C.c_int64, C.c_void_p]
         L.segpa_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64,
                                   C.c_int64, C.c_int64, C.c_void_p]
+        L.segpa_segments_mass_layout.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]
+        L.segpa_attention_mass.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_void_p, C.c_int64,
+                                           C.c_int64, C.c_void_p, C.c_int64, C.c_void_p]
+        L.segpa_mass_select.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
         L.segpa_destroy.argtypes = [C.c_void_p]
         _lib = L
     return _lib
@@ -339,6 +344,30 @@ def segpa_merge(cache: int, out_a, lse_a, out_b, lse_b, out, lse, stream=None) -
         assert t.is_cuda and t.dim() == 2 and t.stride(1) == 1 and t.stride(0) == lse.stride(0)
     _check(lib().segpa_merge(cache, out_a.data_ptr(), lse_a.data_ptr(), out_b.data_ptr(), lse_b.data_ptr(), out.data_ptr(),
                              lse.data_ptr(), out.stride(0), lse.stride(0), out.shape[0], _stream_ptr(stream)))
+
+
+def segpa_segments_mass_layout(segs: int) -> np.ndarray:
+    """int64 offsets [n_segments + 1] of the attention-mass / selection arrays."""
+    n = C.c_int32()
+    _check(lib().segpa_segments_mass_layout(segs, None, 0, C.byref(n)))
+    offs = np.zeros(n.value + 1, dtype=np.int64)
+    _check(lib().segpa_segments_mass_layout(segs, offs.ctypes.data_as(C.c_void_p), n.value + 1, C.byref(n)))
+    return offs
+
+
+def segpa_attention_mass(cache: int, segs: int, q, softmax_scale: float, lse, mass, stream=None) -> None:
+    """q: torch bf16 [T][Hq][D]; lse: fp32 [Hq][T] from segpa_attention_fwd; mass: fp32 device, layout above."""
+    assert q.is_cuda and lse.is_cuda and mass.is_cuda and mass.dtype.is_floating_point and mass.is_contiguous()
+    assert q.stride(2) == 1 and q.stride(1) == q.shape[2] and lse.stride(1) == 1
+    _check(lib().segpa_attention_mass(cache, segs, q.data_ptr(), q.stride(0), softmax_scale, lse.data_ptr(), lse.stride(0),
+                                      q.shape[0], mass.data_ptr(), mass.numel(), _stream_ptr(stream)))
+
+
+def segpa_mass_select(cache: int, segs: int, mass, tau: float, selected, n_selected, stream=None) -> None:
+    """selected: torch uint8 device (layout of mass); n_selected: torch int32 device [n_segments]."""
+    assert mass.is_cuda and selected.is_cuda and n_selected.is_cuda and selected.numel() >= mass.numel()
+    _check(lib().segpa_mass_select(cache, segs, mass.data_ptr(), tau, selected.data_ptr(), n_selected.data_ptr(),
+                                   _stream_ptr(stream)))
 
 
 def segpa_last_launch_count(cache: int) -> int:

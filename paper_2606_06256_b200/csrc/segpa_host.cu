@@ -122,6 +122,7 @@ void staging_free(Staging& s) {
 // workspace); recycled through the cache's free list instead of cudaMalloc / cudaFree per build.
 struct SegBuf {
     Staging blob;
+    Staging mass_blob;    // attention-mass plan (items, per-CTA slices, layout), uploaded at the first mass call
     int* counter = nullptr;
     float* ws_o = nullptr;
     float* ws_ml = nullptr;
@@ -131,6 +132,7 @@ struct SegBuf {
 void segbuf_free(SegBuf* b) {
     if (!b) return;
     staging_free(b->blob);
+    staging_free(b->mass_blob);
     if (b->counter) cudaFree(b->counter);
     if (b->ws_o) cudaFree(b->ws_o);
     if (b->ws_ml) cudaFree(b->ws_ml);
@@ -149,6 +151,10 @@ struct segpa_segments {
     std::vector<int32_t> pages;
     std::vector<CombDev> combs;
     std::vector<int32_t> cta_off;   // items of CTA q: [cta_off[q], cta_off[q+1])
+    std::vector<int64_t> mass_off;  // [n + 1]: layout of the attention-mass array (kv_len rounded up to 128 per segment)
+    mutable bool mass_planned = false;   // mass plan built and uploaded (lazily, by the first segpa_attention_mass)
+    mutable int mass_n_cta = 0;
+    mutable size_t m_off_items = 0, m_off_cta = 0, m_off_layout = 0, m_off_kvlen = 0;
     segpa_plan_stats_t stats{};
     int tiles_per_item = 1;
     // device
@@ -208,6 +214,7 @@ void free_segments_obj(segpa_cache* c, segpa_segments* s) {
     if (!s) return;
     if (s->buf) {
         staging_release(s->buf->blob, s->last_stream);
+        if (s->mass_planned) staging_release(s->buf->mass_blob, s->last_stream);
         c->free_bufs.push_back(s->buf);
     }
     delete s;
@@ -783,6 +790,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 S->pages.insert(S->pages.end(), (size_t)(lst_hi - vis_b), zero_page);
             }
             S->segs.push_back(sd);
+            if (S->mass_off.empty()) S->mass_off.push_back(0);
+            S->mass_off.push_back(S->mass_off.back() + cdiv(kv_len, kBlockKeys) * kBlockKeys);
             vis_tokens += kv_len - first_vis_page * P + sink_pages * P;
             q_rows = std::max<int64_t>(q_rows, r.q_row_start + r.q_len);
             pairs += visible_pairs(kv_len - r.q_len, kv_len - 1, W);
@@ -1139,6 +1148,152 @@ segpa_status_t segpa_merge(segpa_cache_t* c, const void* out_a, const float* lse
     cudaError_t e = launch_merge((const uint16_t*)out_a, lse_a, (const uint16_t*)out_b, lse_b, (uint16_t*)out, lse, row_stride,
                                  lse_stride, T, Hq, D, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "merge: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_segments_mass_layout(const segpa_segments_t* s, int64_t* offsets_out, int32_t cap, int32_t* n_out) {
+    if (!s) return fail(SEGPA_ERR_INVALID, "segments_mass_layout: null argument");
+    if (n_out) *n_out = (int32_t)s->segs.size();
+    if (offsets_out)
+        for (int32_t i = 0; i < cap && i < (int32_t)s->mass_off.size(); ++i) offsets_out[i] = s->mass_off[(size_t)i];
+    return SEGPA_OK;
+}
+
+namespace {
+
+// builds and uploads the attention-mass plan of a segments object (once)
+segpa_status_t plan_mass(segpa_cache* c, const segpa_segments* s, cudaStream_t st) {
+    if (s->mass_planned) return SEGPA_OK;
+    const int TT = kTileRows / c->G;
+    std::vector<MassItem> items;
+    for (size_t si = 0; si < s->segs.size(); ++si) {
+        const SegDev& sg = s->segs[si];
+        const int64_t p0 = sg.kv_len - sg.q_len, W = sg.window, ns = sg.n_sink;
+        const int ppb = kBlockKeys / c->desc.page_size;
+        const int kb_first = sg.first_page / ppb, kb_end = kb_first + sg.n_pages_listed / ppb;
+        for (int kb = kb_first; kb < kb_end; ++kb) {
+            const int64_t lo_key = (int64_t)kb * kBlockKeys, hi_key = lo_key + kBlockKeys - 1;
+            // rows (positions) that see a key of the block: causal p >= lo_key; window p <= hi_key + W - 1, or a sink block
+            const int64_t p_first = std::max(p0, lo_key);
+            const int64_t p_last = (lo_key < ns) ? (int64_t)sg.kv_len - 1 : std::min<int64_t>(sg.kv_len - 1, hi_key + W - 1);
+            if (p_first > p_last) continue;
+            items.push_back(MassItem{(int)si, kb, (int)((p_first - p0) / TT), (int)((p_last - p0) / TT + 1)});
+        }
+    }
+    const int n_items = (int)items.size();
+    const int n_cta = std::min(n_items, c->num_sms);
+    std::vector<int32_t> cta_off((size_t)n_cta + 1, 0);
+    std::vector<MassItem> ordered;
+    if (n_items > 0) {
+        // LPT over the persistent grid, cost = query tiles of the item (+1 for the K block load)
+        std::vector<int> order((size_t)n_items);
+        for (int i = 0; i < n_items; ++i) order[(size_t)i] = i;
+        auto cost = [&](int i) { return items[(size_t)i].t_hi - items[(size_t)i].t_lo + 1; };
+        std::sort(order.begin(), order.end(), [&](int a, int b) { return cost(a) != cost(b) ? cost(a) > cost(b) : a < b; });
+        std::vector<int64_t> heap((size_t)n_cta);
+        for (int q = 0; q < n_cta; ++q) heap[(size_t)q] = q;
+        std::vector<std::vector<int>> per((size_t)n_cta);
+        auto gt = std::greater<int64_t>();
+        for (int idx : order) {
+            std::pop_heap(heap.begin(), heap.end(), gt);
+            int64_t& top = heap.back();
+            per[(size_t)(top & 1023)].push_back(idx);
+            top += (int64_t)cost(idx) * 1024;
+            std::push_heap(heap.begin(), heap.end(), gt);
+        }
+        for (int q = 0; q < n_cta; ++q) {
+            for (int idx : per[(size_t)q]) ordered.push_back(items[(size_t)idx]);
+            cta_off[(size_t)q + 1] = (int32_t)ordered.size();
+        }
+    }
+    std::vector<int32_t> kv_lens(s->segs.size());
+    for (size_t i = 0; i < s->segs.size(); ++i) kv_lens[i] = s->segs[i].kv_len;
+    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    s->m_off_items = 0;
+    s->m_off_cta = al(std::max<size_t>(1, ordered.size()) * sizeof(MassItem));
+    s->m_off_layout = al(s->m_off_cta + cta_off.size() * sizeof(int32_t));
+    s->m_off_kvlen = al(s->m_off_layout + s->mass_off.size() * sizeof(int64_t));
+    const size_t bytes = al(s->m_off_kvlen + kv_lens.size() * sizeof(int32_t));
+    Staging& sg = s->buf->mass_blob;
+    cudaError_t e = staging_acquire(sg, bytes);
+    if (e == cudaSuccess) {
+        uint8_t* hb = (uint8_t*)sg.h;
+        if (!ordered.empty()) memcpy(hb + s->m_off_items, ordered.data(), ordered.size() * sizeof(MassItem));
+        memcpy(hb + s->m_off_cta, cta_off.data(), cta_off.size() * sizeof(int32_t));
+        memcpy(hb + s->m_off_layout, s->mass_off.data(), s->mass_off.size() * sizeof(int64_t));
+        memcpy(hb + s->m_off_kvlen, kv_lens.data(), kv_lens.size() * sizeof(int32_t));
+        e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+    }
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(e == cudaErrorMemoryAllocation ? SEGPA_ERR_OOM : SEGPA_ERR_CUDA, "attention_mass: %s", cudaGetErrorString(e)); }
+    s->mass_n_cta = n_cta;
+    s->mass_planned = true;
+    return SEGPA_OK;
+}
+
+}  // namespace
+
+segpa_status_t segpa_attention_mass(segpa_cache_t* c, const segpa_segments_t* s, const void* q, int64_t q_row_stride, float scale,
+                                    const float* lse, int64_t lse_stride, int64_t T, float* mass, int64_t mass_len,
+                                    void* cuda_stream) {
+    if (!c || !s || !q || !lse || !mass) return fail(SEGPA_ERR_INVALID, "attention_mass: null argument");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "attention_mass: planning-only cache has no device");
+    if (s->cache != c || std::find(c->seg_objs.begin(), c->seg_objs.end(), s) == c->seg_objs.end())
+        return fail(SEGPA_ERR_STATE, "attention_mass: segments were not built by this cache (or were freed)");
+    const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
+    if (T < s->stats.q_rows || lse_stride < T) return fail(SEGPA_ERR_INVALID, "attention_mass: T / lse_stride smaller than the plan's rows");
+    if (q_row_stride < (int64_t)Hq * D || (q_row_stride % 8) || ((uintptr_t)q % 16)) return fail(SEGPA_ERR_INVALID, "attention_mass: bad q stride / alignment");
+    if (mass_len < s->mass_off.back()) return fail(SEGPA_ERR_INVALID, "attention_mass: mass has %lld entries, the layout needs %lld", (long long)mass_len, (long long)s->mass_off.back());
+    if (!(scale > 0.f) || !(scale < 1e30f)) return fail(SEGPA_ERR_INVALID, "attention_mass: softmax_scale must be positive and finite");
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->last_stream = st;
+    segpa_status_t rc = plan_mass(c, s, st);
+    if (rc != SEGPA_OK) return rc;
+    MassParams p{};
+    const char* why = encode_q_map(&p.q_map, q, T, Hq, D, c->G, kTileRows / c->G, q_row_stride);
+    if (why) return fail(SEGPA_ERR_CUDA, "attention_mass: %s", why);
+    const uint8_t* mb = (const uint8_t*)s->buf->mass_blob.d;
+    const uint8_t* db = (const uint8_t*)s->buf->blob.d;
+    p.segs = (const SegDev*)(db + s->off_segs);
+    p.pages = (const int*)(db + s->off_pages);
+    p.items = (const MassItem*)(mb + s->m_off_items);
+    p.cta_off = (const int*)(mb + s->m_off_cta);
+    p.mass_off = (const long long*)(mb + s->m_off_layout);
+    p.k_pool = c->k_pool;
+    p.lse = lse;
+    p.mass = mass;
+    p.lse_stride = lse_stride;
+    p.scale = scale;
+    p.n_cta = s->mass_n_cta;
+    p.G = c->G;
+    p.D = D;
+    p.P = c->desc.page_size;
+    p.tile_tokens = kTileRows / c->G;
+    p.page_bytes = c->page_bytes;
+    cudaError_t e = cudaMemsetAsync(mass, 0, (size_t)s->mass_off.back() * sizeof(float), st);
+    if (e == cudaSuccess) e = launch_attention_mass(p, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_mass: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_mass_select(segpa_cache_t* c, const segpa_segments_t* s, const float* mass, float tau, uint8_t* selected,
+                                 int32_t* n_selected, void* cuda_stream) {
+    if (!c || !s || !mass || !selected || !n_selected) return fail(SEGPA_ERR_INVALID, "mass_select: null argument");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "mass_select: planning-only cache has no device");
+    if (s->cache != c || std::find(c->seg_objs.begin(), c->seg_objs.end(), s) == c->seg_objs.end())
+        return fail(SEGPA_ERR_STATE, "mass_select: segments were not built by this cache (or were freed)");
+    if (!(tau > 0.f) || !(tau <= 1.f)) return fail(SEGPA_ERR_INVALID, "mass_select: tau must be in (0, 1]");
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    s->last_stream = st;
+    segpa_status_t rc = plan_mass(c, s, st);
+    if (rc != SEGPA_OK) return rc;
+    const uint8_t* mb = (const uint8_t*)s->buf->mass_blob.d;
+    cudaError_t e = cudaMemsetAsync(selected, 0, (size_t)s->mass_off.back(), st);
+    if (e == cudaSuccess)
+        e = launch_mass_select(mass, (const long long*)(mb + s->m_off_layout), (const int*)(mb + s->m_off_kvlen), (int)s->segs.size(), tau,
+                               selected, n_selected, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "mass_select: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;
 }
 

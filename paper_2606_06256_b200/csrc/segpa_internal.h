@@ -140,6 +140,35 @@ cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, con
 cudaError_t launch_merge(const uint16_t* out_a, const float* lse_a, const uint16_t* out_b, const float* lse_b, uint16_t* out,
                          float* lse, long long row_stride, long long lse_stride, long long T, int Hq, int D, cudaStream_t st);
 
+// ---------------------------------------------------------------------------------------------
+// Attention mass (SelectImportantTokens by-product): one work item = one 128-key block of a
+// segment and the range of query tiles that can see it.
+// ---------------------------------------------------------------------------------------------
+struct MassItem {
+    int seg;
+    int kb;                 // 128-key block of the segment's stream
+    int t_lo, t_hi;         // query tiles [t_lo, t_hi) (tile = tile_tokens tokens x G heads) with a row that sees a key of the block
+};
+
+struct MassParams {
+    TensorMap q_map;             // same map as FwdParams::q_map
+    const SegDev* segs;
+    const MassItem* items;
+    const int* cta_off;          // [n_cta + 1]
+    const int* pages;
+    const long long* mass_off;   // [n_segments]: first entry of each segment in `mass`
+    const uint8_t* k_pool;
+    const float* lse;            // [Hq][lse_stride] from segpa_attention_fwd
+    float* mass;
+    long long lse_stride;
+    float scale;
+    int n_cta;
+    int G, D, P, tile_tokens, page_bytes;
+};
+cudaError_t launch_attention_mass(const MassParams& p, cudaStream_t st);
+cudaError_t launch_mass_select(const float* mass, const long long* mass_off_dev, const int* kv_len_dev, int n_segments, float tau,
+                               unsigned char* selected, int* n_selected, cudaStream_t st);
+
 // kernel launchers (each returns the CUDA error of its launch)
 cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const ScatterJob* jobs_dev, int n_jobs,
                                  const int* page_ids_dev, long long total_chunks, int D, int P, cudaStream_t st);

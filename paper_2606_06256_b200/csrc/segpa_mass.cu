@@ -1,0 +1,309 @@
+// Attention mass per key (by-product for SelectImportantTokens, Alg. 1 line 19):
+//     mass[s][j] = sum over the query rows t and query heads g of segment s of p(t, g, j),
+//     p(t, g, j) = exp(scale * q . k_j - LSE(t, g)) for visible j, 0 otherwise,
+// recomputed from Q, the paged K and the LSE the fused attention wrote (the probabilities themselves never
+// exist in memory).  Transposed formulation so that the sum over queries is an in-thread sum:
+//     S^T = K_block Q_tile^T    (M = 128 keys = TMEM lanes, N = 128 query rows = columns)
+// tcgen05.mma with both operands K-major from shared memory (K pages by bulk copy, Q tiles by TMA), accumulator
+// double-buffered in TMEM; one thread per key applies the visibility rule and ex2 to its 128 columns and keeps the
+// running sum in a register.  A CTA owns a (segment, key block) item and loops over the query tiles that can see
+// it: every mass entry is written exactly once, by one thread (deterministic, no atomics).
+// Bound: the dense contraction is half of the attention kernel's (no PV) and the exponentials are the same, so the
+// MUFU pipe (16 ex2 / clk / SM = 1024 clk per 128x128 tile) limits it at twice the MMA time.
+//
+// 8 warps: 0 loader (K block, Q tiles, per-column LSE / position arrays), 1 MMA issuer, 2-3 idle, 4-7 exp warpgroup.
+#include "segpa_internal.h"
+#include "sm100_ptx.cuh"
+
+namespace segpa {
+using namespace ptx;
+
+namespace {
+
+constexpr int kMassThreads = 256;
+
+struct MassAux {
+    float lse2[kTileRows];   // LSE of column c in log2 units
+    int pos[kTileRows];      // query position of column c; -1: no such row
+    int pmin, pmax;          // over the valid columns
+    int pad[2];
+};
+
+struct MassBars {
+    uint64_t k_full, k_empty;
+    uint64_t q_full[2], q_empty[2];
+    uint64_t aux_full[2], aux_empty[2];
+    uint64_t s_full[2], s_empty[2];
+    uint32_t tmem_base;
+};
+
+}  // namespace
+
+template <int D>
+__global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const __grid_constant__ MassParams p) {
+    constexpr int kTileBytes = kTileRows * D * 2;
+    constexpr int kHalves = D / 64;
+    constexpr uint32_t kSBO = kHalves * kAtomBytes;
+    extern __shared__ uint8_t smem_raw[];
+    __shared__ MassBars bars;
+    __shared__ MassAux aux[2];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
+    const uint32_t sK = smem_u32(smem);
+    const uint32_t sQ = sK + kTileBytes;          // two Q stages
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
+    const int i_lo = p.cta_off[blockIdx.x], i_hi = p.cta_off[blockIdx.x + 1];
+
+    if (threadIdx.x == 0) {
+        mbar_init(smem_u32(&bars.k_full), 1);
+        mbar_init(smem_u32(&bars.k_empty), 1);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(smem_u32(&bars.q_full[s]), 1);
+            mbar_init(smem_u32(&bars.q_empty[s]), 1);
+            mbar_init(smem_u32(&bars.aux_full[s]), 1);
+            mbar_init(smem_u32(&bars.aux_empty[s]), 128);
+            mbar_init(smem_u32(&bars.s_full[s]), 1);
+            mbar_init(smem_u32(&bars.s_empty[s]), 128);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 2) {
+        tmem_alloc(smem_u32(&bars.tmem_base), 256);
+        tmem_relinquish();
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = bars.tmem_base;
+
+    if (warp == 0) {
+        // ------------------------------------------------------------------ loader
+        uint32_t n_k = 0, n_t = 0;      // K fills, tile fills so far
+        if (lane == 0) prefetch_tmap(&p.q_map);
+        for (int ii = i_lo; ii < i_hi; ++ii) {
+            const MassItem it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            if (lane == 0) {
+                mbar_wait(smem_u32(&bars.k_empty), (n_k & 1) ^ 1);
+                mbar_arrive_expect_tx(smem_u32(&bars.k_full), kTileBytes);
+            }
+            __syncwarp();
+            if (lane < ppb) {
+                const int page = p.pages[sg.page_off + (long long)(it.kb * ppb - sg.first_page) + lane];
+                bulk_g2s(sK + lane * p.page_bytes, p.k_pool + (size_t)page * p.page_bytes, p.page_bytes, smem_u32(&bars.k_full));
+            }
+            ++n_k;
+            const int p0 = sg.kv_len - sg.q_len;
+            for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
+                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                // per-column LSE and position of this tile (columns past the segment's rows: position -1)
+                if (lane == 0) mbar_wait(smem_u32(&bars.aux_empty[st]), ph ^ 1);
+                __syncwarp();
+                const int tok0 = ti * TT;
+                const int n_rows = min(TT, sg.q_len - tok0) * G;
+                int pmin = INT32_MAX, pmax = -1;
+                for (int c = lane; c < kTileRows; c += 32) {
+                    int pos = -1;
+                    float l2 = 0.f;
+                    if (c < n_rows) {
+                        const int tok = tok0 + c / G, head = sg.kv_head * G + c % G;
+                        pos = p0 + tok;
+                        l2 = p.lse[(long long)head * p.lse_stride + sg.q_row_start + tok] * 1.4426950408889634f;
+                        pmin = min(pmin, pos);
+                        pmax = max(pmax, pos);
+                    }
+                    aux[st].pos[c] = pos;
+                    aux[st].lse2[c] = l2;
+                }
+                pmin = __reduce_min_sync(0xffffffffu, pmin);
+                pmax = __reduce_max_sync(0xffffffffu, pmax);
+                if (lane == 0) { aux[st].pmin = pmin; aux[st].pmax = pmax; }
+                __syncwarp();
+                if (lane == 0) {
+                    mbar_arrive(smem_u32(&bars.aux_full[st]));
+                    mbar_wait(smem_u32(&bars.q_empty[st]), ph ^ 1);
+                    mbar_arrive_expect_tx(smem_u32(&bars.q_full[st]), (uint32_t)(64 * 2 * G * TT) * kHalves);
+#pragma unroll
+                    for (int h = 0; h < kHalves; ++h)
+                        tma_load_3d(sQ + st * kTileBytes + h * (kTileRows * 128), &p.q_map, h * 64, sg.kv_head * G,
+                                    (int)(sg.q_row_start + tok0), smem_u32(&bars.q_full[st]));
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp == 1) {
+        // ------------------------------------------------------------------ MMA issuer: S^T = K Q^T
+        constexpr uint32_t idesc = make_idesc_bf16(128, 128, 0, 0);
+        const uint64_t dk0 = make_desc_sw128(sK, 16, kSBO);             // A: K block image (page layout)
+        const uint64_t dq0 = make_desc_sw128(sQ, 16, kAtomBytes);       // B: Q tile image (TMA box layout)
+        uint32_t n_k = 0, n_t = 0;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
+            const MassItem it = p.items[ii];
+            mbar_wait(smem_u32(&bars.k_full), n_k & 1);
+            ++n_k;
+            for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
+                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                mbar_wait(smem_u32(&bars.q_full[st]), ph);
+                mbar_wait(smem_u32(&bars.s_empty[st]), ph ^ 1);
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint64_t dq = dq0 + (uint64_t)((st * kTileBytes) >> 4);
+#pragma unroll
+                    for (int kk = 0; kk < D / 16; ++kk) {
+                        const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
+                        const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                        mma_ss(tmem + st * 128, dk0 + ok, dq + oq, idesc, kk > 0 ? 1u : 0u);
+                    }
+                    tc_commit(smem_u32(&bars.s_full[st]));
+                    tc_commit(smem_u32(&bars.q_empty[st]));
+                    if (ti + 1 == it.t_hi) tc_commit(smem_u32(&bars.k_empty));
+                }
+                __syncwarp();
+            }
+        }
+    } else if (warp >= 4) {
+        // ------------------------------------------------------------------ exp warpgroup: thread = key
+        const int wq = warp & 3;
+        const int kr = wq * 32 + lane;                                   // key row inside the block
+        const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
+        const float sl2 = p.scale * 1.4426950408889634f;
+        uint32_t n_t = 0;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
+            const MassItem it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            const int key = it.kb * kBlockKeys + kr;
+            const int blk_lo = it.kb * kBlockKeys, blk_hi = blk_lo + kBlockKeys - 1;
+            const bool is_sink_key = key < sg.n_sink;
+            float acc = 0.f;
+            for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
+                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                mbar_wait(smem_u32(&bars.aux_full[st]), ph);
+                mbar_wait(smem_u32(&bars.s_full[st]), ph);
+                tc_fence_after();
+                const MassAux& ax = aux[st];
+                // the whole block is visible to every valid column of the tile: causal (blk_hi <= pmin) and inside
+                // the window of the latest query (blk_lo > pmax - W); columns without a row have position -1
+                const bool all_rows = ax.pos[kTileRows - 1] >= 0;
+                const bool full = all_rows && blk_hi <= ax.pmin && blk_lo > ax.pmax - sg.window;
+                float part = 0.f;
+#pragma unroll
+                for (int cb = 0; cb < 4; ++cb) {
+                    uint32_t s[32];
+                    tmem_ld32(tmem + lane_base + st * 128 + cb * 32, s);
+                    tmem_wait_ld();
+                    if (full) {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) part += fast_exp2(fmaf(__uint_as_float(s[e]), sl2, -ax.lse2[cb * 32 + e]));
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) {
+                            const int pos = ax.pos[cb * 32 + e];
+                            const bool vis = key <= pos && (key > pos - sg.window || is_sink_key);
+                            const float pe = fast_exp2(fmaf(__uint_as_float(s[e]), sl2, -ax.lse2[cb * 32 + e]));
+                            part += vis ? pe : 0.f;
+                        }
+                    }
+                }
+                acc += part;
+                tc_fence_before();
+                mbar_arrive(smem_u32(&bars.s_empty[st]));
+                mbar_arrive(smem_u32(&bars.aux_empty[st]));
+            }
+            if (key < sg.kv_len) p.mass[p.mass_off[it.seg] + key] = acc;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) tmem_dealloc(tmem, 256);
+}
+
+template <int D>
+static cudaError_t launch_mass_one(const MassParams& p, cudaStream_t st) {
+    constexpr int smem = 3 * kTileRows * D * 2 + 1024;
+    static bool configured = false;
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(attention_mass_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    attention_mass_kernel<D><<<p.n_cta, kMassThreads, smem, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_attention_mass(const MassParams& p, cudaStream_t st) {
+    if (p.n_cta == 0) return cudaSuccess;
+    return p.D == 128 ? launch_mass_one<128>(p, st) : launch_mass_one<64>(p, st);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Selection: per segment, the smallest set of keys whose cumulative mass reaches tau * (total mass)
+// ("the smallest set of tokens whose cumulative attention mass exceeds a threshold tau").
+// One block per segment; bisection over the bit pattern of the (non-negative) fp32 masses finds the largest
+// threshold t with sum{m >= t} >= tau * total; keys with m > t are selected, and of the keys with m == t as
+// many (lowest positions first) as are still needed.  Sums run in a fixed order (deterministic).
+// ---------------------------------------------------------------------------------------------
+__device__ float block_sum(float v, float* red) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    __syncthreads();
+    if (lane == 0) red[warp] = v;
+    __syncthreads();
+    float t = 0.f;
+    for (int w = 0; w < (int)(blockDim.x >> 5); ++w) t += red[w];
+    return t;
+}
+
+__global__ void mass_select_kernel(const float* __restrict__ mass, const long long* __restrict__ mass_off, const int* __restrict__ kv_len,
+                                   float tau, unsigned char* __restrict__ selected, int* __restrict__ n_selected) {
+    __shared__ float red[32];
+    const int seg = blockIdx.x, n = kv_len[seg];
+    const float* m = mass + mass_off[seg];
+    unsigned char* sel = selected + mass_off[seg];
+    float tot = 0.f;
+    for (int j = threadIdx.x; j < n; j += blockDim.x) tot += m[j];
+    tot = block_sum(tot, red);
+    const float need = tau * tot;
+    // largest bit pattern t with sum{m >= t} >= need (masses are >= 0: their bit patterns order like the values)
+    unsigned lo = 0u, hi = 0x7f800000u;
+    while (lo < hi) {
+        const unsigned mid = lo + (hi - lo + 1) / 2;
+        float sum = 0.f;
+        for (int j = threadIdx.x; j < n; j += blockDim.x) sum += (__float_as_uint(m[j]) >= mid) ? m[j] : 0.f;
+        sum = block_sum(sum, red);
+        if (sum >= need) lo = mid; else hi = mid - 1;
+    }
+    float above = 0.f;
+    for (int j = threadIdx.x; j < n; j += blockDim.x) above += (__float_as_uint(m[j]) > lo) ? m[j] : 0.f;
+    above = block_sum(above, red);
+    const float tval = __uint_as_float(lo);
+    // ties at the threshold: take the lowest positions until the mass is reached
+    int ties_needed = 0;
+    if (tval > 0.f) {
+        const float rest = need - above;
+        ties_needed = rest > 0.f ? (int)ceilf(rest / tval) : 0;
+    }
+    __syncthreads();
+    // sequential over positions for the tie rule (one thread; n is a stream length, the pass is a few microseconds)
+    if (threadIdx.x == 0) {
+        int taken = 0, cnt = 0;
+        for (int j = 0; j < n; ++j) {
+            const unsigned b = __float_as_uint(m[j]);
+            unsigned char s = 0;
+            if (b > lo) s = 1;
+            else if (b == lo && taken < ties_needed) { s = 1; ++taken; }
+            sel[j] = s;
+            cnt += s;
+        }
+        n_selected[seg] = cnt;
+    }
+}
+
+cudaError_t launch_mass_select(const float* mass, const long long* mass_off_dev, const int* kv_len_dev, int n_segments, float tau,
+                               unsigned char* selected, int* n_selected, cudaStream_t st) {
+    if (n_segments <= 0) return cudaSuccess;
+    mass_select_kernel<<<n_segments, 1024, 0, st>>>(mass, mass_off_dev, kv_len_dev, tau, selected, n_selected);
+    return cudaGetLastError();
+}
+
+}  // namespace segpa

@@ -1,0 +1,91 @@
+"""GPU parity of segpa_attention_mass / segpa_mass_select (SelectImportantTokens by-product).
+
+Oracle: the attention oracle's own probabilities p(t, g, j) (want_p), summed over a segment's rows and group heads.
+Tolerance: p is recomputed as ex2 of an fp32 score (bf16 products, fp32 accumulate) minus
+the fp32 LSE the forward pass wrote (|dLSE| <= 1e-3 by the forward tolerance, measured ~1e-6), so each term is off by
+at most ~1e-3 relative: |gpu - oracle| <= 4e-3 * oracle + 1e-3 per key; the total mass equals rows x G within 1e-3."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+from paper_2606_06256_b200.workloads import GLOBAL, LOCAL
+from tests.gpu_helpers import GpuRun
+from tests.helpers import run_oracle
+
+pytestmark = pytest.mark.gpu
+
+CASES = [
+    (8, 2, 128, 16, [{"kv_len": 700, "heads": {0: (GLOBAL, 0, 0, 300), 1: (LOCAL, 100, 0, 300)}}]),
+    (8, 2, 64, 32, [{"kv_len": 515, "heads": {0: (LOCAL, 64, 4, 515), 1: (GLOBAL, 0, 0, 130)}},
+                    {"kv_len": 1300, "heads": {0: (GLOBAL, 0, 0, 1), 1: (LOCAL, 300, 130, 3)}}]),
+    (28, 4, 128, 32, [{"kv_len": 900, "heads": {0: (GLOBAL, 0, 0, 200), 1: (LOCAL, 257, 0, 200), 2: (LOCAL, 4096, 0, 77), 3: (GLOBAL, 0, 0, 19)}}]),
+]
+
+
+@pytest.mark.parametrize("case", range(len(CASES)))
+def test_attention_mass_matches_oracle_column_sums(case):
+    Hq, Hkv, D, P, reqs = CASES[case]
+    w = wl.make_workload("mass%d" % case, Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=500 + case)
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        segs = g.segs[0]
+        offs = B.segpa_segments_mass_layout(segs)
+        mass = torch.full((int(offs[-1]),), -1.0, dtype=torch.float32, device=g.dev)
+        B.segpa_attention_mass(g.cache, segs, q, w.scale, lse, mass)
+        m2 = torch.zeros_like(mass)
+        B.segpa_attention_mass(g.cache, segs, q, w.scale, lse, m2)          # deterministic
+        torch.cuda.synchronize()
+        assert torch.equal(mass, m2)
+        mass = mass.cpu().numpy().astype(np.float64)
+        kv_max = max(s.kv_len for s in w.streams)
+        res = run_oracle(w, 0, g.k_pool, g.v_pool, q, want_p=kv_max)
+        sm = w.stream_map()
+        for si, s in enumerate(w.layer_segments(0)):
+            kv = sm[(0, s.kv_head, s.seq_id)].kv_len
+            want = res.p[s.q_row_start:s.q_row_start + s.q_len, s.kv_head * w.G:(s.kv_head + 1) * w.G, :kv].sum(axis=(0, 1))
+            got = mass[offs[si]:offs[si] + kv]
+            assert np.all(np.abs(got - want) <= 4e-3 * want + 1e-3), (si, np.abs(got - want).max())
+            assert abs(got.sum() - s.q_len * w.G) <= 1e-3 * s.q_len * w.G          # every row's p sums to 1
+            assert np.all(mass[offs[si] + kv:offs[si + 1]] == 0)                   # padding
+            assert np.all(got[want == 0] == 0)                                     # keys nobody sees
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("tau", [0.05, 0.5, 0.9, 1.0])
+def test_mass_select_is_the_smallest_covering_set(tau):
+    Hq, Hkv, D, P, reqs = CASES[0]
+    w = wl.make_workload("sel", Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=600)
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        segs = g.segs[0]
+        offs = B.segpa_segments_mass_layout(segs)
+        mass = torch.zeros((int(offs[-1]),), dtype=torch.float32, device=g.dev)
+        B.segpa_attention_mass(g.cache, segs, q, w.scale, lse, mass)
+        sel = torch.full((int(offs[-1]),), 7, dtype=torch.uint8, device=g.dev)
+        cnt = torch.zeros((len(offs) - 1,), dtype=torch.int32, device=g.dev)
+        B.segpa_mass_select(g.cache, segs, mass, tau, sel, cnt)
+        torch.cuda.synchronize()
+        m, sl, cn = mass.cpu().numpy().astype(np.float64), sel.cpu().numpy(), cnt.cpu().numpy()
+        sm = w.stream_map()
+        for si, s in enumerate(w.layer_segments(0)):
+            kv = sm[(0, s.kv_head, s.seq_id)].kv_len
+            mm, ss = m[offs[si]:offs[si] + kv], sl[offs[si]:offs[si] + kv].astype(bool)
+            tot = mm.sum()
+            assert ss.sum() == cn[si] and np.all(sl[offs[si] + kv:offs[si + 1]] == 0)
+            # valid: covers tau of the mass; every selected key is at least as heavy as every unselected one
+            assert mm[ss].sum() >= tau * tot * (1 - 1e-5)
+            if (~ss).any() and ss.any():
+                assert mm[ss].min() >= mm[~ss].max()
+            # smallest: without its lightest member the set no longer covers tau (up to fp32 summation noise)
+            if ss.any():
+                assert mm[ss].sum() - mm[ss].min() < tau * tot * (1 + 1e-5)
+            # what is unique: the size of the smallest covering set (compare with a sort-based restatement)
+            order = np.sort(mm)[::-1]
+            k_star = int(np.searchsorted(np.cumsum(order), tau * tot * (1 - 1e-6)) + 1)
+            assert abs(int(cn[si]) - min(k_star, kv)) <= 1
+    finally:
+        g.close()
