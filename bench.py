@@ -474,6 +474,57 @@ def run_rope(args):
                       "gpu_launches": args.steps}))
 
 
+def run_mass(args):
+    """`--config mass`: the step after the hot path (attention mass + salient-token selection, PAPER.md:198, 296;
+    SURVEY 8(f) NEXT #4) on cfg2.  The contraction is S^T = K Q^T only: 2*D FLOPs per attended (query, key, q-head)."""
+    import torch
+    from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    w = wl.config2()
+    peaks, peaks_src = load_peaks()
+    k_pool, v_pool = wl.pool_values(w, dev)
+    cache = H.create_cache(w, 0)
+    H.append_workload(cache, w, k_pool, v_pool)
+    segs = H.build_layer(cache, w, 0)
+    q = wl.q_values(w, 0, dev)
+    out = torch.empty_like(q)
+    lse = torch.empty((w.Hq, w.T[0]), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+    B.segpa_attention_fwd(cache, segs, q, w.scale, out, lse, stream=stream)
+    offs = B.segpa_segments_mass_layout(segs)
+    mass = torch.zeros((int(offs[-1]),), dtype=torch.float32, device=dev)
+    sel = torch.zeros((int(offs[-1]),), dtype=torch.uint8, device=dev)
+    cnt = torch.zeros((len(offs) - 1,), dtype=torch.int32, device=dev)
+    flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+    flops = wl.useful_flops(w, 0) // 2
+    ms_mass, ms_sel = [], []
+    for i in range(max(3, args.warmup) + args.steps):
+        flush_buf.fill_(1)
+        torch.cuda.synchronize()
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record(stream)
+        B.segpa_attention_mass(cache, segs, q, w.scale, lse, mass, stream=stream)
+        e1.record(stream)
+        B.segpa_mass_select(cache, segs, mass, 0.7, sel, cnt, stream=stream)
+        e2.record(stream)
+        e2.synchronize()
+        if i >= max(3, args.warmup):
+            ms_mass.append(e0.elapsed_time(e1))
+            ms_sel.append(e1.elapsed_time(e2))
+    t, ts = float(np.mean(ms_mass)), float(np.mean(ms_sel))
+    tf = flops / (t * 1e-3) / 1e12
+    B.segpa_destroy(cache)
+    print(json.dumps({"metric": "attention_mass_useful_tflops", "value": tf, "unit": "TFLOP/s (useful: 2*D per attended (query, key, q-head) pair)",
+                      "n_gpus": 1, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": t, "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+                      "config": {"workload": "attention mass over " + w.name, "l2_flush_between_steps": True, "select_ms": ts, "tau": 0.7},
+                      "roofline": {"bound": "tensor", "achieved": tf, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s", "frac": tf / peaks["bf16_tflops"],
+                                   "traffic": None, "useful_flops": flops, "peak_source": peaks_src,
+                                   "kernel": "attention_mass_kernel; MUFU co-limited: 1024 ex2 cycles per 512 MMA cycles per tile"},
+                      "gpu_launches": 2 * args.steps}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -492,6 +543,8 @@ def main():
         args.warmup = 3
     if args.config == "rope" and args.impl == "ours":
         run_rope(args)
+    elif args.config == "mass" and args.impl == "ours":
+        run_mass(args)
     elif args.impl == "reference":
         run_reference(args)
     else:

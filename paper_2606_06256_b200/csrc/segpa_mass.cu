@@ -11,7 +11,7 @@
 // Bound: the dense contraction is half of the attention kernel's (no PV) and the exponentials are the same, so the
 // MUFU pipe (16 ex2 / clk / SM = 1024 clk per 128x128 tile) limits it at twice the MMA time.
 //
-// 8 warps: 0 loader (K block, Q tiles, per-column LSE / position arrays), 1 MMA issuer, 2-3 idle, 4-7 exp warpgroup.
+// 8 warps: 0 loader (K block, Q tiles), 1 MMA issuer, 2 per-column LSE / position arrays, 3 TMEM, 4-7 exp warpgroup.
 #include "segpa_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -22,7 +22,7 @@ namespace {
 
 constexpr int kMassThreads = 256;
 
-struct MassAux {
+struct alignas(16) MassAux {
     float lse2[kTileRows];   // LSE of column c in log2 units
     int pos[kTileRows];      // query position of column c; -1: no such row
     int pmin, pmax;          // over the valid columns
@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
         }
         fence_mbar_init();
     }
-    if (warp == 2) {
+    if (warp == 3) {
         tmem_alloc(smem_u32(&bars.tmem_base), 256);
         tmem_relinquish();
     }
@@ -93,34 +93,10 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                 bulk_g2s(sK + lane * p.page_bytes, p.k_pool + (size_t)page * p.page_bytes, p.page_bytes, smem_u32(&bars.k_full));
             }
             ++n_k;
-            const int p0 = sg.kv_len - sg.q_len;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
                 const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
-                // per-column LSE and position of this tile (columns past the segment's rows: position -1)
-                if (lane == 0) mbar_wait(smem_u32(&bars.aux_empty[st]), ph ^ 1);
-                __syncwarp();
                 const int tok0 = ti * TT;
-                const int n_rows = min(TT, sg.q_len - tok0) * G;
-                int pmin = INT32_MAX, pmax = -1;
-                for (int c = lane; c < kTileRows; c += 32) {
-                    int pos = -1;
-                    float l2 = 0.f;
-                    if (c < n_rows) {
-                        const int tok = tok0 + c / G, head = sg.kv_head * G + c % G;
-                        pos = p0 + tok;
-                        l2 = p.lse[(long long)head * p.lse_stride + sg.q_row_start + tok] * 1.4426950408889634f;
-                        pmin = min(pmin, pos);
-                        pmax = max(pmax, pos);
-                    }
-                    aux[st].pos[c] = pos;
-                    aux[st].lse2[c] = l2;
-                }
-                pmin = __reduce_min_sync(0xffffffffu, pmin);
-                pmax = __reduce_max_sync(0xffffffffu, pmax);
-                if (lane == 0) { aux[st].pmin = pmin; aux[st].pmax = pmax; }
-                __syncwarp();
                 if (lane == 0) {
-                    mbar_arrive(smem_u32(&bars.aux_full[st]));
                     mbar_wait(smem_u32(&bars.q_empty[st]), ph ^ 1);
                     mbar_arrive_expect_tx(smem_u32(&bars.q_full[st]), (uint32_t)(64 * 2 * G * TT) * kHalves);
 #pragma unroll
@@ -129,6 +105,47 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                                     (int)(sg.q_row_start + tok0), smem_u32(&bars.q_full[st]));
                 }
                 __syncwarp();
+            }
+        }
+    } else if (warp == 2) {
+        // ------------------------------------------------------------------ per-column LSE / position arrays of each tile
+        uint32_t n_t = 0;
+        for (int ii = i_lo; ii < i_hi; ++ii) {
+            const MassItem it = p.items[ii];
+            const SegDev sg = p.segs[it.seg];
+            const int p0 = sg.kv_len - sg.q_len;
+            for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
+                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                const int tok0 = ti * TT;
+                const int n_rows = min(TT, sg.q_len - tok0) * G;
+                // columns past the segment's rows: position -1 (their scores are garbage and never counted)
+                int pos[4], pmin = INT32_MAX, pmax = -1;
+                float l2[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int c = lane + 32 * u;
+                    pos[u] = -1;
+                    l2[u] = 0.f;
+                    if (c < n_rows) {
+                        const int tok = tok0 + c / G, head = sg.kv_head * G + c % G;
+                        pos[u] = p0 + tok;
+                        l2[u] = p.lse[(long long)head * p.lse_stride + sg.q_row_start + tok] * 1.4426950408889634f;
+                        pmin = min(pmin, pos[u]);
+                        pmax = max(pmax, pos[u]);
+                    }
+                }
+                pmin = __reduce_min_sync(0xffffffffu, pmin);
+                pmax = __reduce_max_sync(0xffffffffu, pmax);
+                if (lane == 0) mbar_wait(smem_u32(&bars.aux_empty[st]), ph ^ 1);
+                __syncwarp();
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    aux[st].pos[lane + 32 * u] = pos[u];
+                    aux[st].lse2[lane + 32 * u] = l2[u];
+                }
+                if (lane == 0) { aux[st].pmin = pmin; aux[st].pmax = pmax; }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&bars.aux_full[st]));
             }
         }
     } else if (warp == 1) {
@@ -193,14 +210,26 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                     tmem_wait_ld();
                     if (full) {
 #pragma unroll
-                        for (int e = 0; e < 32; ++e) part += fast_exp2(fmaf(__uint_as_float(s[e]), sl2, -ax.lse2[cb * 32 + e]));
+                        for (int e = 0; e < 32; e += 4) {
+                            const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[cb * 32 + e]);
+                            part += fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
+                            part += fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
+                            part += fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
+                            part += fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
+                        }
                     } else {
 #pragma unroll
-                        for (int e = 0; e < 32; ++e) {
-                            const int pos = ax.pos[cb * 32 + e];
-                            const bool vis = key <= pos && (key > pos - sg.window || is_sink_key);
-                            const float pe = fast_exp2(fmaf(__uint_as_float(s[e]), sl2, -ax.lse2[cb * 32 + e]));
-                            part += vis ? pe : 0.f;
+                        for (int e = 0; e < 32; e += 4) {
+                            const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[cb * 32 + e]);
+                            const int4 p4 = *reinterpret_cast<const int4*>(&ax.pos[cb * 32 + e]);
+                            const float lv[4] = {l4.x, l4.y, l4.z, l4.w};
+                            const int pv[4] = {p4.x, p4.y, p4.z, p4.w};
+#pragma unroll
+                            for (int u = 0; u < 4; ++u) {
+                                const bool vis = key <= pv[u] && (key > pv[u] - sg.window || is_sink_key);
+                                const float pe = fast_exp2(fmaf(__uint_as_float(s[e + u]), sl2, -lv[u]));
+                                part += vis ? pe : 0.f;
+                            }
                         }
                     }
                 }
@@ -215,7 +244,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
 
     tc_fence_before();
     __syncthreads();
-    if (warp == 2) tmem_dealloc(tmem, 256);
+    if (warp == 3) tmem_dealloc(tmem, 256);
 }
 
 template <int D>
