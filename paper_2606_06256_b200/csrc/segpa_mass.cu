@@ -11,7 +11,8 @@
 // Bound: the dense contraction is half of the attention kernel's (no PV) and the exponentials are the same, so the
 // MUFU pipe (16 ex2 / clk / SM = 1024 clk per 128x128 tile) limits it at twice the MMA time.
 //
-// 8 warps: 0 loader (K block, Q tiles), 1 MMA issuer, 2 per-column LSE / position arrays, 3 TMEM, 4-7 exp warpgroup.
+// 12 warps: 0 loader (K block, Q tiles), 1 MMA issuer, 2-3 per-column LSE / position arrays (3 also owns TMEM), 4-7 and 8-11 the two
+// exp warpgroups (each takes half of a tile's query columns).
 #include "segpa_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -20,7 +21,7 @@ using namespace ptx;
 
 namespace {
 
-constexpr int kMassThreads = 256;
+constexpr int kMassThreads = 384;   // 4 service warps + two exp warpgroups
 
 struct alignas(16) MassAux {
     float lse2[kTileRows];   // LSE of column c in log2 units
@@ -29,9 +30,11 @@ struct alignas(16) MassAux {
     int pad[2];
 };
 
+constexpr int kQStages = 4;   // Q tiles in flight (the S accumulator and the per-column arrays are double-buffered)
+
 struct MassBars {
     uint64_t k_full, k_empty;
-    uint64_t q_full[2], q_empty[2];
+    uint64_t q_full[kQStages], q_empty[kQStages];
     uint64_t aux_full[2], aux_empty[2];
     uint64_t s_full[2], s_empty[2];
     uint32_t tmem_base;
@@ -47,9 +50,10 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
     extern __shared__ uint8_t smem_raw[];
     __shared__ MassBars bars;
     __shared__ MassAux aux[2];
+    __shared__ float half_sum[kTileRows];   // partial mass of the second exp warpgroup, added by the first
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
     const uint32_t sK = smem_u32(smem);
-    const uint32_t sQ = sK + kTileBytes;          // two Q stages
+    const uint32_t sQ = sK + kTileBytes;          // kQStages Q stages
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
     const int i_lo = p.cta_off[blockIdx.x], i_hi = p.cta_off[blockIdx.x + 1];
@@ -57,13 +61,15 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
     if (threadIdx.x == 0) {
         mbar_init(smem_u32(&bars.k_full), 1);
         mbar_init(smem_u32(&bars.k_empty), 1);
-        for (int s = 0; s < 2; ++s) {
+        for (int s = 0; s < kQStages; ++s) {
             mbar_init(smem_u32(&bars.q_full[s]), 1);
             mbar_init(smem_u32(&bars.q_empty[s]), 1);
+        }
+        for (int s = 0; s < 2; ++s) {
             mbar_init(smem_u32(&bars.aux_full[s]), 1);
-            mbar_init(smem_u32(&bars.aux_empty[s]), 128);
+            mbar_init(smem_u32(&bars.aux_empty[s]), 256);
             mbar_init(smem_u32(&bars.s_full[s]), 1);
-            mbar_init(smem_u32(&bars.s_empty[s]), 128);
+            mbar_init(smem_u32(&bars.s_empty[s]), 256);
         }
         fence_mbar_init();
     }
@@ -94,7 +100,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             }
             ++n_k;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
-                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                const uint32_t st = n_t % kQStages, ph = (n_t / kQStages) & 1;
                 const int tok0 = ti * TT;
                 if (lane == 0) {
                     mbar_wait(smem_u32(&bars.q_empty[st]), ph ^ 1);
@@ -107,8 +113,10 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                 __syncwarp();
             }
         }
-    } else if (warp == 2) {
+    } else if (warp == 2 || warp == 3) {
         // ------------------------------------------------------------------ per-column LSE / position arrays of each tile
+        // (two warps, one per stage: warp 2 serves the even tiles, warp 3 the odd ones -- a tile costs one
+        // round trip to L2 for the LSE values, which one warp alone cannot hide)
         uint32_t n_t = 0;
         for (int ii = i_lo; ii < i_hi; ++ii) {
             const MassItem it = p.items[ii];
@@ -116,22 +124,29 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             const int p0 = sg.kv_len - sg.q_len;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
                 const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                if ((int)st != warp - 2) continue;
                 const int tok0 = ti * TT;
                 const int n_rows = min(TT, sg.q_len - tok0) * G;
                 // columns past the segment's rows: position -1 (their scores are garbage and never counted)
                 int pos[4], pmin = INT32_MAX, pmax = -1;
                 float l2[4];
+                // the four LSE loads of a lane are issued together (clamped to a valid row), then used
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const int c = lane + 32 * u;
-                    pos[u] = -1;
-                    l2[u] = 0.f;
-                    if (c < n_rows) {
-                        const int tok = tok0 + c / G, head = sg.kv_head * G + c % G;
-                        pos[u] = p0 + tok;
-                        l2[u] = p.lse[(long long)head * p.lse_stride + sg.q_row_start + tok] * 1.4426950408889634f;
+                    const int cc = min(lane + 32 * u, n_rows - 1);
+                    const int tok = tok0 + cc / G, head = sg.kv_head * G + cc % G;
+                    pos[u] = p0 + tok;
+                    l2[u] = p.lse[(long long)head * p.lse_stride + sg.q_row_start + tok];
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    if (lane + 32 * u < n_rows) {
+                        l2[u] *= 1.4426950408889634f;
                         pmin = min(pmin, pos[u]);
                         pmax = max(pmax, pos[u]);
+                    } else {
+                        pos[u] = -1;
+                        l2[u] = 0.f;
                     }
                 }
                 pmin = __reduce_min_sync(0xffffffffu, pmin);
@@ -159,12 +174,13 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             mbar_wait(smem_u32(&bars.k_full), n_k & 1);
             ++n_k;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
+                const uint32_t qs = n_t % kQStages, qph = (n_t / kQStages) & 1;
                 const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
-                mbar_wait(smem_u32(&bars.q_full[st]), ph);
+                mbar_wait(smem_u32(&bars.q_full[qs]), qph);
                 mbar_wait(smem_u32(&bars.s_empty[st]), ph ^ 1);
                 tc_fence_after();
                 if (elect_one()) {
-                    const uint64_t dq = dq0 + (uint64_t)((st * kTileBytes) >> 4);
+                    const uint64_t dq = dq0 + (uint64_t)((qs * kTileBytes) >> 4);
 #pragma unroll
                     for (int kk = 0; kk < D / 16; ++kk) {
                         const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
@@ -172,15 +188,18 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                         mma_ss(tmem + st * 128, dk0 + ok, dq + oq, idesc, kk > 0 ? 1u : 0u);
                     }
                     tc_commit(smem_u32(&bars.s_full[st]));
-                    tc_commit(smem_u32(&bars.q_empty[st]));
+                    tc_commit(smem_u32(&bars.q_empty[qs]));
                     if (ti + 1 == it.t_hi) tc_commit(smem_u32(&bars.k_empty));
                 }
                 __syncwarp();
             }
         }
     } else if (warp >= 4) {
-        // ------------------------------------------------------------------ exp warpgroup: thread = key
+        // ------------------------------------------------------------------ exp warpgroups: thread = (key, half of the columns)
+        // warps 4-7 take the query columns [0, 64) of every tile, warps 8-11 the columns [64, 128): the per-tile
+        // chain (TMEM load, 64 ex2, sum) is half as long; the two partial sums of a key are added in a fixed order
         const int wq = warp & 3;
+        const int hf = (warp - 4) >> 2;                                  // which half of the columns
         const int kr = wq * 32 + lane;                                   // key row inside the block
         const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
         const float sl2 = p.scale * 1.4426950408889634f;
@@ -202,43 +221,45 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                 // the window of the latest query (blk_lo > pmax - W); columns without a row have position -1
                 const bool all_rows = ax.pos[kTileRows - 1] >= 0;
                 const bool full = all_rows && blk_hi <= ax.pmin && blk_lo > ax.pmax - sg.window;
-                float part = 0.f;
+                uint32_t s[64];
+                tmem_ld32(tmem + lane_base + st * 128 + hf * 64, s);
+                tmem_ld32(tmem + lane_base + st * 128 + hf * 64 + 32, s + 32);
+                tmem_wait_ld();
+                float pa = 0.f, pb = 0.f, pc = 0.f, pd = 0.f;
+                if (full) {
 #pragma unroll
-                for (int cb = 0; cb < 4; ++cb) {
-                    uint32_t s[32];
-                    tmem_ld32(tmem + lane_base + st * 128 + cb * 32, s);
-                    tmem_wait_ld();
-                    if (full) {
+                    for (int e = 0; e < 64; e += 4) {
+                        const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[hf * 64 + e]);
+                        pa += fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
+                        pb += fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
+                        pc += fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
+                        pd += fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
+                    }
+                } else {
 #pragma unroll
-                        for (int e = 0; e < 32; e += 4) {
-                            const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[cb * 32 + e]);
-                            part += fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
-                            part += fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
-                            part += fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
-                            part += fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
-                        }
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 32; e += 4) {
-                            const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[cb * 32 + e]);
-                            const int4 p4 = *reinterpret_cast<const int4*>(&ax.pos[cb * 32 + e]);
-                            const float lv[4] = {l4.x, l4.y, l4.z, l4.w};
-                            const int pv[4] = {p4.x, p4.y, p4.z, p4.w};
-#pragma unroll
-                            for (int u = 0; u < 4; ++u) {
-                                const bool vis = key <= pv[u] && (key > pv[u] - sg.window || is_sink_key);
-                                const float pe = fast_exp2(fmaf(__uint_as_float(s[e + u]), sl2, -lv[u]));
-                                part += vis ? pe : 0.f;
-                            }
-                        }
+                    for (int e = 0; e < 64; e += 4) {
+                        const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[hf * 64 + e]);
+                        const int4 p4 = *reinterpret_cast<const int4*>(&ax.pos[hf * 64 + e]);
+                        const float e0 = fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
+                        const float e1 = fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
+                        const float e2 = fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
+                        const float e3 = fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
+                        pa += (key <= p4.x && (key > p4.x - sg.window || is_sink_key)) ? e0 : 0.f;
+                        pb += (key <= p4.y && (key > p4.y - sg.window || is_sink_key)) ? e1 : 0.f;
+                        pc += (key <= p4.z && (key > p4.z - sg.window || is_sink_key)) ? e2 : 0.f;
+                        pd += (key <= p4.w && (key > p4.w - sg.window || is_sink_key)) ? e3 : 0.f;
                     }
                 }
-                acc += part;
+                acc += (pa + pb) + (pc + pd);
                 tc_fence_before();
                 mbar_arrive(smem_u32(&bars.s_empty[st]));
                 mbar_arrive(smem_u32(&bars.aux_empty[st]));
             }
-            if (key < sg.kv_len) p.mass[p.mass_off[it.seg] + key] = acc;
+            // mass = (columns [0, 64)) + (columns [64, 128)), added by the first warpgroup: one writer per entry
+            if (hf == 1) half_sum[kr] = acc;
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+            if (hf == 0 && key < sg.kv_len) p.mass[p.mass_off[it.seg] + key] = acc + half_sum[kr];
+            asm volatile("bar.sync 2, 256;" ::: "memory");
         }
     }
 
@@ -249,7 +270,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
 
 template <int D>
 static cudaError_t launch_mass_one(const MassParams& p, cudaStream_t st) {
-    constexpr int smem = 3 * kTileRows * D * 2 + 1024;
+    constexpr int smem = (1 + kQStages) * kTileRows * D * 2 + 1024;
     static bool configured = false;
     if (!configured) {
         cudaError_t e = cudaFuncSetAttribute(attention_mass_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
