@@ -477,6 +477,10 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const int pos = sg.kv_len - sg.q_len + tok;      // query position i
                 const int key_lo = max(0, pos - sg.window + 1);  // visible keys [key_lo, pos]
                 const bool warp_has_rows = wq * 32 < tr.n_rows;  // decode-shaped tiles: most warps hold no row
+                // positions are non-decreasing along the lanes, so the warp-wide extremes of the visible column range
+                // are those of the first and the last lane: formed once per item, no votes or reductions per block
+                const int pos_w0 = __shfl_sync(0xffffffffu, pos, 0), pos_w1 = __shfl_sync(0xffffffffu, pos, 31);
+                const int klo_w0 = __shfl_sync(0xffffffffu, key_lo, 0), klo_w1 = __shfl_sync(0xffffffffu, key_lo, 31);
                 float m_used = -INFINITY, l = 0.f;
 
                 const int nb = n_blocks(tr);
@@ -491,7 +495,9 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         // visible columns of this block: c <= cmax and (c >= cmin or c < csink)
                         const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;
                         const int csink = sg.n_sink - j * kBlockKeys;        // same for every row of the segment
-                        const bool need_mask = __any_sync(0xffffffffu, cmax < kBlockKeys - 1 || (cmin > 0 && csink < kBlockKeys));
+                        const int mn_cmin = klo_w0 - j * kBlockKeys, mx_cmin = klo_w1 - j * kBlockKeys;   // over the warp's rows
+                        const int mn_cmax = pos_w0 - j * kBlockKeys, mx_cmax = pos_w1 - j * kBlockKeys;
+                        const bool need_mask = mn_cmax < kBlockKeys - 1 || (mx_cmin > 0 && csink < kBlockKeys);
                         // the whole score row of this thread: 128 fp32 columns -> registers, one wait
                         uint32_t s[kBlockKeys];
 #pragma unroll
@@ -502,8 +508,6 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         if (need_mask) {
                             // boundary block (causal diagonal / window edge / sink edge).  Per 32-column chunk, warp-uniformly:
                             // all visible -> untouched; all masked -> no exp at all; ragged -> element mask in registers
-                            const int mn_cmin = __reduce_min_sync(0xffffffffu, cmin), mx_cmin = __reduce_max_sync(0xffffffffu, cmin);
-                            const int mn_cmax = __reduce_min_sync(0xffffffffu, cmax), mx_cmax = __reduce_max_sync(0xffffffffu, cmax);
                             if (sg.n_sink == 0) {
 #pragma unroll
                                 for (int c = 0; c < 4; ++c) {
