@@ -819,8 +819,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         for (size_t i = 1; i < ivs.size(); ++i)
             if (ivs[i].kv_head == ivs[i - 1].kv_head && ivs[i].lo < ivs[i - 1].hi) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: two segments of kv_head %d overlap on rows [%lld, %lld)", ivs[i].kv_head, (long long)ivs[i].lo, (long long)std::min(ivs[i].hi, ivs[i - 1].hi)); }
 
-        // scheduler: split long tiles along KV when the grid would be unbalanced, then order
-        // longest-first; CTAs pull items from a shared cursor (greedy LPT).
+        // scheduler: split long tiles along KV when the grid would be unbalanced (decode-shaped global heads),
+        // then assign the items to the CTAs of the persistent grid (LPT, below)
         int64_t total_cost = 0;
         for (auto& t : tiles) total_cost += t.cost;
         const int64_t chunk = std::max<int64_t>(8, cdiv(total_cost, (int64_t)c->num_sms * 4));
