@@ -379,3 +379,28 @@ def test_lse_merge_of_split_key_sets(j0):
         assert torch.equal(o2, out[0:1]) and torch.equal(l2, lse[:, 0:1])
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_workloads(seed):
+    """Seeded random small workloads over the whole argument space (shape, page size, lengths, class, window,
+    sinks, several requests), product kernel, against the oracle."""
+    rng = np.random.default_rng(4242 + seed)
+    Hkv = int(rng.choice([1, 2, 4]))
+    G = int(rng.choice([1, 2, 4, 7, 8, 16]))
+    D = int(rng.choice([64, 128]))
+    P = int(rng.choice([16, 32]))
+    reqs = []
+    for _ in range(int(rng.integers(1, 5))):
+        kv_len = int(rng.choice([1, 2, 17, 129, 700, 1500, 2600])) + int(rng.integers(0, 50))
+        heads = {}
+        for h in range(Hkv):
+            cls = GLOBAL if rng.random() < 0.35 else LOCAL
+            W = int(rng.choice([1, 2, 63, 64, 65, 128, 300, 5000]))
+            n_sink = int(rng.choice([0, 0, 4, 70, 200])) if cls == LOCAL else 0
+            q_len = int(min(kv_len, rng.choice([1, 1, 3, 40, 129, 10 ** 6])))
+            heads[h] = (cls, W, n_sink, q_len)
+        reqs.append({"kv_len": kv_len, "heads": heads})
+    w = wl.make_workload("rand%d" % seed, Hq=Hkv * G, Hkv=Hkv, D=D, P=P, requests=reqs, seed=9000 + seed)
+    print(Hkv, G, D, P, reqs)
+    print(_run_full(w, "tc", 2, "rand%d" % seed))
