@@ -731,11 +731,14 @@ int attention_tc_tiles_per_item() {
 template <int D, int NT>
 static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
     using C = Cfg<D, NT>;
-    static bool configured = false;
-    if (!configured) {
+    // the opt-in to > 48 KB of dynamic shared memory is per device: remember which devices have it
+    static bool configured[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
         cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<D, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     attention_tc_kernel<D, NT><<<p.n_cta, kThreads, C::kSmemBytes, st>>>(p);
     return cudaGetLastError();

@@ -271,11 +271,14 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
 template <int D>
 static cudaError_t launch_mass_one(const MassParams& p, cudaStream_t st) {
     constexpr int smem = (1 + kQStages) * kTileRows * D * 2 + 1024;
-    static bool configured = false;
-    if (!configured) {
+    // the opt-in to > 48 KB of dynamic shared memory is per device: remember which devices have it
+    static bool configured[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || !configured[dev]) {
         cudaError_t e = cudaFuncSetAttribute(attention_mass_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
-        configured = true;
+        if (dev >= 0 && dev < 64) configured[dev] = true;
     }
     attention_mass_kernel<D><<<p.n_cta, kMassThreads, smem, st>>>(p);
     return cudaGetLastError();
