@@ -64,13 +64,16 @@ constexpr float kRescaleThreshold = 8.0f;  // log2 units: O is rescaled only whe
 #define TRACE(tag, arg) do { } while (0)
 #endif
 
+constexpr int kOutWarpBytes = 32 * 128;
+
 template <int D, int NT>
 struct Cfg {
     static constexpr int kTileBytes = kTileRows * D * 2;      // Q tile, K block or V block
     static constexpr int kStages = (D == 128) ? 4 : 8;   // > 114 KB of smem either way: one CTA per SM (it owns all of TMEM)
     static constexpr int kSmemQ = NT * kTileBytes;
     static constexpr int kSmemKV = kStages * kTileBytes;
-    static constexpr int kSmemBytes = kSmemQ + kSmemKV + 1024 /*align slack*/;
+    static constexpr int kSmemOut = 4 * kOutWarpBytes;      // epilogue staging: 32 rows x 64 bf16 columns per warp
+    static constexpr int kSmemBytes = kSmemQ + kSmemKV + kSmemOut + 1024 /*align slack*/;
     static constexpr int kHalves = D / 64;
     static constexpr uint32_t kSBO = kHalves * kAtomBytes;
 };
@@ -180,6 +183,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
     extern __shared__ uint8_t smem_raw[];
     __shared__ Bars bars;
     __shared__ float2 stats[2][kTileRows];   // (m in log2 units, l) of a finished tile, softmax -> epilogue
+    __shared__ int out_row16[kTileRows];     // epilogue: where each row of the tile goes in `out` (16-byte units, -1: nowhere)
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
     const uint32_t sQ = smem_u32(smem);
     const uint32_t sKV = sQ + C::kSmemQ;
@@ -684,15 +688,22 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                     }
                     if (valid) { p.ws_ml[base * 2] = ml.x; p.ws_ml[base * 2 + 1] = ml.y; }
                 } else {
+                    // Row r of the tile is one contiguous D-element row of `out`, but consecutive rows are far apart:
+                    // a store straight from the TMEM layout (lane = row) touches 32 lines per instruction.  So each
+                    // warp transposes its 32 rows through shared memory, 64 columns at a time (16-byte chunks
+                    // XOR-swizzled by row, conflict-free both ways), and stores 4 full 128-byte lines per instruction.
                     const float inv = 1.f / ml.y;
-                    uint16_t* orow = p.out + row * p.out_row_stride + (long long)head * D;
+                    const long long off16 = (row * p.out_row_stride + (long long)head * D) >> 3;
+                    out_row16[r] = valid ? (int)off16 : -1;
+                    const uint32_t stg = sKV + C::kSmemKV + wq * kOutWarpBytes;
+                    uint4* out16 = reinterpret_cast<uint4*>(p.out);
+#pragma unroll 1
+                    for (int h = 0; h < D / 64; ++h) {
 #pragma unroll 2
-                    for (int c = 0; c < D / 16; ++c) {
-                        uint32_t v[16];
-                        tmem_ld16(tO + c * 16, v);
-                        tmem_wait_ld();
-                        if (valid) {
-                            uint4* dst = reinterpret_cast<uint4*>(orow + c * 16);
+                        for (int c = 0; c < 4; ++c) {
+                            uint32_t v[16];
+                            tmem_ld16(tO + h * 64 + c * 16, v);
+                            tmem_wait_ld();
 #pragma unroll
                             for (int e = 0; e < 2; ++e) {
                                 uint4 o;
@@ -700,13 +711,26 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                                 o.y = pack_bf16x2(__uint_as_float(v[8 * e + 2]) * inv, __uint_as_float(v[8 * e + 3]) * inv);
                                 o.z = pack_bf16x2(__uint_as_float(v[8 * e + 4]) * inv, __uint_as_float(v[8 * e + 5]) * inv);
                                 o.w = pack_bf16x2(__uint_as_float(v[8 * e + 6]) * inv, __uint_as_float(v[8 * e + 7]) * inv);
-                                dst[e] = o;
+                                sts128(stg + lane * 128 + (((2 * c + e) ^ (lane & 7)) << 4), o);
                             }
                         }
+                        if (h == D / 64 - 1 && has_blk) {   // O_t is in registers / shared memory now: the next item may overwrite it
+                            tc_fence_before();
+                            mbar_arrive(smem_u32(&bars.o_free[tile]));
+                        }
+                        __syncwarp();
+#pragma unroll 4
+                        for (int i = 0; i < 8; ++i) {
+                            const int rr = i * 4 + (lane >> 3);
+                            const int ro = out_row16[wq * 32 + rr];
+                            const uint4 o = lds128(stg + rr * 128 + (((lane & 7) ^ (rr & 7)) << 4));
+                            if (ro >= 0) out16[(long long)ro + h * 8 + (lane & 7)] = o;
+                        }
+                        __syncwarp();
                     }
                     if (valid && p.lse) p.lse[(long long)head * p.lse_stride + row] = (ml.x + log2f(ml.y)) * 0.6931471805599453f;
                 }
-                if (has_blk) {
+                if (has_blk && it.partial_slot >= 0) {
                     tc_fence_before();
                     mbar_arrive(smem_u32(&bars.o_free[tile]));   // O_t may be overwritten by the next item
                 }
