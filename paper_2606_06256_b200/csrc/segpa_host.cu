@@ -147,7 +147,8 @@ struct segpa_segments {
     std::vector<segpa_segment_req_t> reqs;
     std::vector<SegDev> segs;
     std::vector<ItemDev> items;
-    std::vector<segpa_item_t> items_pub;
+    struct ItemMeta { int32_t tile; int32_t split; int32_t n_splits; };
+    std::vector<ItemMeta> item_meta;   // per item (same order as items): what segpa_segments_items reports besides ItemDev
     std::vector<int32_t> pages;
     std::vector<CombDev> combs;
     std::vector<int32_t> cta_off;   // items of CTA q: [cta_off[q], cta_off[q+1])
@@ -161,6 +162,31 @@ struct segpa_segments {
     SegBuf* buf = nullptr;
     mutable cudaStream_t last_stream = nullptr;   // stream of the last upload / attention_fwd
     size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0, off_cta = 0;
+
+    // back to the state of a fresh object, keeping the vectors' storage (objects are recycled through the
+    // cache: a plan is built on the critical path of every layer and must not go through malloc / page faults)
+    void reset() {
+        cache = nullptr; layer = 0;
+        reqs.clear(); segs.clear(); items.clear(); item_meta.clear(); pages.clear(); combs.clear(); cta_off.clear(); mass_off.clear();
+        mass_planned = false; mass_n_cta = 0;
+        m_off_items = m_off_cta = m_off_layout = m_off_kvlen = 0;
+        stats = segpa_plan_stats_t{};
+        tiles_per_item = 1;
+        buf = nullptr; last_stream = nullptr;
+        off_segs = off_items = off_pages = off_combs = off_cta = 0;
+    }
+};
+
+// build_segments scratch, kept in the cache between calls (same reason)
+struct PlanTile { int seg, t0, n_tok, kb_lo, kb_hi, cost; bool sink; };
+struct PlanIv { int32_t kv_head; int64_t lo, hi; };
+struct PlanScratch {
+    std::vector<PlanTile> tiles;
+    std::vector<PlanIv> ivs;
+    std::vector<int> order, start, item_cta, count, cursor;
+    std::vector<int64_t> heap;
+    std::vector<ItemDev> it2;
+    std::vector<segpa_segments::ItemMeta> im2;
 };
 
 struct segpa_cache {
@@ -176,9 +202,10 @@ struct segpa_cache {
     int64_t n_free = 0;
     std::unordered_map<StreamKey, StreamRec, StreamKeyHash> streams;
     std::vector<segpa_segments*> seg_objs;
-    std::vector<SegBuf*> free_bufs;
-    std::vector<uint32_t> dup_mark;  // append_pages: duplicate detection stamps
-    uint32_t dup_stamp = 0;
+    std::vector<SegBuf*> free_bufs;   // released device storage, oldest first
+    size_t n_seg_bufs = 0;            // SegBufs alive (in free_bufs or owned by a segments object)
+    std::vector<segpa_segments*> free_seg_objs;   // recycled host-side plan objects
+    PlanScratch plan;
     Staging append_stage[2];         // alternating, so staging a batch does not wait for the previous one
     int append_turn = 0;
     int num_sms = 148;
@@ -217,7 +244,12 @@ void free_segments_obj(segpa_cache* c, segpa_segments* s) {
         if (s->mass_planned) staging_release(s->buf->mass_blob, s->last_stream);
         c->free_bufs.push_back(s->buf);
     }
-    delete s;
+    if (c->free_seg_objs.size() < 64) {
+        s->reset();
+        c->free_seg_objs.push_back(s);
+    } else {
+        delete s;
+    }
 }
 
 inline int64_t cdiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
@@ -358,6 +390,7 @@ segpa_status_t segpa_destroy(segpa_cache_t* c) {
     if (!c->planning_only) cudaDeviceSynchronize();
     for (auto* s : c->seg_objs) free_segments_obj(c, s);
     for (auto* b : c->free_bufs) segbuf_free(b);
+    for (auto* s : c->free_seg_objs) delete s;
     staging_free(c->append_stage[0]);
     staging_free(c->append_stage[1]);
     if (c->st_q) cudaFree(c->st_q);
@@ -431,20 +464,16 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                     if (r.page_ids[k] < 0 || r.page_ids[k] >= c->desc.num_pages) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page id %d out of range", i, r.page_ids[k]);
                     if (c->refcnt[r.page_ids[k]] != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page %d is not free", i, r.page_ids[k]);
                 }
-                // duplicates inside one request: stamp array, O(n)
-                if (c->dup_mark.size() != c->refcnt.size()) c->dup_mark.assign(c->refcnt.size(), 0);
-                const uint32_t stamp = ++c->dup_stamp;
-                for (int32_t k = 0; k < r.n_page_ids; ++k) {
-                    if (c->dup_mark[r.page_ids[k]] == stamp) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: duplicate page id %d", i, r.page_ids[k]);
-                    c->dup_mark[r.page_ids[k]] = stamp;
-                }
+                // (a duplicate inside the request is caught while it is applied, below: no second pass over the pool state)
             } else {
                 if (need > c->n_free) APPEND_FAIL(SEGPA_ERR_OOM, "append_pages[%d]: pool exhausted (%lld pages needed, %lld free)", i, (long long)need, (long long)c->n_free);
             }
 
             // the request is valid: apply it
             StreamRec& rec = c->streams[key];
-            undo.push_back(Undo{key, created, cur_len, (size_t)need});
+            undo.push_back(Undo{key, created, cur_len, 0});
+            rec.pages.reserve(rec.pages.size() + (size_t)need);
+            if (!attach) touched.reserve(touched.size() + (size_t)need + 1);
             if (!attach) {
                 ScatterJob jb{};
                 jb.k_src = (const uint16_t*)r.k_src;
@@ -461,6 +490,10 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
             }
             for (int64_t k = 0; k < need; ++k) {
                 const int32_t id = r.page_ids ? r.page_ids[k] : pop_free_page(c);
+                // every id of a copy request was free when the request was checked: one that is taken now was
+                // taken by an earlier entry of this same request
+                if (!attach && r.page_ids && c->refcnt[id] != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: duplicate page id %d", i, id);
+                ++undo.back().n_new;
                 if (c->refcnt[id] == 0) --c->n_free;
                 ++c->refcnt[id];
                 rec.pages.push_back(id);
@@ -724,20 +757,34 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
     const int TT = kTileRows / G;               // tokens per 128-row tile (GQA packing)
     const int item_tok = TT * tiles_per_item;
 
-    segpa_segments* S = new (std::nothrow) segpa_segments();
-    if (!S) return fail(SEGPA_ERR_OOM, "build_segments: host allocation failed");
+    segpa_segments* S = nullptr;
+    if (!c->free_seg_objs.empty()) {
+        S = c->free_seg_objs.back();
+        c->free_seg_objs.pop_back();
+    } else {
+        S = new (std::nothrow) segpa_segments();
+        if (!S) return fail(SEGPA_ERR_OOM, "build_segments: host allocation failed");
+    }
     S->cache = c;
     S->layer = layer;
     S->tiles_per_item = tiles_per_item;
-    struct TileTmp { int seg, t0, n_tok, kb_lo, kb_hi, cost; bool sink; };
-    std::vector<TileTmp> tiles;
+    using TileTmp = PlanTile;
+    PlanScratch& ps = c->plan;
+    std::vector<TileTmp>& tiles = ps.tiles;
+    tiles.clear();
     int64_t q_rows = 0, pairs = 0, vis_tokens = 0;
     try {
         S->reqs.assign(reqs, reqs + n);
         S->segs.reserve((size_t)n);
+        {
+            size_t n_tiles_max = 0;
+            for (int32_t s = 0; s < n; ++s) n_tiles_max += (size_t)(std::max(reqs[s].q_len, 1) + item_tok - 1) / (size_t)item_tok;
+            tiles.reserve(n_tiles_max);
+        }
         // validation + per-segment metadata
-        struct Iv { int32_t kv_head; int64_t lo, hi; };
-        std::vector<Iv> ivs;
+        using Iv = PlanIv;
+        std::vector<Iv>& ivs = ps.ivs;
+        ivs.clear();
         for (int32_t s = 0; s < n; ++s) {
             const segpa_segment_req_t& r = reqs[s];
             if (r.kv_head < 0 || r.kv_head >= c->desc.num_kv_heads) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: kv_head %d out of range", s, r.kv_head); }
@@ -825,6 +872,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         for (auto& t : tiles) total_cost += t.cost;
         const int64_t chunk = std::max<int64_t>(8, cdiv(total_cost, (int64_t)c->num_sms * 4));
         int n_split_tiles = 0, n_slots = 0;
+        S->items.reserve(tiles.size() + (size_t)c->num_sms * 8);
+        S->item_meta.reserve(tiles.size() + (size_t)c->num_sms * 8);
         for (size_t ti = 0; ti < tiles.size(); ++ti) {
             const TileTmp& t = tiles[ti];
             const int cost = t.cost;
@@ -843,7 +892,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 const int hi = t.sink ? t.kb_hi : t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
                 const int slot = (parts > 1 || strided) ? n_slots++ : -1;
                 S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, t.sink ? t.cost : hi - lo});
-                S->items_pub.push_back(segpa_item_t{t.seg, t.t0, t.n_tok, lo, hi, parts > 1 ? p : -1, parts, (int32_t)ti, 0, 0});
+                S->item_meta.push_back(segpa_segments::ItemMeta{(int32_t)ti, parts > 1 ? p : -1, parts});
             }
         }
         // LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid (min-heap on
@@ -852,53 +901,64 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         // only: the plan is built on the critical path of every layer.
         const int n_items_all = (int)S->items.size();
         const int n_cta = std::min(n_items_all, c->num_sms);
-        std::vector<int> order((size_t)n_items_all);
-        for (int i = 0; i < n_items_all; ++i) order[(size_t)i] = i;
-        std::sort(order.begin(), order.end(), [&](int a, int b) {
-            return S->items[a].cost != S->items[b].cost ? S->items[a].cost > S->items[b].cost : a < b;
-        });
-        const int n_rounds = (n_items_all + n_cta - 1) / n_cta;
-        int cap = n_rounds + 8;      // slots per CTA (LPT can give a CTA a few more than the average count)
-        std::vector<int> slot, count;
-        for (;;) {
-            slot.assign((size_t)n_cta * cap, -1);
-            count.assign((size_t)n_cta, 0);
-            std::vector<int64_t> heap((size_t)n_cta);   // min-heap on the single key load * 1024 + cta
-            for (int q = 0; q < n_cta; ++q) heap[(size_t)q] = q;
-            auto gt = std::greater<int64_t>();
-            bool overflow = false;
-            for (int idx : order) {
-                std::pop_heap(heap.begin(), heap.end(), gt);
-                int64_t& top = heap.back();
-                const int q = (int)(top & 1023);
-                if (count[(size_t)q] == cap) { overflow = true; break; }
-                slot[(size_t)q * cap + count[(size_t)q]++] = idx;
-                const int64_t blocks3 = 3 * (int64_t)S->items[idx].cost;
-                top += (((S->items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2) * 1024;   // strided: two chains
-                std::push_heap(heap.begin(), heap.end(), gt);
-            }
-            if (!overflow) break;
-            cap *= 2;
+        // descending cost, ties by ascending index: a counting sort (costs are block counts, small integers)
+        std::vector<int>& order = ps.order;
+        order.resize((size_t)n_items_all);
+        {
+            int max_cost = 0;
+            for (const ItemDev& it : S->items) max_cost = std::max(max_cost, it.cost);
+            std::vector<int>& start = ps.start;
+            start.assign((size_t)max_cost + 2, 0);
+            for (const ItemDev& it : S->items) ++start[(size_t)(max_cost - it.cost) + 1];
+            for (int k2 = 0; k2 <= max_cost; ++k2) start[(size_t)k2 + 1] += start[(size_t)k2];
+            for (int i = 0; i < n_items_all; ++i) order[(size_t)start[(size_t)(max_cost - S->items[(size_t)i].cost)]++] = i;
         }
-        std::vector<ItemDev> it2;
-        std::vector<segpa_item_t> ip2;
-        it2.reserve(order.size());
-        ip2.reserve(order.size());
-        S->cta_off.assign((size_t)n_cta + 1, 0);
-        int64_t kv_blocks = 0;
-        for (int q = 0; q < n_cta; ++q) {
-            for (int k2 = 0; k2 < count[(size_t)q]; ++k2) {
-                const int idx = slot[(size_t)q * cap + k2];
-                it2.push_back(S->items[idx]);
-                segpa_item_t pub = S->items_pub[idx];
-                pub.cta = q;
-                ip2.push_back(pub);
-                kv_blocks += S->items[idx].cost;
+        // LPT: each item, in that order, goes to the least-loaded CTA.  The loads are kept as one ascending run of
+        // keys load * 1024 + cta (distinct, so the minimum is unique) inside a longer array: the minimum leaves at
+        // the head, the CTA's new key is inserted from the tail.  With costs descending the new key belongs at or
+        // near the tail, so an assignment costs a few moves (a binary heap's dependent loads per level cost more)
+        std::vector<int64_t>& run = ps.heap;
+        run.resize((size_t)n_cta + (size_t)n_items_all);
+        for (int q = 0; q < n_cta; ++q) run[(size_t)q] = q;
+        std::vector<int>&item_cta = ps.item_cta, &count = ps.count, &cursor = ps.cursor;
+        item_cta.resize((size_t)n_items_all);
+        count.assign((size_t)n_cta, 0);
+        {
+            int64_t* a = run.data();
+            const ItemDev* items = S->items.data();
+            size_t head = 0, tail = (size_t)n_cta;
+            for (int idx : order) {
+                const int64_t top = a[head++];
+                const int q = (int)(top & 1023);
+                item_cta[(size_t)idx] = q;
+                ++count[(size_t)q];
+                const int64_t blocks3 = 3 * (int64_t)items[idx].cost;
+                const int64_t key = top + (((items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2) * 1024;   // strided: two chains
+                size_t pos = tail++;
+                while (pos > head && a[pos - 1] > key) {
+                    a[pos] = a[pos - 1];
+                    --pos;
+                }
+                a[pos] = key;
             }
-            S->cta_off[(size_t)q + 1] = (int32_t)it2.size();
+        }
+        // per-CTA slices: CTA by CTA, each CTA's items in the order they were assigned (descending cost)
+        S->cta_off.assign((size_t)n_cta + 1, 0);
+        for (int q = 0; q < n_cta; ++q) S->cta_off[(size_t)q + 1] = S->cta_off[(size_t)q] + count[(size_t)q];
+        std::vector<ItemDev>& it2 = ps.it2;
+        std::vector<segpa_segments::ItemMeta>& im2 = ps.im2;
+        it2.resize((size_t)n_items_all);
+        im2.resize((size_t)n_items_all);
+        cursor.assign(S->cta_off.begin(), S->cta_off.end() - 1);
+        int64_t kv_blocks = 0;
+        for (int idx : order) {
+            const int at = cursor[(size_t)item_cta[(size_t)idx]]++;
+            it2[(size_t)at] = S->items[(size_t)idx];
+            im2[(size_t)at] = S->item_meta[(size_t)idx];
+            kv_blocks += S->items[(size_t)idx].cost;
         }
         S->items.swap(it2);
-        S->items_pub.swap(ip2);
+        S->item_meta.swap(im2);
 
         segpa_plan_stats_t& stt = S->stats;
         stt.n_segments = n;
@@ -928,13 +988,26 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         S->off_cta = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
         const size_t blob_bytes = al(S->off_cta + S->cta_off.size() * sizeof(int32_t));
         // device storage: recycled from the cache's free list (no cudaMalloc / cudaMallocHost in steady state)
+        // Oldest first, and only one whose last use has completed on the device: a caller that enqueues steps
+        // back to back (host planning of step k+1 under the kernels of step k) must not be made to wait here.
+        // While none is ready the cache grows, up to twice the live objects + 2; past that the oldest is waited for.
         SegBuf* B = nullptr;
-        if (!c->free_bufs.empty()) {
-            B = c->free_bufs.back();
-            c->free_bufs.pop_back();
-        } else {
+        for (size_t i = 0; i < c->free_bufs.size() && !B; ++i) {
+            SegBuf* cand = c->free_bufs[i];
+            if (!cand->blob.pending || cudaEventQuery(cand->blob.ev) == cudaSuccess) {
+                B = cand;
+                c->free_bufs.erase(c->free_bufs.begin() + (long)i);
+            }
+        }
+        cudaGetLastError();   // (cudaErrorNotReady from the queries is not an error)
+        if (!B && !c->free_bufs.empty() && c->n_seg_bufs >= 2 * (c->seg_objs.size() + 1) + 2) {
+            B = c->free_bufs.front();
+            c->free_bufs.erase(c->free_bufs.begin());
+        }
+        if (!B) {
             B = new (std::nothrow) SegBuf();
             if (!B) { delete S; return fail(SEGPA_ERR_OOM, "build_segments: host allocation failed"); }
+            ++c->n_seg_bufs;
         }
         S->buf = B;
         S->last_stream = st;
@@ -991,9 +1064,16 @@ segpa_status_t segpa_segments_stats(const segpa_segments_t* s, segpa_plan_stats_
 
 segpa_status_t segpa_segments_items(const segpa_segments_t* s, segpa_item_t* items_out, int32_t cap, int32_t* n_out) {
     if (!s) return fail(SEGPA_ERR_INVALID, "segments_items: null argument");
-    if (n_out) *n_out = (int32_t)s->items_pub.size();
-    if (items_out)
-        for (int32_t i = 0; i < cap && i < (int32_t)s->items_pub.size(); ++i) items_out[i] = s->items_pub[(size_t)i];
+    if (n_out) *n_out = (int32_t)s->items.size();
+    if (items_out) {
+        int32_t cta = 0;
+        for (int32_t i = 0; i < cap && i < (int32_t)s->items.size(); ++i) {
+            while (cta + 1 < (int32_t)s->cta_off.size() && i >= s->cta_off[(size_t)cta + 1]) ++cta;
+            const ItemDev& it = s->items[(size_t)i];
+            const segpa_segments::ItemMeta& m = s->item_meta[(size_t)i];
+            items_out[i] = segpa_item_t{it.seg, it.t0, it.n_tok, it.kb_lo, it.kb_hi, m.split, m.n_splits, m.tile, cta, 0};
+        }
+    }
     return SEGPA_OK;
 }
 

@@ -243,6 +243,64 @@ def test_batched_append_matches_per_stream_append():
     print(compare(w, 0, k, v, q, outs[0][0], outs[0][1], label="batched append"))
 
 
+def test_copy_append_rejects_duplicate_ids_and_rolls_back():
+    """A copy-mode request that names a page twice fails as a whole: pool state and streams are as before
+    (the duplicate is detected while the request is applied, so the partial application must be undone)."""
+    w = wl.config1()
+    dev = torch.device("cuda:0")
+    cache = H.create_cache(w, 0)
+    try:
+        rows = torch.zeros((40, w.D), dtype=torch.bfloat16, device=dev)
+        good = (0, 0, 7, rows, rows, 40, [3, 4, 5])
+        bad = (0, 1, 7, rows, rows, 40, [8, 9, 8])
+        before = B.segpa_pool_stats(cache)
+        with pytest.raises(B.SegpaError, match="duplicate page id 8"):
+            B.segpa_append_pages_batch(cache, [good, bad])
+        assert B.segpa_pool_stats(cache) == before          # the valid first request was undone too
+        with pytest.raises(B.SegpaError):
+            B.segpa_stream_info(cache, 0, 0, 7)
+        B.segpa_append_pages_batch(cache, [good, (0, 1, 7, rows, rows, 40, [8, 9, 10])])
+        used, free = B.segpa_pool_stats(cache)
+        assert used == before[0] + 6 and free == before[1] - 6
+        with pytest.raises(B.SegpaError, match="not free"):
+            B.segpa_append_pages(cache, 0, 0, 9, rows, rows, 40, page_ids=[5, 11, 12])
+        torch.cuda.synchronize()
+    finally:
+        B.segpa_destroy(cache)
+
+
+def test_back_to_back_steps_without_host_sync():
+    """Steps enqueued back to back (store, plan, attend; the previous step's plan freed while its kernel may
+    still run): plan storage is only reused once its last use has completed on the device, so every step
+    gives the bits of a step run alone."""
+    reqs = [{"kv_len": 3000 + 211 * r, "heads": {0: (GLOBAL, 0, 0, 3000 + 211 * r), 1: (LOCAL, 512, 0, 3000 + 211 * r)}} for r in range(3)]
+    w = wl.make_workload("pipelined", Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=5)
+    dev = torch.device("cuda:0")
+    k, v = wl.pool_values(w, dev)
+    q = wl.q_values(w, 0, dev)
+    cache = H.create_cache(w, 0)
+    try:
+        batch = B.AppendBatch(H.append_requests(w, k, v))
+        sb = B.SegmentBatch(H.segment_reqs(w, 0))
+        outs, prev = [], None
+        for step in range(6):
+            if prev is not None:
+                B.segpa_free_segments(cache, prev)
+            B.segpa_clear_streams(cache)
+            B.segpa_append_pages_batch(cache, batch)
+            prev = B.segpa_build_segments(cache, 0, sb)
+            out = torch.full_like(q, OUT_SENTINEL)
+            lse = torch.full((w.Hq, w.T[0]), LSE_SENTINEL, dtype=torch.float32, device=dev)
+            B.segpa_attention_fwd(cache, prev, q, w.scale, out, lse)
+            outs.append((out, lse))
+        torch.cuda.synchronize()
+        for o, l in outs[1:]:
+            assert torch.equal(o, outs[0][0]) and torch.equal(l, outs[0][1])
+        print(compare(w, 0, k, v, q, outs[0][0], outs[0][1], label="back-to-back steps"))
+    finally:
+        B.segpa_destroy(cache)
+
+
 def test_host_buffer_entry_point_matches_device_path():
     w = wl.config1()
     g = GpuRun(w, "tc", 2)
