@@ -76,6 +76,7 @@ struct Staging {
     size_t cap = 0;
     cudaEvent_t ev = nullptr;
     bool pending = false;
+    cudaEvent_t up = nullptr;   // upload of h -> d has completed (staging_upload)
 };
 
 cudaError_t staging_acquire(Staging& s, size_t bytes) {
@@ -107,6 +108,19 @@ cudaError_t staging_acquire(Staging& s, size_t bytes) {
     return cudaSuccess;
 }
 
+// h -> d on the cache's own copy stream, then `st` waits for it: descriptors go up while the work already queued
+// in `st` (the previous step's kernels) is still running, instead of queueing behind it.  Safe because the pair
+// is only handed out (staging_acquire) once its last consumer has finished.
+cudaError_t staging_upload(Staging& s, size_t bytes, cudaStream_t up_stream, cudaStream_t st) {
+    if (!up_stream) return cudaMemcpyAsync(s.d, s.h, bytes, cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaSuccess;
+    if (!s.up) e = cudaEventCreateWithFlags(&s.up, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(s.d, s.h, bytes, cudaMemcpyHostToDevice, up_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(s.up, up_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s.up, 0);
+    return e;
+}
+
 void staging_release(Staging& s, cudaStream_t st) {
     if (s.ev && cudaEventRecord(s.ev, st) == cudaSuccess) s.pending = true;
 }
@@ -115,6 +129,7 @@ void staging_free(Staging& s) {
     if (s.h) cudaFreeHost(s.h);
     if (s.d) cudaFree(s.d);
     if (s.ev) cudaEventDestroy(s.ev);
+    if (s.up) cudaEventDestroy(s.up);
     s = Staging();
 }
 
@@ -206,9 +221,11 @@ struct segpa_cache {
     size_t n_seg_bufs = 0;            // SegBufs alive (in free_bufs or owned by a segments object)
     std::vector<segpa_segments*> free_seg_objs;   // recycled host-side plan objects
     PlanScratch plan;
+    std::vector<int32_t> append_touched;   // append_pages_batch scratch, kept between calls
     Staging append_stage[2];         // alternating, so staging a batch does not wait for the previous one
     int append_turn = 0;
     int num_sms = 148;
+    cudaStream_t up_stream = nullptr;   // descriptor uploads (staging_upload)
     int kernel_kind = 1;  // 0 = SIMT bring-up kernel (SEGPA_KERNEL=simt), 1 = tcgen05
     int last_launches = 0;
     // host-buffer entry point staging
@@ -360,6 +377,10 @@ segpa_status_t segpa_create_cache(const segpa_cache_desc_t* d, segpa_cache_t** o
         }
         c->num_sms = prop.multiProcessorCount;
         DeviceGuard g(d->device);
+        if (cudaStreamCreateWithFlags(&c->up_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            cudaGetLastError();
+            c->up_stream = nullptr;   // uploads then go through the caller's stream
+        }
         const size_t bytes = (size_t)segpa_pool_bytes(d);
         if (d->k_pool) {
             c->own_pool = false;
@@ -393,6 +414,7 @@ segpa_status_t segpa_destroy(segpa_cache_t* c) {
     for (auto* s : c->free_seg_objs) delete s;
     staging_free(c->append_stage[0]);
     staging_free(c->append_stage[1]);
+    if (c->up_stream) cudaStreamDestroy(c->up_stream);
     if (c->st_q) cudaFree(c->st_q);
     if (c->st_out) cudaFree(c->st_out);
     if (c->st_lse) cudaFree(c->st_lse);
@@ -411,8 +433,18 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
     struct Undo { StreamKey key; bool created; int64_t old_len; size_t n_new; };
     std::vector<Undo> undo;
     std::vector<ScatterJob> jobs;
-    std::vector<int32_t> touched;     // page ids the scatter kernel indexes, job after job
+    std::vector<int32_t>& touched = c->append_touched;     // page ids the scatter kernel indexes, job after job
+    touched.clear();
     long long total_chunks = 0;
+    try {
+        size_t ub = 0;   // one allocation at most (an upper bound of the ids listed: new pages + a refilled last page per job)
+        for (int32_t i = 0; i < n; ++i) ub += (size_t)(std::max<int64_t>(reqs[i].n_tokens, 0) / P) + 2;
+        touched.reserve(ub);
+        undo.reserve((size_t)n);
+        jobs.reserve((size_t)n);
+    } catch (const std::bad_alloc&) {
+        return fail(SEGPA_ERR_OOM, "append_pages: host allocation failed");
+    }
     auto rollback = [&]() {
         for (size_t u = undo.size(); u-- > 0;) {
             auto it = c->streams.find(undo[u].key);
@@ -454,26 +486,18 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 if (!r.page_ids) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs page_ids", i);
                 if (cur_len % P != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs the stream length (%lld) to be a multiple of page_size", i, (long long)cur_len);
                 if (r.n_page_ids != need) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs %lld page ids, got %d", i, (long long)need, r.n_page_ids);
-                for (int32_t k = 0; k < r.n_page_ids; ++k) {
-                    if (r.page_ids[k] < 0 || r.page_ids[k] >= c->desc.num_pages) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page id %d out of range", i, r.page_ids[k]);
-                    if (!c->planning_only && c->refcnt[r.page_ids[k]] == 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach of page %d which holds no data", i, r.page_ids[k]);
-                }
             } else if (r.page_ids) {
                 if (r.n_page_ids != need) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: need %lld page ids, got %d", i, (long long)need, r.n_page_ids);
-                for (int32_t k = 0; k < r.n_page_ids; ++k) {
-                    if (r.page_ids[k] < 0 || r.page_ids[k] >= c->desc.num_pages) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page id %d out of range", i, r.page_ids[k]);
-                    if (c->refcnt[r.page_ids[k]] != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page %d is not free", i, r.page_ids[k]);
-                }
-                // (a duplicate inside the request is caught while it is applied, below: no second pass over the pool state)
             } else {
                 if (need > c->n_free) APPEND_FAIL(SEGPA_ERR_OOM, "append_pages[%d]: pool exhausted (%lld pages needed, %lld free)", i, (long long)need, (long long)c->n_free);
             }
 
-            // the request is valid: apply it
+            // Apply the request.  The given page ids are checked as they are taken (one pass over the pool state,
+            // which is random access into a table far larger than the host caches); a bad id undoes this request's
+            // partial application together with the earlier requests (rollback).
             StreamRec& rec = c->streams[key];
             undo.push_back(Undo{key, created, cur_len, 0});
             rec.pages.reserve(rec.pages.size() + (size_t)need);
-            if (!attach) touched.reserve(touched.size() + (size_t)need + 1);
             if (!attach) {
                 ScatterJob jb{};
                 jb.k_src = (const uint16_t*)r.k_src;
@@ -489,10 +513,25 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 jobs.push_back(jb);
             }
             for (int64_t k = 0; k < need; ++k) {
-                const int32_t id = r.page_ids ? r.page_ids[k] : pop_free_page(c);
-                // every id of a copy request was free when the request was checked: one that is taken now was
-                // taken by an earlier entry of this same request
-                if (!attach && r.page_ids && c->refcnt[id] != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: duplicate page id %d", i, id);
+                int32_t id;
+                if (r.page_ids) {
+                    id = r.page_ids[k];
+                    if (k + 16 < need) {   // the table is walked in the (random) order of the ids: fetch ahead
+                        const int32_t nx = r.page_ids[k + 16];
+                        if (nx >= 0 && nx < c->desc.num_pages) __builtin_prefetch(&c->refcnt[nx], 1);
+                    }
+                    if (id < 0 || id >= c->desc.num_pages) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page id %d out of range", i, id);
+                    const int32_t rc = c->refcnt[id];
+                    if (attach) {
+                        if (!c->planning_only && rc == 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach of page %d which holds no data", i, id);
+                    } else if (rc != 0) {
+                        // taken: by an earlier entry of this very request (duplicate), or before it
+                        if (std::find(r.page_ids, r.page_ids + k, id) != r.page_ids + k) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: duplicate page id %d", i, id);
+                        APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: page %d is not free", i, id);
+                    }
+                } else {
+                    id = pop_free_page(c);
+                }
                 ++undo.back().n_new;
                 if (c->refcnt[id] == 0) --c->n_free;
                 ++c->refcnt[id];
@@ -517,7 +556,7 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
         if (e == cudaSuccess) {
             memcpy(sg.h, jobs.data(), jobs.size() * sizeof(ScatterJob));
             memcpy((uint8_t*)sg.h + jobs_bytes, touched.data(), touched.size() * sizeof(int32_t));
-            e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+            e = staging_upload(sg, bytes, c->up_stream, st);
         }
         if (e == cudaSuccess)
             e = launch_scatter_pages(c->k_pool, c->v_pool, (const ScatterJob*)sg.d, (int)jobs.size(),
@@ -827,10 +866,16 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             {
                 const int64_t lst_lo = sd.first_page, lst_hi = sd.first_page + sd.n_pages_listed;
                 const int64_t vis_a = std::max(lst_lo, first_vis_page), vis_b = std::min(lst_hi, n_stream_pages);
-                for (int64_t pg = 0; pg < sink_pages; ++pg)
-                    if (rec.pages[(size_t)pg] < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: sink page %lld of the stream was evicted", s, (long long)pg); }
-                for (int64_t pg = vis_a; pg < vis_b; ++pg)
-                    if (rec.pages[(size_t)pg] < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: visible page %lld of the stream was evicted", s, (long long)pg); }
+                // (holes are negative ids: a branch-free minimum first, the search for the message only on failure)
+                int32_t min_id = 0;
+                for (int64_t pg = 0; pg < sink_pages; ++pg) min_id = std::min(min_id, rec.pages[(size_t)pg]);
+                for (int64_t pg = vis_a; pg < vis_b; ++pg) min_id = std::min(min_id, rec.pages[(size_t)pg]);
+                if (min_id < 0) {
+                    for (int64_t pg = 0; pg < sink_pages; ++pg)
+                        if (rec.pages[(size_t)pg] < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: sink page %lld of the stream was evicted", s, (long long)pg); }
+                    for (int64_t pg = vis_a; pg < vis_b; ++pg)
+                        if (rec.pages[(size_t)pg] < 0) { delete S; return fail(SEGPA_ERR_INVALID, "build_segments: segment %d: visible page %lld of the stream was evicted", s, (long long)pg); }
+                }
                 S->pages.insert(S->pages.end(), rec.pages.begin(), rec.pages.begin() + sink_pages);
                 S->pages.insert(S->pages.end(), (size_t)(vis_a - lst_lo - sink_pages), zero_page);
                 S->pages.insert(S->pages.end(), rec.pages.begin() + vis_a, rec.pages.begin() + vis_b);
@@ -888,8 +933,9 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             if (parts > 1 || strided)
                 S->combs.push_back(CombDev{t.seg, t.t0, t.n_tok, n_slots, parts, strided ? 1 : 0, 0, 0});
             for (int p = 0; p < parts; ++p) {
-                const int lo = t.sink ? t.kb_lo : t.kb_lo + (int)((int64_t)cost * p / parts);
-                const int hi = t.sink ? t.kb_hi : t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
+                // (parts == 1, nearly every tile: no divisions on this path)
+                const int lo = (t.sink || parts == 1) ? t.kb_lo : t.kb_lo + (int)((int64_t)cost * p / parts);
+                const int hi = (t.sink || parts == 1) ? t.kb_hi : t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
                 const int slot = (parts > 1 || strided) ? n_slots++ : -1;
                 S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, t.sink ? t.cost : hi - lo});
                 S->item_meta.push_back(segpa_segments::ItemMeta{(int32_t)ti, parts > 1 ? p : -1, parts});
@@ -1034,7 +1080,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         memcpy(hb + S->off_pages, S->pages.data(), S->pages.size() * sizeof(int32_t));
         if (!S->combs.empty()) memcpy(hb + S->off_combs, S->combs.data(), S->combs.size() * sizeof(CombDev));
         memcpy(hb + S->off_cta, S->cta_off.data(), S->cta_off.size() * sizeof(int32_t));
-        e = cudaMemcpyAsync(B->blob.d, B->blob.h, blob_bytes, cudaMemcpyHostToDevice, st);
+        e = staging_upload(B->blob, blob_bytes, c->up_stream, st);
         if (e != cudaSuccess) {
             cudaGetLastError();
             free_segments_obj(c, S);
