@@ -4,10 +4,10 @@
 // See DESIGN.md section 5.2.
 //
 // One persistent CTA per SM, 16 warps, warp-specialised:
-//   warp 0        K/V loader: one bulk copy per physical page into a ring of K/V stages
+//   warp 0 / 3    K loader / V loader: one bulk copy per physical page into a ring of K/V stages
 //   warp 1        MMA issuer (whole warp walks the schedule, one elected lane issues)
 //   warp 2        Q loader: two TMA boxes per 128-row tile, next item's Q prefetched into L2
-//   warp 3        TMEM allocation, otherwise idle
+//                 (warp 3 also allocates TMEM)
 //   warps 4..7    softmax warpgroup of tile 0 (thread = query row)
 //   warps 8..11   softmax warpgroup of tile 1 (NT = 2: two 128-row tiles of adjacent tokens share
 //                 every K/V stage and ping-pong on the tensor pipe)
@@ -36,6 +36,7 @@ namespace {
 constexpr int kLoaderWarp = 0;
 constexpr int kMmaWarp = 1;
 constexpr int kQWarp = 2;
+constexpr int kVLoaderWarp = 3;   // (also allocates and frees TMEM)
 constexpr int kFirstSoftmaxWarp = 4;
 constexpr int kFirstEpilogueWarp = 12;
 constexpr int kThreads = 512;
@@ -223,10 +224,17 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
     tc_fence_after();
     const uint32_t tmem = bars.tmem_base;
 
-    if (warp == kLoaderWarp) {
-        // ------------------------------------------------------------------ K/V loader
+    if (warp == kLoaderWarp || warp == kVLoaderWarp) {
+        // ------------------------------------------------------------------ K/V loaders
+        // Two warps: warp 0 fills the K stages, warp 3 the V stages (ring order K(j), V(j): even fills are K, odd
+        // fills are V, and kStages is even, so a stage always belongs to the same warp).  The stages of K(j+1) and
+        // V(j) are freed by the same step and both are needed by the next one; one warp issuing them one after the
+        // other (about 600 cycles per stage of bulk copies plus the page-id fetch) put the second on the critical
+        // path of every step (pipeline trace).
         reg_dec<kRegsLow>();
-        uint32_t fill = 0;  // stage fills so far
+        const int kv = (warp == kLoaderWarp) ? 0 : 1;
+        const uint8_t* pool = (kv == 0) ? p.k_pool : p.v_pool;
+        uint32_t n_blk = 0;  // blocks filled so far (this warp's fill number is 2 * n_blk + kv)
         for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
@@ -241,21 +249,19 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const int j = blk(x);
                 const int page = page_next;
                 if (lane < ppb && x + 1 < n_steps) page_next = pg[(long long)blk(x + 1) * ppb];
-                for (int kv = 0; kv < 2; ++kv) {
-                    const uint32_t st = fill % C::kStages, ph = (fill / C::kStages) & 1;
-                    TRACE(1, j * 2 + kv);
-                    if (lane == 0) {
-                        mbar_wait(smem_u32(&bars.kv_empty[st]), ph ^ 1);
-                        mbar_arrive_expect_tx(smem_u32(&bars.kv_full[st]), C::kTileBytes);
-                    }
-                    TRACE(2, j * 2 + kv);
-                    __syncwarp();
-                    if (lane < ppb) {
-                        const uint8_t* src = (kv == 0 ? p.k_pool : p.v_pool) + (size_t)page * p.page_bytes;
-                        bulk_g2s(sKV + st * C::kTileBytes + lane * p.page_bytes, src, p.page_bytes, smem_u32(&bars.kv_full[st]));
-                    }
-                    ++fill;
+                const uint32_t fill = 2 * n_blk + kv;
+                const uint32_t st = fill % C::kStages, ph = (fill / C::kStages) & 1;
+                TRACE(1, j * 2 + kv);
+                if (lane == 0) {
+                    mbar_wait(smem_u32(&bars.kv_empty[st]), ph ^ 1);
+                    mbar_arrive_expect_tx(smem_u32(&bars.kv_full[st]), C::kTileBytes);
                 }
+                TRACE(2, j * 2 + kv);
+                __syncwarp();
+                if (lane < ppb)
+                    bulk_g2s(sKV + st * C::kTileBytes + lane * p.page_bytes, pool + (size_t)page * p.page_bytes, p.page_bytes,
+                             smem_u32(&bars.kv_full[st]));
+                ++n_blk;
             }
         }
     } else if (warp == kMmaWarp) {
@@ -456,8 +462,6 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 __syncwarp();
             }
         }
-    } else if (warp == 3) {
-        reg_dec<kRegsLow>();
     } else if (warp < kFirstEpilogueWarp) {
         // ------------------------------------------------------------------ softmax warpgroups
         reg_inc<kRegsSoftmax>();

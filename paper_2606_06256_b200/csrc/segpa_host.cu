@@ -972,6 +972,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         {
             int64_t* a = run.data();
             const ItemDev* items = S->items.data();
+            const int64_t fixed3 = 2;   // the fixed per-item term, in thirds of a block (a sweep over 0..6 moved cfg2 / cfg4 by < 0.5 %)
             size_t head = 0, tail = (size_t)n_cta;
             for (int idx : order) {
                 const int64_t top = a[head++];
@@ -979,7 +980,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 item_cta[(size_t)idx] = q;
                 ++count[(size_t)q];
                 const int64_t blocks3 = 3 * (int64_t)items[idx].cost;
-                const int64_t key = top + (((items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + 2) * 1024;   // strided: two chains
+                const int64_t key = top + (((items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + fixed3) * 1024;   // strided: two chains
                 size_t pos = tail++;
                 while (pos > head && a[pos - 1] > key) {
                     a[pos] = a[pos - 1];
