@@ -87,8 +87,36 @@ class ClockSampler:
         self.samples = []
         self.proc = None
         self.idx = gpu_index
+        self.nvml = None          # (module, handle): NVML read from a thread every ~2 ms; nvidia-smi -lms is the fallback
+        self.nv_samples = []      # (sm_mhz, reasons bitmask)
+        self.nv_max = None
+        self.stop_flag = False
+
+    def _cuda_index_to_nvml(self, pynvml):
+        """NVML enumerates all GPUs of the box, CUDA only the visible ones: map through CUDA_VISIBLE_DEVICES / UUID."""
+        vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+        if vis:
+            ent = [x.strip() for x in vis.split(",") if x.strip()]
+            if self.idx < len(ent):
+                e = ent[self.idx]
+                if e.isdigit():
+                    return pynvml.nvmlDeviceGetHandleByIndex(int(e))
+                return pynvml.nvmlDeviceGetHandleByUUID(e.encode() if hasattr(e, "encode") else e)
+        return pynvml.nvmlDeviceGetHandleByIndex(self.idx)
 
     def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = self._cuda_index_to_nvml(pynvml)
+            self.nv_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+            self.nvml = (pynvml, h)
+            self.th = threading.Thread(target=self._poll, daemon=True)
+            self.th.start()
+            return
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
                                           "--format=csv,noheader,nounits", "-lms", "100"],
@@ -98,11 +126,34 @@ class ClockSampler:
         except Exception:
             self.proc = None
 
+    def _poll(self):
+        pynvml, h = self.nvml
+        while not self.stop_flag:
+            try:
+                sm = float(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                try:
+                    rs = int(pynvml.nvmlDeviceGetCurrentClocksEventReasons(h))
+                except Exception:
+                    rs = int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                self.nv_samples.append((sm, rs))
+            except Exception:
+                pass
+            time.sleep(0.002)
+
     def _read(self):
         for line in self.proc.stdout:
             self.samples.append(line.strip())
 
     def stop(self):
+        if self.nvml is not None:
+            self.stop_flag = True
+            self.th.join(timeout=1)
+            pynvml, _ = self.nvml
+            bits = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20, "sw_power_cap": 0x4}
+            sm = [a for a, _ in self.nv_samples]
+            reasons = sorted(n for n, b in bits.items() if any(r & b for _, r in self.nv_samples))
+            return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": self.nv_max, "reasons": reasons,
+                    "samples": len(sm), "how": "NVML, every 2 ms during the timed region"}
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
@@ -126,7 +177,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(n)
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "how": "nvidia-smi -lms 100"}
 
 
 # ---------------------------------------------------------------------------------------------
@@ -560,7 +611,7 @@ def run_mass(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="2")
