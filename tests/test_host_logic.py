@@ -286,3 +286,43 @@ def test_config_plans_match_closed_forms():
         used, free = B.segpa_pool_stats(c)
         assert used == len({int(p) for s in w.streams for p in s.page_ids})
         B.segpa_destroy(c)
+
+
+def test_lpt_assignment_matches_plain_heap_restatement():
+    """The scheduler's CTA assignment (counting sort + sorted-run insertion in the library) equals the textbook
+    statement of LPT written with heapq: items by descending cost (ties: creation order), each to the CTA with
+    the smallest (load, cta); load grows by 3 * blocks + 2 thirds of a block-time.
+    Workloads without strided or sink items, where the cost is kb_hi - kb_lo."""
+    import heapq
+    os.environ["SEGPA_TC_TILES"] = "2"
+    rng = np.random.default_rng(3)
+    for trial in range(4):
+        n_req = int(rng.integers(2, 7))
+        reqs = []
+        for r in range(n_req):
+            L = int(rng.integers(200, 9000))
+            reqs.append({"kv_len": L, "heads": {0: (GLOBAL, 0, 0, L), 1: (LOCAL, int(rng.choice([256, 1024, 3000])), 0, L)}})
+        w = wl.make_workload("lpt%d" % trial, Hq=8, Hkv=2, D=128, P=16, requests=reqs, seed=trial)
+        c = B.segpa_create_cache(num_layers=1, num_q_heads=w.Hq, num_kv_heads=w.Hkv, head_dim=w.D, page_size=w.P,
+                                 num_pages=w.num_pages, device=-1)
+        H.append_workload(c, w)
+        segs = H.build_layer(c, w, 0)
+        items = B.segpa_segments_items(segs)
+        n_cta = min(len(items), 148)
+        created = sorted(range(len(items)), key=lambda i: (items[i]["tile"], max(items[i]["split"], 0)))
+        order = sorted(created, key=lambda i: -(items[i]["kb_hi"] - items[i]["kb_lo"]))   # stable: ties keep creation order
+        heap = [(0, q) for q in range(n_cta)]
+        heapq.heapify(heap)
+        expect = {}
+        per_cta = {q: [] for q in range(n_cta)}
+        for i in order:
+            load, q = heapq.heappop(heap)
+            expect[i] = q
+            per_cta[q].append(i)
+            heapq.heappush(heap, (load + 3 * (items[i]["kb_hi"] - items[i]["kb_lo"]) + 2, q))
+        assert [items[i]["cta"] for i in range(len(items))] == [expect[i] for i in range(len(items))]
+        # and the list is laid out CTA by CTA in assignment order
+        flat = [i for q in range(n_cta) for i in per_cta[q]]
+        assert flat == list(range(len(items)))
+        B.segpa_free_segments(c, segs)
+        B.segpa_destroy(c)
