@@ -72,6 +72,10 @@ typedef struct {
     int64_t num_pages;    /* pool capacity in pages; one page holds P tokens of ONE KV head */
     void *k_pool;         /* optional caller-owned device memory of segpa_pool_bytes() bytes, */
     void *v_pool;         /*   else NULL (library allocates). Contents are library-private.     */
+    int32_t tiles_per_item; /* 128-row query tiles a work item of the attention kernel holds: 0 = default (2:
+                               two tiles share every K/V stage), or 1 / 2.  A tuning knob of the one kernel,
+                               fixed for the cache's lifetime; results do not depend on it beyond rounding order. */
+    int32_t reserved;     /* 0 */
 } segpa_cache_desc_t;
 
 /* Bytes needed for each of k_pool / v_pool when the caller owns them ((num_pages + 1) pages: the
@@ -82,7 +86,7 @@ int64_t segpa_pool_bytes(const segpa_cache_desc_t *desc);
  * Create a cache.  The pool is zero-filled.  Physical page layout is private to the library
  * (a page is stored as the shared-memory image the attention kernel consumes, so that one bulk
  * copy moves a page).
- * Errors: INVALID (null, counts < 1, Hq % Hkv != 0), UNSUPPORTED (head_dim, page_size, G > 16,
+ * Errors: INVALID (null, counts < 1, Hq % Hkv != 0, tiles_per_item not in 0..2), UNSUPPORTED (head_dim, page_size, G > 16,
  * device is not compute capability 10.x), CUDA, OOM.
  */
 segpa_status_t segpa_create_cache(const segpa_cache_desc_t *desc, segpa_cache_t **out);

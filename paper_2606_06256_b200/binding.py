@@ -12,6 +12,9 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libsegpa.so")
+# test build: the same sources compiled with -DSEGPA_BRINGUP (adds the SIMT cross-check kernel and one extra
+# symbol, segpa_bringup_use_simt); never loaded unless a test asks for it with use_library("bringup")
+BRINGUP_LIB_PATH = os.path.join(_HERE, "libsegpa_bringup.so")
 
 OK, ERR_INVALID, ERR_OOM, ERR_CUDA, ERR_UNSUPPORTED, ERR_STATE = range(6)
 GLOBAL, LOCAL = 0, 1
@@ -37,7 +40,8 @@ class SegpaError(RuntimeError):
 class CacheDesc(C.Structure):
     _fields_ = [("num_layers", C.c_int32), ("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32),
                 ("head_dim", C.c_int32), ("page_size", C.c_int32), ("device", C.c_int32),
-                ("num_pages", C.c_int64), ("k_pool", C.c_void_p), ("v_pool", C.c_void_p)]
+                ("num_pages", C.c_int64), ("k_pool", C.c_void_p), ("v_pool", C.c_void_p),
+                ("tiles_per_item", C.c_int32), ("reserved", C.c_int32)]
 
 
 class SegmentReq(C.Structure):
@@ -71,15 +75,34 @@ class Item(C.Structure):
 
 
 _lib = None
+_libs = {}
+_which = "product"
+
+
+def use_library(which: str) -> None:
+    """"product" (libsegpa.so, the default) or "bringup" (the test build): the library the functions below call."""
+    global _lib, _which
+    assert which in ("product", "bringup")
+    _which = which
+    _lib = _libs.get(which)
+
+
+def segpa_bringup_use_simt(cache: int, on: bool = True) -> None:
+    """Test build only: run this cache's plans on the SIMT cross-check kernel."""
+    assert _which == "bringup", "segpa_bringup_use_simt exists only in libsegpa_bringup.so"
+    L = lib()
+    L.segpa_bringup_use_simt.argtypes = [C.c_void_p, C.c_int32]
+    _check(L.segpa_bringup_use_simt(cache, 1 if on else 0))
 
 
 def lib():
     global _lib
     if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise ImportError("libsegpa.so is not built (%s); run `python -c 'import __graft_entry__ as g; g.build()'` "
-                              "or `python paper_2606_06256_b200/build.py`. There is no fallback path." % LIB_PATH)
-        L = C.CDLL(LIB_PATH)
+        path = LIB_PATH if _which == "product" else BRINGUP_LIB_PATH
+        if not os.path.exists(path):
+            raise ImportError("%s is not built (%s); run `python -c 'import __graft_entry__ as g; g.build()'` "
+                              "or `python paper_2606_06256_b200/build.py`. There is no fallback path." % (os.path.basename(path), path))
+        L = C.CDLL(path)
         L.segpa_pool_bytes.restype = C.c_int64
         L.segpa_last_error.restype = C.c_char_p
         L.segpa_version.restype = C.c_int32
@@ -119,6 +142,7 @@ def lib():
         L.segpa_mass_select.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
         L.segpa_destroy.argtypes = [C.c_void_p]
         _lib = L
+        _libs[_which] = L
     return _lib
 
 
@@ -138,9 +162,10 @@ def _stream_ptr(stream) -> Optional[int]:
 # ---------------------------------------------------------------------------------------------
 
 def segpa_create_cache(*, num_layers: int, num_q_heads: int, num_kv_heads: int, head_dim: int,
-                       page_size: int, num_pages: int, device: int = 0, k_pool: int = 0, v_pool: int = 0) -> int:
+                       page_size: int, num_pages: int, device: int = 0, k_pool: int = 0, v_pool: int = 0,
+                       tiles_per_item: int = 0) -> int:
     d = CacheDesc(num_layers, num_q_heads, num_kv_heads, head_dim, page_size, device, num_pages,
-                  k_pool or None, v_pool or None)
+                  k_pool or None, v_pool or None, tiles_per_item, 0)
     out = C.c_void_p()
     _check(lib().segpa_create_cache(C.byref(d), C.byref(out)))
     return out.value

@@ -749,13 +749,6 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
 }
 
 // ---------------------------------------------------------------------------------------------
-int attention_tc_tiles_per_item() {
-    // SEGPA_TC_TILES=1|2 (bring-up knob; read at every build_segments call)
-    const char* e = getenv("SEGPA_TC_TILES");
-    const int t = e ? atoi(e) : 2;
-    return (t == 1) ? 1 : 2;
-}
-
 template <int D, int NT>
 static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
     using C = Cfg<D, NT>;

@@ -50,6 +50,9 @@ struct StreamKeyHash {
 struct StreamRec {
     std::vector<int32_t> pages;
     int64_t kv_len = 0;
+    // append_pages_batch: index of this stream's last COPY job in the batch with stamp `batch_stamp`
+    uint64_t batch_stamp = 0;
+    int32_t batch_job = -1;
 };
 
 struct DeviceGuard {
@@ -213,7 +216,8 @@ struct segpa_cache {
     uint8_t* k_pool = nullptr;
     uint8_t* v_pool = nullptr;
     std::vector<int32_t> refcnt;
-    std::vector<int32_t> free_list;  // may hold stale entries (refcnt != 0): skipped on pop
+    std::vector<int32_t> free_list;  // may hold stale entries (refcnt != 0: pages taken by caller-given id): skipped on pop
+    std::vector<uint8_t> in_free;    // page id is somewhere in free_list (so a release never adds a second entry)
     int64_t n_free = 0;
     std::unordered_map<StreamKey, StreamRec, StreamKeyHash> streams;
     std::vector<segpa_segments*> seg_objs;
@@ -224,9 +228,11 @@ struct segpa_cache {
     std::vector<int32_t> append_touched;   // append_pages_batch scratch, kept between calls
     Staging append_stage[2];         // alternating, so staging a batch does not wait for the previous one
     int append_turn = 0;
+    uint64_t batch_stamp = 0;        // one per append_pages_batch call (StreamRec::batch_stamp)
     int num_sms = 148;
     cudaStream_t up_stream = nullptr;   // descriptor uploads (staging_upload)
-    int kernel_kind = 1;  // 0 = SIMT bring-up kernel (SEGPA_KERNEL=simt), 1 = tcgen05
+    int kernel_kind = 1;  // 1 = tcgen05 (the product); 0 = SIMT cross-check kernel, only in the test build (-DSEGPA_BRINGUP)
+    int tiles_per_item = 2;   // 128-row tiles per work item (desc.tiles_per_item; fixed at create)
     int last_launches = 0;
     // host-buffer entry point staging
     uint16_t* st_q = nullptr;
@@ -241,6 +247,7 @@ int32_t pop_free_page(segpa_cache* c) {
     while (!c->free_list.empty()) {
         int32_t id = c->free_list.back();
         c->free_list.pop_back();
+        c->in_free[(size_t)id] = 0;
         if (c->refcnt[id] == 0) return id;
     }
     return -1;
@@ -248,7 +255,10 @@ int32_t pop_free_page(segpa_cache* c) {
 
 void release_page(segpa_cache* c, int32_t id) {
     if (--c->refcnt[id] == 0) {
-        c->free_list.push_back(id);
+        if (!c->in_free[(size_t)id]) {
+            c->free_list.push_back(id);
+            c->in_free[(size_t)id] = 1;
+        }
         ++c->n_free;
     }
 }
@@ -341,6 +351,7 @@ segpa_status_t segpa_create_cache(const segpa_cache_desc_t* d, segpa_cache_t** o
     if ((d->k_pool == nullptr) != (d->v_pool == nullptr))
         return fail(SEGPA_ERR_INVALID, "create_cache: give both k_pool and v_pool or neither");
     if (d->device < -1) return fail(SEGPA_ERR_INVALID, "create_cache: bad device %d", d->device);
+    if (d->tiles_per_item < 0 || d->tiles_per_item > 2) return fail(SEGPA_ERR_INVALID, "create_cache: tiles_per_item %d (0 = default, 1 or 2)", d->tiles_per_item);
 
     segpa_cache* c = new (std::nothrow) segpa_cache();
     if (!c) return fail(SEGPA_ERR_OOM, "create_cache: host allocation failed");
@@ -348,12 +359,12 @@ segpa_status_t segpa_create_cache(const segpa_cache_desc_t* d, segpa_cache_t** o
     c->G = d->num_q_heads / d->num_kv_heads;
     c->page_bytes = d->page_size * d->head_dim * 2;
     c->planning_only = (d->device == -1);
-    const char* kk = getenv("SEGPA_KERNEL");
-    c->kernel_kind = (kk && strcmp(kk, "simt") == 0) ? 0 : 1;
+    c->tiles_per_item = d->tiles_per_item == 0 ? 2 : d->tiles_per_item;
     try {
         c->refcnt.assign((size_t)d->num_pages, 0);
         c->free_list.resize((size_t)d->num_pages);
         for (int64_t i = 0; i < d->num_pages; ++i) c->free_list[(size_t)i] = (int32_t)(d->num_pages - 1 - i);
+        c->in_free.assign((size_t)d->num_pages, 1);
     } catch (const std::bad_alloc&) {
         delete c;
         return fail(SEGPA_ERR_OOM, "create_cache: host allocation failed");
@@ -435,6 +446,7 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
     std::vector<ScatterJob> jobs;
     std::vector<int32_t>& touched = c->append_touched;     // page ids the scatter kernel indexes, job after job
     touched.clear();
+    const uint64_t stamp = ++c->batch_stamp;
     long long total_chunks = 0;
     try {
         size_t ub = 0;   // one allocation at most (an upper bound of the ids listed: new pages + a refilled last page per job)
@@ -498,6 +510,16 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
             StreamRec& rec = c->streams[key];
             undo.push_back(Undo{key, created, cur_len, 0});
             rec.pages.reserve(rec.pages.size() + (size_t)need);
+            if (!attach && cur_len % P != 0) {
+                // The new rows start inside the stream's partial last page.  That page must be this stream's alone:
+                // a page attached by another stream (reference count > 1) would be overwritten under it.
+                if (c->refcnt[rec.pages.back()] > 1) {
+                    APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: the stream's partial last page %d is shared with another stream (reference count %d); copying into it would overwrite that stream's view", i, rec.pages.back(), c->refcnt[rec.pages.back()]);
+                }
+                // An earlier COPY job of this batch that ended in the same page must not zero-fill the slots this
+                // job writes (both run in one launch, unordered): its writes stop at its own last token.
+                if (rec.batch_stamp == stamp && rec.batch_job >= 0) jobs[(size_t)rec.batch_job].n_write = jobs[(size_t)rec.batch_job].n_tokens;
+            }
             if (!attach) {
                 ScatterJob jb{};
                 jb.k_src = (const uint16_t*)r.k_src;
@@ -509,7 +531,10 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 jb.first_slot = (int)(cur_len % P);
                 jb.n_pages = (int)need + (cur_len % P != 0 ? 1 : 0);
                 if (cur_len % P != 0) touched.push_back(rec.pages.back());   // (a partial last page is never a hole: evict_pages refuses it)
-                total_chunks += ((long long)jb.n_pages * P - jb.first_slot) * (D >> 3);
+                jb.n_write = (long long)jb.n_pages * P - jb.first_slot;     // rows + the zero-filled tail of the last page
+                total_chunks += jb.n_write * (D >> 3);
+                rec.batch_stamp = stamp;
+                rec.batch_job = (int32_t)jobs.size();
                 jobs.push_back(jb);
             }
             for (int64_t k = 0; k < need; ++k) {
@@ -747,6 +772,7 @@ segpa_status_t segpa_clear_streams(segpa_cache_t* c) {
     std::fill(c->refcnt.begin(), c->refcnt.end(), 0);
     c->free_list.resize((size_t)c->desc.num_pages);
     for (int64_t i = 0; i < c->desc.num_pages; ++i) c->free_list[(size_t)i] = (int32_t)(c->desc.num_pages - 1 - i);
+    std::fill(c->in_free.begin(), c->in_free.end(), 1);
     c->n_free = c->desc.num_pages;
     return SEGPA_OK;
 }
@@ -792,7 +818,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
     const int P = c->desc.page_size, G = c->G, D = c->desc.head_dim;
     const int ppb = kBlockKeys / P;
     const int32_t zero_page = (int32_t)c->desc.num_pages;
-    const int tiles_per_item = (c->kernel_kind == 1) ? attention_tc_tiles_per_item() : 1;
+    const int tiles_per_item = (c->kernel_kind == 1) ? c->tiles_per_item : 1;
     const int TT = kTileRows / G;               // tokens per 128-row tile (GQA packing)
     const int item_tok = TT * tiles_per_item;
 
@@ -1202,10 +1228,16 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     cudaMemsetAsync(d_trace, 0, 16 * kTraceCap * 8, st);
     p.trace = d_trace;
 #endif
-    if (c->kernel_kind == 0) e = cudaMemsetAsync(s->buf->counter, 0, 256, st);   // only the SIMT kernel pulls from a cursor
     int launches = 0;
+#ifdef SEGPA_BRINGUP
+    if (c->kernel_kind == 0) {   // test build only: the SIMT cross-check kernel over the same plan (it pulls items from a cursor)
+        e = cudaMemsetAsync(s->buf->counter, 0, 256, st);
+        if (e == cudaSuccess) e = launch_attention_simt(p, st);
+        ++launches;
+    } else
+#endif
     if (e == cudaSuccess) {
-        e = (c->kernel_kind == 0) ? launch_attention_simt(p, st) : launch_attention_tc(p, st);
+        e = launch_attention_tc(p, st);
         ++launches;
     }
     if (e == cudaSuccess && p.n_combs > 0) {
@@ -1425,5 +1457,17 @@ segpa_status_t segpa_mass_select(segpa_cache_t* c, const segpa_segments_t* s, co
 }
 
 int32_t segpa_last_launch_count(const segpa_cache_t* c) { return c ? c->last_launches : 0; }
+
+#ifdef SEGPA_BRINGUP
+// Test build only (libsegpa_bringup.so; not declared in include/segpa.h, not in the product library): run the
+// plans of this cache on the SIMT cross-check kernel -- a second opinion on the pool layout, the builder and the
+// scheduler that shares no kernel code with the tcgen05 path.  Call before build_segments.
+segpa_status_t segpa_bringup_use_simt(segpa_cache_t* c, int32_t on) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "bringup_use_simt: null cache");
+    if (!c->seg_objs.empty()) return fail(SEGPA_ERR_STATE, "bringup_use_simt: segments objects exist");
+    c->kernel_kind = on ? 0 : 1;
+    return SEGPA_OK;
+}
+#endif
 
 }  // extern "C"

@@ -114,6 +114,8 @@ struct ScatterJob {
     long long page_off;          // index of this job's first touched page id in the batch's id array
     int first_slot;              // slot of the first new token inside the first touched page
     int n_pages;                 // touched pages (the partial last page of the stream + new pages)
+    long long n_write;           // slots written from first_slot on: n_tokens rows, then zeros; = n_tokens when a later
+                                 // job of the same batch continues the stream inside this job's last page
 };
 
 // cos / sin of delta_pos * theta_d for the D/2 rotation pairs (host-computed in fp64)
@@ -172,9 +174,10 @@ cudaError_t launch_mass_select(const float* mass, const long long* mass_off_dev,
 // kernel launchers (each returns the CUDA error of its launch)
 cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const ScatterJob* jobs_dev, int n_jobs,
                                  const int* page_ids_dev, long long total_chunks, int D, int P, cudaStream_t st);
-cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st);
+#ifdef SEGPA_BRINGUP
+cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st);   // test build only (libsegpa_bringup.so)
+#endif
 cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st);
 cudaError_t launch_combine(const FwdParams& p, cudaStream_t st);
-int attention_tc_tiles_per_item();
 
 }  // namespace segpa

@@ -1,5 +1,5 @@
-// Small kernels of libsegpa.so: page scatter (append), split-KV combine, and the SIMT bring-up
-// attention kernel (selected with SEGPA_KERNEL=simt; the product kernel is segpa_attn_tc.cu).
+// Small kernels of libsegpa.so: page scatter (append), RoPEAlign, row gather, split-KV combine, LSE merge; and,
+// in the test build only (-DSEGPA_BRINGUP -> libsegpa_bringup.so), the SIMT cross-check attention kernel.
 #include "segpa_internal.h"
 
 #include <cuda_bf16.h>
@@ -31,6 +31,7 @@ __global__ void scatter_pages_kernel(uint8_t* __restrict__ k_pool, uint8_t* __re
         const int page = page_ids[jb.page_off + gs / P];
         const int slot = (int)(gs % P);
         const size_t dst = (size_t)page * ((size_t)P * D * 2) + page_elem_offset_bytes(D, slot, c * 8);
+        if (n >= jb.n_write) continue;   // tail slots that a later job of this batch fills (same stream, same page)
         uint4 kv = make_uint4(0, 0, 0, 0), vv = make_uint4(0, 0, 0, 0);
         if (n < jb.n_tokens) {
             kv = *reinterpret_cast<const uint4*>(jb.k_src + n * jb.src_stride + c * 8);
@@ -283,8 +284,9 @@ cudaError_t launch_merge(const uint16_t* out_a, const float* lse_a, const uint16
     return cudaGetLastError();
 }
 
+#ifdef SEGPA_BRINGUP
 // ---------------------------------------------------------------------------------------------
-// SIMT bring-up attention: same plan, same outputs, no tensor cores.  One warp per query row;
+// SIMT cross-check attention (test build only): same plan, same outputs, no tensor cores.  One warp per query row;
 // lanes split the head dim; keys visited one at a time.  Exists to validate the pool layout, the
 // builder and the scheduler independently of the tcgen05 kernel.
 // ---------------------------------------------------------------------------------------------
@@ -357,5 +359,6 @@ cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st) {
     attention_simt_kernel<<<p.num_sms * 4, 256, 0, st>>>(p);
     return cudaGetLastError();
 }
+#endif  // SEGPA_BRINGUP
 
 }  // namespace segpa

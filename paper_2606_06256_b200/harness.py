@@ -10,9 +10,9 @@ from . import binding as B
 from . import workloads as wl
 
 
-def create_cache(w: wl.Workload, device: int = 0) -> int:
+def create_cache(w: wl.Workload, device: int = 0, tiles_per_item: int = 0) -> int:
     return B.segpa_create_cache(num_layers=w.num_layers, num_q_heads=w.Hq, num_kv_heads=w.Hkv, head_dim=w.D,
-                                page_size=w.P, num_pages=w.num_pages, device=device)
+                                page_size=w.P, num_pages=w.num_pages, device=device, tiles_per_item=tiles_per_item)
 
 
 def append_requests(w: wl.Workload, k_pool=None, v_pool=None) -> List[tuple]:

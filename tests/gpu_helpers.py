@@ -1,8 +1,6 @@
 """GPU-side test plumbing: run a Workload through libsegpa.so and compare with the oracle."""
 from __future__ import annotations
 
-import os
-
 import numpy as np
 import torch
 
@@ -15,15 +13,22 @@ TOL_OUT_MAX, TOL_OUT_MEAN, TOL_LSE = 2e-2, 2e-3, 1e-3     # BASELINE.json:north_
 
 
 class GpuRun:
+    """kernel "tc": the product library.  kernel "simt": the test build (libsegpa_bringup.so) with its SIMT
+    cross-check kernel -- the binding is switched to that library for the lifetime of the run."""
+
     def __init__(self, w: wl.Workload, kernel: str = "tc", tiles: int = 1, k_pool=None, v_pool=None):
-        os.environ["SEGPA_KERNEL"] = kernel
-        os.environ["SEGPA_TC_TILES"] = str(tiles)
+        assert kernel in ("tc", "simt")
         self.w = w
         self.dev = torch.device("cuda:0")
         if k_pool is None:
             k_pool, v_pool = wl.pool_values(w, self.dev)
         self.k_pool, self.v_pool = k_pool, v_pool
-        self.cache = H.create_cache(w, 0)
+        self.bringup = kernel == "simt"
+        if self.bringup:
+            B.use_library("bringup")
+        self.cache = H.create_cache(w, 0, tiles_per_item=tiles)
+        if self.bringup:
+            B.segpa_bringup_use_simt(self.cache)
         H.append_workload(self.cache, w, k_pool, v_pool)
         self.segs = {}
 
@@ -42,6 +47,8 @@ class GpuRun:
     def close(self):
         B.segpa_destroy(self.cache)
         self.cache = None
+        if self.bringup:
+            B.use_library("product")
 
 
 def compare(w, layer, k_pool, v_pool, q, out, lse, rows=None, label=""):
@@ -69,9 +76,10 @@ def compare(w, layer, k_pool, v_pool, q, out, lse, rows=None, label=""):
     return msg
 
 
-def sample_rows(w, layer, n_random=256, seed=0):
-    """Stratified row sample: heads and tails of each segment, rows around tile and
-    128-key block edges, plus seeded uniform rows."""
+def sample_rows(w, layer, n_random=256, seed=0, tile_edges=8, block_edges=6, ends=40, dense_tail=0):
+    """Stratified row sample: the first and last `ends` rows of each segment (`dense_tail`: at
+    least that many last rows), rows around `tile_edges` tile edges and `block_edges` 128-key block edges spread
+    over the segment, plus seeded uniform rows (n_random over the layer).  Every row it picks is compared."""
     rng = np.random.default_rng(seed)
     rows = set()
     sm = w.stream_map()
@@ -79,20 +87,20 @@ def sample_rows(w, layer, n_random=256, seed=0):
     for s in w.layer_segments(layer):
         q0, ql = s.q_row_start, s.q_len
         kv = sm[(s.layer, s.kv_head, s.seq_id)].kv_len
-        for t in list(range(min(ql, 40))) + list(range(max(0, ql - 40), ql)):
+        for t in list(range(min(ql, ends))) + list(range(max(0, ql - max(ends, dense_tail)), ql)):
             rows.add(q0 + t)
-        for edge in range(TT, ql, TT * max(1, ql // (TT * 8))):
+        for edge in range(TT, ql, TT * max(1, ql // (TT * tile_edges))):
             for d in (-1, 0, 1):
                 if 0 <= edge + d < ql:
                     rows.add(q0 + edge + d)
         # rows whose position sits at a 128-key block edge
         p0 = kv - ql
-        for blk in range((p0 // 128 + 1) * 128, kv, 128 * max(1, (kv - p0) // (128 * 6))):
+        for blk in range((p0 // 128 + 1) * 128, kv, 128 * max(1, (kv - p0) // (128 * block_edges))):
             for d in (-1, 0, 1):
                 t = blk + d - p0
                 if 0 <= t < ql:
                     rows.add(q0 + t)
-        if ql > 80:
+        if ql > 2 * ends:
             for t in rng.integers(0, ql, size=max(4, n_random // max(1, len(w.layer_segments(layer))))):
                 rows.add(q0 + int(t))
     return np.array(sorted(rows), dtype=np.int64)

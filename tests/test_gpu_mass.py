@@ -54,6 +54,57 @@ def test_attention_mass_matches_oracle_column_sums(case):
         g.close()
 
 
+def test_attention_mass_at_cfg2_size():
+    """The mass kernel on the whole of cfg2 (32 segments, 16713 rows: the multi-CTA LPT, the Q ring wrapping around
+    many times, wholly visible tiles on the fast path), compared with the oracle on the longest request's GLOBAL
+    segment and one of its LOCAL segments (every key of both; the oracle's p summed over the segment's rows in
+    chunks, on the two KV heads only: the oracle is handed q restricted to their 8 query heads)."""
+    import oracle
+    w = wl.config2()
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        segs = g.segs[0]
+        offs = B.segpa_segments_mass_layout(segs)
+        mass = torch.full((int(offs[-1]),), -1.0, dtype=torch.float32, device=g.dev)
+        B.segpa_attention_mass(g.cache, segs, q, w.scale, lse, mass)
+        torch.cuda.synchronize()
+        mass = mass.cpu().numpy().astype(np.float64)
+        all_segs = w.layer_segments(0)
+        sm = w.stream_map()
+        # every segment: total mass = rows x G, padding 0
+        for si, s in enumerate(all_segs):
+            kv = sm[(0, s.kv_head, s.seq_id)].kv_len
+            assert abs(mass[offs[si]:offs[si] + kv].sum() - s.q_len * w.G) <= 1e-3 * s.q_len * w.G
+            assert np.all(mass[offs[si] + kv:offs[si + 1]] == 0)
+        seq = int(np.argmax(w.notes["lengths"]))
+        heads = (0, 5)                                         # GLOBAL head 0, LOCAL head 5 (W = 1024)
+        pick = [si for si, s in enumerate(all_segs) if s.seq_id == seq and s.kv_head in heads]
+        assert [all_segs[si].head_class for si in pick] == [GLOBAL, LOCAL]
+        table, pt_off, kv_lens, index = wl.csr_page_tables(w, 0)
+        qh = torch.cat([torch.arange(h * w.G, (h + 1) * w.G) for h in heads]).to(q.device)
+        q_sub = q[:, qh].contiguous()                          # [T][8][D]: the oracle sees a 2-KV-head problem
+        tup = [(index[(all_segs[si].kv_head, seq)], k, all_segs[si].head_class, all_segs[si].window, all_segs[si].n_sink,
+                all_segs[si].q_row_start, all_segs[si].q_len) for k, si in enumerate(pick)]
+        L = w.notes["lengths"][seq]
+        q0 = all_segs[pick[0]].q_row_start
+        want = np.zeros((2, L))
+        for lo in range(0, L, 512):
+            rows = np.arange(q0 + lo, q0 + min(L, lo + 512))
+            res = oracle.oracle_attention(Hq=2 * w.G, Hkv=2, D=w.D, P=w.P, k_pool=g.k_pool, v_pool=g.v_pool, page_table=table,
+                                          pt_offsets=pt_off, kv_lens=kv_lens, segments=tup, q=q_sub, T=w.T[0], scale=w.scale,
+                                          row_subset=rows, want_p=L)
+            for k in range(2):
+                want[k] += res.p[:, k * w.G:(k + 1) * w.G, :].sum(axis=(0, 1))
+        for k, si in enumerate(pick):
+            got = mass[offs[si]:offs[si] + L]
+            err = np.abs(got - want[k])
+            assert np.all(err <= 4e-3 * want[k] + 1e-3), (si, err.max(), int(np.argmax(err)))
+            assert np.all(got[want[k] == 0] == 0)
+    finally:
+        g.close()
+
+
 @pytest.mark.parametrize("tau", [0.05, 0.5, 0.9, 1.0])
 def test_mass_select_is_the_smallest_covering_set(tau):
     Hq, Hkv, D, P, reqs = CASES[0]

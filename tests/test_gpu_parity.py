@@ -269,6 +269,66 @@ def test_copy_append_rejects_duplicate_ids_and_rolls_back():
         B.segpa_destroy(cache)
 
 
+def test_two_copy_jobs_of_one_batch_extend_the_same_stream():
+    """segpa.h: a later request of a batch may extend the same stream.  Job A (10 tokens) ends inside a page and
+    zero-fills its tail; job B (3 tokens, then 40 more) starts in that same page, in the same scatter launch:
+    A's zero-fill must not reach B's slots.  Read back with segpa_gather_rows; repeated to catch a race."""
+    w = wl.config1()
+    dev = torch.device("cuda:0")
+    D, P = w.D, w.P
+    torch.manual_seed(7)
+    k = torch.randn((53, D), device=dev).to(torch.bfloat16)
+    v = torch.randn((53, D), device=dev).to(torch.bfloat16)
+    for rep in range(20):
+        cache = H.create_cache(w, 0)
+        try:
+            B.segpa_append_pages_batch(cache, [(0, 0, 5, k[:10], v[:10], 10, None),
+                                               (0, 0, 5, k[10:13], v[10:13], 3, None),
+                                               (0, 1, 9, k[:7], v[:7], 7, [100]),
+                                               (0, 0, 5, k[13:], v[13:], 40, None)])
+            kv_len, ids = B.segpa_stream_info(cache, 0, 0, 5)
+            assert kv_len == 53 and len(ids) == 4
+            ko, vo = torch.zeros_like(k), torch.zeros_like(v)
+            B.segpa_gather_rows(cache, 0, 0, 5, 0, 53, ko, vo)
+            torch.cuda.synchronize()
+            assert torch.equal(ko, k) and torch.equal(vo, v), rep
+            # the tail of the stream's last page (slots 5..15 of page 3) is still zero-filled
+            B.segpa_append_pages(cache, 0, 0, 77, None, None, 16, page_ids=ids[3:4])
+            kt, vt = torch.ones((16, D), dtype=torch.bfloat16, device=dev), torch.ones((16, D), dtype=torch.bfloat16, device=dev)
+            B.segpa_gather_rows(cache, 0, 0, 77, 0, 16, kt, vt)
+            torch.cuda.synchronize()
+            assert torch.equal(kt[:5], k[48:]) and not kt[5:].any() and not vt[5:].any()
+        finally:
+            B.segpa_destroy(cache)
+
+
+def test_copy_into_a_shared_partial_page_is_refused():
+    """A page can be the partial tail of two streams (B attaches A's pages, A's length not a multiple of P).  A COPY
+    append into that page through either stream would overwrite slots the other stream sees: INVALID, nothing applied."""
+    w = wl.config1()
+    dev = torch.device("cuda:0")
+    rows = torch.ones((24, w.D), dtype=torch.bfloat16, device=dev)
+    more = torch.full((8, w.D), 2.0, dtype=torch.bfloat16, device=dev)
+    cache = H.create_cache(w, 0)
+    try:
+        B.segpa_append_pages(cache, 0, 0, 1, rows, rows, 24, page_ids=[10, 11])
+        B.segpa_append_pages(cache, 0, 0, 2, None, None, 24, page_ids=[10, 11])       # stream 2 shares both pages
+        before = B.segpa_pool_stats(cache)
+        for seq in (1, 2):
+            with pytest.raises(B.SegpaError, match="shared with another stream"):
+                B.segpa_append_pages(cache, 0, 0, seq, more, more, 8)
+            assert B.segpa_stream_info(cache, 0, 0, seq)[0] == 24
+        assert B.segpa_pool_stats(cache) == before
+        B.segpa_free_stream(cache, 0, 0, 2)                                            # sole owner again: allowed
+        B.segpa_append_pages(cache, 0, 0, 1, more, more, 8)
+        ko = torch.zeros((32, w.D), dtype=torch.bfloat16, device=dev)
+        B.segpa_gather_rows(cache, 0, 0, 1, 0, 32, ko, None)
+        torch.cuda.synchronize()
+        assert torch.equal(ko[:24], rows) and torch.equal(ko[24:], more)
+    finally:
+        B.segpa_destroy(cache)
+
+
 def test_back_to_back_steps_without_host_sync():
     """Steps enqueued back to back (store, plan, attend; the previous step's plan freed while its kernel may
     still run): plan storage is only reused once its last use has completed on the device, so every step
@@ -351,12 +411,15 @@ def test_cfg2_sampled(tiles):
 
 
 def test_cfg3_sampled():
+    """cfg3 at full size: every stratified row is compared (64 tile edges and 64 block edges of the 64K-row GLOBAL
+    segment, its first / last rows, 512 uniform rows) and the whole 1024-row suffix 64512..65535 that the seven
+    LOCAL heads query, densely."""
     w = wl.config3()
     g = GpuRun(w, "tc", 2)
     try:
         q, out, lse = g.layer(0)
-        rows = sample_rows(w, 0, n_random=64, seed=3)
-        rows = rows[:: max(1, len(rows) // 300)]
+        rows = sample_rows(w, 0, n_random=4096, seed=3, tile_edges=64, block_edges=64, dense_tail=1024)
+        assert len(rows) > 2000 and np.isin(np.arange(64512, 65536), rows).all()
         print(len(rows), compare(w, 0, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg3"))
     finally:
         g.close()
@@ -386,15 +449,56 @@ def test_cfg4_decode_only_sampled():
         g.close()
 
 
-def test_cfg5_two_layers_sampled():
-    w = wl.config5(num_layers=2)
+def test_cfg5_all_layers_sampled():
+    """cfg5 at full size, ALL 28 layers (BASELINE.json configs[4]; SURVEY 8(c) "cfg5 is compared per layer"): about
+    300 stratified rows per layer, all 28 query heads.  The 16 GLOBAL (layer, head) pairs of the seeded class map sit
+    in layers 2, 4, 7, 9, ...: the G = 7 / P = 32 GLOBAL path at 32K is compared wherever it occurs."""
+    w = wl.config5()
+    gl_layers = sorted({p // w.Hkv for p in w.notes["global_pairs"]})
+    assert len(w.notes["global_pairs"]) == 16 and 0 not in gl_layers and 1 not in gl_layers and len(gl_layers) >= 10
     g = GpuRun(w, "tc", 2)
     try:
-        for layer in range(2):
+        n_global_checked = 0
+        for layer in range(w.num_layers):
             q, out, lse = g.layer(layer)
-            rows = sample_rows(w, layer, n_random=64, seed=5)
-            rows = rows[:: max(1, len(rows) // 300)]
-            print(len(rows), compare(w, layer, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg5 L%d" % layer))
+            rows = sample_rows(w, layer, n_random=256, seed=50 + layer, tile_edges=8, block_edges=8, ends=24)
+            assert 250 <= len(rows) <= 500, len(rows)
+            msg = compare(w, layer, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg5 L%d" % layer)
+            n_gl = sum(s.head_class == GLOBAL for s in w.layer_segments(layer))
+            n_global_checked += n_gl
+            print(len(rows), "global heads: %d" % n_gl, msg)
+            del q, out, lse
+        assert n_global_checked == 16
+    finally:
+        g.close()
+
+
+# ----------------------------------------------------- the paper's micro-benchmark shape (PAPER.md:354-356, Fig. 9(e)-(h))
+def test_fig9_decode_128k():
+    """Qwen3-32B-shaped layer, 4 GLOBAL + 4 LOCAL (sink 4 + window 316 = the paper's 320 visible keys) KV heads, one
+    decode query over a 131072-token context: twice the longest stream of the five configs.  Compared in full."""
+    w = wl.fig9(131072, "decode", num_layers=1)
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        st = B.segpa_segments_stats(g.segs[0])
+        assert st["n_split_tiles"] >= 4 and B.segpa_last_launch_count(g.cache) == 2      # split-KV + combine
+        print(compare(w, 0, g.k_pool, g.v_pool, q, out, lse, label="fig9 decode 128K"), st)
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("ctx_k", [32, 128])
+def test_fig9_prefill_sampled(ctx_k):
+    """The same shape fully prefilled (q_len = L) at 32K and 128K: stratified rows, all 32 query heads."""
+    w = wl.fig9(ctx_k * 1024, "prefill", num_layers=1)
+    g = GpuRun(w, "tc", 2)
+    try:
+        q, out, lse = g.layer(0)
+        rows = sample_rows(w, 0, n_random=256, seed=90 + ctx_k, tile_edges=12, block_edges=12, ends=16)
+        rows = np.unique(np.concatenate([rows, np.arange(w.T[0] - 160, w.T[0])]))
+        assert len(rows) >= 300
+        print(len(rows), compare(w, 0, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="fig9 prefill %dK" % ctx_k))
     finally:
         g.close()
 

@@ -13,9 +13,9 @@ from paper_2606_06256_b200.workloads import GLOBAL, LOCAL
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
-def plan_cache(Hq=8, Hkv=2, D=128, P=16, num_pages=4096, layers=1):
+def plan_cache(Hq=8, Hkv=2, D=128, P=16, num_pages=4096, layers=1, tiles=0):
     return B.segpa_create_cache(num_layers=layers, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=D, page_size=P,
-                                num_pages=num_pages, device=-1)
+                                num_pages=num_pages, device=-1, tiles_per_item=tiles)
 
 
 def test_library_exports_every_declared_symbol():
@@ -26,6 +26,23 @@ def test_library_exports_every_declared_symbol():
     for name in declared:
         assert hasattr(L, name), name
     assert B.segpa_version() == 1
+
+
+def test_product_library_has_no_second_backend():
+    """BASELINE north_star "no multi-backend dispatch": the SIMT cross-check kernel and its switch exist only in
+    the test build (libsegpa_bringup.so, -DSEGPA_BRINGUP); the product library holds neither, and reads no
+    SEGPA_* environment variable."""
+    import subprocess
+    L = ctypes.CDLL(B.LIB_PATH)
+    assert not hasattr(L, "segpa_bringup_use_simt")
+    syms = subprocess.run(["nm", "-C", B.LIB_PATH], capture_output=True, text=True).stdout
+    assert "attention_simt" not in syms and "attention_tc_kernel" in syms
+    blob = open(B.LIB_PATH, "rb").read()
+    assert b"SEGPA_KERNEL" not in blob and b"SEGPA_TC_TILES" not in blob and b"SEGPA_TRACE" not in blob
+    T = ctypes.CDLL(B.BRINGUP_LIB_PATH)
+    assert hasattr(T, "segpa_bringup_use_simt")
+    with pytest.raises(B.SegpaError, match="tiles_per_item"):
+        plan_cache(tiles=3)
 
 
 def test_no_cpu_fallback_without_gpu():
@@ -135,12 +152,11 @@ def test_visible_page_selection_and_tiles(P):
         cls = int(rng.integers(0, 2))
         W = int(rng.choice([1, 2, P - 1, P, P + 1, 127, 128, 129, 700, 5000]))
         G = int(rng.choice([1, 4, 7, 8]))
-        c = plan_cache(Hq=2 * G, Hkv=2, P=P, num_pages=1024)
         npg = (kv_len + P - 1) // P
         ids = rng.permutation(1024)[:npg].astype(np.int32)
-        B.segpa_append_pages(c, 0, 1, 42, None, None, kv_len, page_ids=ids)
         for tiles in (1, 2):
-            os.environ["SEGPA_TC_TILES"] = str(tiles)
+            c = plan_cache(Hq=2 * G, Hkv=2, P=P, num_pages=1024, tiles=tiles)
+            B.segpa_append_pages(c, 0, 1, 42, None, None, kv_len, page_ids=ids)
             segs = B.segpa_build_segments(c, 0, [(42, 1, cls, W, 0, 10, q_len)])
             first, got = B.segpa_segments_pages(segs, 0)
             efirst, exp = _expected_pages(kv_len, q_len, cls, W, P, ids, 1024)
@@ -187,12 +203,11 @@ def test_visible_page_selection_and_tiles(P):
             tot = [sum(3 * x + 2 for x in cs) for cs in loads.values()]
             assert max(tot) - min(tot) <= 3 * max(costs) + 2
             B.segpa_free_segments(c, segs)
-        B.segpa_destroy(c)
+            B.segpa_destroy(c)
 
 
 def test_split_kv_plan_for_decode():
-    os.environ["SEGPA_TC_TILES"] = "1"
-    c = plan_cache(num_pages=4096)
+    c = plan_cache(num_pages=4096, tiles=1)
     B.segpa_append_pages(c, 0, 0, 0, None, None, 30000, page_ids=np.arange(1875))
     segs = B.segpa_build_segments(c, 0, [(0, 0, GLOBAL, 0, 0, 0, 1)])
     st = B.segpa_segments_stats(segs)
@@ -274,7 +289,6 @@ def test_sinks_select_two_page_ranges_and_eviction_is_checked():
 
 def test_config_plans_match_closed_forms():
     """Useful work of the five BASELINE configs as planned by the library == generator closed forms."""
-    os.environ["SEGPA_TC_TILES"] = "2"
     for cfg in (1, 2, 3, 4):
         w = wl.CONFIGS[cfg]()
         c = B.segpa_create_cache(num_layers=1, num_q_heads=w.Hq, num_kv_heads=w.Hkv, head_dim=w.D, page_size=w.P,
@@ -294,7 +308,6 @@ def test_lpt_assignment_matches_plain_heap_restatement():
     the smallest (load, cta); load grows by 3 * blocks + 2 thirds of a block-time.
     Workloads without strided or sink items, where the cost is kb_hi - kb_lo."""
     import heapq
-    os.environ["SEGPA_TC_TILES"] = "2"
     rng = np.random.default_rng(3)
     for trial in range(4):
         n_req = int(rng.integers(2, 7))

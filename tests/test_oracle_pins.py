@@ -330,6 +330,56 @@ def test_T12_torch_sdpa_causal_midsize():
     assert np.abs(res.lse - torch.logsumexp(S, dim=-1).numpy()).max() < 1e-12
 
 
+# ---------------------------------------------------------------------- row_subset path (T13)
+@pytest.mark.parametrize("P", [4, 16])
+def test_T13_row_subset_equals_full_run_bit_for_bit(P):
+    """Every full-size expected value goes through oracle_attention(row_subset=R) (subset_find + the
+    subset-indexed outputs): pin it to the full run at rows R, bit for bit, for out, lse, p and pairs.
+    R is handed over unsorted with duplicates and holds rows of every kind: covered by all heads, by one
+    KV head only (the other head's q range is shorter), the first and the last row of a segment, and -- second
+    request -- rows that other requests own.  `pairs` is checked against the T2 closed form, not the full run."""
+    reqs = [{"kv_len": 67, "heads": {0: (GLOBAL, 0, 0, 67), 1: (LOCAL, 9, 3, 20)}},
+            {"kv_len": 33, "heads": {0: (LOCAL, 5, 0, 33), 1: (GLOBAL, 0, 0, 1)}}]
+    w = tiny(0, None, requests=reqs, P=P, seed=77)
+    k, v, q = values(w)
+    T = w.T[0]
+    full = run_oracle(w, 0, k, v, q, want_p=67)
+    R = np.array([99, 0, 66, 47, 46, 5, 67, 98, 5, 66, 13, 80], dtype=np.int64)     # unsorted, 5 and 66 twice
+    assert R.max() < T
+    sub = run_oracle(w, 0, k, v, q, row_subset=R, want_p=67)
+    rows = sub.rows
+    assert np.array_equal(rows, np.unique(R))
+    cov = covered_mask(w, 0, rows)
+    assert cov.any() and (~cov).any()                       # rows 0..46 are not covered by kv head 1 (q_len 20)
+    # bit for bit (NaN where no segment covers the pair, on both sides)
+    assert np.array_equal(sub.out, full.out[rows], equal_nan=True)
+    assert np.array_equal(sub.lse, full.lse[:, rows], equal_nan=True)
+    assert np.array_equal(sub.p, full.p[rows])
+    assert np.isnan(sub.out[~cov]).all() and np.isnan(sub.lse.T[~cov]).all()
+    assert not np.isnan(sub.out[cov]).any()
+    # pairs of the subset: closed-form counts of exactly these rows
+    sm = w.stream_map()
+    want = 0
+    for s in w.segments:
+        kv_len = sm[(0, s.kv_head, s.seq_id)].kv_len
+        for r in rows:
+            t = int(r) - s.q_row_start
+            if 0 <= t < s.q_len:
+                want += w.G * _count(kv_len - s.q_len + t, s.head_class, s.window, s.n_sink)
+    assert sub.pairs == want
+    # a subset that no segment covers at all is legal and evaluates nothing
+    w2 = tiny(20, {0: (GLOBAL, 0, 0, 4), 1: (LOCAL, 3, 0, 2)}, P=P, seed=5)
+    k2, v2, q2 = values(w2)
+    w2.T = [9]                                              # rows 4..8 exist in q / out but belong to nobody
+    q2 = wl.randn_bf16((9, w2.Hq, w2.D), 11)
+    none = run_oracle(w2, 0, k2, v2, q2, row_subset=np.array([8, 5]))
+    assert none.pairs == 0 and np.isnan(none.out).all() and np.isnan(none.lse).all()
+    # the whole row range as a subset is the full run
+    allr = run_oracle(w, 0, k, v, q, row_subset=np.arange(T)[::-1].copy(), want_p=67)
+    assert np.array_equal(allr.out, full.out, equal_nan=True) and np.array_equal(allr.lse, full.lse, equal_nan=True)
+    assert allr.pairs == full.pairs
+
+
 # ------------------------------------------------------------------------------------ rejections
 def test_oracle_rejects_invalid():
     w = tiny(10, {0: (GLOBAL, 0, 0, 11), 1: (LOCAL, 3, 0, 5)})
