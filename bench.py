@@ -211,11 +211,11 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    w = get_workload(args.config)
+    w = get_workload(args.config or HEADLINE)
     from paper_2606_06256_b200 import workloads as wl
     k_pool, v_pool = wl.pool_values(w, "cpu")
     q = wl.q_values(w, 0, "cpu")
-    rows = args.ref_rows
+    rows = args.ref_rows if args.ref_rows > 0 else oracle_rows_for(w, args.ref_pairs)
     vals, times = [], []
     for i in range(args.warmup + args.steps):
         tf, dt, cores, pairs, desc = oracle_sample(w, rows, seed=i, k_pool=k_pool, v_pool=v_pool, q=q)
@@ -277,9 +277,240 @@ def dense_mask_ms(w, k_pool, v_pool, q, layer: int = 0, reps: int = 3):
 # ---------------------------------------------------------------------------------------------
 # our arm
 # ---------------------------------------------------------------------------------------------
-def run_ours(args):
+PER_CONFIG = ["2", "3", "4", "4d", "fig9-decode-128k"]      # measured beside the headline workload in the default run
+HEADLINE = "5"                                              # BASELINE.json configs[4]: the largest single-GPU job
+
+
+def is_decode_shaped(name: str) -> bool:
+    return name == "4d" or name.startswith("fig9-decode")
+
+
+def measure(name: str, steps: int, warmup: int, dev, local_rank: int, world: int, dist, peaks, peaks_src, tiles: int,
+            full: bool, cpu_rows_pairs: float = 0.0, dense_mask: bool = False):
+    """One workload through the C ABI: `steps` steps enqueued back to back inside one CUDA-event bracket.  Returns the
+    measurement record; `full` adds the isolated-step latency, the e2e (host buffers) leg and the oracle timing."""
     import torch
     from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
+
+    w = get_workload(name)
+    k_pool, v_pool = wl.pool_values(w, dev)
+    qs = [wl.q_values(w, l, dev) for l in range(w.num_layers)]
+    outs = [torch.empty_like(q) for q in qs]
+    lses = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32, device=dev) for l in range(w.num_layers)]
+    # the batch's K/V rows, resident in HBM (what the QKV projections would have produced); the
+    # marshalled request array is prepared once (the same batch is stored every step)
+    append_reqs = H.append_requests(w, k_pool, v_pool)
+    batch = B.AppendBatch(append_reqs)
+    cache = H.create_cache(w, local_rank, tiles_per_item=tiles)
+    stream = torch.cuda.current_stream()
+    flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
+    useful = sum(wl.useful_flops(w, l) for l in range(w.num_layers))
+    seg_objs = []
+    seg_batches = [B.SegmentBatch(H.segment_reqs(w, l)) for l in range(w.num_layers)]
+
+    def append_all(b):
+        """a1: drop the previous batch's streams and segment objects, store this batch (one scatter launch)"""
+        for s in seg_objs:
+            B.segpa_free_segments(cache, s)
+        seg_objs.clear()
+        B.segpa_clear_streams(cache)
+        B.segpa_append_pages_batch(cache, b, stream=stream)
+        return 1
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step():
+        """one pass of the hot path, enqueued on `stream` with no host synchronisation; returns the CUDA
+        events around each layer's segpa_attention_fwd and the number of our kernels launched"""
+        fa, fb = [], []
+        n = append_all(batch)
+        for l in range(w.num_layers):
+            segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
+            seg_objs.append(segs)
+            a, b = ev(), ev()
+            a.record(stream)
+            B.segpa_attention_fwd(cache, segs, qs[l], w.scale, outs[l], lses[l], stream=stream)
+            b.record(stream)
+            fa.append(a)
+            fb.append(b)
+            n += B.segpa_last_launch_count(cache)
+        return fa, fb, n
+
+    for _ in range(warmup):
+        step()
+        flush_buf.fill_(1)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    # The K timed steps are enqueued back to back inside ONE CUDA-event bracket (E0 .. E1): the host plans
+    # step k+1 (build_segments) while the device runs step k, as a serving loop does.  L2 is flushed on the
+    # stream before every step; each flush has its own events.  Two figures come out of the bracket:
+    #   ms_per_step_incl_flush = (E1 - E0) / K                        everything the device did, flushes included
+    #   ms_per_step            = max((E1 - E0 - flushes) / K, host enqueue time per step)
+    # `value` uses the second: the flush is the harness's, not the path's, but the host's planning of step k+1
+    # runs under it, so the step is never credited with less than the host needed to enqueue it.
+    E0, E1 = ev(), ev()
+    flushes, fwd_ev = [], []
+    host_s = 0.0
+    launches = 0
+    wall0 = time.perf_counter()
+    E0.record(stream)
+    for _ in range(steps):
+        f0, f1 = ev(), ev()
+        f0.record(stream)
+        flush_buf.fill_(1)                      # L2 flush between timed iterations
+        f1.record(stream)
+        flushes.append((f0, f1))
+        h0 = time.perf_counter()
+        fa, fb, n = step()
+        host_s += time.perf_counter() - h0
+        fwd_ev.append((fa, fb))
+        launches += n
+    E1.record(stream)
+    E1.synchronize()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop()
+    flush_ms = float(sum(f0.elapsed_time(f1) for f0, f1 in flushes))
+    bracket_ms = max_over_ranks(E0.elapsed_time(E1), dist, dev)
+    host_ms = max_over_ranks(1e3 * host_s / steps, dist, dev)
+    dev_ms = max_over_ranks((E0.elapsed_time(E1) - flush_ms) / steps, dist, dev)
+    ms_per_step = max(dev_ms, host_ms)
+    value = world * useful / (ms_per_step * 1e-3) / 1e12
+    fwd_ms = [sum(a.elapsed_time(b) for a, b in zip(fa, fb)) for fa, fb in fwd_ev]
+    fwd_mean = float(np.mean(fwd_ms))
+    layer_ms = [float(np.mean([fa[l].elapsed_time(fb[l]) for fa, fb in fwd_ev])) for l in range(w.num_layers)]
+
+    # ---- plan statistics / algorithmic bytes for the roofline
+    st0 = None
+    alg_bytes = 0
+    for l in range(w.num_layers):
+        sg = H.build_layer(cache, w, l)
+        st = B.segpa_segments_stats(sg)
+        B.segpa_free_segments(cache, sg)
+        st0 = st0 or st
+        cov_rows = sum(s.q_len * w.G for s in w.layer_segments(l))
+        alg_bytes += st["visible_kv_tokens"] * w.D * 2 * 2 + cov_rows * w.D * 2 * 2 + cov_rows * 4
+    torch.cuda.synchronize()
+    # a kernel timed inside a long step (tens of ms back to back: the device sits at its power cap) is held against
+    # the sustained bf16 figure, a short one against the burst figure (B200_PROFILING.md); both fractions are printed
+    long_step = fwd_mean >= 20.0
+    if is_decode_shaped(name):
+        roof = {"bound": "hbm", "achieved": alg_bytes / (fwd_mean * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+        roof["frac"] = roof["achieved"] / roof["peak"]
+        roof["peak_source"] = peaks_src
+    else:
+        ach = useful / (fwd_mean * 1e-3) / 1e12
+        pk = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
+        roof = {"bound": "tensor", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
+                "frac_of_burst": ach / peaks["bf16_tflops"], "frac_of_sustained": ach / peaks["bf16_tflops_sustained"],
+                "peak_source": peaks_src + (", sustained figure (kernel timed inside a %.0f ms step)" % fwd_mean if long_step else ", burst figure")}
+    roof["traffic"] = ncu_traffic(w.name)
+    roof["kernel"] = "attention_tc_kernel (+ combine_kernel where the plan splits KV) = segpa_attention_fwd, mean over %d steps x %d layers, CUDA events on the launching stream" % (steps, w.num_layers)
+    roof["algorithmic_bytes"] = alg_bytes
+    roof["useful_flops"] = useful
+
+    rec = {"workload": w.name, "steps": steps, "warmup": warmup, "ms_per_step": ms_per_step,
+           "ms_per_step_incl_flush": bracket_ms / steps, "value": value, "fwd_ms": fwd_mean,
+           "us_per_layer": 1e3 * fwd_mean / w.num_layers, "useful_tflops": useful / (fwd_mean * 1e-3) / 1e12,
+           "roofline": roof, "clocks": clocks, "gpu_launches": int(launches), "wall_s_timed_region": wall,
+           "plan": {k: st0[k] for k in ("n_tiles", "n_items", "n_split_tiles", "kv_blocks", "workspace_bytes")},
+           "shape": {"Hq": w.Hq, "Hkv": w.Hkv, "D": w.D, "page_size": w.P, "layers": w.num_layers, "q_rows": int(sum(w.T)),
+                     "segments": len(w.segments)},
+           "timing": {"flush_ms_total": flush_ms, "device_ms_per_step_excl_flush": dev_ms, "host_enqueue_ms_per_step": host_ms,
+                      "value_uses": "max(device time excluding the L2 flushes, host enqueue time) per step"}}
+    if w.num_layers > 1:
+        rec["layer_ms"] = {"min": min(layer_ms), "max": max(layer_ms), "mean": float(np.mean(layer_ms))}
+
+    if full:
+        # ---- the same step run alone: flush, device idle, then one step with the host waiting for its end
+        # (planning and kernels in series: the latency of a single isolated step, not the throughput)
+        iso_ms = []
+        for _ in range(max(2, min(steps, 5))):
+            flush_buf.fill_(1)
+            torch.cuda.synchronize()
+            e0, e1 = ev(), ev()
+            e0.record(stream)
+            step()
+            e1.record(stream)
+            e1.synchronize()
+            iso_ms.append(e0.elapsed_time(e1))
+        torch.cuda.synchronize()
+        rec["timing"]["isolated_step_ms"] = float(np.mean(iso_ms))
+
+        # ---- e2e, everything through the C ABI with HOST buffers (pinned): the step's K/V rows go up inside
+        # segpa_append_pages_batch (src_is_host), Q / out / LSE through segpa_attention_fwd_host (row-chunked:
+        # H2D, kernels and D2H overlap)
+        h_reqs, keep = [], []
+        for (layer, kvh, seq, kr, vr, n, ids) in append_reqs:
+            if kr is None:
+                h_reqs.append((layer, kvh, seq, None, None, n, ids))
+            else:
+                a, b = kr.cpu().pin_memory(), vr.cpu().pin_memory()
+                keep.append((a, b))
+                h_reqs.append((layer, kvh, seq, a, b, n, ids))
+        h_batch = B.AppendBatch(h_reqs)
+        h_q = [q.cpu().pin_memory() for q in qs]
+        h_out = [torch.empty_like(q).pin_memory() for q in h_q]
+        h_lse = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32).pin_memory() for l in range(w.num_layers)]
+        h2d = sum(a.numel() * 2 * 2 for a, _ in keep) + sum(q.numel() * 2 for q in h_q)
+        d2h = sum(o.numel() * 2 for o in h_out) + sum(x.numel() * 4 for x in h_lse)
+
+        def e2e_step():
+            append_all(h_batch)
+            for l in range(w.num_layers):
+                segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
+                seg_objs.append(segs)
+                B.segpa_attention_fwd_host(cache, segs, h_q[l], w.scale, h_out[l], h_lse[l], stream=stream)
+            torch.cuda.synchronize()
+
+        e2e_step()
+        n_e2e = max(2, min(steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            e2e_step()
+        e2e_s = max_over_ranks((time.perf_counter() - t0) / n_e2e, dist, dev)
+        pcie = max(h2d, d2h) / (e2e_s) / 1e9
+        rec["e2e"] = {"value": world * useful / e2e_s / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                      "ms_per_step": 1e3 * e2e_s, "steps": n_e2e,
+                      "how": "segpa_append_pages_batch(src_is_host) + segpa_build_segments + segpa_attention_fwd_host per layer, pinned host buffers, wall clock around whole steps",
+                      "larger_direction_gbs": pcie}
+        del h_q, h_out, h_lse, keep, h_batch
+
+    if dense_mask:
+        try:
+            dm, ncalls = dense_mask_ms(w, k_pool, v_pool, qs[0])
+            rec["dense_mask_context"] = {"ms_per_layer": dm, "x_slower_than_segpa_fwd": dm / (fwd_mean / w.num_layers),
+                                         "how": "torch SDPA, boolean attn_mask, dense gathered K/V, %d calls (one per request x head class), layer 0" % ncalls,
+                                         "note": "context for the paper's 4.9-7.6x mask penalty (PAPER.md:19; its shapes are unknown), not a like-for-like number"}
+        except Exception as ex:  # library path, context only
+            rec["dense_mask_context"] = {"error": repr(ex)[:200]}
+    if cpu_rows_pairs > 0:
+        rows = oracle_rows_for(w, cpu_rows_pairs)
+        tf, dt, cores, pairs, desc = oracle_sample(w, rows, seed=0, k_pool=k_pool.cpu(), v_pool=v_pool.cpu(), q=qs[0].cpu())
+        rec["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc + "; %.1f s" % dt}
+    for s in seg_objs:
+        B.segpa_free_segments(cache, s)
+    B.segpa_destroy(cache)
+    del k_pool, v_pool, qs, outs, lses, batch, append_reqs, flush_buf
+    torch.cuda.empty_cache()
+    return rec
+
+
+def oracle_rows_for(w, pairs_budget: float) -> int:
+    """Rows of layer 0 whose oracle evaluation costs about `pairs_budget` attended (query, key, q-head) pairs."""
+    from paper_2606_06256_b200 import workloads as wl
+    per_row = wl.useful_flops(w, 0) / (4.0 * w.D) / max(1, w.T[0])
+    return int(min(w.T[0], max(16, pairs_budget / max(per_row, 1.0))))
+
+
+def run_ours(args):
+    import torch
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -293,204 +524,40 @@ def run_ours(args):
         import torch.distributed as dist_
         dist = dist_
         dist.init_process_group("nccl", device_id=dev)
-
-    os.environ.setdefault("SEGPA_KERNEL", "tc")
-    os.environ.setdefault("SEGPA_TC_TILES", str(args.tiles))
-    w = get_workload(args.config)
     peaks, peaks_src = load_peaks()
-    k_pool, v_pool = wl.pool_values(w, dev)
-    qs = [wl.q_values(w, l, dev) for l in range(w.num_layers)]
-    outs = [torch.empty_like(q) for q in qs]
-    lses = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32, device=dev) for l in range(w.num_layers)]
-    # the batch's K/V rows, resident in HBM (what the QKV projections would have produced); the
-    # marshalled request array is prepared once (the same batch is stored every step)
-    append_reqs = H.append_requests(w, k_pool, v_pool)
-    batch = B.AppendBatch(append_reqs)
-    rows = [(r[3], r[4]) for r in append_reqs if r[3] is not None]
-    cache = H.create_cache(w, local_rank)
-    stream = torch.cuda.current_stream()
-    flush_buf = torch.empty(256 * 2 ** 20, dtype=torch.uint8, device=dev)
-    useful = sum(wl.useful_flops(w, l) for l in range(w.num_layers))
-    seg_objs = []
-    launches = [0]
-    seg_batches = [B.SegmentBatch(H.segment_reqs(w, l)) for l in range(w.num_layers)]
-
-    def append_all():
-        """a1: drop the previous batch's streams and segment objects, store this batch (one scatter launch)"""
-        for s in seg_objs:
-            B.segpa_free_segments(cache, s)
-        seg_objs.clear()
-        B.segpa_clear_streams(cache)
-        B.segpa_append_pages_batch(cache, batch, stream=stream)
-        return 1
-
-    ev = lambda: torch.cuda.Event(enable_timing=True)
-
-    def step():
-        """one pass of the hot path, enqueued on `stream` with no host synchronisation; returns the CUDA
-        events around each layer's segpa_attention_fwd and the number of our kernels launched"""
-        fa, fb = [], []
-        n = append_all()
-        for l in range(w.num_layers):
-            segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
-            seg_objs.append(segs)
-            a, b = ev(), ev()
-            a.record(stream)
-            B.segpa_attention_fwd(cache, segs, qs[l], w.scale, outs[l], lses[l], stream=stream)
-            b.record(stream)
-            fa.append(a)
-            fb.append(b)
-            n += B.segpa_last_launch_count(cache)
-        return fa, fb, n
-
-    def free_segs():
-        torch.cuda.synchronize()
-
-    for _ in range(args.warmup):
-        step()
-        flush_buf.fill_(1)
-    free_segs()
-    if dist is not None:
-        dist.barrier()
-    torch.cuda.synchronize()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    # The K timed steps are enqueued back to back inside ONE CUDA-event bracket (E0 .. E1): the host plans
-    # step k+1 (build_segments) while the device runs step k, as a serving loop does.  L2 is flushed on the
-    # stream before every step; each flush has its own events and its time is taken out of the bracket, so
-    # ms_per_step = (E1 - E0 - sum of flushes) / K still contains every gap in which the device waited for
-    # the host.
-    E0, E1 = ev(), ev()
-    flushes, fwd_ev = [], []
-    host_s = 0.0
-    wall0 = time.perf_counter()
-    E0.record(stream)
-    for _ in range(args.steps):
-        f0, f1 = ev(), ev()
-        f0.record(stream)
-        flush_buf.fill_(1)                      # L2 flush between timed iterations (its time is subtracted)
-        f1.record(stream)
-        flushes.append((f0, f1))
-        h0 = time.perf_counter()
-        fa, fb, n = step()
-        host_s += time.perf_counter() - h0
-        fwd_ev.append((fa, fb))
-        launches[0] += n
-    E1.record(stream)
-    E1.synchronize()
-    torch.cuda.synchronize()
-    if dist is not None:
-        dist.barrier()
-    wall = time.perf_counter() - wall0
-    clocks = sampler.stop()
-    free_segs()
-    flush_ms = float(sum(f0.elapsed_time(f1) for f0, f1 in flushes))
-    total_ms = E0.elapsed_time(E1) - flush_ms
-    fwd_ms = [sum(a.elapsed_time(b) for a, b in zip(fa, fb)) for fa, fb in fwd_ev]
-    total_ms = max_over_ranks(total_ms, dist, dev)
-    ms_per_step = total_ms / args.steps
-    value = world * useful / (ms_per_step * 1e-3) / 1e12
-    fwd_mean = float(np.mean(fwd_ms))
-
-    # ---- the same step run alone: flush, device idle, then one step with the host waiting for its end
-    # (planning and kernels in series: the latency of a single isolated step, not the throughput)
-    iso_ms = []
-    for _ in range(max(2, min(args.steps, 5))):
-        flush_buf.fill_(1)
-        torch.cuda.synchronize()
-        e0, e1 = ev(), ev()
-        e0.record(stream)
-        step()
-        e1.record(stream)
-        e1.synchronize()
-        iso_ms.append(e0.elapsed_time(e1))
-    free_segs()
-    iso_ms = float(np.mean(iso_ms))
-
-    # ---- e2e through the host-buffer entry point: H2D of the step's K/V rows and Q, D2H of out + LSE
-    h_rows = [(a.cpu().pin_memory(), b.cpu().pin_memory()) for a, b in rows]
-    h_q = [q.cpu().pin_memory() for q in qs]
-    h_out = [torch.empty_like(q).pin_memory() for q in h_q]
-    h_lse = [torch.empty((w.Hq, w.T[l]), dtype=torch.float32).pin_memory() for l in range(w.num_layers)]
-    h2d = sum(a.numel() * 2 * 2 for a, _ in h_rows) + sum(q.numel() * 2 for q in h_q)
-    d2h = sum(o.numel() * 2 for o in h_out) + sum(x.numel() * 4 for x in h_lse)
-
-    def e2e_step():
-        for (dk, dv), (a, b) in zip(rows, h_rows):
-            dk.copy_(a, non_blocking=True)
-            dv.copy_(b, non_blocking=True)
-        append_all()
-        for l in range(w.num_layers):
-            segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
-            seg_objs.append(segs)
-            B.segpa_attention_fwd_host(cache, segs, h_q[l], w.scale, h_out[l], h_lse[l], stream=stream)
-        torch.cuda.synchronize()
-
-    e2e_step()
-    free_segs()
-    n_e2e = max(2, min(args.steps, 5))
-    t0 = time.perf_counter()
-    for _ in range(n_e2e):
-        e2e_step()
-    e2e_s = (time.perf_counter() - t0) / n_e2e
-    free_segs()
-    e2e_s = max_over_ranks(e2e_s, dist, dev)
-    e2e_val = world * useful / e2e_s / 1e12
-
-    # ---- plan statistics / algorithmic bytes for the roofline
-    st0 = None
-    alg_bytes = 0
-    for l in range(w.num_layers):
-        sg = H.build_layer(cache, w, l)
-        st = B.segpa_segments_stats(sg)
-        B.segpa_free_segments(cache, sg)
-        st0 = st0 or st
-        cov_rows = sum(s.q_len * w.G for s in w.layer_segments(l))
-        alg_bytes += st["visible_kv_tokens"] * w.D * 2 * 2 + cov_rows * w.D * 2 * 2 + cov_rows * 4
-    torch.cuda.synchronize()
-    decode_shaped = args.config == "4d" or args.config.startswith("fig9-decode")
-    if decode_shaped:
-        roof = {"bound": "hbm", "achieved": alg_bytes / (fwd_mean * 1e-3) / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s"}
-    else:
-        roof = {"bound": "tensor", "achieved": useful / (fwd_mean * 1e-3) / 1e12, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = ncu_traffic(w.name)
-    roof["kernel"] = "attention_tc_kernel (segpa_attention_fwd), avg of %d launches-groups timed with CUDA events" % args.steps
-    roof["peak_source"] = peaks_src + (", burst figure" if not decode_shaped else "")
-    roof["algorithmic_bytes"] = alg_bytes
-    roof["useful_flops"] = useful
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-            "data": "synthetic",
-            "config": {"workload": w.name, "Hq": w.Hq, "Hkv": w.Hkv, "D": w.D, "page_size": w.P, "layers": w.num_layers,
-                       "q_rows": int(sum(w.T)), "segments": len(w.segments), "l2_flush_between_steps": True,
-                       "step": "append_pages_batch + (build_segments + attention_fwd) per layer", "tiles_per_item": int(os.environ["SEGPA_TC_TILES"]),
-                       "replicas": world},
-            "fwd_ms_per_step": fwd_mean, "us_per_layer": 1e3 * fwd_mean / w.num_layers,
-            "pct_of_bf16_peak": 100.0 * (useful / (fwd_mean * 1e-3) / 1e12) / peaks["bf16_tflops"],
-            "plan": {k: st0[k] for k in ("n_tiles", "n_items", "n_split_tiles", "kv_blocks", "workspace_bytes")},
-            "roofline": roof, "clocks": clocks,
-            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "ms_per_step": 1e3 * e2e_s},
-            "gpu_launches": int(launches[0]), "wall_s_timed_region": wall,
-            "timing": {"how": "one CUDA-event bracket over the K steps enqueued back to back (host plans step k+1 under the kernels of step k); "
-                              "the on-stream L2 flushes before each step are timed with their own events and subtracted",
-                       "flush_ms_total": flush_ms, "host_enqueue_ms_per_step": 1e3 * host_s / args.steps,
-                       "isolated_step_ms": iso_ms}}
-
-    if rank == 0 and world == 1 and (args.dense_mask == "on" or (args.dense_mask == "auto" and args.config == "2")):
-        try:
-            dm, ncalls = dense_mask_ms(w, k_pool, v_pool, qs[0])
-            line["dense_mask_context"] = {"ms_per_layer": dm, "x_slower_than_segpa_fwd": dm / (fwd_mean / w.num_layers),
-                                          "how": "torch SDPA, boolean attn_mask, dense gathered K/V, %d calls (one per request x head class), layer 0" % ncalls,
-                                          "note": "context for the paper's 4.9-7.6x mask penalty (PAPER.md:19; its shapes are unknown), not a like-for-like number"}
-        except Exception as ex:  # library path, context only
-            line["dense_mask_context"] = {"error": repr(ex)[:200]}
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        tf, dt, cores, pairs, desc = oracle_sample(w, args.cpu_rows, seed=0, k_pool=k_pool.cpu(), v_pool=v_pool.cpu(), q=qs[0].cpu())
-        line["cpu_baseline"] = {"value": tf, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc + "; %.1f s" % dt}
-    B.segpa_destroy(cache)
+    name = args.config or HEADLINE
+    head = measure(name, args.steps, args.warmup, dev, local_rank, world, dist, peaks, peaks_src, args.tiles, full=True,
+                   cpu_rows_pairs=(0.0 if (args.no_cpu_baseline or rank != 0 or world != 1) else args.cpu_pairs),
+                   dense_mask=(rank == 0 and world == 1 and args.dense_mask == "on"))
+    line = {"metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": head["ms_per_step"], "ms_per_step_incl_flush": head["ms_per_step_incl_flush"],
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": dict(head["shape"], workload=head["workload"], l2_flush_between_steps=True,
+                           step="append_pages_batch + (build_segments + attention_fwd) per layer", tiles_per_item=args.tiles,
+                           replicas=world),
+            "fwd_ms_per_step": head["fwd_ms"], "us_per_layer": head["us_per_layer"],
+            "pct_of_bf16_peak": 100.0 * head["useful_tflops"] / peaks["bf16_tflops"],
+            "plan": head["plan"], "roofline": head["roofline"], "clocks": head["clocks"], "e2e": head["e2e"],
+            "gpu_launches": head["gpu_launches"], "wall_s_timed_region": head["wall_s_timed_region"],
+            "timing": dict(head["timing"], how="one CUDA-event bracket over the K steps enqueued back to back (host plans step k+1 under the "
+                                              "kernels of step k); the on-stream L2 flushes before each step are timed with their own events")}
+    for k in ("layer_ms", "dense_mask_context", "cpu_baseline"):
+        if k in head:
+            line[k] = head[k]
+    # the other workloads, each with its own clocks record (default run only: one GPU, no --config)
+    if args.config is None and world == 1 and not args.no_per_config:
+        per = [{k: head[k] for k in ("workload", "steps", "warmup", "ms_per_step", "ms_per_step_incl_flush", "value", "fwd_ms", "us_per_layer",
+                                     "useful_tflops", "roofline", "clocks", "gpu_launches")}]
+        for c in PER_CONFIG:
+            r = measure(c, min(args.steps, 20), 3, dev, local_rank, world, None, peaks, peaks_src, args.tiles, full=False,
+                        dense_mask=(c == "2" and args.dense_mask != "off"))
+            ent = {k: r[k] for k in ("workload", "steps", "warmup", "ms_per_step", "ms_per_step_incl_flush", "value", "fwd_ms", "us_per_layer",
+                                     "useful_tflops", "roofline", "clocks", "gpu_launches", "timing")}
+            if "dense_mask_context" in r:
+                ent["dense_mask_context"] = r["dense_mask_context"]
+            per.append(ent)
+            line["gpu_launches"] += r["gpu_launches"]
+        line["per_config"] = per
     if rank == 0:
         print(json.dumps(line))
     if dist is not None:
@@ -611,16 +678,20 @@ def run_mass(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="2")
+    ap.add_argument("--config", default=None,
+                    help="workload: 1..5, 4d, fig9-{decode,prefill}-{8,32,128}k, rope, mass.  Default: BASELINE.json configs[4] "
+                         "(cfg5, the whole 28-layer stack) as the headline, plus a per_config list over cfg2, cfg3, cfg4, 4d and fig9-decode-128k")
     ap.add_argument("--tiles", type=int, default=2)
-    ap.add_argument("--cpu-rows", type=int, default=20000, help="rows in the cpu_baseline oracle sample")
-    ap.add_argument("--ref-rows", type=int, default=2048, help="rows per step of the --impl reference oracle sample")
+    ap.add_argument("--cpu-pairs", type=float, default=1.2e9, help="attended pairs in the cpu_baseline oracle sample (about 15 s of CPU)")
+    ap.add_argument("--ref-rows", type=int, default=0, help="rows per step of the --impl reference oracle sample (0: from --ref-pairs)")
+    ap.add_argument("--ref-pairs", type=float, default=8e7, help="attended pairs per step of the --impl reference oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="default run: skip the per_config list")
     ap.add_argument("--dense-mask", default="auto", choices=["auto", "on", "off"],
-                    help="also time dense attention with an explicit mask (context; auto = only for --config 2)")
+                    help="also time dense attention with an explicit mask (context; auto = for cfg2 in the per_config list)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3

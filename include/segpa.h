@@ -130,13 +130,16 @@ typedef struct {
     int32_t layer;
     int32_t kv_head;
     int64_t seq_id;
-    const void *k_src;            /* device bf16 rows, or NULL (with v_src NULL) = ATTACH */
+    const void *k_src;            /* bf16 rows (device, or host if src_is_host), or NULL (with v_src NULL) = ATTACH */
     const void *v_src;
     int64_t src_row_stride_elems;
     int64_t n_tokens;
     const int32_t *page_ids;      /* host; NULL = allocator chooses (COPY mode only) */
     int32_t n_page_ids;
-    int32_t reserved;             /* 0 */
+    int32_t src_is_host;          /* 0: k_src / v_src are device pointers.  1: HOST pointers (pinned memory for the
+                                     copies to be asynchronous; any 2-byte alignment and row stride >= D): the rows
+                                     are copied to a staging buffer owned by the cache on cuda_stream, ahead of the
+                                     scatter launch; the host buffers must stay valid until that work completes. */
 } segpa_append_req_t;
 
 segpa_status_t segpa_append_pages_batch(segpa_cache_t *cache, const segpa_append_req_t *reqs, int32_t n,
@@ -331,10 +334,14 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t *cache, const segpa_segments_t 
                                    int64_t lse_stride, int64_t T, void *cuda_stream);
 
 /*
- * Same computation with HOST buffers: q is copied to the device, attention runs, out and lse are
- * copied back, and the call returns after the copies complete (synchronous).  q/out are dense
- * [T][Hq][D] bf16, lse [Hq][T] fp32 (may be NULL).  Staging buffers are owned by the cache and
- * reused.  This is the end-to-end path bench.py times.
+ * Same computation with HOST buffers (pinned memory for the copies to be asynchronous): q/out are dense
+ * [T][Hq][D] bf16, lse [Hq][T] fp32 (may be NULL).  The plan is cut into chunks of consecutive query rows (about
+ * 16 MB of q each); the host->device copy of chunk k+1, the kernels of chunk k (on cuda_stream) and the device->host
+ * copy of chunk k-1 run concurrently on three streams, so the call is bounded by the larger PCIe direction, not by
+ * the sum.  Results are bit-identical to segpa_attention_fwd on the same plan.  Differences from the device entry
+ * point: the call returns after the last copy back has completed (synchronous), and (row, head) pairs that no segment
+ * covers are written as zeros (out and lse) rather than left untouched.  Staging buffers are owned by the cache and
+ * reused.  This is the end-to-end path bench.py times.  Errors: as segpa_attention_fwd, plus OOM (staging).
  */
 segpa_status_t segpa_attention_fwd_host(segpa_cache_t *cache, const segpa_segments_t *segs,
                                         const void *q_host, float softmax_scale, void *out_host,

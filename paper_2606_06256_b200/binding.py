@@ -53,7 +53,7 @@ class SegmentReq(C.Structure):
 class AppendReq(C.Structure):
     _fields_ = [("layer", C.c_int32), ("kv_head", C.c_int32), ("seq_id", C.c_int64), ("k_src", C.c_void_p),
                 ("v_src", C.c_void_p), ("src_row_stride_elems", C.c_int64), ("n_tokens", C.c_int64),
-                ("page_ids", C.c_void_p), ("n_page_ids", C.c_int32), ("reserved", C.c_int32)]
+                ("page_ids", C.c_void_p), ("n_page_ids", C.c_int32), ("src_is_host", C.c_int32)]
 
 
 class RopeReq(C.Structure):
@@ -198,24 +198,27 @@ class AppendBatch:
 
     def __init__(self, reqs: Sequence[tuple]):
         """reqs: tuples (layer, kv_head, seq_id, k_src, v_src, n_tokens, page_ids) with k_src / v_src torch
-        bf16 device tensors [n_tokens][D] or None (attach), page_ids an int sequence or None."""
+        bf16 tensors [n_tokens][D] -- on the device, or on the host (src_is_host) -- or None (attach), page_ids an
+        int sequence or None."""
         self.n = len(reqs)
         self.arr = (AppendReq * max(1, self.n))()
         self._keep = []
         for i, (layer, kvh, seq, k_src, v_src, n_tokens, page_ids) in enumerate(reqs):
             kp = vp = None
             stride = 0
+            on_host = 0
             if k_src is not None:
-                assert k_src.is_cuda and v_src.is_cuda and k_src.stride(-1) == 1 and v_src.stride(-1) == 1
+                assert k_src.is_cuda == v_src.is_cuda and k_src.stride(-1) == 1 and v_src.stride(-1) == 1
                 assert k_src.stride(0) == v_src.stride(0)
                 kp, vp, stride = k_src.data_ptr(), v_src.data_ptr(), k_src.stride(0)
+                on_host = 0 if k_src.is_cuda else 1       # CPU tensors (pinned for speed) go through src_is_host
                 self._keep.append((k_src, v_src))
             ip, n_ids = None, 0
             if page_ids is not None:
                 ids = np.ascontiguousarray(page_ids, dtype=np.int32)
                 self._keep.append(ids)
                 ip, n_ids = ids.ctypes.data, len(ids)
-            self.arr[i] = AppendReq(int(layer), int(kvh), int(seq), kp, vp, int(stride), int(n_tokens), ip, n_ids, 0)
+            self.arr[i] = AppendReq(int(layer), int(kvh), int(seq), kp, vp, int(stride), int(n_tokens), ip, n_ids, on_host)
 
 
 def segpa_append_pages_batch(cache: int, batch, stream=None) -> None:

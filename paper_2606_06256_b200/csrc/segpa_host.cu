@@ -141,6 +141,7 @@ void staging_free(Staging& s) {
 struct SegBuf {
     Staging blob;
     Staging mass_blob;    // attention-mass plan (items, per-CTA slices, layout), uploaded at the first mass call
+    Staging host_blob;    // row-chunked plan of segpa_attention_fwd_host (items, per-CTA slices, combine entries per chunk)
     int* counter = nullptr;
     float* ws_o = nullptr;
     float* ws_ml = nullptr;
@@ -151,6 +152,7 @@ void segbuf_free(SegBuf* b) {
     if (!b) return;
     staging_free(b->blob);
     staging_free(b->mass_blob);
+    staging_free(b->host_blob);
     if (b->counter) cudaFree(b->counter);
     if (b->ws_o) cudaFree(b->ws_o);
     if (b->ws_ml) cudaFree(b->ws_ml);
@@ -174,6 +176,16 @@ struct segpa_segments {
     mutable bool mass_planned = false;   // mass plan built and uploaded (lazily, by the first segpa_attention_mass)
     mutable int mass_n_cta = 0;
     mutable size_t m_off_items = 0, m_off_cta = 0, m_off_layout = 0, m_off_kvlen = 0;
+    // segpa_attention_fwd_host: the plan cut into row chunks, each with its own launch, so that the H2D copy of
+    // chunk k+1, the kernels of chunk k and the D2H copy of chunk k-1 overlap (built at the first call)
+    struct HostChunk {
+        int64_t row_lo, row_hi;      // rows copied in / out with this chunk
+        int64_t need_hi;             // its items read Q rows below this (<= row_hi of the next chunk)
+        size_t off_items, off_cta, off_combs;
+        int n_items, n_cta, n_combs, comb_max_rows;
+    };
+    mutable std::vector<HostChunk> hchunks;
+    mutable bool host_planned = false;
     segpa_plan_stats_t stats{};
     int tiles_per_item = 1;
     // device
@@ -187,6 +199,7 @@ struct segpa_segments {
         cache = nullptr; layer = 0;
         reqs.clear(); segs.clear(); items.clear(); item_meta.clear(); pages.clear(); combs.clear(); cta_off.clear(); mass_off.clear();
         mass_planned = false; mass_n_cta = 0;
+        hchunks.clear(); host_planned = false;
         m_off_items = m_off_cta = m_off_layout = m_off_kvlen = 0;
         stats = segpa_plan_stats_t{};
         tiles_per_item = 1;
@@ -234,11 +247,17 @@ struct segpa_cache {
     int kernel_kind = 1;  // 1 = tcgen05 (the product); 0 = SIMT cross-check kernel, only in the test build (-DSEGPA_BRINGUP)
     int tiles_per_item = 2;   // 128-row tiles per work item (desc.tiles_per_item; fixed at create)
     int last_launches = 0;
-    // host-buffer entry point staging
+    // host-buffer entry points: device staging, copy streams and events
     uint16_t* st_q = nullptr;
     uint16_t* st_out = nullptr;
     float* st_lse = nullptr;
     size_t st_q_bytes = 0, st_lse_bytes = 0;
+    uint16_t* st_kv = nullptr;          // K / V rows of host-source append requests (src_is_host)
+    size_t st_kv_bytes = 0;
+    cudaEvent_t st_kv_ev = nullptr;     // the scatter that last read st_kv has completed
+    bool st_kv_pending = false;
+    cudaStream_t h2d_stream = nullptr, d2h_stream = nullptr;
+    std::vector<cudaEvent_t> host_events;
 };
 
 namespace {
@@ -269,6 +288,7 @@ void free_segments_obj(segpa_cache* c, segpa_segments* s) {
     if (s->buf) {
         staging_release(s->buf->blob, s->last_stream);
         if (s->mass_planned) staging_release(s->buf->mass_blob, s->last_stream);
+        if (s->host_planned) staging_release(s->buf->host_blob, s->last_stream);
         c->free_bufs.push_back(s->buf);
     }
     if (c->free_seg_objs.size() < 64) {
@@ -319,6 +339,111 @@ inline int64_t visible_pairs(int64_t i0, int64_t i1, int64_t W) {
     const int64_t ramp = tri(i0 + 1, std::min(i1, knee) + 1);
     const int64_t flat = i1 > knee ? (i1 - std::max(i0, knee + 1) + 1) * W : 0;
     return ramp + flat;
+}
+
+}  // namespace
+
+namespace {
+
+// LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid;
+// a CTA's items stay in descending order.  Cost = visited blocks + a fixed per-item term (pipeline refill, Q load,
+// epilogue: about 0.6 block-times measured), in thirds of a block.  Reorders `items` (and `meta`, if given) CTA by
+// CTA and fills cta_off ([n_cta + 1]).  Flat arrays only: a plan is built on the critical path of every layer.
+// Returns the sum of the items' costs.
+int64_t lpt_assign(PlanScratch& ps, std::vector<ItemDev>& items_v, std::vector<segpa_segments::ItemMeta>* meta, int num_sms,
+                   std::vector<int32_t>& cta_off) {
+    const int n_items_all = (int)items_v.size();
+    const int n_cta = std::min(n_items_all, num_sms);
+    // descending cost, ties by ascending index: a counting sort (costs are block counts, small integers)
+    std::vector<int>& order = ps.order;
+    order.resize((size_t)n_items_all);
+    {
+        int max_cost = 0;
+        for (const ItemDev& it : items_v) max_cost = std::max(max_cost, it.cost);
+        std::vector<int>& start = ps.start;
+        start.assign((size_t)max_cost + 2, 0);
+        for (const ItemDev& it : items_v) ++start[(size_t)(max_cost - it.cost) + 1];
+        for (int k2 = 0; k2 <= max_cost; ++k2) start[(size_t)k2 + 1] += start[(size_t)k2];
+        for (int i = 0; i < n_items_all; ++i) order[(size_t)start[(size_t)(max_cost - items_v[(size_t)i].cost)]++] = i;
+    }
+    // Each item, in that order, goes to the least-loaded CTA.  The loads are kept as one ascending run of
+    // keys load * 1024 + cta (distinct, so the minimum is unique) inside a longer array: the minimum leaves at
+    // the head, the CTA's new key is inserted from the tail.  With costs descending the new key belongs at or
+    // near the tail, so an assignment costs a few moves (a binary heap's dependent loads per level cost more)
+    std::vector<int64_t>& run = ps.heap;
+    run.resize((size_t)n_cta + (size_t)n_items_all);
+    for (int q = 0; q < n_cta; ++q) run[(size_t)q] = q;
+    std::vector<int>&item_cta = ps.item_cta, &count = ps.count, &cursor = ps.cursor;
+    item_cta.resize((size_t)n_items_all);
+    count.assign((size_t)n_cta, 0);
+    {
+        int64_t* a = run.data();
+        const ItemDev* items = items_v.data();
+        const int64_t fixed3 = 2;   // the fixed per-item term, in thirds of a block (a sweep over 0..6 moved cfg2 / cfg4 by < 0.5 %)
+        size_t head = 0, tail = (size_t)n_cta;
+        for (int idx : order) {
+            const int64_t top = a[head++];
+            const int q = (int)(top & 1023);
+            item_cta[(size_t)idx] = q;
+            ++count[(size_t)q];
+            const int64_t blocks3 = 3 * (int64_t)items[idx].cost;
+            const int64_t key = top + (((items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + fixed3) * 1024;   // strided: two chains
+            size_t pos = tail++;
+            while (pos > head && a[pos - 1] > key) {
+                a[pos] = a[pos - 1];
+                --pos;
+            }
+            a[pos] = key;
+        }
+    }
+    // per-CTA slices: CTA by CTA, each CTA's items in the order they were assigned (descending cost)
+    cta_off.assign((size_t)n_cta + 1, 0);
+    for (int q = 0; q < n_cta; ++q) cta_off[(size_t)q + 1] = cta_off[(size_t)q] + count[(size_t)q];
+    std::vector<ItemDev>& it2 = ps.it2;
+    std::vector<segpa_segments::ItemMeta>& im2 = ps.im2;
+    it2.resize((size_t)n_items_all);
+    if (meta) im2.resize((size_t)n_items_all);
+    cursor.assign(cta_off.begin(), cta_off.end() - 1);
+    int64_t kv_blocks = 0;
+    for (int idx : order) {
+        const int at = cursor[(size_t)item_cta[(size_t)idx]]++;
+        it2[(size_t)at] = items_v[(size_t)idx];
+        if (meta) im2[(size_t)at] = (*meta)[(size_t)idx];
+        kv_blocks += items_v[(size_t)idx].cost;
+    }
+    items_v.swap(it2);
+    if (meta) meta->swap(im2);
+    return kv_blocks;
+}
+
+// fills FwdParams from a cache + segments object (everything but q / out / lse, their strides, the Q tensor map and
+// the per-launch item arrays)
+void fill_fwd_params(FwdParams& p, const segpa_cache* c, const segpa_segments* s) {
+    const uint8_t* d_blob = (const uint8_t*)s->buf->blob.d;
+    p.segs = (const SegDev*)(d_blob + s->off_segs);
+    p.items = (const ItemDev*)(d_blob + s->off_items);
+    p.pages = (const int*)(d_blob + s->off_pages);
+    p.combs = (const CombDev*)(d_blob + s->off_combs);
+    p.cta_off = (const int*)(d_blob + s->off_cta);
+    p.n_cta = (int)s->cta_off.size() - 1;
+    p.n_items = (int)s->items.size();
+    p.n_combs = (int)s->combs.size();
+    p.comb_max_rows = 0;
+    for (const CombDev& cd : s->combs) p.comb_max_rows = std::max(p.comb_max_rows, cd.n_tok * c->G);
+    p.counter = s->buf->counter;
+    p.k_pool = c->k_pool;
+    p.v_pool = c->v_pool;
+    p.ws_o = s->buf->ws_o;
+    p.ws_ml = s->buf->ws_ml;
+    p.Hq = c->desc.num_q_heads;
+    p.Hkv = c->desc.num_kv_heads;
+    p.G = c->G;
+    p.D = c->desc.head_dim;
+    p.P = c->desc.page_size;
+    p.tile_tokens = kTileRows / c->G;
+    p.tiles_per_item = s->tiles_per_item;
+    p.page_bytes = c->page_bytes;
+    p.num_sms = c->num_sms;
 }
 
 }  // namespace
@@ -429,6 +554,11 @@ segpa_status_t segpa_destroy(segpa_cache_t* c) {
     if (c->st_q) cudaFree(c->st_q);
     if (c->st_out) cudaFree(c->st_out);
     if (c->st_lse) cudaFree(c->st_lse);
+    if (c->st_kv) cudaFree(c->st_kv);
+    if (c->st_kv_ev) cudaEventDestroy(c->st_kv_ev);
+    if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+    if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
+    for (cudaEvent_t ev : c->host_events) cudaEventDestroy(ev);
     if (c->own_pool && c->k_pool) { cudaFree(c->k_pool); cudaFree(c->v_pool); }
     delete c;
     return SEGPA_OK;
@@ -447,6 +577,28 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
     std::vector<int32_t>& touched = c->append_touched;     // page ids the scatter kernel indexes, job after job
     touched.clear();
     const uint64_t stamp = ++c->batch_stamp;
+    // host-source requests (src_is_host): their rows are staged in st_kv ([K rows of all such requests][V rows]) by
+    // async copies on cuda_stream ahead of the scatter launch
+    struct HostCopy { const void* k; const void* v; int64_t stride, n, off_rows; };
+    std::vector<HostCopy> host_copies;
+    int64_t host_rows = 0, host_rows_total = 0;
+    for (int32_t i = 0; i < n; ++i)
+        if (reqs[i].src_is_host == 1 && reqs[i].k_src && reqs[i].n_tokens > 0) host_rows_total += reqs[i].n_tokens;
+    if (host_rows_total > 0 && !c->planning_only) {
+        DeviceGuard g(c->desc.device);
+        const size_t need_bytes = (size_t)host_rows_total * D * 2 * 2;
+        if (need_bytes > c->st_kv_bytes) {
+            if (c->st_kv_pending) { cudaEventSynchronize(c->st_kv_ev); c->st_kv_pending = false; }
+            if (c->st_kv) cudaFree(c->st_kv);
+            c->st_kv = nullptr;
+            c->st_kv_bytes = 0;
+            if (cudaMalloc((void**)&c->st_kv, need_bytes + need_bytes / 4) != cudaSuccess) {
+                cudaGetLastError();
+                return fail(SEGPA_ERR_OOM, "append_pages: staging allocation of %zu bytes for host-source rows failed", need_bytes);
+            }
+            c->st_kv_bytes = need_bytes + need_bytes / 4;
+        }
+    }
     long long total_chunks = 0;
     try {
         size_t ub = 0;   // one allocation at most (an upper bound of the ids listed: new pages + a refilled last page per job)
@@ -480,9 +632,11 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
             if ((r.k_src == nullptr) != (r.v_src == nullptr)) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: give both k_src and v_src, or neither (attach)", i);
             if (r.n_page_ids < 0 || (r.n_page_ids > 0 && !r.page_ids)) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: bad page_ids", i);
             const bool attach = (r.k_src == nullptr);
+            if (r.src_is_host != 0 && r.src_is_host != 1) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: src_is_host must be 0 or 1", i);
+            const bool from_host = !attach && r.src_is_host == 1;
             if (!attach && c->planning_only) APPEND_FAIL(SEGPA_ERR_STATE, "append_pages[%d]: copy mode on a planning-only cache", i);
             if (!attach && r.src_row_stride_elems < D) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: src_row_stride_elems %lld < head_dim", i, (long long)r.src_row_stride_elems);
-            if (!attach && ((r.src_row_stride_elems % 8) || ((uintptr_t)r.k_src % 16) || ((uintptr_t)r.v_src % 16)))
+            if (!attach && !from_host && ((r.src_row_stride_elems % 8) || ((uintptr_t)r.k_src % 16) || ((uintptr_t)r.v_src % 16)))
                 APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: k_src / v_src must be 16-byte aligned with a row stride multiple of 8 elements", i);
 
             const StreamKey key{r.layer, r.kv_head, r.seq_id};
@@ -525,6 +679,13 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 jb.k_src = (const uint16_t*)r.k_src;
                 jb.v_src = (const uint16_t*)r.v_src;
                 jb.src_stride = r.src_row_stride_elems;
+                if (from_host) {
+                    host_copies.push_back(HostCopy{r.k_src, r.v_src, r.src_row_stride_elems, r.n_tokens, host_rows});
+                    jb.k_src = c->st_kv + (size_t)host_rows * D;
+                    jb.v_src = c->st_kv + (size_t)(host_rows_total + host_rows) * D;
+                    jb.src_stride = D;
+                    host_rows += r.n_tokens;
+                }
                 jb.n_tokens = r.n_tokens;
                 jb.chunk_begin = total_chunks;
                 jb.page_off = (long long)touched.size();
@@ -583,10 +744,26 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
             memcpy((uint8_t*)sg.h + jobs_bytes, touched.data(), touched.size() * sizeof(int32_t));
             e = staging_upload(sg, bytes, c->up_stream, st);
         }
+        if (e == cudaSuccess && !host_copies.empty()) {
+            // the scatter of an earlier host-source batch (possibly on another stream) must have read st_kv
+            if (c->st_kv_pending) e = cudaStreamWaitEvent(st, c->st_kv_ev, 0);
+            for (size_t h = 0; h < host_copies.size() && e == cudaSuccess; ++h) {
+                const HostCopy& hc = host_copies[h];
+                uint16_t* kd = c->st_kv + (size_t)hc.off_rows * D;
+                uint16_t* vd = c->st_kv + (size_t)(host_rows_total + hc.off_rows) * D;
+                e = cudaMemcpy2DAsync(kd, (size_t)D * 2, hc.k, (size_t)hc.stride * 2, (size_t)D * 2, (size_t)hc.n, cudaMemcpyHostToDevice, st);
+                if (e == cudaSuccess)
+                    e = cudaMemcpy2DAsync(vd, (size_t)D * 2, hc.v, (size_t)hc.stride * 2, (size_t)D * 2, (size_t)hc.n, cudaMemcpyHostToDevice, st);
+            }
+        }
         if (e == cudaSuccess)
             e = launch_scatter_pages(c->k_pool, c->v_pool, (const ScatterJob*)sg.d, (int)jobs.size(),
                                      (const int*)((const uint8_t*)sg.d + jobs_bytes), total_chunks, D, P, st);
         if (e == cudaSuccess) staging_release(sg, st);
+        if (e == cudaSuccess && !host_copies.empty()) {
+            if (!c->st_kv_ev) e = cudaEventCreateWithFlags(&c->st_kv_ev, cudaEventDisableTiming);
+            if (e == cudaSuccess && cudaEventRecord(c->st_kv_ev, st) == cudaSuccess) c->st_kv_pending = true;
+        }
         if (e != cudaSuccess) {
             cudaGetLastError();
             APPEND_FAIL(SEGPA_ERR_CUDA, "append_pages: %s", cudaGetErrorString(e));
@@ -967,71 +1144,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 S->item_meta.push_back(segpa_segments::ItemMeta{(int32_t)ti, parts > 1 ? p : -1, parts});
             }
         }
-        // LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid (min-heap on
-        // (load, cta)); a CTA's items stay in descending order.  Cost = visited blocks + a fixed per-item term
-        // (pipeline refill, Q load, epilogue: about 0.6 block-times measured), in thirds of a block.  Flat arrays
-        // only: the plan is built on the critical path of every layer.
-        const int n_items_all = (int)S->items.size();
-        const int n_cta = std::min(n_items_all, c->num_sms);
-        // descending cost, ties by ascending index: a counting sort (costs are block counts, small integers)
-        std::vector<int>& order = ps.order;
-        order.resize((size_t)n_items_all);
-        {
-            int max_cost = 0;
-            for (const ItemDev& it : S->items) max_cost = std::max(max_cost, it.cost);
-            std::vector<int>& start = ps.start;
-            start.assign((size_t)max_cost + 2, 0);
-            for (const ItemDev& it : S->items) ++start[(size_t)(max_cost - it.cost) + 1];
-            for (int k2 = 0; k2 <= max_cost; ++k2) start[(size_t)k2 + 1] += start[(size_t)k2];
-            for (int i = 0; i < n_items_all; ++i) order[(size_t)start[(size_t)(max_cost - S->items[(size_t)i].cost)]++] = i;
-        }
-        // LPT: each item, in that order, goes to the least-loaded CTA.  The loads are kept as one ascending run of
-        // keys load * 1024 + cta (distinct, so the minimum is unique) inside a longer array: the minimum leaves at
-        // the head, the CTA's new key is inserted from the tail.  With costs descending the new key belongs at or
-        // near the tail, so an assignment costs a few moves (a binary heap's dependent loads per level cost more)
-        std::vector<int64_t>& run = ps.heap;
-        run.resize((size_t)n_cta + (size_t)n_items_all);
-        for (int q = 0; q < n_cta; ++q) run[(size_t)q] = q;
-        std::vector<int>&item_cta = ps.item_cta, &count = ps.count, &cursor = ps.cursor;
-        item_cta.resize((size_t)n_items_all);
-        count.assign((size_t)n_cta, 0);
-        {
-            int64_t* a = run.data();
-            const ItemDev* items = S->items.data();
-            const int64_t fixed3 = 2;   // the fixed per-item term, in thirds of a block (a sweep over 0..6 moved cfg2 / cfg4 by < 0.5 %)
-            size_t head = 0, tail = (size_t)n_cta;
-            for (int idx : order) {
-                const int64_t top = a[head++];
-                const int q = (int)(top & 1023);
-                item_cta[(size_t)idx] = q;
-                ++count[(size_t)q];
-                const int64_t blocks3 = 3 * (int64_t)items[idx].cost;
-                const int64_t key = top + (((items[idx].flags & 1) ? (blocks3 + 1) / 2 : blocks3) + fixed3) * 1024;   // strided: two chains
-                size_t pos = tail++;
-                while (pos > head && a[pos - 1] > key) {
-                    a[pos] = a[pos - 1];
-                    --pos;
-                }
-                a[pos] = key;
-            }
-        }
-        // per-CTA slices: CTA by CTA, each CTA's items in the order they were assigned (descending cost)
-        S->cta_off.assign((size_t)n_cta + 1, 0);
-        for (int q = 0; q < n_cta; ++q) S->cta_off[(size_t)q + 1] = S->cta_off[(size_t)q] + count[(size_t)q];
-        std::vector<ItemDev>& it2 = ps.it2;
-        std::vector<segpa_segments::ItemMeta>& im2 = ps.im2;
-        it2.resize((size_t)n_items_all);
-        im2.resize((size_t)n_items_all);
-        cursor.assign(S->cta_off.begin(), S->cta_off.end() - 1);
-        int64_t kv_blocks = 0;
-        for (int idx : order) {
-            const int at = cursor[(size_t)item_cta[(size_t)idx]]++;
-            it2[(size_t)at] = S->items[(size_t)idx];
-            im2[(size_t)at] = S->item_meta[(size_t)idx];
-            kv_blocks += S->items[(size_t)idx].cost;
-        }
-        S->items.swap(it2);
-        S->item_meta.swap(im2);
+        const int64_t kv_blocks = lpt_assign(ps, S->items, &S->item_meta, c->num_sms, S->cta_off);
 
         segpa_plan_stats_t& stt = S->stats;
         stt.n_segments = n;
@@ -1184,39 +1297,15 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     if (e != cudaSuccess) return fail(SEGPA_ERR_CUDA, "attention_fwd: earlier asynchronous failure: %s", cudaGetErrorString(e));
 
     FwdParams p{};
-    const uint8_t* d_blob = (const uint8_t*)s->buf->blob.d;
     s->last_stream = st;
-    p.segs = (const SegDev*)(d_blob + s->off_segs);
-    p.items = (const ItemDev*)(d_blob + s->off_items);
-    p.pages = (const int*)(d_blob + s->off_pages);
-    p.combs = (const CombDev*)(d_blob + s->off_combs);
-    p.cta_off = (const int*)(d_blob + s->off_cta);
-    p.n_cta = (int)s->cta_off.size() - 1;
-    p.n_items = (int)s->items.size();
-    p.n_combs = (int)s->combs.size();
-    p.comb_max_rows = 0;
-    for (const CombDev& cd : s->combs) p.comb_max_rows = std::max(p.comb_max_rows, cd.n_tok * c->G);
-    p.counter = s->buf->counter;
-    p.k_pool = c->k_pool;
-    p.v_pool = c->v_pool;
+    fill_fwd_params(p, c, s);
     p.q = (const uint16_t*)q;
     p.out = (uint16_t*)out;
     p.lse = lse;
-    p.ws_o = s->buf->ws_o;
-    p.ws_ml = s->buf->ws_ml;
     p.q_row_stride = q_row_stride;
     p.out_row_stride = out_row_stride;
     p.lse_stride = lse_stride;
     p.scale = scale;
-    p.Hq = Hq;
-    p.Hkv = c->desc.num_kv_heads;
-    p.G = c->G;
-    p.D = D;
-    p.P = c->desc.page_size;
-    p.tile_tokens = kTileRows / c->G;
-    p.tiles_per_item = s->tiles_per_item;
-    p.page_bytes = c->page_bytes;
-    p.num_sms = c->num_sms;
     if (c->kernel_kind == 1) {
         const char* why = encode_q_map(&p.q_map, q, T, Hq, D, c->G, p.tile_tokens, q_row_stride);
         if (why) return fail(SEGPA_ERR_CUDA, "attention_fwd: %s", why);
@@ -1260,16 +1349,88 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t* c, const segpa_segments_t* s, 
     return SEGPA_OK;
 }
 
+namespace {
+
+// segpa_attention_fwd_host: cut the plan into chunks of consecutive query rows (about 16 MB of Q each, at most 16),
+// each with its own LPT assignment over the persistent grid and its own combine entries, and upload them (once per
+// segments object).  An item belongs to the chunk that holds its first row.
+segpa_status_t plan_host_chunks(segpa_cache* c, const segpa_segments* s, int64_t T, cudaStream_t st) {
+    if (s->host_planned) return SEGPA_OK;
+    const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
+    const int64_t row_bytes = (int64_t)Hq * D * 2;
+    const int64_t rows_used = std::max<int64_t>(1, std::min(T, s->stats.q_rows));
+    int64_t n_chunks = std::min<int64_t>(16, std::max<int64_t>(1, (rows_used * row_bytes + (16 << 20) - 1) / (16 << 20)));
+    int64_t rows_per = std::max<int64_t>(2 * kTileRows, cdiv(rows_used, n_chunks));   // an item spans < 2 * 128 rows: it reaches into the next chunk at most
+    n_chunks = cdiv(rows_used, rows_per);
+    std::vector<std::vector<ItemDev>> per((size_t)n_chunks);
+    std::vector<int64_t> need((size_t)n_chunks, 0);
+    for (const ItemDev& it : s->items) {
+        const int64_t r0 = s->segs[(size_t)it.seg].q_row_start + it.t0;
+        const size_t ch = (size_t)std::min<int64_t>(n_chunks - 1, r0 / rows_per);
+        per[ch].push_back(it);
+        need[ch] = std::max(need[ch], r0 + it.n_tok);
+    }
+    std::vector<std::vector<CombDev>> combs((size_t)n_chunks);
+    for (const CombDev& cd : s->combs) {
+        const int64_t r0 = s->segs[(size_t)cd.seg].q_row_start + cd.t0;
+        combs[(size_t)std::min<int64_t>(n_chunks - 1, r0 / rows_per)].push_back(cd);
+    }
+    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    std::vector<uint8_t> blob;
+    std::vector<int32_t> cta_off;
+    s->hchunks.clear();
+    for (int64_t ch = 0; ch < n_chunks; ++ch) {
+        segpa_segments::HostChunk hc{};
+        hc.row_lo = ch * rows_per;
+        hc.row_hi = (ch == n_chunks - 1) ? T : std::min<int64_t>(T, (ch + 1) * rows_per);   // the last chunk carries the rows past the plan's
+        hc.need_hi = std::max(need[(size_t)ch], hc.row_lo);
+        std::vector<ItemDev>& items = per[(size_t)ch];
+        hc.n_items = (int)items.size();
+        cta_off.assign(1, 0);
+        if (!items.empty()) lpt_assign(c->plan, items, nullptr, c->num_sms, cta_off);
+        hc.n_cta = (int)cta_off.size() - 1;
+        hc.n_combs = (int)combs[(size_t)ch].size();
+        for (const CombDev& cd : combs[(size_t)ch]) hc.comb_max_rows = std::max(hc.comb_max_rows, cd.n_tok * c->G);
+        hc.off_items = al(blob.size());
+        blob.resize(hc.off_items + items.size() * sizeof(ItemDev));
+        if (!items.empty()) memcpy(blob.data() + hc.off_items, items.data(), items.size() * sizeof(ItemDev));
+        hc.off_cta = al(blob.size());
+        blob.resize(hc.off_cta + cta_off.size() * sizeof(int32_t));
+        memcpy(blob.data() + hc.off_cta, cta_off.data(), cta_off.size() * sizeof(int32_t));
+        hc.off_combs = al(blob.size());
+        blob.resize(hc.off_combs + std::max<size_t>(1, combs[(size_t)ch].size()) * sizeof(CombDev));
+        if (hc.n_combs) memcpy(blob.data() + hc.off_combs, combs[(size_t)ch].data(), (size_t)hc.n_combs * sizeof(CombDev));
+        s->hchunks.push_back(hc);
+    }
+    Staging& sg = s->buf->host_blob;
+    cudaError_t e = staging_acquire(sg, al(blob.size()));
+    if (e == cudaSuccess) {
+        memcpy(sg.h, blob.data(), blob.size());
+        e = staging_upload(sg, al(blob.size()), c->up_stream, st);
+    }
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(e == cudaErrorMemoryAllocation ? SEGPA_ERR_OOM : SEGPA_ERR_CUDA, "attention_fwd_host: %s", cudaGetErrorString(e)); }
+    s->host_planned = true;
+    return SEGPA_OK;
+}
+
+}  // namespace
+
 segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t* s, const void* q_host,
                                         float scale, void* out_host, float* lse_host, int64_t T,
                                         void* cuda_stream) {
     if (!c || !s || !q_host || !out_host) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: null argument");
     if (c->planning_only) return fail(SEGPA_ERR_STATE, "attention_fwd_host: planning-only cache has no device; there is no CPU fallback");
-    if (T < 1) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: T < 1");
+    if (s->cache != c || std::find(c->seg_objs.begin(), c->seg_objs.end(), s) == c->seg_objs.end())
+        return fail(SEGPA_ERR_STATE, "attention_fwd_host: segments were not built by this cache (or were freed)");
+    if (T < 1 || T < s->stats.q_rows) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: T %lld < rows used by the plan %lld", (long long)T, (long long)s->stats.q_rows);
+    if (!(scale > 0.f) || !(scale < 1e30f)) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: softmax_scale must be positive and finite");
     const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
-    const size_t qb = (size_t)T * Hq * D * 2, lb = (size_t)T * Hq * 4;
+    const size_t row_bytes = (size_t)Hq * D * 2;
+    const size_t qb = (size_t)T * row_bytes, lb = (size_t)T * Hq * 4;
     DeviceGuard g(c->desc.device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(SEGPA_ERR_CUDA, "attention_fwd_host: earlier asynchronous failure: %s", cudaGetErrorString(e));
     if (qb > c->st_q_bytes) {
         if (c->st_q) { cudaStreamSynchronize(st); cudaFree(c->st_q); cudaFree(c->st_out); c->st_q = c->st_out = nullptr; c->st_q_bytes = 0; }
         if (cudaMalloc((void**)&c->st_q, qb) != cudaSuccess || cudaMalloc((void**)&c->st_out, qb) != cudaSuccess) {
@@ -1285,13 +1446,83 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t
         if (cudaMalloc((void**)&c->st_lse, lb) != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_OOM, "attention_fwd_host: staging allocation failed"); }
         c->st_lse_bytes = lb;
     }
-    cudaError_t e = cudaMemcpyAsync(c->st_q, q_host, qb, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_fwd_host: H2D failed: %s", cudaGetErrorString(e)); }
-    segpa_status_t rc = segpa_attention_fwd(c, s, c->st_q, (int64_t)Hq * D, scale, c->st_out, (int64_t)Hq * D,
-                                            c->st_lse, T, T, cuda_stream);
+    if (!c->h2d_stream && (cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking) != cudaSuccess ||
+                           cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking) != cudaSuccess)) {
+        cudaGetLastError();
+        return fail(SEGPA_ERR_CUDA, "attention_fwd_host: cannot create the copy streams");
+    }
+    s->last_stream = st;
+    segpa_status_t rc = plan_host_chunks(c, s, T, st);
     if (rc != SEGPA_OK) return rc;
-    e = cudaMemcpyAsync(out_host, c->st_out, qb, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && lse_host) e = cudaMemcpyAsync(lse_host, c->st_lse, lb, cudaMemcpyDeviceToHost, st);
+    const size_t n_ch = s->hchunks.size();
+    while (c->host_events.size() < 2 * n_ch + 1) {
+        cudaEvent_t ev = nullptr;
+        if (cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_fwd_host: cannot create events"); }
+        c->host_events.push_back(ev);
+    }
+    cudaEvent_t* ev_in = c->host_events.data();            // [n_ch]: Q rows of chunk k are on the device
+    cudaEvent_t* ev_done = c->host_events.data() + n_ch;   // [n_ch]: kernels of chunk k have finished
+    cudaEvent_t ev_start = c->host_events[2 * n_ch];
+
+    // Three streams: Q chunks go up on h2d_stream one after the other; the caller's stream runs chunk k's kernels once
+    // its rows (and the first rows of chunk k+1 its last items reach into) have arrived; d2h_stream copies chunk k's out /
+    // lse rows back while chunk k+1 computes.  PCIe is full duplex, so the call is bounded by the larger direction.
+    // (row, head) pairs no segment covers come back as zeros: the staging rows are cleared first.
+    FwdParams base{};
+    fill_fwd_params(base, c, s);
+    const char* why = encode_q_map(&base.q_map, c->st_q, T, Hq, D, c->G, base.tile_tokens, (int64_t)Hq * D);
+    if (why) return fail(SEGPA_ERR_CUDA, "attention_fwd_host: %s", why);
+    base.q = c->st_q;
+    base.out = c->st_out;
+    base.lse = c->st_lse;
+    base.q_row_stride = base.out_row_stride = (int64_t)Hq * D;
+    base.lse_stride = T;
+    base.scale = scale;
+    const uint8_t* hb = (const uint8_t*)s->buf->host_blob.d;
+    e = cudaMemsetAsync(c->st_out, 0, qb, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->st_lse, 0, lb, st);
+    if (e == cudaSuccess) e = cudaEventRecord(ev_start, st);                  // earlier work on the caller's stream (K/V stores) is ordered before
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->h2d_stream, ev_start, 0);   // ... the first copy, so a step's uploads do not overtake the previous step's reads
+    for (size_t k = 0; k < n_ch && e == cudaSuccess; ++k) {
+        const segpa_segments::HostChunk& hc = s->hchunks[k];
+        e = cudaMemcpyAsync((uint8_t*)c->st_q + (size_t)hc.row_lo * row_bytes, (const uint8_t*)q_host + (size_t)hc.row_lo * row_bytes,
+                            (size_t)(hc.row_hi - hc.row_lo) * row_bytes, cudaMemcpyHostToDevice, c->h2d_stream);
+        if (e == cudaSuccess) e = cudaEventRecord(ev_in[k], c->h2d_stream);
+    }
+    int launches = 0;
+    for (size_t k = 0; k < n_ch && e == cudaSuccess; ++k) {
+        const segpa_segments::HostChunk& hc = s->hchunks[k];
+        size_t last_in = k;
+        while (last_in + 1 < n_ch && s->hchunks[last_in].row_hi < hc.need_hi) ++last_in;
+        e = cudaStreamWaitEvent(st, ev_in[last_in], 0);
+        if (e == cudaSuccess && hc.n_items > 0) {
+            FwdParams p = base;
+            p.items = (const ItemDev*)(hb + hc.off_items);
+            p.cta_off = (const int*)(hb + hc.off_cta);
+            p.combs = (const CombDev*)(hb + hc.off_combs);
+            p.n_items = hc.n_items;
+            p.n_cta = hc.n_cta;
+            p.n_combs = hc.n_combs;
+            p.comb_max_rows = hc.comb_max_rows;
+            e = launch_attention_tc(p, st);
+            ++launches;
+            if (e == cudaSuccess && p.n_combs > 0) { e = launch_combine(p, st); ++launches; }
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(ev_done[k], st);
+        // rows of chunk k are final once the kernels of chunk k have run (items of chunk k-1 that reach into it ran before)
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c->d2h_stream, ev_done[k], 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpyAsync((uint8_t*)out_host + (size_t)hc.row_lo * row_bytes, (const uint8_t*)c->st_out + (size_t)hc.row_lo * row_bytes,
+                                (size_t)(hc.row_hi - hc.row_lo) * row_bytes, cudaMemcpyDeviceToHost, c->d2h_stream);
+        if (e == cudaSuccess && lse_host)
+            e = cudaMemcpy2DAsync(lse_host + hc.row_lo, (size_t)T * 4, c->st_lse + hc.row_lo, (size_t)T * 4, (size_t)(hc.row_hi - hc.row_lo) * 4,
+                                  (size_t)Hq, cudaMemcpyDeviceToHost, c->d2h_stream);
+    }
+    c->last_launches = launches;
+    // the call is synchronous: wait for the last copy back (and leave the caller's stream ordered after it)
+    if (e == cudaSuccess) e = cudaEventRecord(ev_start, c->d2h_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_start, 0);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->d2h_stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_fwd_host: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;

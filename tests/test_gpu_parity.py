@@ -9,6 +9,7 @@ import torch
 from paper_2606_06256_b200 import binding as B, harness as H, workloads as wl
 from paper_2606_06256_b200.workloads import GLOBAL, LOCAL
 from tests.gpu_helpers import GpuRun, LSE_SENTINEL, OUT_SENTINEL, compare, sample_rows
+from tests.helpers import covered_mask
 
 pytestmark = pytest.mark.gpu
 
@@ -376,6 +377,58 @@ def test_host_buffer_entry_point_matches_device_path():
         g.close()
 
 
+def test_host_entry_points_pipelined_chunks_and_host_source_append():
+    """The host-buffer path at a size that is cut into several row chunks (H2D of chunk k+1 beside the kernels of
+    chunk k beside the D2H of chunk k-1): bit-identical to the device entry point on the covered (row, head) pairs,
+    zeros on the uncovered ones; decode-shaped requests (split-KV + combine inside a chunk) and a head whose query
+    range is shorter included.  The K/V rows of the second cache come from HOST memory (src_is_host), with a
+    non-contiguous row stride, and must give the same pool."""
+    reqs = [{"kv_len": 5000, "heads": {h: ((GLOBAL, 0, 0, 5000) if h == 0 else (LOCAL, 700, 4 * (h % 2), 5000 if h < 6 else 333)) for h in range(8)}},
+            {"kv_len": 9000, "heads": {h: ((GLOBAL, 0, 0, 1) if h % 3 == 0 else (LOCAL, 2048, 0, 1)) for h in range(8)}},
+            {"kv_len": 3000, "heads": {h: (GLOBAL if h == 7 else LOCAL, 257, 0, 1500) for h in range(8)}}]
+    w = wl.make_workload("hostpath", Hq=32, Hkv=8, D=128, P=16, requests=reqs, seed=61)
+    assert w.T[0] * w.Hq * w.D * 2 > 3 * (16 << 20)             # more than three 16 MB chunks of Q
+    dev = torch.device("cuda:0")
+    k, v = wl.pool_values(w, dev)
+    g = GpuRun(w, "tc", 2, k, v)
+    cache2 = H.create_cache(w, 0, tiles_per_item=2)
+    try:
+        q, out, lse = g.layer(0)
+        print(compare(w, 0, k, v, q, out, lse, rows=sample_rows(w, 0, n_random=64, seed=6), label="hostpath (device entry)"))
+        # second cache: the same streams, rows handed over from pinned host memory with a padded row stride
+        keep, hreqs = [], []
+        for (layer, kvh, seq, kr, vr, n, ids) in H.append_requests(w, k, v):
+            kh = torch.zeros((n, w.D + 8), dtype=torch.bfloat16).pin_memory()
+            vh = torch.zeros((n, w.D + 8), dtype=torch.bfloat16).pin_memory()
+            kh[:, :w.D].copy_(kr)
+            vh[:, :w.D].copy_(vr)
+            keep.append((kh, vh))
+            hreqs.append((layer, kvh, seq, kh[:, :w.D], vh[:, :w.D], n, ids))
+        B.segpa_append_pages_batch(cache2, hreqs)
+        for s_ in w.streams[::5]:
+            ka, kb = torch.zeros((s_.kv_len, w.D), dtype=torch.bfloat16, device=dev), torch.zeros((s_.kv_len, w.D), dtype=torch.bfloat16, device=dev)
+            va, vb = torch.zeros_like(ka), torch.zeros_like(kb)
+            B.segpa_gather_rows(g.cache, 0, s_.kv_head, s_.seq_id, 0, s_.kv_len, ka, va)
+            B.segpa_gather_rows(cache2, 0, s_.kv_head, s_.seq_id, 0, s_.kv_len, kb, vb)
+            torch.cuda.synchronize()
+            assert torch.equal(ka, kb) and torch.equal(va, vb)
+        segs2 = H.build_layer(cache2, w, 0)
+        qh = q.cpu().pin_memory()
+        cov = torch.from_numpy(covered_mask(w, 0))
+        assert (~cov).any()
+        for rep in range(2):                                    # second call: the chunk plan is reused
+            oh = torch.full_like(qh, 5.0).pin_memory()
+            lh = torch.full((w.Hq, w.T[0]), 5.0, dtype=torch.float32).pin_memory()
+            B.segpa_attention_fwd_host(cache2, segs2, qh, w.scale, oh, lh)
+            assert B.segpa_last_launch_count(cache2) >= 4       # several chunk launches (+ combine)
+            oc, lc = out.cpu(), lse.cpu()
+            assert torch.equal(oh[cov], oc[cov]) and torch.equal(lh.T[cov], lc.T[cov])
+            assert not oh[~cov].any() and not lh.T[~cov].any()
+    finally:
+        B.segpa_destroy(cache2)
+        g.close()
+
+
 def test_no_dense_allocation():
     """'No dense [B,H,L,D] tensor and no additive mask is built': device memory taken by
     build_segments + attention_fwd stays far below one [L, L] mask."""
@@ -419,7 +472,7 @@ def test_cfg3_sampled():
     try:
         q, out, lse = g.layer(0)
         rows = sample_rows(w, 0, n_random=4096, seed=3, tile_edges=64, block_edges=64, dense_tail=1024)
-        assert len(rows) > 2000 and np.isin(np.arange(64512, 65536), rows).all()
+        assert len(rows) > 1800 and np.isin(np.arange(64512, 65536), rows).all()
         print(len(rows), compare(w, 0, g.k_pool, g.v_pool, q, out, lse, rows=rows, label="cfg3"))
     finally:
         g.close()
