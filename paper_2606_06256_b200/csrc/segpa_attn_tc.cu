@@ -45,10 +45,6 @@ constexpr int kHalfKeys = 64;
 constexpr int kRegsLow = 72;
 constexpr int kRegsSoftmax = 192;
 constexpr int kRegsEpilogue = 56;
-#ifndef SEGPA_POLY_MASK
-#define SEGPA_POLY_MASK 0x00
-#endif
-constexpr unsigned kPolyMask = SEGPA_POLY_MASK;   // bit q: pair q of every 8 pairs takes the polynomial exp2
 constexpr float kRescaleThreshold = 8.0f;  // log2 units: O is rescaled only when the max grows by > 2^8
 
 // Pipeline trace (debug builds with -DSEGPA_TRACE only): lane 0 of every warp of CTA 0 logs
@@ -579,8 +575,6 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         TRACE(23, j);
                         const float mref = (m_used == -INFINITY) ? 0.f : m_used;
                         // p = 2^(s*scale*log2e - m) (masked columns: 2^-inf = 0), row sum, bf16 P -> TMEM (aliases S[0, 64))
-                        // exp2 is split between the MUFU pipe and the FMA pipe (exp2_poly2): the two are
-                        // co-limiters of this loop, kPolyMask picks the pairs (of every 8) that go to the FMA pipe
                         const uint64_t sl2x2 = pack2(sl2, sl2), nmx2 = pack2(-mref, -mref);
                         uint64_t rsa = pack2(0.f, 0.f), rsb = pack2(0.f, 0.f);
 #pragma unroll
@@ -601,15 +595,9 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                             for (int q = 0; q < 16; ++q) {
                                 const int e = c * 32 + 2 * q;
                                 const uint64_t x = ffma2(pack2(__uint_as_float(s[e]), __uint_as_float(s[e + 1])), sl2x2, nmx2);
-                                float p0, p1;
-                                if ((kPolyMask >> (q & 7)) & 1) {
-                                    exp2_poly2(x, p0, p1);
-                                } else {
-                                    float x0, x1;
-                                    unpack2(x, x0, x1);
-                                    p0 = fast_exp2(x0);
-                                    p1 = fast_exp2(x1);
-                                }
+                                float x0, x1;
+                                unpack2(x, x0, x1);
+                                const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
                                 if (q & 1) rsb = fadd2(rsb, pack2(p0, p1)); else rsa = fadd2(rsa, pack2(p0, p1));
                                 pk[q] = pack_bf16x2(p0, p1);
                             }

@@ -76,11 +76,6 @@ __device__ __forceinline__ void tma_prefetch_3d(const void* tmap, int c0, int c1
 __device__ __forceinline__ void prefetch_tmap(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
 }
-// generic-proxy smem writes -> visible to the async proxy (UMMA / TMA reads)
-__device__ __forceinline__ void fence_proxy_async_smem() {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-
 // ------------------------------------------------------------------------------- tcgen05
 __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
@@ -163,18 +158,7 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* r) {
         : "r"(taddr)
         : "memory");
 }
-// registers -> TMEM: this thread's lane, 32 / 16 consecutive 32-bit columns
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};" ::"r"(taddr),
-        "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
-        "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]), "r"(r[16]), "r"(r[17]), "r"(r[18]),
-        "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]), "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]),
-        "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
+// registers -> TMEM: this thread's lane, 16 consecutive 32-bit columns
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
     asm volatile(
         "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
@@ -184,13 +168,6 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
         : "memory");
 }
 
-
-// ------------------------------------------------------------------------------- cp.async (LDGSTS)
-// 16-byte global -> shared copy; src_bytes = 0 writes zeros instead
-__device__ __forceinline__ void cp_async16(uint32_t dst_smem, const void* src, uint32_t src_bytes) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst_smem), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------- register budget
 template <int N>
@@ -217,32 +194,6 @@ __device__ __forceinline__ uint64_t fadd2(uint64_t a, uint64_t b) {
     asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
     return d;
 }
-__device__ __forceinline__ uint64_t fsub2(uint64_t a, uint64_t b) {
-    uint64_t d;
-    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-
-// 2^x for a pair on the FMA pipe (no MUFU): round-to-nearest split x = j + f, f in [-0.5, 0.5], degree-3
-// minimax polynomial for 2^f (max relative error 7.5e-5, well below the bf16 rounding of P), exponent
-// added as an integer.  x is clamped to >= -126 (2^-126 stands in for 0; -inf inputs become ~1e-38).
-__device__ __forceinline__ void exp2_poly2(uint64_t x, float& p0, float& p1) {
-    float x0, x1;
-    unpack2(x, x0, x1);
-    x = pack2(fmaxf(x0, -126.f), fmaxf(x1, -126.f));
-    const uint64_t magic = pack2(12582912.f, 12582912.f);                    // 1.5 * 2^23
-    const uint64_t t = fadd2(x, magic);                                      // low mantissa bits = round(x)
-    const uint64_t f = fsub2(x, fsub2(t, magic));
-    uint64_t p = ffma2(f, pack2(0.0551716610789299f, 0.0551716610789299f), pack2(0.2426111251115799f, 0.2426111251115799f));
-    p = ffma2(p, f, pack2(0.6932609677314758f, 0.6932609677314758f));
-    p = ffma2(p, f, pack2(0.9999280571937561f, 0.9999280571937561f));
-    float t0, t1, q0, q1;
-    unpack2(t, t0, t1);
-    unpack2(p, q0, q1);
-    p0 = __uint_as_float(__float_as_uint(q0) + (__float_as_uint(t0) << 23));
-    p1 = __uint_as_float(__float_as_uint(q1) + (__float_as_uint(t1) << 23));
-}
-
 __device__ __forceinline__ float max3(float a, float b, float c) {
     float d;
     asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
