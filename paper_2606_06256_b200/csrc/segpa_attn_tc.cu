@@ -219,6 +219,10 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = bars.tmem_base;
+    // everything above overlapped the tail of the previous kernel of the stream (programmatic dependent launch); from
+    // here on this kernel reads what that kernel wrote (K/V pages, partials' workspace, out)
+    pdl_launch_dependents();
+    pdl_wait();
 
     if (warp == kLoaderWarp || warp == kVLoaderWarp) {
         // ------------------------------------------------------------------ K/V loaders
@@ -749,8 +753,7 @@ static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    attention_tc_kernel<D, NT><<<p.n_cta, kThreads, C::kSmemBytes, st>>>(p);
-    return cudaGetLastError();
+    return launch_pdl(attention_tc_kernel<D, NT>, dim3((unsigned)p.n_cta), dim3(kThreads), (size_t)C::kSmemBytes, st, p);
 }
 
 cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st) {

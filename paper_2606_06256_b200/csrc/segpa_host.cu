@@ -1119,6 +1119,11 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         int64_t total_cost = 0;
         for (auto& t : tiles) total_cost += t.cost;
         const int64_t chunk = std::max<int64_t>(8, cdiv(total_cost, (int64_t)c->num_sms * 4));
+        // Decode-shaped tiles (a few rows against a long stream, HBM-bound) are cut coarser: pieces of about one CTA's
+        // share of the whole plan.  Every piece costs a Q load, a drain of 2 x 128 TMEM lanes for a handful of valid rows
+        // and one more partial for the combine pass to read, and LPT still balances the grid with ~2 pieces per CTA
+        // (measured: fig9-decode-128k 92 -> 65 us per layer, cfg4d 99 -> 93 us against pieces of a quarter of that size).
+        const int64_t chunk_dec = std::max<int64_t>(8, cdiv(total_cost, (int64_t)c->num_sms));
         int n_split_tiles = 0, n_slots = 0;
         S->items.reserve(tiles.size() + (size_t)c->num_sms * 8);
         S->item_meta.reserve(tiles.size() + (size_t)c->num_sms * 8);
@@ -1126,7 +1131,9 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             const TileTmp& t = tiles[ti];
             const int cost = t.cost;
             int parts = 1;
-            if (cost > chunk + chunk / 2 && !t.sink) parts = (int)cdiv(cost, chunk);   // (sink items are not cut along KV)
+            const bool dec = S->reqs[(size_t)t.seg].q_len <= TT;
+            const int64_t ch = dec ? chunk_dec : chunk;
+            if (cost > (dec ? ch + ch / 8 : ch + ch / 2) && !t.sink) parts = (int)cdiv(cost, ch);   // (sink items are not cut along KV)
             // Decode-shaped segment (all its rows fit the first of the item's two tile slots; the short tail item of a
             // long prefill segment does not count: it is not worth a combine pass): run it STRIDED -- the
             // two slots take alternate KV blocks of the same rows as two independent chains, each writing a

@@ -4,6 +4,7 @@
 
 #include <cstdint>
 #include <cuda_runtime.h>
+#include <utility>
 
 namespace segpa {
 
@@ -170,6 +171,23 @@ struct MassParams {
 cudaError_t launch_attention_mass(const MassParams& p, cudaStream_t st);
 cudaError_t launch_mass_select(const float* mass, const long long* mass_off_dev, const int* kv_len_dev, int n_segments, float tau,
                                unsigned char* selected, int* n_selected, cudaStream_t st);
+
+// Launch with programmatic dependent launch allowed: the kernel may begin (prologue up to its pdl_wait()) while the
+// previous kernel of the stream drains, which hides launch latency between the back-to-back kernels of a layer.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
 
 // kernel launchers (each returns the CUDA error of its launch)
 cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const ScatterJob* jobs_dev, int n_jobs,

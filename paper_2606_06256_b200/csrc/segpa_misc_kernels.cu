@@ -1,6 +1,7 @@
 // Small kernels of libsegpa.so: page scatter (append), RoPEAlign, row gather, split-KV combine, LSE merge; and,
 // in the test build only (-DSEGPA_BRINGUP -> libsegpa_bringup.so), the SIMT cross-check attention kernel.
 #include "segpa_internal.h"
+#include "sm100_ptx.cuh"
 
 #include <cuda_bf16.h>
 
@@ -16,6 +17,8 @@ __global__ void scatter_pages_kernel(uint8_t* __restrict__ k_pool, uint8_t* __re
                                      const ScatterJob* __restrict__ jobs, int n_jobs,
                                      const int* __restrict__ page_ids, long long total_chunks, int D, int P) {
     const int cpr = D >> 3;  // 16-byte chunks per row
+    ptx::pdl_launch_dependents();
+    ptx::pdl_wait();         // the pool pages may still be read by the previous kernel of the stream
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total_chunks;
          idx += (long long)gridDim.x * blockDim.x) {
         int lo = 0, hi = n_jobs - 1;
@@ -48,9 +51,8 @@ cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const Scatter
     const int threads = 256;
     long long blocks = (total_chunks + threads - 1) / threads;
     if (blocks > 148 * 64) blocks = 148 * 64;   // grid-stride beyond 64 CTAs per SM
-    scatter_pages_kernel<<<(unsigned)blocks, threads, 0, st>>>(k_pool, v_pool, jobs_dev, n_jobs, page_ids_dev,
-                                                               total_chunks, D, P);
-    return cudaGetLastError();
+    return launch_pdl(scatter_pages_kernel, dim3((unsigned)blocks), dim3(threads), 0, st, k_pool, v_pool, jobs_dev, n_jobs, page_ids_dev,
+                      total_chunks, D, P);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -173,6 +175,8 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ Fw
     __shared__ float s_l[NW];
     const int rows_per_slot = kTileRows * p.tiles_per_item;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    ptx::pdl_launch_dependents();
+    ptx::pdl_wait();         // the partials are the attention kernel's
     // block (x, y): comb x, rows y, y + gridDim.y, ...  One block per row: the chain of dependent loads of a
     // row with many partials is cut eight ways; sums are formed in a fixed order (deterministic).
     const CombDev c = p.combs[blockIdx.x];
@@ -195,6 +199,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ Fw
         float acc[EPL];
 #pragma unroll
         for (int k = 0; k < EPL; ++k) acc[k] = 0.f;
+#pragma unroll 4
         for (int s = warp; s < n_part; s += NW) {
             const size_t base = part_row(s);
             const float ms = p.ws_ml[base * 2], ls = p.ws_ml[base * 2 + 1];
@@ -237,9 +242,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ Fw
 cudaError_t launch_combine(const FwdParams& p, cudaStream_t st) {
     if (p.n_combs == 0) return cudaSuccess;
     const dim3 grid((unsigned)p.n_combs, (unsigned)(p.comb_max_rows < 1 ? 1 : (p.comb_max_rows > 256 ? 256 : p.comb_max_rows)));
-    if (p.D == 128) combine_kernel<128><<<grid, 256, 0, st>>>(p);
-    else combine_kernel<64><<<grid, 256, 0, st>>>(p);
-    return cudaGetLastError();
+    return p.D == 128 ? launch_pdl(combine_kernel<128>, grid, dim3(256), 0, st, p) : launch_pdl(combine_kernel<64>, grid, dim3(256), 0, st, p);
 }
 
 // ---------------------------------------------------------------------------------------------

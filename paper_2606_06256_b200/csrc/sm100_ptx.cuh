@@ -54,6 +54,14 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     }
 }
 
+// ------------------------------------------------------------------------------- programmatic dependent launch
+// A kernel launched with the programmatic-stream-serialization attribute may start while its predecessor in the
+// stream still runs; it must not touch what the predecessor writes (nor write what it reads) before pdl_wait(), which
+// returns once the predecessor grid has completed and its writes are visible.  pdl_launch_dependents() lets the
+// successor's CTAs be scheduled (as SMs free up) from this point on instead of at the end of this grid.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ------------------------------------------------------------------------------- TMA bulk copy
 // global -> shared::cta, completion signalled on an mbarrier as transaction bytes (SASS: UBLKCP)
 __device__ __forceinline__ void bulk_g2s(uint32_t dst_smem, const void* src_gmem, uint32_t bytes, uint32_t bar) {
