@@ -79,8 +79,11 @@ def _u16(a) -> np.ndarray:
 def oracle_attention(*, Hq: int, Hkv: int, D: int, P: int, k_pool, v_pool,
                      page_table: np.ndarray, pt_offsets: np.ndarray, kv_lens: np.ndarray,
                      segments: Sequence[tuple], q, T: int, scale: float,
-                     row_subset: Optional[np.ndarray] = None, want_p: int = 0) -> OracleResult:
+                     row_subset: Optional[np.ndarray] = None, want_p: int = 0,
+                     seg_offsets: Optional[np.ndarray] = None, seg_lens: Optional[np.ndarray] = None) -> OracleResult:
     """segments: tuples (stream_idx, kv_head, head_class, window, n_sink, q_row_start, q_len).
+    seg_offsets / seg_lens: optional head-segment table (CSR over streams): each segment of a stream
+    starts on a fresh page of the stream's page table.
 
     k_pool/v_pool: [num_pages][P][D] bf16 (torch) or uint16 bits; q: [T][Hq][D] likewise.
     """
@@ -107,6 +110,12 @@ def oracle_attention(*, Hq: int, Hkv: int, D: int, P: int, k_pool, v_pool,
     p = np.zeros((rows, Hq, want_p), dtype=np.float64) if want_p else None
     pairs = C.c_int64(0)
     shape = _Shape(Hq, Hkv, D, P)
+    so_ptr = sl_ptr = None
+    if seg_offsets is not None:
+        seg_offsets = np.ascontiguousarray(seg_offsets, dtype=np.int64)
+        seg_lens = np.ascontiguousarray(seg_lens, dtype=np.int64)
+        assert len(seg_offsets) == len(kv_lens) + 1 and seg_offsets[-1] == len(seg_lens)
+        so_ptr, sl_ptr = seg_offsets.ctypes.data_as(C.c_void_p), seg_lens.ctypes.data_as(C.c_void_p)
     rc = lib.oracle_attention(
         C.byref(shape), kp.ctypes.data_as(C.c_void_p), vp.ctypes.data_as(C.c_void_p),
         C.c_int64(num_pages), page_table.ctypes.data_as(C.c_void_p),
@@ -116,7 +125,7 @@ def oracle_attention(*, Hq: int, Hkv: int, D: int, P: int, k_pool, v_pool,
         sub_ptr, C.c_int64(rows if row_subset is not None else 0),
         out.ctypes.data_as(C.c_void_p), lse.ctypes.data_as(C.c_void_p),
         p.ctypes.data_as(C.c_void_p) if p is not None else None, C.c_int64(want_p),
-        C.byref(pairs))
+        C.byref(pairs), so_ptr, sl_ptr)
     if rc != 0:
         raise ValueError("oracle_attention rejected the input (code %d)" % rc)
     return OracleResult(out, lse, int(pairs.value), p, row_subset)

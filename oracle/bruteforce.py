@@ -18,13 +18,22 @@ def widen(bits: np.ndarray) -> np.ndarray:
 
 
 def dense_masked_attention(q_bits, k_pool_bits, v_pool_bits, page_ids, kv_len, P,
-                           head_class, W, n_sink, scale):
-    """q_bits [q_len][D] of ONE q head; returns (O [q_len][D], LSE [q_len], p [q_len][kv_len])."""
+                           head_class, W, n_sink, scale, chunk_lens=None):
+    """q_bits [q_len][D] of ONE q head; returns (O [q_len][D], LSE [q_len], p [q_len][kv_len]).
+    chunk_lens: the stream's head segments, each on its own consecutive pages of page_ids; the dense
+    stream is the concatenation of the segments' rows (None: one segment)."""
     q = widen(np.asarray(q_bits))
     q_len = q.shape[0]
-    pages = np.asarray(page_ids)[: (kv_len + P - 1) // P]
-    K = widen(np.asarray(k_pool_bits)[pages]).reshape(-1, q.shape[1])[:kv_len]
-    V = widen(np.asarray(v_pool_bits)[pages]).reshape(-1, q.shape[1])[:kv_len]
+    Kp, Vp = [], []
+    first = 0
+    for n in ([kv_len] if chunk_lens is None else list(chunk_lens)):
+        npg = (n + P - 1) // P
+        pages = np.asarray(page_ids)[first:first + npg]
+        Kp.append(widen(np.asarray(k_pool_bits)[pages]).reshape(-1, q.shape[1])[:n])
+        Vp.append(widen(np.asarray(v_pool_bits)[pages]).reshape(-1, q.shape[1])[:n])
+        first += npg
+    K, V = np.concatenate(Kp), np.concatenate(Vp)
+    assert K.shape[0] == kv_len
     S = np.float64(np.float32(scale)) * (q @ K.T)
     i = (kv_len - q_len + np.arange(q_len))[:, None]
     j = np.arange(kv_len)[None, :]

@@ -21,8 +21,14 @@
  *        LOCAL : W(i) = S_sink U [max(0,i-w), i]   PAPER.md:219 (Sec. 4.2), with w = W - 1
  *                (W counts the keys INCLUDING the query's own position: reading A1; the paper's
  *                 example i=1000, w=256 -> 744..1000 is W = 257)
- *   3. for j in V(i), ascending: k_j = Kpool[pt[j / P]][j % P][:], v_j likewise;
+ *   3. for j in V(i), ascending: k_j = Kpool[pt[page(j)]][slot(j)][:], v_j likewise;
  *      s_j = scale * sum_d q_d k_{j,d}
+ *      A head's stream is the concatenation of its head segments, each mapped to its OWN consecutive virtual
+ *      pages ("T_seg maps each head segment (l, h, s) to the virtual pages"): with segment lengths
+ *      n_0, n_1, ... token j lies in the segment s with  t_s <= j < t_s + n_s  (t_s = n_0 + ... + n_{s-1}), at offset
+ *      o = j - t_s, so  page(j) = (ceil(n_0 / P) + ... + ceil(n_{s-1} / P)) + o / P  and  slot(j) = o % P.  A segment whose
+ *      length is not a multiple of P leaves the rest of its last page unused in mid-stream (ragged chunk tails,
+ *      SURVEY 8(f) NEXT #1).  Without a segment table the stream is one segment: page(j) = j / P, slot(j) = j % P.
  *   4. m = max_j s_j ; l = sum_j exp(s_j - m) ; p_j = exp(s_j - m) / l     (two passes)
  *   5. O[row][head][:] = sum_j p_j v_j ;  LSE[head][row] = m + ln l         (natural log of the
  *      SCALED scores: reading A6; pinned by the Q=0 closed form LSE = ln #V)
@@ -37,7 +43,9 @@
  * counts incl. the paper's i=1000 example, W=1 exactness, LOCAL(W>=kv_len) == GLOBAL, page
  * permutation / page size invariance, softmax row sums, constant-V, LSE merge identity
  * (PAPER.md:302), power-of-two scale, GQA == replicated MHA, poison, batch
- * independence / aliasing, torch fp64 causal SDPA at mid size.
+ * independence / aliasing, torch fp64 causal SDPA at mid size; the row_subset path against the full
+ * run (T13); the head-segment table against the brute force's own concatenation of segments, against the
+ * dense stream when every segment is a page multiple, and against a dense re-layout of the same tokens (T14).
  */
 #include <math.h>
 #include <stdint.h>
@@ -100,6 +108,23 @@ static int visible(int64_t j, int64_t i, int32_t head_class, int64_t W, int64_t 
     return 0;
 }
 
+/*
+ * Token j of a stream -> index of its (page, slot) in the stream's page table (step 3).
+ * seg_lens[0 .. n_seg) are the lengths of the stream's head segments (n_seg == 0: one segment, the whole stream).
+ * Returns page_index * P + slot.
+ */
+static int64_t locate(const int64_t *seg_lens, int64_t n_seg, int64_t P, int64_t j)
+{
+    if (n_seg == 0) return j;
+    int64_t t = 0, page0 = 0;
+    for (int64_t s = 0; s < n_seg; ++s) {
+        if (j < t + seg_lens[s]) return (page0 + (j - t) / P) * P + (j - t) % P;
+        t += seg_lens[s];
+        page0 += (seg_lens[s] + P - 1) / P;
+    }
+    return -1;   /* not reached: the segment lengths sum to kv_len (validated) */
+}
+
 /* position of row r inside the sorted subset, or -1 */
 static int64_t subset_find(const int64_t *subset, int64_t n, int64_t r)
 {
@@ -123,6 +148,9 @@ static int64_t subset_find(const int64_t *subset, int64_t n, int64_t r)
  * p_out (optional)   : [rows][Hq][p_stride] softmax probabilities p_j at index j (0 elsewhere is
  *                      the caller's job), rows indexed like out.
  * pairs_out (opt.)   : number of (query, key) pairs evaluated, summed over q heads.
+ * seg_offsets/seg_lens: head-segment table (optional; NULL = every stream is one segment): the segments of
+ *                      stream s are seg_lens[seg_offsets[s] .. seg_offsets[s+1]); they must sum to kv_lens[s] and
+ *                      the stream's page table must hold sum ceil(n / P) pages.
  */
 int oracle_attention(const oracle_shape_t *shape,
                      const uint16_t *k_pool, const uint16_t *v_pool, int64_t num_pages,
@@ -132,7 +160,8 @@ int oracle_attention(const oracle_shape_t *shape,
                      const uint16_t *q, int64_t q_row_stride, int64_t T, float scale_f32,
                      const int64_t *row_subset, int64_t n_subset,
                      double *out, double *lse, double *p_out, int64_t p_stride,
-                     int64_t *pairs_out)
+                     int64_t *pairs_out,
+                     const int64_t *seg_offsets, const int64_t *seg_lens)
 {
     const int64_t Hq = shape->num_q_heads, Hkv = shape->num_kv_heads;
     const int64_t D = shape->head_dim, P = shape->page_size;
@@ -153,8 +182,19 @@ int oracle_attention(const oracle_shape_t *shape,
         if (sg->n_sink < 0) return -7;
         if (sg->q_row_start < 0 || sg->q_row_start + sg->q_len > T) return -8;
         const int64_t npg = pt_offsets[sg->stream + 1] - pt_offsets[sg->stream];
-        if (npg * P < kv_len) return -9;
-        for (int64_t pg = 0; pg < (kv_len + P - 1) / P; ++pg) {
+        int64_t need_pages = (kv_len + P - 1) / P;
+        if (seg_offsets && seg_offsets[sg->stream + 1] > seg_offsets[sg->stream]) {
+            int64_t tot = 0;
+            need_pages = 0;
+            for (int64_t k = seg_offsets[sg->stream]; k < seg_offsets[sg->stream + 1]; ++k) {
+                if (seg_lens[k] < 1) return -11;
+                tot += seg_lens[k];
+                need_pages += (seg_lens[k] + P - 1) / P;
+            }
+            if (tot != kv_len) return -12;
+        }
+        if (npg < need_pages) return -9;
+        for (int64_t pg = 0; pg < need_pages; ++pg) {
             int32_t id = page_table[pt_offsets[sg->stream] + pg];
             if (id < 0 || id >= num_pages) return -10;
         }
@@ -165,6 +205,8 @@ int oracle_attention(const oracle_shape_t *shape,
         const oracle_segment_t *sg = &segs[s];
         const int64_t kv_len = kv_lens[sg->stream];
         const int32_t *pt = page_table + pt_offsets[sg->stream];
+        const int64_t *sl = seg_offsets ? seg_lens + seg_offsets[sg->stream] : NULL;
+        const int64_t n_sl = seg_offsets ? seg_offsets[sg->stream + 1] - seg_offsets[sg->stream] : 0;
         const int64_t units = (int64_t)sg->q_len * G;
         int64_t pairs_seg = 0;
 #pragma omp parallel for schedule(dynamic, 4) reduction(+ : pairs_seg)
@@ -189,7 +231,8 @@ int oracle_attention(const oracle_shape_t *shape,
             int64_t nvis = 0;
             for (int64_t j = 0; j <= i; ++j) {
                 if (!visible(j, i, sg->head_class, sg->window, sg->n_sink)) continue;
-                const uint16_t *kp = k_pool + ((int64_t)pt[j / P] * P + (j % P)) * D;
+                const int64_t u = locate(sl, n_sl, P, j);
+                const uint16_t *kp = k_pool + ((int64_t)pt[u / P] * P + (u % P)) * D;
                 double acc = 0.0;
                 for (int64_t d = 0; d < D; ++d) acc += qd[d] * bf16_to_f64(kp[d]);
                 sc[j] = scale * acc;
@@ -208,7 +251,8 @@ int oracle_attention(const oracle_shape_t *shape,
             for (int64_t j = 0; j <= i; ++j) {
                 if (!visible(j, i, sg->head_class, sg->window, sg->n_sink)) continue;
                 const double p = exp(sc[j] - m) / l;
-                const uint16_t *vp = v_pool + ((int64_t)pt[j / P] * P + (j % P)) * D;
+                const int64_t u = locate(sl, n_sl, P, j);
+                const uint16_t *vp = v_pool + ((int64_t)pt[u / P] * P + (u % P)) * D;
                 for (int64_t d = 0; d < D; ++d) op[d] += p * bf16_to_f64(vp[d]);
                 if (p_out && j < p_stride) p_out[(orow * Hq + head) * p_stride + j] = p;
             }

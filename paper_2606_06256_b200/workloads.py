@@ -13,6 +13,8 @@ Logical layouts handed to both sides (plain, row-major):
     q              : [T][Hq][D]        bf16      (per layer)
     stream         : (layer, kv_head, seq_id) -> kv_len, page_ids[ceil(kv_len/P)]
                      token j lives in page page_ids[j // P], slot j % P
+                     (a stream with chunk_lens is the concatenation of head segments, each starting on a
+                     fresh page: page_ids then holds sum ceil(n_s / P) pages and a segment's last page may be partial)
     segment        : (seq_id, kv_head, class, window W, n_sink, q_row_start, q_len)
 """
 from __future__ import annotations
@@ -39,6 +41,10 @@ class Stream:
     page_ids: np.ndarray            # int32 [ceil(kv_len / P)]
     n_shared_prefix_pages: int = 0  # leading pages that alias another stream's pages
     shared_from: Optional[Tuple[int, int, int]] = None  # (layer, kv_head, seq_id) of the owner
+    chunk_lens: Optional[List[int]] = None  # head segments (reused chunks), each on its own pages; None = one segment
+
+    def chunks(self) -> List[int]:
+        return [self.kv_len] if self.chunk_lens is None else list(self.chunk_lens)
 
 
 @dataclass
@@ -131,10 +137,26 @@ def q_values(w: Workload, layer: int, device="cpu") -> torch.Tensor:
 
 def stream_rows(pool: torch.Tensor, s: Stream, P: int, lo_page: int = 0) -> torch.Tensor:
     """Rows [n][D] of a stream's tokens starting at page index lo_page (plain gather, no arithmetic)."""
+    if s.chunk_lens is not None:
+        assert lo_page == 0
+        return torch.cat([chunk_rows(pool, s, P, c) for c in range(len(s.chunk_lens))])
     idx = torch.from_numpy(s.page_ids[lo_page:].astype(np.int64)).to(pool.device)
     rows = pool[idx].reshape(-1, pool.shape[-1])
     n = s.kv_len - lo_page * P
     return rows[:n].contiguous()
+
+
+def chunk_pages(s: Stream, P: int, c: int) -> np.ndarray:
+    """page ids of head segment c of a stream (each segment starts on a fresh page)."""
+    lens = s.chunks()
+    first = sum(_pages_for(n, P) for n in lens[:c])
+    return s.page_ids[first:first + _pages_for(lens[c], P)]
+
+
+def chunk_rows(pool: torch.Tensor, s: Stream, P: int, c: int) -> torch.Tensor:
+    """Rows [n_c][D] of head segment c of a stream."""
+    idx = torch.from_numpy(chunk_pages(s, P, c).astype(np.int64)).to(pool.device)
+    return pool[idx].reshape(-1, pool.shape[-1])[:s.chunks()[c]].contiguous()
 
 
 # ----------------------------------------------------------------------------------------------
@@ -151,6 +173,20 @@ def csr_page_tables(w: Workload, layer: int):
     kv_lens = np.array([s.kv_len for s in ss], dtype=np.int64)
     index = {(s.kv_head, s.seq_id): i for i, s in enumerate(ss)}
     return table, offs, kv_lens, index
+
+
+def csr_segment_tables(w: Workload, layer: int):
+    """Head-segment table of the layer's streams (same stream order as csr_page_tables): (seg_offsets int64 [n+1],
+    seg_lens int64), or (None, None) when every stream is a single segment."""
+    ss = w.layer_streams(layer)
+    if all(s.chunk_lens is None for s in ss):
+        return None, None
+    offs = np.zeros(len(ss) + 1, dtype=np.int64)
+    lens: List[int] = []
+    for i, s in enumerate(ss):
+        lens += s.chunks()
+        offs[i + 1] = len(lens)
+    return offs, np.array(lens, dtype=np.int64)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -195,15 +231,21 @@ def make_workload(name: str, *, Hq: int, Hkv: int, D: int, P: int, requests, see
                   identity_pages: bool = False) -> Workload:
     """Generic builder used by the tests.
 
-    requests: list of dicts {kv_len, heads: {kv_head: (class, W, n_sink, q_len)}}; each request's
-    q rows are packed consecutively, q_row_start shared by its heads; a head with a shorter q_len
-    takes the LAST q_len rows of the request's row range (bottom-right).
+    requests: list of dicts {kv_len, heads: {kv_head: (class, W, n_sink, q_len)}[, chunks: [n_0, n_1, ...]]}; each
+    request's q rows are packed consecutively, q_row_start shared by its heads; a head with a shorter q_len
+    takes the LAST q_len rows of the request's row range (bottom-right).  "chunks" (summing to
+    kv_len) makes every stream of the request a concatenation of head segments of those lengths, each on its own
+    pages (reused chunks of arbitrary length: ragged chunk tails).
     """
     rng = np.random.default_rng(seed)
+
+    def npages(r):
+        return sum(_pages_for(n, P) for n in r["chunks"]) if "chunks" in r else _pages_for(r["kv_len"], P)
     n_live = 0
     for _ in range(num_layers):
         for r in requests:
-            n_live += len(r["heads"]) * _pages_for(r["kv_len"], P)
+            assert "chunks" not in r or sum(r["chunks"]) == r["kv_len"]
+            n_live += len(r["heads"]) * npages(r)
     num_pages = max(1, int(math.ceil(pool_factor * n_live)))
     place = np.arange(n_live, dtype=np.int32) if identity_pages else _place(rng, n_live, num_pages)
     streams, segments, T = [], [], []
@@ -213,8 +255,9 @@ def make_workload(name: str, *, Hq: int, Hkv: int, D: int, P: int, requests, see
         for sid, r in enumerate(requests):
             qmax = max(h[3] for h in r["heads"].values())
             for kvh, (cls, W, n_sink, q_len) in sorted(r["heads"].items()):
-                npg = _pages_for(r["kv_len"], P)
-                streams.append(Stream(layer, kvh, sid, r["kv_len"], place[cur:cur + npg].copy()))
+                npg = npages(r)
+                streams.append(Stream(layer, kvh, sid, r["kv_len"], place[cur:cur + npg].copy(),
+                                      chunk_lens=list(r["chunks"]) if "chunks" in r else None))
                 cur += npg
                 segments.append(Segment(layer, sid, kvh, cls, W, n_sink, row + qmax - q_len, q_len))
             row += qmax

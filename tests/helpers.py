@@ -25,10 +25,11 @@ def run_oracle(w: wl.Workload, layer, k_pool, v_pool, q, row_subset=None, want_p
     segs = segments if segments is not None else w.layer_segments(layer)
     tup = [(index[(s.kv_head, s.seq_id)], s.kv_head, s.head_class, s.window, s.n_sink,
             s.q_row_start, s.q_len) for s in segs]
+    seg_offsets, seg_lens = wl.csr_segment_tables(w, layer)
     return oracle.oracle_attention(Hq=w.Hq, Hkv=w.Hkv, D=w.D, P=w.P, k_pool=k_pool, v_pool=v_pool,
                                    page_table=table, pt_offsets=offs, kv_lens=kv_lens, segments=tup,
                                    q=q, T=w.T[layer], scale=w.scale, row_subset=row_subset,
-                                   want_p=want_p)
+                                   want_p=want_p, seg_offsets=seg_offsets, seg_lens=seg_lens)
 
 
 def covered_mask(w: wl.Workload, layer, rows=None) -> np.ndarray:

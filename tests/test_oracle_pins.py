@@ -12,6 +12,8 @@ T9  GQA == replicated MHA (contiguous groups)
 T10 poison: non-visible K/V never enter the softmax
 T11 batch independence and page-table aliasing
 T12 library special case: torch fp64 causal SDPA at mid size
+T13 the row_subset path equals the full run bit for bit
+T14 head-segment table (ragged chunk tails): brute force, page-multiple split == dense, dense re-layout
 """
 import math
 import os
@@ -378,6 +380,96 @@ def test_T13_row_subset_equals_full_run_bit_for_bit(P):
     allr = run_oracle(w, 0, k, v, q, row_subset=np.arange(T)[::-1].copy(), want_p=67)
     assert np.array_equal(allr.out, full.out, equal_nan=True) and np.array_equal(allr.lse, full.lse, equal_nan=True)
     assert allr.pairs == full.pairs
+
+
+# ------------------------------------------------------------------- head-segment table (T14)
+RAGGED_CHUNKS = [
+    # (P, chunk lengths): tails of every size, single-token segments, a segment of exactly one page, many segments per block
+    (4, [5, 3, 1, 8, 2, 7, 6]),
+    (4, [4, 4, 9, 1, 1, 1]),
+    (16, [17, 1, 30, 16, 3]),
+    (16, [1, 66]),
+]
+
+
+@pytest.mark.parametrize("case", range(len(RAGGED_CHUNKS)))
+def test_T14_segment_table_against_bruteforce_concatenation(case):
+    """A stream made of head segments, each on its own consecutive pages: the oracle locates token j
+    through the segment table; the brute force concatenates the segments' rows into a dense stream first.  All
+    classes / windows / sinks of the T1 grid that matter at a tail: windows that end, start and straddle a ragged tail."""
+    P, chunks = RAGGED_CHUNKS[case]
+    kv_len = sum(chunks)
+    worst = 0.0
+    for q_len in sorted({1, kv_len // 2, kv_len}):
+        for W in sorted({1, 2, P, P + 1, chunks[-1], chunks[-1] + 1, kv_len}):
+            for n_sink in (0, 3, chunks[0] + 1):
+                w = tiny(0, None, P=P, seed=300 + case, requests=[
+                    {"kv_len": kv_len, "chunks": chunks, "heads": {0: (GLOBAL, 0, 0, q_len), 1: (LOCAL, W, n_sink, q_len)}}])
+                k, v, q = values(w)
+                res = run_oracle(w, 0, k, v, q, want_p=kv_len)
+                sm = w.stream_map()
+                for s in w.segments:
+                    st = sm[(0, s.kv_head, 0)]
+                    assert len(st.page_ids) == sum((n + P - 1) // P for n in chunks) > (kv_len + P - 1) // P - 1
+                    for g in range(w.G):
+                        h = s.kv_head * w.G + g
+                        qb = bits(q)[s.q_row_start:s.q_row_start + s.q_len, h]
+                        O, L, p = bruteforce.dense_masked_attention(qb, bits(k), bits(v), st.page_ids, kv_len, P, s.head_class,
+                                                                   s.window, s.n_sink, w.scale, chunk_lens=chunks)
+                        rows = slice(s.q_row_start, s.q_row_start + s.q_len)
+                        worst = max(worst, np.abs(res.out[rows, h] - O).max(), np.abs(res.lse[h, rows] - L).max(),
+                                    np.abs(res.p[rows, h, :kv_len] - p).max())
+    assert worst < 1e-12, worst
+
+
+def test_T14_page_multiple_segments_equal_the_dense_stream():
+    """Splitting a stream into segments at page multiples changes nothing: same page table, same tokens -> the oracle
+    must return the dense stream's result bit for bit (the segment table then only restates j -> page j / P)."""
+    P = 4
+    heads = {0: (GLOBAL, 0, 0, 40), 1: (LOCAL, 7, 2, 25)}
+    wd = tiny(40, heads, P=P, seed=9)
+    ws = tiny(0, None, P=P, seed=9, requests=[{"kv_len": 40, "chunks": [8, 4, 16, 12], "heads": heads}])
+    assert all(np.array_equal(a.page_ids, b.page_ids) for a, b in zip(wd.streams, ws.streams))
+    k, v, q = values(wd)
+    a = run_oracle(wd, 0, k, v, q, want_p=40)
+    b = run_oracle(ws, 0, k, v, q, want_p=40)
+    assert np.array_equal(a.out, b.out, equal_nan=True) and np.array_equal(a.lse, b.lse, equal_nan=True) and np.array_equal(a.p, b.p)
+    assert a.pairs == b.pairs
+
+
+def test_T14_ragged_layout_equals_dense_relayout_and_ignores_the_tails():
+    """The same tokens stored (a) as ragged segments and (b) densely in another pool give bit-identical results, and
+    the unused slots after a segment's tail never enter the softmax (poisoned with NaN / 1e30)."""
+    P, chunks = 16, [17, 1, 30, 16, 3]
+    kv_len = sum(chunks)
+    heads = {0: (GLOBAL, 0, 0, kv_len), 1: (LOCAL, 20, 2, 40)}
+    wr = tiny(0, None, P=P, seed=21, requests=[{"kv_len": kv_len, "chunks": chunks, "heads": heads}])
+    wdn = tiny(kv_len, heads, P=P, seed=22)
+    kr, vr, q = values(wr)
+    kd, vd = torch.zeros((wdn.num_pages, P, wr.D), dtype=torch.bfloat16), torch.zeros((wdn.num_pages, P, wr.D), dtype=torch.bfloat16)
+    for sr, sd in zip(wr.streams, wdn.streams):
+        rows_k, rows_v = wl.stream_rows(kr, sr, P), wl.stream_rows(vr, sr, P)
+        assert rows_k.shape[0] == kv_len
+        for j in range(kv_len):
+            kd[int(sd.page_ids[j // P]), j % P] = rows_k[j]
+            vd[int(sd.page_ids[j // P]), j % P] = rows_v[j]
+    a = run_oracle(wr, 0, kr, vr, q, want_p=kv_len)
+    b = run_oracle(wdn, 0, kd, vd, q, want_p=kv_len)
+    assert np.array_equal(a.out, b.out, equal_nan=True) and np.array_equal(a.lse, b.lse, equal_nan=True) and np.array_equal(a.p, b.p)
+    # poison the dead slots behind every segment's tail
+    kp, vp = kr.clone(), vr.clone()
+    for s in wr.streams:
+        for c, n in enumerate(chunks):
+            if n % P:
+                last = int(wl.chunk_pages(s, P, c)[-1])
+                kp[last, n % P:] = float("nan")
+                vp[last, n % P:] = 1e30
+    c2 = run_oracle(wr, 0, kp, vp, q, want_p=kv_len)
+    assert np.array_equal(a.out, c2.out, equal_nan=True) and np.array_equal(a.lse, c2.lse, equal_nan=True)
+    # a segment table that does not add up is rejected
+    wr.streams[0].chunk_lens = [17, 1, 30, 16, 4]
+    with pytest.raises(ValueError):
+        run_oracle(wr, 0, kr, vr, q)
 
 
 # ------------------------------------------------------------------------------------ rejections
