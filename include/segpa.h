@@ -23,11 +23,15 @@
  *
  * Terms
  *   stream   = (layer, kv_head, seq_id): the ordered tokens of ONE KV head of one request, of
- *              length kv_len, backed by ceil(kv_len / page_size) physical pages; token j lives in
- *              page pt[j / page_size], slot j % page_size.  It is the concatenation of the paper's
- *              head segments (l, h, s), each mapped to consecutive virtual pages by T_seg and to
- *              physical pages by T_page; here virtual page v of a stream is simply
- *              index v of its page table.
+ *              length kv_len.  It is the concatenation of the paper's head segments (l, h, s), each
+ *              mapped to its own consecutive virtual pages by T_seg and to physical pages by T_page
+ *              (PAPER.md:235); virtual page v of a stream is index v of its page table.  A stream
+ *              written by COPY appends alone is ONE head segment: token j lives in page
+ *              pt[j / page_size], slot j % page_size.  Every ATTACH adds a head segment that starts on
+ *              a fresh page (so does the first COPY after one): a segment whose length is not a multiple
+ *              of page_size leaves the rest of its last page unused in mid-stream ("ragged chunk
+ *              tail"), and the page table holds sum ceil(n_s / page_size) pages.  Token indices,
+ *              positions and windows never see those unused slots.
  *   segment  = execution segment: one (request, KV head) unit of a layer's attention call, i.e.
  *              one tuple (h, B_h, |U_h|, p) of the per-layer varlen metadata M_l,
  *              plus its query rows.
@@ -96,16 +100,21 @@ segpa_status_t segpa_create_cache(const segpa_cache_desc_t *desc, segpa_cache_t 
  *
  *  - COPY mode (k_src and v_src non-NULL): device bf16 rows; row t of the new tokens is at
  *    k_src + t * src_row_stride_elems (D contiguous elements).  Rows are scattered into the
- *    stream's pages by a kernel on cuda_stream.  If the stream's last page is partial the new
- *    tokens first fill it; further pages are taken from page_ids (host int32, in order,
- *    n_page_ids of them, each must be free) or, if page_ids == NULL, from the allocator.
+ *    stream's pages by a kernel on cuda_stream.  If the stream's last page is partial, was started
+ *    by a COPY append of this stream and is referenced by no other stream, the new tokens first fill
+ *    it; otherwise (the last head segment was attached, or another stream has attached that page)
+ *    they start a new head segment on a fresh page and the partial page keeps its unused slots.
+ *    Further pages are taken from page_ids (host int32, in order, n_page_ids of them = the number
+ *    of pages the new tokens start, each must be free) or, if page_ids == NULL, from the allocator.
  *    Slots of a newly started page beyond the stream's end are zero-filled (masked probabilities
  *    multiply them, so they must stay finite).
  *  - ATTACH mode (k_src == v_src == NULL, page_ids non-NULL): the pages already hold the data
  *    (filled earlier through another stream); they are appended to this stream's page table
  *    without copying and their reference count is incremented.  This is both PIC chunk splicing
  *    ("directly reusing the prefix-robust local segments") and shared-prefix
- *    aliasing.  Requires the stream's current length to be a multiple of page_size, and
+ *    aliasing.  The attached tokens are a head segment of their own: they start on a fresh page
+ *    whatever the stream's current length, n_tokens may be any length >= 1 (a reused chunk need not
+ *    be a multiple of page_size; only the first n_tokens slots of the pages belong to the stream) and
  *    n_page_ids == ceil(n_tokens / page_size).  On a planning-only cache pages may be attached
  *    without ever having been filled.
  *
@@ -378,7 +387,8 @@ segpa_status_t segpa_segments_mass_layout(const segpa_segments_t *segs, int64_t 
  * with the same segments; the probabilities are recomputed on the tensor cores (S^T = K Q^T per 128-key block),
  * they are never stored.  Entries of keys no query sees, and the padding up to the next multiple of 128, are 0.
  * mass: device fp32 with at least offsets[n] entries.  Asynchronous on cuda_stream; deterministic.
- * Errors: INVALID, STATE (planning-only cache, foreign or stale segments), OOM, CUDA.
+ * Errors: INVALID, STATE (planning-only cache, foreign or stale segments), UNSUPPORTED (a segment's stream has
+ * ragged chunk tails: the mass kernel works on single-segment streams), OOM, CUDA.
  */
 segpa_status_t segpa_attention_mass(segpa_cache_t *cache, const segpa_segments_t *segs, const void *q,
                                     int64_t q_row_stride_elems, float softmax_scale, const float *lse,

@@ -107,7 +107,9 @@ struct TileRange {
 // visits the sink blocks first and then its window blocks (two KV block ranges per item); when the two
 // ranges touch they are merged into one and the gap is masked per element.  In a strided item tile 0 takes
 // the sink blocks.
-__device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev& sg, int tile, int TT, int G) {
+// KV blocks, pages and the 64-key halves below are all in SLOT space (head segments start on fresh pages, so
+// a ragged stream has unused slots behind a segment's tail; slot = token for a dense stream), positions in token space.
+__device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev& sg, const PadDev* __restrict__ pads, int tile, int TT, int G) {
     TileRange r;
     const bool strided = (it.flags & 1) != 0;
     const int tok_lo = it.t0 + (strided ? 0 : tile * TT);
@@ -118,11 +120,18 @@ __device__ __forceinline__ TileRange tile_range(const ItemDev& it, const SegDev&
     r.step = 1;
     if (r.n_rows == 0) return r;
     const int i0 = sg.kv_len - sg.q_len + tok_lo, i1 = sg.kv_len - sg.q_len + tok_hi - 1;
-    r.lo64 = max(it.kb_lo * 2, max(0, i0 - sg.window + 1) / kHalfKeys);
-    r.hi64 = min(it.kb_hi * 2, i1 / kHalfKeys + 1);
+    // slots of the first and the last key the tile's rows see, and of its last sink key
+    // (ragged stream: looked up by the host, ItemDev::slots; a strided item's two tile slots hold the same rows)
+    int3 sl = make_int3(max(0, i0 - sg.window + 1), i1, min(sg.n_sink, i1 + 1) - 1);
+    if (sg.n_pads > 0) {   // (selects, not an indexed access: `it` must stay in registers)
+        const bool first = strided || tile == 0;
+        sl = make_int3(first ? it.slots[0][0] : it.slots[1][0], first ? it.slots[0][1] : it.slots[1][1], first ? it.slots[0][2] : it.slots[1][2]);
+    }
+    r.lo64 = max(it.kb_lo * 2, sl.x / kHalfKeys);
+    r.hi64 = min(it.kb_hi * 2, sl.y / kHalfKeys + 1);
     if (r.hi64 < r.lo64) r.hi64 = r.lo64;
     if (sg.n_sink > 0 && it.kb_lo == 0) {
-        r.sink64 = (min(sg.n_sink, i1 + 1) + kHalfKeys - 1) / kHalfKeys;
+        r.sink64 = (sl.z + 1 + kHalfKeys - 1) / kHalfKeys;
         r.sb = (r.sink64 + 1) >> 1;
         if (r.hi64 > r.lo64 && r.sb >= (r.lo64 >> 1)) { r.lo64 = 0; r.sink64 = r.sb = 0; }   // ranges touch: merge
         if (strided && tile != 0) r.sink64 = r.sb = 0;
@@ -157,12 +166,12 @@ __device__ __forceinline__ int half_mask(const TileRange& r, int j) {
 // [0, sb) followed by window blocks [lo, hi) (one range [0, hi) when they touch).
 struct ItemBlocks { int sb, lo, hi; };
 template <int NT>
-__device__ __forceinline__ ItemBlocks item_blocks(const ItemDev& it, const SegDev& sg, int TT, int G) {
+__device__ __forceinline__ ItemBlocks item_blocks(const ItemDev& it, const SegDev& sg, const PadDev* __restrict__ pads, int TT, int G) {
     ItemBlocks b;
     b.sb = 0; b.lo = INT_MAX; b.hi = 0;
 #pragma unroll
     for (int t = 0; t < NT; ++t) {
-        const TileRange tr = tile_range(it, sg, t, TT, G);
+        const TileRange tr = tile_range(it, sg, pads, t, TT, G);
         if (tr.n_rows == 0) continue;
         b.sb = max(b.sb, tr.sb);
         if (tr.hi > tr.lo) { b.lo = min(b.lo, tr.lo); b.hi = max(b.hi, tr.hi); }
@@ -174,7 +183,9 @@ __device__ __forceinline__ ItemBlocks item_blocks(const ItemDev& it, const SegDe
 
 }  // namespace
 
-template <int D, int NT>
+// RG: the plan has ragged streams (head segments with partial last pages in mid-stream).  The dense
+// instantiation carries none of that code: inlined into the softmax loop it cost cfg2 3 % even when never taken.
+template <int D, int NT, bool RG>
 __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_constant__ FwdParams p) {
     using C = Cfg<D, NT>;
     extern __shared__ uint8_t smem_raw[];
@@ -238,7 +249,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         for (int ii = i_lo; ii < i_hi; ++ii) {
             const ItemDev it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
-            const ItemBlocks ib = item_blocks<NT>(it, sg, TT, G);
+            const ItemBlocks ib = item_blocks<NT>(it, sg, p.pads, TT, G);
             const int n_steps = ib.sb + ib.hi - ib.lo;
             // page ids are fetched one block ahead: the dependent global load of the next block is in flight
             // while this block's copies are issued (decode-shaped items consume a block every ~1500 cycles)
@@ -401,9 +412,9 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             if (!flush) {
                 const ItemDev it = p.items[ii];
                 const SegDev sg = p.segs[it.seg];
-                ib = item_blocks<NT>(it, sg, TT, G);
+                ib = item_blocks<NT>(it, sg, p.pads, TT, G);
 #pragma unroll
-                for (int t = 0; t < NT; ++t) tr[t] = tile_range(it, sg, t, TT, G);
+                for (int t = 0; t < NT; ++t) tr[t] = tile_range(it, sg, p.pads, t, TT, G);
 #pragma unroll
                 for (int t = 0; t < NT; ++t)
                     if (tr[t].n_rows > 0 && !has_blocks(tr[t])) {
@@ -436,7 +447,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                 const SegDev sgn = p.segs[itn.seg];
 #pragma unroll
                 for (int t = 0; t < NT; ++t) {
-                    const TileRange trn = tile_range(itn, sgn, t, TT, G);
+                    const TileRange trn = tile_range(itn, sgn, p.pads, t, TT, G);
                     if (trn.n_rows == 0) continue;
 #pragma unroll
                     for (int h = 0; h < C::kHalves; ++h)
@@ -446,7 +457,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             __syncwarp();
 #pragma unroll
             for (int t = 0; t < NT; ++t) {
-                const TileRange tr = tile_range(it, sg, t, TT, G);
+                const TileRange tr = tile_range(it, sg, p.pads, t, TT, G);
                 if (tr.n_rows == 0) continue;
                 TRACE(40, t);
                 mbar_wait(smem_u32(&bars.q_empty[t]), (n_fill[t] & 1) ^ 1);   // last QK^T on the old Q is done
@@ -477,7 +488,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             for (int ii = i_lo; ii < i_hi; ++ii) {
                 const ItemDev it = p.items[ii];
                 const SegDev sg = p.segs[it.seg];
-                const TileRange tr = tile_range(it, sg, tile, TT, G);
+                const TileRange tr = tile_range(it, sg, p.pads, tile, TT, G);
                 if (tr.n_rows == 0) continue;
 
                 const int rc = min(r, tr.n_rows - 1);            // rows past the end mirror the last valid row
@@ -500,11 +511,27 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                     tc_fence_after();
                     TRACE(21, j);
                     if (warp_has_rows) {
+                        // Column c of block j is slot 128 j + c.  In a dense stream that is token 128 j + c; in a ragged one
+                        // (head segments on their own pages) the block either lies inside one head segment
+                        // (token = slot - pad, same form) or holds a segment tail: unused slots and a change of pad (ragged_blk)
+                        int tokb = j * kBlockKeys;      // token of column 0
+                        bool ragged_blk = false;
+                        if (RG && sg.n_pads > 0) {
+                            int padv = 0, prev = 0;
+                            for (int k = 0; k < sg.n_pads; ++k) {
+                                const PadDev pd = p.pads[sg.pad_off + k];
+                                const int seg0 = pd.tok + pd.pad, tail = pd.tok + prev;   // unused slots [tail, seg0)
+                                if (seg0 <= j * kBlockKeys) padv = pd.pad;
+                                else if (tail < (j + 1) * kBlockKeys) ragged_blk = true;
+                                prev = pd.pad;
+                            }
+                            tokb -= padv;
+                        }
                         // visible columns of this block: c <= cmax and (c >= cmin or c < csink)
-                        const int cmin = key_lo - j * kBlockKeys, cmax = pos - j * kBlockKeys;
-                        const int csink = sg.n_sink - j * kBlockKeys;        // same for every row of the segment
-                        const int mn_cmin = klo_w0 - j * kBlockKeys, mx_cmin = klo_w1 - j * kBlockKeys;   // over the warp's rows
-                        const int mn_cmax = pos_w0 - j * kBlockKeys, mx_cmax = pos_w1 - j * kBlockKeys;
+                        const int cmin = key_lo - tokb, cmax = pos - tokb;
+                        const int csink = sg.n_sink - tokb;        // same for every row of the segment
+                        const int mn_cmin = klo_w0 - tokb, mx_cmin = klo_w1 - tokb;   // over the warp's rows
+                        const int mn_cmax = pos_w0 - tokb, mx_cmax = pos_w1 - tokb;
                         const bool need_mask = mn_cmax < kBlockKeys - 1 || (mx_cmin > 0 && csink < kBlockKeys);
                         // the whole score row of this thread: 128 fp32 columns -> registers, one wait
                         uint32_t s[kBlockKeys];
@@ -513,7 +540,43 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
                         tmem_wait_ld();
                         TRACE(22, j);
                         bool dead[4] = {false, false, false, false};   // 32-column chunk masked for every row of the warp
-                        if (need_mask) {
+                        if (RG && ragged_blk) {
+                            // The block holds the tail of a head segment.  Visible columns as a 128-bit set, built from
+                            // intervals: for every head segment that reaches into the block, its columns [ra, rb) hold the
+                            // tokens c + off; of those, the window [key_lo, pos] and the sinks [0, n_sink) are visible.
+                            uint32_t vis[4] = {0u, 0u, 0u, 0u};
+                            auto add_bits = [&vis](int a, int b) {
+#pragma unroll
+                                for (int w = 0; w < 4; ++w) {
+                                    const int lo = min(max(a - 32 * w, 0), 32), hi = min(max(b - 32 * w, 0), 32);
+                                    if (hi > lo) vis[w] |= (hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
+                                }
+                            };
+                            const int B = j * kBlockKeys;
+                            int start = 0, pad_c = 0;
+                            for (int k = 0; k <= sg.n_pads; ++k) {
+                                int end = INT_MAX, nstart = 0, npad = 0;
+                                if (k < sg.n_pads) {
+                                    const PadDev pd = p.pads[sg.pad_off + k];
+                                    end = pd.tok + pad_c;
+                                    nstart = pd.tok + pd.pad;
+                                    npad = pd.pad;
+                                }
+                                const int ra = max(start, B) - B, rb = min(end, B + kBlockKeys) - B;
+                                if (ra < rb) {
+                                    const int off = B - pad_c;
+                                    add_bits(max(ra, key_lo - off), min(rb, pos - off + 1));
+                                    add_bits(ra, min(rb, min(sg.n_sink, pos + 1) - off));
+                                }
+                                start = nstart;
+                                pad_c = npad;
+                            }
+#pragma unroll
+                            for (int c = 0; c < 4; ++c) dead[c] = __all_sync(0xffffffffu, vis[c] == 0u);
+#pragma unroll
+                            for (int e = 0; e < kBlockKeys; ++e)
+                                if (!((vis[e >> 5] >> (e & 31)) & 1u)) s[e] = 0xff800000u;   // -inf
+                        } else if (need_mask) {
                             // boundary block (causal diagonal / window edge / sink edge).  Per 32-column chunk, warp-uniformly:
                             // all visible -> untouched; all masked -> no exp at all; ragged -> element mask in registers
                             if (sg.n_sink == 0) {
@@ -643,7 +706,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
             const SegDev sg = p.segs[it.seg];
 #pragma unroll 1
             for (int tile = 0; tile < NT; ++tile) {
-                const TileRange tr = tile_range(it, sg, tile, TT, G);
+                const TileRange tr = tile_range(it, sg, p.pads, tile, TT, G);
                 if (tr.n_rows == 0) continue;
                 const uint32_t tO = tmem + lane_base + 256 + tile * 128;
                 const bool has_blk = has_blocks(tr);
@@ -741,7 +804,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int D, int NT>
+template <int D, int NT, bool RG>
 static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
     using C = Cfg<D, NT>;
     // the opt-in to > 48 KB of dynamic shared memory is per device: remember which devices have it
@@ -749,17 +812,21 @@ static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
     int dev = 0;
     cudaGetDevice(&dev);
     if (dev < 0 || dev >= 64 || !configured[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<D, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<D, NT, RG>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    return launch_pdl(attention_tc_kernel<D, NT>, dim3((unsigned)p.n_cta), dim3(kThreads), (size_t)C::kSmemBytes, st, p);
+    return launch_pdl(attention_tc_kernel<D, NT, RG>, dim3((unsigned)p.n_cta), dim3(kThreads), (size_t)C::kSmemBytes, st, p);
 }
 
 cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st) {
     if (p.n_items == 0) return cudaSuccess;
-    if (p.tiles_per_item == 2) return p.D == 128 ? launch_one<128, 2>(p, st) : launch_one<64, 2>(p, st);
-    return p.D == 128 ? launch_one<128, 1>(p, st) : launch_one<64, 1>(p, st);
+    if (p.has_ragged) {
+        if (p.tiles_per_item == 2) return p.D == 128 ? launch_one<128, 2, true>(p, st) : launch_one<64, 2, true>(p, st);
+        return p.D == 128 ? launch_one<128, 1, true>(p, st) : launch_one<64, 1, true>(p, st);
+    }
+    if (p.tiles_per_item == 2) return p.D == 128 ? launch_one<128, 2, false>(p, st) : launch_one<64, 2, false>(p, st);
+    return p.D == 128 ? launch_one<128, 1, false>(p, st) : launch_one<64, 1, false>(p, st);
 }
 
 }  // namespace segpa

@@ -47,9 +47,25 @@ struct StreamKeyHash {
         return (size_t)h;
     }
 };
+// Head segments: a stream is the concatenation of head segments, each on its own consecutive
+// pages, so a segment whose length is not a multiple of P leaves unused slots behind its tail in mid-stream.  The
+// stream is kept in SLOT space (slot = page index * P + slot in page): token j sits at slot j + pad(j), where pad(j)
+// is the cumulative number of unused slots before j's segment.  Only the points where the padding grows are stored.
+struct PadPoint {
+    int64_t tok;   // first token of a head segment that starts on a fresh page after a partial one
+    int64_t pad;   // unused slots before it, cumulative: tokens >= tok (up to the next point) sit at slot tok' + pad
+};
 struct StreamRec {
     std::vector<int32_t> pages;
     int64_t kv_len = 0;
+    std::vector<PadPoint> pads;   // ascending; empty = the stream is dense (token j in page j / P, slot j % P)
+    bool tail_open = false;       // the partial last page was started by a COPY append of this stream (it may be filled further)
+    int64_t slot_len() const { return kv_len + (pads.empty() ? 0 : pads.back().pad); }
+    int64_t slot_of(int64_t tok) const {
+        int64_t pad = 0;
+        for (const PadPoint& pp : pads) { if (pp.tok <= tok) pad = pp.pad; else break; }
+        return tok + pad;
+    }
     // append_pages_batch: index of this stream's last COPY job in the batch with stamp `batch_stamp`
     uint64_t batch_stamp = 0;
     int32_t batch_job = -1;
@@ -170,9 +186,11 @@ struct segpa_segments {
     struct ItemMeta { int32_t tile; int32_t split; int32_t n_splits; };
     std::vector<ItemMeta> item_meta;   // per item (same order as items): what segpa_segments_items reports besides ItemDev
     std::vector<int32_t> pages;
+    std::vector<PadDev> pads;       // token -> slot maps of the ragged streams among the segments
     std::vector<CombDev> combs;
     std::vector<int32_t> cta_off;   // items of CTA q: [cta_off[q], cta_off[q+1])
     std::vector<int64_t> mass_off;  // [n + 1]: layout of the attention-mass array (kv_len rounded up to 128 per segment)
+    bool has_ragged = false;             // some segment's stream has head segments with partial last pages
     mutable bool mass_planned = false;   // mass plan built and uploaded (lazily, by the first segpa_attention_mass)
     mutable int mass_n_cta = 0;
     mutable size_t m_off_items = 0, m_off_cta = 0, m_off_layout = 0, m_off_kvlen = 0;
@@ -191,20 +209,20 @@ struct segpa_segments {
     // device
     SegBuf* buf = nullptr;
     mutable cudaStream_t last_stream = nullptr;   // stream of the last upload / attention_fwd
-    size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0, off_cta = 0;
+    size_t off_segs = 0, off_items = 0, off_pages = 0, off_combs = 0, off_cta = 0, off_pads = 0;
 
     // back to the state of a fresh object, keeping the vectors' storage (objects are recycled through the
     // cache: a plan is built on the critical path of every layer and must not go through malloc / page faults)
     void reset() {
         cache = nullptr; layer = 0;
-        reqs.clear(); segs.clear(); items.clear(); item_meta.clear(); pages.clear(); combs.clear(); cta_off.clear(); mass_off.clear();
-        mass_planned = false; mass_n_cta = 0;
+        reqs.clear(); segs.clear(); items.clear(); item_meta.clear(); pages.clear(); pads.clear(); combs.clear(); cta_off.clear(); mass_off.clear();
+        mass_planned = false; mass_n_cta = 0; has_ragged = false;
         hchunks.clear(); host_planned = false;
         m_off_items = m_off_cta = m_off_layout = m_off_kvlen = 0;
         stats = segpa_plan_stats_t{};
         tiles_per_item = 1;
         buf = nullptr; last_stream = nullptr;
-        off_segs = off_items = off_pages = off_combs = off_cta = 0;
+        off_segs = off_items = off_pages = off_combs = off_cta = off_pads = 0;
     }
 };
 
@@ -345,6 +363,23 @@ inline int64_t visible_pairs(int64_t i0, int64_t i1, int64_t W) {
 
 namespace {
 
+// Cuts the token range [t0, t0 + n) of a stream at its head-segment boundaries: f(tok_lo, n_piece, slot_lo) for
+// every maximal piece whose tokens are consecutive in slot space.
+template <class F>
+void for_each_piece(const StreamRec& rec, int64_t t0, int64_t n, F f) {
+    int64_t t = t0;
+    const int64_t end = t0 + n;
+    size_t k = 0;
+    int64_t pad = 0;
+    while (k < rec.pads.size() && rec.pads[k].tok <= t) pad = rec.pads[k++].pad;
+    while (t < end) {
+        const int64_t stop = (k < rec.pads.size()) ? std::min(end, rec.pads[k].tok) : end;
+        f(t, stop - t, t + pad);
+        t = stop;
+        if (k < rec.pads.size() && rec.pads[k].tok <= t) pad = rec.pads[k++].pad;
+    }
+}
+
 // LPT: items by descending cost, each given to the least-loaded CTA of the persistent grid;
 // a CTA's items stay in descending order.  Cost = visited blocks + a fixed per-item term (pipeline refill, Q load,
 // epilogue: about 0.6 block-times measured), in thirds of a block.  Reorders `items` (and `meta`, if given) CTA by
@@ -423,6 +458,7 @@ void fill_fwd_params(FwdParams& p, const segpa_cache* c, const segpa_segments* s
     p.segs = (const SegDev*)(d_blob + s->off_segs);
     p.items = (const ItemDev*)(d_blob + s->off_items);
     p.pages = (const int*)(d_blob + s->off_pages);
+    p.pads = (const PadDev*)(d_blob + s->off_pads);
     p.combs = (const CombDev*)(d_blob + s->off_combs);
     p.cta_off = (const int*)(d_blob + s->off_cta);
     p.n_cta = (int)s->cta_off.size() - 1;
@@ -444,6 +480,7 @@ void fill_fwd_params(FwdParams& p, const segpa_cache* c, const segpa_segments* s
     p.tiles_per_item = s->tiles_per_item;
     p.page_bytes = c->page_bytes;
     p.num_sms = c->num_sms;
+    p.has_ragged = s->has_ragged ? 1 : 0;
 }
 
 }  // namespace
@@ -571,7 +608,7 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
     const int P = c->desc.page_size, D = c->desc.head_dim;
 
     // Requests are applied to the host state in order; `undo` lets a later failure restore it exactly.
-    struct Undo { StreamKey key; bool created; int64_t old_len; size_t n_new; };
+    struct Undo { StreamKey key; bool created; int64_t old_len; size_t n_new; size_t old_pads; bool old_tail_open; };
     std::vector<Undo> undo;
     std::vector<ScatterJob> jobs;
     std::vector<int32_t>& touched = c->append_touched;     // page ids the scatter kernel indexes, job after job
@@ -618,6 +655,8 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 rec.pages.pop_back();
             }
             rec.kv_len = undo[u].old_len;
+            rec.pads.resize(undo[u].old_pads);
+            rec.tail_open = undo[u].old_tail_open;
             if (undo[u].created) c->streams.erase(it);
         }
     };
@@ -643,14 +682,23 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
             auto it = c->streams.find(key);
             const bool created = (it == c->streams.end());
             const int64_t cur_len = created ? 0 : it->second.kv_len;
-            const int64_t cur_pages = cdiv(cur_len, P);
+            const int64_t cur_slots_raw = created ? 0 : it->second.slot_len();
+            const int64_t cur_pages = created ? 0 : (int64_t)it->second.pages.size();   // = ceil(slot_len / P)
+            // The new tokens continue inside the stream's partial last page only if that page was started by a COPY
+            // append of this very stream and nobody else refers to it.  Otherwise (ATTACH of a reused chunk; new tokens
+            // after an attached chunk whose length is not a multiple of P; a last page shared with another stream) they
+            // form a new head segment on a fresh page, and the rest of the partial page stays unused in mid-stream
+            // (every head segment has its own consecutive pages).
+            const bool partial = cur_slots_raw % P != 0;
+            const bool in_place = partial && !attach && it->second.tail_open && c->refcnt[it->second.pages.back()] == 1;
+            const int64_t new_pad = (partial && !in_place) ? P - cur_slots_raw % P : 0;
+            const int64_t cur_slots = cur_slots_raw + new_pad;
             const int64_t new_len = cur_len + r.n_tokens;
-            if (new_len > (int64_t)INT32_MAX - 2 * kBlockKeys) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: stream too long", i);
-            const int64_t need = cdiv(new_len, P) - cur_pages;
+            if (cur_slots + r.n_tokens > (int64_t)INT32_MAX - 2 * kBlockKeys) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: stream too long", i);
+            const int64_t need = cdiv(cur_slots + r.n_tokens, P) - cur_pages;
 
             if (attach) {
                 if (!r.page_ids) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs page_ids", i);
-                if (cur_len % P != 0) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs the stream length (%lld) to be a multiple of page_size", i, (long long)cur_len);
                 if (r.n_page_ids != need) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: attach needs %lld page ids, got %d", i, (long long)need, r.n_page_ids);
             } else if (r.page_ids) {
                 if (r.n_page_ids != need) APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: need %lld page ids, got %d", i, (long long)need, r.n_page_ids);
@@ -662,14 +710,10 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
             // which is random access into a table far larger than the host caches); a bad id undoes this request's
             // partial application together with the earlier requests (rollback).
             StreamRec& rec = c->streams[key];
-            undo.push_back(Undo{key, created, cur_len, 0});
+            undo.push_back(Undo{key, created, cur_len, 0, rec.pads.size(), rec.tail_open});
             rec.pages.reserve(rec.pages.size() + (size_t)need);
-            if (!attach && cur_len % P != 0) {
-                // The new rows start inside the stream's partial last page.  That page must be this stream's alone:
-                // a page attached by another stream (reference count > 1) would be overwritten under it.
-                if (c->refcnt[rec.pages.back()] > 1) {
-                    APPEND_FAIL(SEGPA_ERR_INVALID, "append_pages[%d]: the stream's partial last page %d is shared with another stream (reference count %d); copying into it would overwrite that stream's view", i, rec.pages.back(), c->refcnt[rec.pages.back()]);
-                }
+            if (new_pad > 0) rec.pads.push_back(PadPoint{cur_len, (rec.pads.empty() ? 0 : rec.pads.back().pad) + new_pad});
+            if (in_place) {
                 // An earlier COPY job of this batch that ended in the same page must not zero-fill the slots this
                 // job writes (both run in one launch, unordered): its writes stop at its own last token.
                 if (rec.batch_stamp == stamp && rec.batch_job >= 0) jobs[(size_t)rec.batch_job].n_write = jobs[(size_t)rec.batch_job].n_tokens;
@@ -689,15 +733,16 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 jb.n_tokens = r.n_tokens;
                 jb.chunk_begin = total_chunks;
                 jb.page_off = (long long)touched.size();
-                jb.first_slot = (int)(cur_len % P);
-                jb.n_pages = (int)need + (cur_len % P != 0 ? 1 : 0);
-                if (cur_len % P != 0) touched.push_back(rec.pages.back());   // (a partial last page is never a hole: evict_pages refuses it)
+                jb.first_slot = (int)(cur_slots % P);
+                jb.n_pages = (int)need + (in_place ? 1 : 0);
+                if (in_place) touched.push_back(rec.pages.back());   // (a partial last page is never a hole: evict_pages refuses it)
                 jb.n_write = (long long)jb.n_pages * P - jb.first_slot;     // rows + the zero-filled tail of the last page
                 total_chunks += jb.n_write * (D >> 3);
                 rec.batch_stamp = stamp;
                 rec.batch_job = (int32_t)jobs.size();
                 jobs.push_back(jb);
             }
+            rec.tail_open = !attach;
             for (int64_t k = 0; k < need; ++k) {
                 int32_t id;
                 if (r.page_ids) {
@@ -799,7 +844,7 @@ segpa_status_t segpa_evict_pages(segpa_cache_t* c, int32_t layer, int32_t kv_hea
     const int P = c->desc.page_size;
     if (first_page_index < 0 || n_pages < 1 || (int64_t)first_page_index + n_pages > (int64_t)rec.pages.size())
         return fail(SEGPA_ERR_INVALID, "evict_pages: range [%d, %d) outside the stream's %zu pages", first_page_index, first_page_index + n_pages, rec.pages.size());
-    if (rec.kv_len % P != 0 && (size_t)first_page_index + n_pages == rec.pages.size())
+    if (rec.slot_len() % P != 0 && (size_t)first_page_index + n_pages == rec.pages.size())
         return fail(SEGPA_ERR_INVALID, "evict_pages: the stream's partial last page cannot be evicted");
     for (int32_t i = 0; i < n_pages; ++i)
         if (rec.pages[(size_t)first_page_index + i] < 0) return fail(SEGPA_ERR_INVALID, "evict_pages: page index %d is already evicted", first_page_index + i);
@@ -815,11 +860,11 @@ namespace {
 // pages covering tokens [first_token, first_token + n) of a stream, uploaded through the append staging
 // buffers; *first_slot = slot of first_token inside the first page.  Returns nullptr and sets *why on error.
 const int* stage_token_range(segpa_cache* c, const StreamRec& rec, int64_t first_token, int64_t n, bool need_exclusive,
-                             cudaStream_t st, int* first_slot, Staging** used, const char** why, segpa_status_t* code) {
+                             cudaStream_t st, int64_t* first_page, Staging** used, const char** why, segpa_status_t* code) {
     const int P = c->desc.page_size;
     *code = SEGPA_ERR_INVALID;
     if (first_token < 0 || n < 1 || first_token + n > rec.kv_len) { *why = "token range outside the stream"; return nullptr; }
-    const int64_t pg_lo = first_token / P, pg_hi = (first_token + n - 1) / P + 1;
+    const int64_t pg_lo = rec.slot_of(first_token) / P, pg_hi = rec.slot_of(first_token + n - 1) / P + 1;
     for (int64_t pg = pg_lo; pg < pg_hi; ++pg) {
         const int32_t id = rec.pages[(size_t)pg];
         if (id < 0) { *why = "the range touches an evicted page"; return nullptr; }
@@ -834,7 +879,7 @@ const int* stage_token_range(segpa_cache* c, const StreamRec& rec, int64_t first
         e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
     }
     if (e != cudaSuccess) { cudaGetLastError(); *why = cudaGetErrorString(e); *code = SEGPA_ERR_CUDA; return nullptr; }
-    *first_slot = (int)(first_token % P);
+    *first_page = pg_lo;
     *used = &sg;
     return (const int*)sg.d;
 }
@@ -866,21 +911,24 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
                 if (g.key == it->first && r.first_token < g.hi && g.lo < r.first_token + r.n_tokens)
                     return fail(SEGPA_ERR_INVALID, "rope_align[%d]: token range overlaps an earlier request of the batch", i);
             seen.push_back(Rng{it->first, r.first_token, r.first_token + r.n_tokens});
-            const int64_t pg_lo = r.first_token / P, pg_hi = (r.first_token + r.n_tokens - 1) / P + 1;
+            const int64_t pg_lo = rec.slot_of(r.first_token) / P, pg_hi = rec.slot_of(r.first_token + r.n_tokens - 1) / P + 1;
             for (int64_t pg = pg_lo; pg < pg_hi; ++pg) {
                 const int32_t id = rec.pages[(size_t)pg];
                 if (id < 0) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: the range touches an evicted page", i);
                 if (c->refcnt[id] > 1) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: page %d is shared with another stream", i, id);
             }
-            RopeJob jb{};
-            jb.chunk_begin = total_chunks;
-            jb.page_off = (long long)ids.size();
-            jb.n_tokens = r.n_tokens;
-            jb.delta_pos = r.delta_pos;   // R(p_on) R(p_off)^-1 = R(delta); the per-pair cos / sin are formed on the device in fp64
-            jb.first_slot = (int)(r.first_token % P);
-            ids.insert(ids.end(), rec.pages.begin() + pg_lo, rec.pages.begin() + pg_hi);
-            total_chunks += r.n_tokens * (D >> 4);
-            jobs.push_back(jb);
+            // one job per piece that is contiguous in slot space (a range may span head segments with ragged tails)
+            for_each_piece(rec, r.first_token, r.n_tokens, [&](int64_t, int64_t n_piece, int64_t slot_lo) {
+                RopeJob jb{};
+                jb.chunk_begin = total_chunks;
+                jb.page_off = (long long)ids.size();
+                jb.n_tokens = n_piece;
+                jb.delta_pos = r.delta_pos;   // R(p_on) R(p_off)^-1 = R(delta); the per-pair cos / sin are formed on the device in fp64
+                jb.first_slot = (int)(slot_lo % P);
+                ids.insert(ids.end(), rec.pages.begin() + slot_lo / P, rec.pages.begin() + (slot_lo + n_piece - 1) / P + 1);
+                total_chunks += n_piece * (D >> 4);
+                jobs.push_back(jb);
+            });
         }
     } catch (const std::bad_alloc&) {
         return fail(SEGPA_ERR_OOM, "rope_align: host allocation failed");
@@ -930,14 +978,22 @@ segpa_status_t segpa_gather_rows(segpa_cache_t* c, int32_t layer, int32_t kv_hea
     if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "gather_rows: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
     DeviceGuard g(c->desc.device);
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int first_slot = 0;
+    int64_t first_page = 0;
     Staging* used = nullptr;
     const char* why = "";
     segpa_status_t code = SEGPA_OK;
-    const int* ids = stage_token_range(c, it->second, first_token, n_tokens, false, st, &first_slot, &used, &why, &code);
+    const StreamRec& rec = it->second;
+    const int* ids = stage_token_range(c, rec, first_token, n_tokens, false, st, &first_page, &used, &why, &code);
     if (!ids) return fail(code, "gather_rows: %s", why);
-    cudaError_t e = launch_gather_rows(c->k_pool, c->v_pool, ids, first_slot, n_tokens, (uint16_t*)k_dst, (uint16_t*)v_dst,
-                                       dst_row_stride_elems, D, c->desc.page_size, st);
+    const int P = c->desc.page_size;
+    cudaError_t e = cudaSuccess;
+    for_each_piece(rec, first_token, n_tokens, [&](int64_t tok_lo, int64_t n_piece, int64_t slot_lo) {
+        if (e != cudaSuccess) return;
+        uint16_t* kd = k_dst ? (uint16_t*)k_dst + (tok_lo - first_token) * dst_row_stride_elems : nullptr;
+        uint16_t* vd = v_dst ? (uint16_t*)v_dst + (tok_lo - first_token) * dst_row_stride_elems : nullptr;
+        e = launch_gather_rows(c->k_pool, c->v_pool, ids + (slot_lo / P - first_page), (int)(slot_lo % P), n_piece, kd, vd,
+                               dst_row_stride_elems, D, P, st);
+    });
     staging_release(*used, st);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "gather_rows: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;
@@ -1042,17 +1098,22 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
 
             const int64_t kv_len = rec.kv_len;
             const int64_t W = (r.head_class == SEGPA_GLOBAL) ? (int64_t)INT32_MAX / 2 : r.window;
+            // Positions are token indices; pages and KV blocks are laid out in slot space (slot = token + the unused slots
+            // behind earlier head segments' tails; the identity for a dense stream)
+            auto slot_of = [&rec](int64_t tok) { return rec.pads.empty() ? tok : rec.slot_of(tok); };
             // Alg. 2 lines 6-10: visible positions of the whole segment
             const int64_t vis_lo = std::max<int64_t>(0, kv_len - r.q_len - W + 1);
+            const int64_t vis_lo_slot = slot_of(vis_lo), last_slot = slot_of(kv_len - 1);
             // S_sink: the first n_sink tokens stay visible to a LOCAL head; they matter only when
             // some query's window starts after position 0 (the last query's does iff kv_len > W)
             const int64_t ns = (r.head_class == SEGPA_LOCAL) ? std::min<int64_t>(r.n_sink, kv_len) : 0;
             const bool has_sink = ns > 0 && kv_len > W;
-            const int64_t sink_pages = has_sink ? std::min(cdiv(std::min(ns, vis_lo), P), vis_lo / P) : 0;   // pages wholly before the window's first page
-            const int64_t seg_kb_lo = has_sink ? 0 : vis_lo / kBlockKeys;
-            const int64_t seg_kb_hi = (kv_len - 1) / kBlockKeys + 1;
-            const int64_t first_vis_page = vis_lo / P;
-            const int64_t n_stream_pages = cdiv(kv_len, P);
+            const int64_t sink_slots = (has_sink && std::min(ns, vis_lo) > 0) ? slot_of(std::min(ns, vis_lo) - 1) + 1 : 0;
+            const int64_t sink_pages = has_sink ? std::min(cdiv(sink_slots, P), vis_lo_slot / P) : 0;   // pages wholly before the window's first page
+            const int64_t seg_kb_lo = has_sink ? 0 : vis_lo_slot / kBlockKeys;
+            const int64_t seg_kb_hi = last_slot / kBlockKeys + 1;
+            const int64_t first_vis_page = vis_lo_slot / P;
+            const int64_t n_stream_pages = (int64_t)rec.pages.size();
             SegDev sd{};
             sd.q_row_start = r.q_row_start;
             sd.page_off = (long long)S->pages.size();
@@ -1064,6 +1125,10 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             sd.kv_head = r.kv_head;
             sd.first_page = (int)(seg_kb_lo * ppb);
             sd.n_pages_listed = (int)((seg_kb_hi - seg_kb_lo) * ppb);
+            sd.pad_off = (int)S->pads.size();
+            sd.n_pads = (int)rec.pads.size();
+            for (const PadPoint& pp : rec.pads) S->pads.push_back(PadDev{(int)pp.tok, (int)pp.pad});
+            if (!rec.pads.empty()) S->has_ragged = true;
             // Alg. 2 line 12: Translate(T_page, U_h): sink pages and recent-window pages (lines 9-10); invisible
             // pages (the evicted middle) and absent ones -> the zero page, never read
             {
@@ -1087,21 +1152,21 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             S->segs.push_back(sd);
             if (S->mass_off.empty()) S->mass_off.push_back(0);
             S->mass_off.push_back(S->mass_off.back() + cdiv(kv_len, kBlockKeys) * kBlockKeys);
-            vis_tokens += kv_len - first_vis_page * P + sink_pages * P;
+            vis_tokens += last_slot + 1 - first_vis_page * P + sink_pages * P;
             q_rows = std::max<int64_t>(q_rows, r.q_row_start + r.q_len);
             pairs += visible_pairs(kv_len - r.q_len, kv_len - 1, W);
             if (has_sink)   // sink keys not already inside the window
                 for (int64_t i = kv_len - r.q_len; i < kv_len; ++i) pairs += std::max<int64_t>(0, std::min(ns, i - W + 1));
-            // tiles: exactly the KV blocks the tile's rows attend to
+            // tiles: exactly the KV blocks (of slots) the tile's rows attend to
             for (int64_t t0 = 0; t0 < r.q_len; t0 += item_tok) {
                 const int64_t n_tok = std::min<int64_t>(item_tok, r.q_len - t0);
                 const int64_t i0 = kv_len - r.q_len + t0, i1 = i0 + n_tok - 1;
                 const int64_t lo = std::max<int64_t>(0, i0 - W + 1);
-                TileTmp tt{s, (int)t0, (int)n_tok, (int)(lo / kBlockKeys), (int)(i1 / kBlockKeys + 1), 0, false};
+                TileTmp tt{s, (int)t0, (int)n_tok, (int)(slot_of(lo) / kBlockKeys), (int)(slot_of(i1) / kBlockKeys + 1), 0, false};
                 tt.cost = tt.kb_hi - tt.kb_lo;
                 if (has_sink) {
                     // two KV block ranges: sink blocks [0, sb) then the window blocks; one range when they touch
-                    const int sb = (int)cdiv(std::min(ns, i1 + 1), kBlockKeys);
+                    const int sb = (int)cdiv(slot_of(std::min(ns, i1 + 1) - 1) + 1, kBlockKeys);
                     tt.cost = (sb >= tt.kb_lo) ? tt.kb_hi : sb + tt.kb_hi - tt.kb_lo;
                     tt.kb_lo = 0;
                     tt.sink = true;
@@ -1147,7 +1212,21 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
                 const int lo = (t.sink || parts == 1) ? t.kb_lo : t.kb_lo + (int)((int64_t)cost * p / parts);
                 const int hi = (t.sink || parts == 1) ? t.kb_hi : t.kb_lo + (int)((int64_t)cost * (p + 1) / parts);
                 const int slot = (parts > 1 || strided) ? n_slots++ : -1;
-                S->items.push_back(ItemDev{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, t.sink ? t.cost : hi - lo});
+                ItemDev itd{t.seg, t.t0, t.n_tok, lo, hi, slot, strided ? 1 : 0, t.sink ? t.cost : hi - lo, {{0, 0, 0}, {0, 0, 0}}, {0, 0}};
+                const segpa_segment_req_t& rq = S->reqs[(size_t)t.seg];
+                const StreamRec& srec = c->streams.find(StreamKey{layer, rq.kv_head, rq.seq_id})->second;
+                if (!srec.pads.empty()) {   // ragged stream: the slots of the tiles' first / last visible key and last sink key
+                    const SegDev& sdv = S->segs[(size_t)t.seg];
+                    for (int tl = 0; tl < 2; ++tl) {
+                        const int64_t tok_lo = t.t0 + (int64_t)tl * TT, tok_hi = std::min<int64_t>(t.t0 + t.n_tok, tok_lo + TT);
+                        if (tok_hi <= tok_lo) continue;
+                        const int64_t i0 = srec.kv_len - rq.q_len + tok_lo, i1 = srec.kv_len - rq.q_len + tok_hi - 1;
+                        itd.slots[tl][0] = (int)srec.slot_of(std::max<int64_t>(0, i0 - sdv.window + 1));
+                        itd.slots[tl][1] = (int)srec.slot_of(i1);
+                        itd.slots[tl][2] = sdv.n_sink > 0 ? (int)srec.slot_of(std::min<int64_t>(sdv.n_sink, i1 + 1) - 1) : -1;
+                    }
+                }
+                S->items.push_back(itd);
                 S->item_meta.push_back(segpa_segments::ItemMeta{(int32_t)ti, parts > 1 ? p : -1, parts});
             }
         }
@@ -1179,7 +1258,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         S->off_pages = al(S->off_items + S->items.size() * sizeof(ItemDev));
         S->off_combs = al(S->off_pages + S->pages.size() * sizeof(int32_t));
         S->off_cta = al(S->off_combs + std::max<size_t>(1, S->combs.size()) * sizeof(CombDev));
-        const size_t blob_bytes = al(S->off_cta + S->cta_off.size() * sizeof(int32_t));
+        S->off_pads = al(S->off_cta + S->cta_off.size() * sizeof(int32_t));
+        const size_t blob_bytes = al(S->off_pads + std::max<size_t>(1, S->pads.size()) * sizeof(PadDev));
         // device storage: recycled from the cache's free list (no cudaMalloc / cudaMallocHost in steady state)
         // Oldest first, and only one whose last use has completed on the device: a caller that enqueues steps
         // back to back (host planning of step k+1 under the kernels of step k) must not be made to wait here.
@@ -1227,6 +1307,7 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
         memcpy(hb + S->off_pages, S->pages.data(), S->pages.size() * sizeof(int32_t));
         if (!S->combs.empty()) memcpy(hb + S->off_combs, S->combs.data(), S->combs.size() * sizeof(CombDev));
         memcpy(hb + S->off_cta, S->cta_off.data(), S->cta_off.size() * sizeof(int32_t));
+        if (!S->pads.empty()) memcpy(hb + S->off_pads, S->pads.data(), S->pads.size() * sizeof(PadDev));
         e = staging_upload(B->blob, blob_bytes, c->up_stream, st);
         if (e != cudaSuccess) {
             cudaGetLastError();
@@ -1639,6 +1720,7 @@ segpa_status_t segpa_attention_mass(segpa_cache_t* c, const segpa_segments_t* s,
     const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
     if (T < s->stats.q_rows || lse_stride < T) return fail(SEGPA_ERR_INVALID, "attention_mass: T / lse_stride smaller than the plan's rows");
     if (q_row_stride < (int64_t)Hq * D || (q_row_stride % 8) || ((uintptr_t)q % 16)) return fail(SEGPA_ERR_INVALID, "attention_mass: bad q stride / alignment");
+    if (s->has_ragged) return fail(SEGPA_ERR_UNSUPPORTED, "attention_mass: a segment's stream has head segments with partial last pages (ragged chunk tails); the mass kernel works on dense streams only");
     if (mass_len < s->mass_off.back()) return fail(SEGPA_ERR_INVALID, "attention_mass: mass has %lld entries, the layout needs %lld", (long long)mass_len, (long long)s->mass_off.back());
     if (!(scale > 0.f) || !(scale < 1e30f)) return fail(SEGPA_ERR_INVALID, "attention_mass: softmax_scale must be positive and finite");
     DeviceGuard g(c->desc.device);

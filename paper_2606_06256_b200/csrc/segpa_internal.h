@@ -39,8 +39,17 @@ struct SegDev {
     int window;             // W (keys incl. self); large for GLOBAL
     int n_sink;
     int kv_head;
-    int first_page;         // absolute page index (position / P) of page_off
+    int first_page;         // absolute page index (slot / P) of page_off
     int n_pages_listed;
+    int pad_off;            // ragged streams (head segments with partial last pages): index of the stream's
+    int n_pads;             //   first PadDev and their number (0: token j sits at slot j)
+};
+
+// Token -> slot map of a ragged stream: tokens >= tok (up to the next entry) sit at slot token + pad; the slots
+// [tok + previous pad, tok + pad) behind the previous head segment's tail hold no token.
+struct PadDev {
+    int tok;
+    int pad;
 };
 
 struct ItemDev {
@@ -52,7 +61,13 @@ struct ItemDev {
     int partial_slot;       // -1: final result written to out/lse; else split-KV partial slot
     int flags;              // bit 0: strided (both tiles hold the same rows and take alternate KV blocks)
     int cost;               // KV blocks the item visits (scheduling only; < kb_hi - kb_lo for sink segments)
+    // Ragged streams only (SegDev::n_pads > 0; zero otherwise): per tile slot t of the item, the slots of the first key
+    // any of its rows sees, of the last one, and of its last sink key (a dense stream has slot = token and the kernel
+    // forms them itself).  Looked up on the host so that no role of the kernel walks the token -> slot map per item.
+    int slots[2][3];
+    int pad_[2];
 };
+static_assert(sizeof(ItemDev) == 64, "ItemDev is read as four 16-byte words");
 
 struct CombDev {
     int seg;
@@ -74,6 +89,7 @@ struct FwdParams {
     const SegDev* segs;
     const ItemDev* items;
     const int* pages;            // translated physical page ids (zero page = num_pages)
+    const PadDev* pads;          // token -> slot maps of the ragged streams (SegDev::pad_off)
     const CombDev* combs;
     const int* cta_off;          // [n_cta + 1]: CTA c of the attention kernel owns items [cta_off[c], cta_off[c+1])
     int n_cta;
@@ -97,6 +113,7 @@ struct FwdParams {
     int tiles_per_item;
     int page_bytes;
     int num_sms;
+    int has_ragged;              // some segment's stream is ragged (SegDev::n_pads > 0): the kernel instantiation with that code
 #ifdef SEGPA_TRACE
     unsigned long long* trace;   // [16 warps][kTraceCap] (tag << 56 | arg << 40 | clock) of CTA 0; debug builds only
 #endif

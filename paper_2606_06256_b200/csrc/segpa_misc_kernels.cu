@@ -318,13 +318,34 @@ __global__ void attention_simt_kernel(FwdParams p) {
             for (int k = 0; k < epl; ++k)
                 qv[k] = bf16_bits_to_float(p.q[row * p.q_row_stride + (long long)head * p.D + lane * epl + k]);
             float m = -INFINITY, l = 0.f;
-            int jlo = max(it.kb_lo * kBlockKeys, i - sg.window + 1);
-            int jhi = min(it.kb_hi * kBlockKeys - 1, i);
+            // the item's KV blocks are ranges of SLOTS (head segments start on fresh pages): first token at
+            // or after a slot, and the slot of a token
+            auto tok_at = [&](int u) {
+                int start = 0, pad_c = 0;
+                for (int k = 0; k < sg.n_pads; ++k) {
+                    const PadDev pd = p.pads[sg.pad_off + k];
+                    if (u < pd.tok + pad_c) return max(u, start) - pad_c;
+                    start = pd.tok + pd.pad;
+                    pad_c = pd.pad;
+                }
+                return max(u, start) - pad_c;
+            };
+            auto slot_of = [&](int j) {
+                int pad = 0;
+                for (int k = 0; k < sg.n_pads; ++k) {
+                    const PadDev pd = p.pads[sg.pad_off + k];
+                    if (pd.tok <= j) pad = pd.pad;
+                }
+                return j + pad;
+            };
+            int jlo = max(tok_at(it.kb_lo * kBlockKeys), i - sg.window + 1);
+            int jhi = min(tok_at(it.kb_hi * kBlockKeys) - 1, i);
             // visible keys: sink tokens [0, n_sink) not already inside the window, then the window
             const int n_sink_keys = (it.kb_lo == 0) ? min(sg.n_sink, jlo) : 0;
             for (int jj = 0; jj < n_sink_keys + max(0, jhi - jlo + 1); ++jj) {
                 const int j = jj < n_sink_keys ? jj : jlo + (jj - n_sink_keys);
-                const int pg = j / p.P, slot = j % p.P;
+                const int u = slot_of(j);
+                const int pg = u / p.P, slot = u % p.P;
                 const int page = p.pages[sg.page_off + (pg - sg.first_page)];
                 const size_t off = (size_t)page * p.page_bytes;
                 float dot = 0.f;

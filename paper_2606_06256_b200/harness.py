@@ -24,6 +24,22 @@ def append_requests(w: wl.Workload, k_pool=None, v_pool=None) -> List[tuple]:
     aliased = [s for s in w.streams if s.shared_from is not None]
     reqs = []
     for s in owners + aliased:
+        if s.chunk_lens is not None:
+            # A stream spliced from reused chunks (PIC): every chunk but the last is first stored under an
+            # id of its own (what an offline cache holds) and then ATTACHED, each chunk on its own pages whatever its
+            # length; the last chunk is the request's new suffix, copied in (it starts a fresh page after the attach).
+            for c, n in enumerate(s.chunk_lens):
+                ids = wl.chunk_pages(s, w.P, c)
+                last = c == len(s.chunk_lens) - 1
+                if k_pool is None:
+                    reqs.append((s.layer, s.kv_head, s.seq_id, None, None, n, ids))
+                elif last:
+                    reqs.append((s.layer, s.kv_head, s.seq_id, wl.chunk_rows(k_pool, s, w.P, c), wl.chunk_rows(v_pool, s, w.P, c), n, ids))
+                else:
+                    src = chunk_source_id(s.seq_id, c)
+                    reqs.append((s.layer, s.kv_head, src, wl.chunk_rows(k_pool, s, w.P, c), wl.chunk_rows(v_pool, s, w.P, c), n, ids))
+                    reqs.append((s.layer, s.kv_head, s.seq_id, None, None, n, ids))
+            continue
         if k_pool is None:
             reqs.append((s.layer, s.kv_head, s.seq_id, None, None, s.kv_len, s.page_ids))
             continue
@@ -36,6 +52,11 @@ def append_requests(w: wl.Workload, k_pool=None, v_pool=None) -> List[tuple]:
             vr = wl.stream_rows(v_pool, s, w.P, lo_page=pp)
             reqs.append((s.layer, s.kv_head, s.seq_id, kr, vr, n_rest, s.page_ids[pp:]))
     return reqs
+
+
+def chunk_source_id(seq_id: int, c: int) -> int:
+    """seq_id under which reused chunk c of a spliced stream is stored before it is attached."""
+    return (c + 1) * (1 << 32) + seq_id
 
 
 def append_workload(cache: int, w: wl.Workload, k_pool=None, v_pool=None, stream=None, batched: bool = True) -> None:

@@ -89,6 +89,96 @@ def test_sinks(case, kernel, tiles):
     print(_run_full(w, kernel, tiles, "sinks%d" % case))
 
 
+RAGGED_TAILS = [
+    # Hq, Hkv, D, P, requests whose streams are spliced from reused chunks of ARBITRARY length: every
+    # chunk sits on its own pages, so a chunk whose length is not a multiple of P leaves a partial page in mid-stream
+    # 3 chunks + suffix; windows that end inside, start inside and straddle a ragged tail; sinks in the first chunk
+    (8, 2, 128, 16, [{"kv_len": 1000, "chunks": [333, 200, 407, 60],
+                      "heads": {0: (GLOBAL, 0, 0, 1000), 1: (LOCAL, 100, 4, 700)}}]),
+    # 12 chunks of the paper's reused-segment sizes scaled down, P = 32, G = 7; decode and short-q heads
+    (28, 4, 128, 32, [{"kv_len": 5243, "chunks": [517, 301, 640, 333, 1025, 96, 31, 700, 449, 512, 639],
+                       "heads": {0: (GLOBAL, 0, 0, 5243), 1: (LOCAL, 1000, 0, 5243), 2: (LOCAL, 4096, 128, 77), 3: (GLOBAL, 0, 0, 1)}}]),
+    # chunks shorter than a 128-slot block (several tails per block), single-token chunks, a chunk of exactly one page; D = 64
+    (8, 2, 64, 16, [{"kv_len": 397, "chunks": [5, 1, 16, 17, 40, 1, 100, 90, 127],
+                     "heads": {0: (GLOBAL, 0, 0, 397), 1: (LOCAL, 33, 6, 397)}},
+                    {"kv_len": 300, "heads": {0: (LOCAL, 64, 0, 300), 1: (GLOBAL, 0, 0, 10)}}]),
+    # long ragged streams with decode-shaped queries (split along KV, strided chains) and W = 1
+    (32, 8, 128, 16, [{"kv_len": 20011, "chunks": [4099, 2050, 8111, 3001, 2750],
+                       "heads": {h: ((GLOBAL, 0, 0, 1) if h % 2 == 0 else (LOCAL, 2048 if h > 1 else 1, 0, 1)) for h in range(8)}}]),
+]
+
+
+@pytest.mark.parametrize("kernel,tiles", VARIANTS)
+@pytest.mark.parametrize("case", range(len(RAGGED_TAILS)))
+def test_ragged_chunk_tails(case, kernel, tiles):
+    """Mid-stream partial pages: streams built by ATTACHING reused chunks of arbitrary length,
+    then COPYING the new suffix (which starts a fresh page), against the oracle's head-segment table."""
+    Hq, Hkv, D, P, reqs = RAGGED_TAILS[case]
+    w = wl.make_workload("tails%d" % case, Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=1500 + case)
+    g = GpuRun(w, kernel, tiles)
+    try:
+        for s_ in w.streams:
+            kv_len, ids = B.segpa_stream_info(g.cache, s_.layer, s_.kv_head, s_.seq_id)
+            assert kv_len == s_.kv_len and np.array_equal(ids, s_.page_ids)
+        q, out, lse = g.layer(0)
+        print(compare(w, 0, g.k_pool, g.v_pool, q, out, lse, label="tails%d[%s,%d]" % (case, kernel, tiles)))
+    finally:
+        g.close()
+
+
+def test_ragged_stream_append_gather_and_rope():
+    """Token-addressed calls on a ragged stream: rows read back with segpa_gather_rows are the stream's tokens in
+    order (ranges that cross ragged tails included); a further COPY append continues inside the suffix's own partial
+    page; a decode step over the grown stream matches the oracle; RoPEAlign over a range that spans two chunks moves
+    exactly those tokens."""
+    import oracle as O
+    P, D = 16, 128
+    chunks = [100, 37, 260, 50]
+    w = wl.make_workload("tails_api", Hq=8, Hkv=2, D=D, P=P, seed=77, pool_factor=3.0,
+                         requests=[{"kv_len": sum(chunks), "chunks": chunks, "heads": {0: (GLOBAL, 0, 0, 9), 1: (LOCAL, 120, 2, 9)}}])
+    g = GpuRun(w, "tc", 2)
+    dev = g.dev
+    try:
+        st = w.stream_map()[(0, 1, 0)]
+        want_k, want_v = wl.stream_rows(g.k_pool, st, P), wl.stream_rows(g.v_pool, st, P)
+        for (t0, n) in [(0, st.kv_len), (90, 60), (99, 2), (137, 300), (396, 51)]:
+            ko, vo = torch.zeros((n, D), dtype=torch.bfloat16, device=dev), torch.zeros((n, D), dtype=torch.bfloat16, device=dev)
+            B.segpa_gather_rows(g.cache, 0, 1, 0, t0, n, ko, vo)
+            torch.cuda.synchronize()
+            assert torch.equal(ko, want_k[t0:t0 + n]) and torch.equal(vo, want_v[t0:t0 + n]), (t0, n)
+        # 7 more tokens: they continue in the suffix's partial page (50 % 16 = 2 slots used), no new ragged tail
+        more_k = wl.randn_bf16((7, D), 4711, dev)
+        more_v = wl.randn_bf16((7, D), 4712, dev)
+        n_pages_before = len(B.segpa_stream_info(g.cache, 0, 1, 0)[1])
+        B.segpa_append_pages(g.cache, 0, 1, 0, more_k, more_v, 7)
+        kv_len, ids = B.segpa_stream_info(g.cache, 0, 1, 0)
+        assert kv_len == st.kv_len + 7 and len(ids) == n_pages_before
+        ko = torch.zeros((20, D), dtype=torch.bfloat16, device=dev)
+        B.segpa_gather_rows(g.cache, 0, 1, 0, st.kv_len - 13, 20, ko, None)
+        torch.cuda.synchronize()
+        assert torch.equal(ko[:13], want_k[-13:]) and torch.equal(ko[13:], more_k)
+        # RoPEAlign tokens [80, 150): the tail of chunk 0, all of chunk 1, the head of chunk 2
+        kb = torch.zeros((st.kv_len, D), dtype=torch.bfloat16, device=dev)
+        B.segpa_gather_rows(g.cache, 0, 1, 0, 0, st.kv_len, kb, None)
+        with pytest.raises(B.SegpaError, match="shared with another stream"):     # the chunks' cached copies still refer to the pages
+            B.segpa_rope_align(g.cache, 0, 1, 0, 80, 70, 1234)
+        for c in range(len(chunks) - 1):
+            B.segpa_free_stream(g.cache, 0, 1, H.chunk_source_id(0, c))
+        B.segpa_rope_align(g.cache, 0, 1, 0, 80, 70, 1234)
+        ka = torch.zeros_like(kb)
+        B.segpa_gather_rows(g.cache, 0, 1, 0, 0, st.kv_len, ka, None)
+        torch.cuda.synchronize()
+        assert torch.equal(ka[:80], kb[:80]) and torch.equal(ka[150:], kb[150:])
+        p_off = np.arange(80, 150)
+        ref = O.rope_align(kb[80:150].float().cpu().numpy().astype(np.float64), p_off, p_off + 1234, 10000.0)
+        got = ka[80:150].float().cpu().numpy().astype(np.float64)
+        a = np.abs(kb[80:150].float().cpu().numpy().astype(np.float64))
+        bound = 2.0 ** -8 * (a[:, :D // 2] + a[:, D // 2:]) + 1e-6
+        assert np.all(np.abs(got - ref) <= np.concatenate([bound, bound], axis=1))
+    finally:
+        g.close()
+
+
 def test_true_eviction_between_sinks_and_window():
     """the middle of a LOCAL head's stream is evicted, its physical pages are reused by another
     stream holding NaN / 1e30; the head's result is unchanged and still matches the oracle."""
@@ -303,29 +393,36 @@ def test_two_copy_jobs_of_one_batch_extend_the_same_stream():
             B.segpa_destroy(cache)
 
 
-def test_copy_into_a_shared_partial_page_is_refused():
+def test_copy_after_a_shared_partial_page_starts_a_new_head_segment():
     """A page can be the partial tail of two streams (B attaches A's pages, A's length not a multiple of P).  A COPY
-    append into that page through either stream would overwrite slots the other stream sees: INVALID, nothing applied."""
+    append through either stream must not write into that page (it would overwrite slots the other stream sees, or
+    expose A's later tokens to B): the new tokens form a new head segment on a fresh page and the rest of
+    the shared page stays unused in mid-stream.  Once the page is the stream's alone again, appends continue in place."""
     w = wl.config1()
     dev = torch.device("cuda:0")
     rows = torch.ones((24, w.D), dtype=torch.bfloat16, device=dev)
     more = torch.full((8, w.D), 2.0, dtype=torch.bfloat16, device=dev)
+    more3 = torch.full((8, w.D), 3.0, dtype=torch.bfloat16, device=dev)
     cache = H.create_cache(w, 0)
     try:
         B.segpa_append_pages(cache, 0, 0, 1, rows, rows, 24, page_ids=[10, 11])
         B.segpa_append_pages(cache, 0, 0, 2, None, None, 24, page_ids=[10, 11])       # stream 2 shares both pages
-        before = B.segpa_pool_stats(cache)
-        for seq in (1, 2):
-            with pytest.raises(B.SegpaError, match="shared with another stream"):
-                B.segpa_append_pages(cache, 0, 0, seq, more, more, 8)
-            assert B.segpa_stream_info(cache, 0, 0, seq)[0] == 24
-        assert B.segpa_pool_stats(cache) == before
-        B.segpa_free_stream(cache, 0, 0, 2)                                            # sole owner again: allowed
-        B.segpa_append_pages(cache, 0, 0, 1, more, more, 8)
-        ko = torch.zeros((32, w.D), dtype=torch.bfloat16, device=dev)
-        B.segpa_gather_rows(cache, 0, 0, 1, 0, 32, ko, None)
+        B.segpa_append_pages(cache, 0, 0, 1, more, more, 8, page_ids=[20])            # page 11 is shared: fresh page
+        B.segpa_append_pages(cache, 0, 0, 2, more3, more3, 8, page_ids=[21])          # attached tail: fresh page
+        for seq, ids, val in ((1, [10, 11, 20], more), (2, [10, 11, 21], more3)):
+            kv_len, got = B.segpa_stream_info(cache, 0, 0, seq)
+            assert kv_len == 32 and list(got) == ids
+            ko = torch.zeros((32, w.D), dtype=torch.bfloat16, device=dev)
+            B.segpa_gather_rows(cache, 0, 0, seq, 0, 32, ko, None)
+            torch.cuda.synchronize()
+            assert torch.equal(ko[:24], rows) and torch.equal(ko[24:], val)
+        # the fresh page is stream 1's alone and was started by its own COPY: the next append fills it in place
+        B.segpa_append_pages(cache, 0, 0, 1, more3[:5], more3[:5], 5)
+        assert list(B.segpa_stream_info(cache, 0, 0, 1)[1]) == [10, 11, 20]
+        ko = torch.zeros((13, w.D), dtype=torch.bfloat16, device=dev)
+        B.segpa_gather_rows(cache, 0, 0, 1, 24, 13, ko, None)
         torch.cuda.synchronize()
-        assert torch.equal(ko[:24], rows) and torch.equal(ko[24:], more)
+        assert torch.equal(ko[:8], more) and torch.equal(ko[8:], more3[:5])
     finally:
         B.segpa_destroy(cache)
 

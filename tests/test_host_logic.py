@@ -84,10 +84,12 @@ def test_pool_bookkeeping_attach_and_refcounts():
     B.segpa_append_pages(c, 0, 0, 2, None, None, 32, page_ids=[5, 9])
     B.segpa_append_pages(c, 0, 0, 2, None, None, 16, page_ids=[7])
     assert B.segpa_pool_stats(c) == (4, 60)
-    # attach requires a page-aligned stream: stream 1 has 40 tokens
-    with pytest.raises(B.SegpaError) as e:
-        B.segpa_append_pages(c, 0, 0, 1, None, None, 16, page_ids=[11])
-    assert e.value.status == B.ERR_INVALID
+    # attach to a stream whose last page is partial (stream 1 has 40 tokens): the attached chunk is a new head segment
+    # on its own pages; the 8 unused slots of page 2 stay unused in mid-stream
+    B.segpa_append_pages(c, 0, 0, 1, None, None, 16, page_ids=[11])
+    kv, ids = B.segpa_stream_info(c, 0, 0, 1)
+    assert kv == 56 and list(ids) == [5, 9, 2, 11]
+    assert B.segpa_pool_stats(c) == (5, 59)
     with pytest.raises(B.SegpaError):
         B.segpa_append_pages(c, 0, 0, 3, None, None, 16, page_ids=[64])               # out of range
     with pytest.raises(B.SegpaError):
@@ -204,6 +206,72 @@ def test_visible_page_selection_and_tiles(P):
             assert max(tot) - min(tot) <= 3 * max(costs) + 2
             B.segpa_free_segments(c, segs)
             B.segpa_destroy(c)
+
+
+@pytest.mark.parametrize("P", [16, 32])
+def test_ragged_streams_are_planned_in_slot_space(P):
+    """Streams spliced from chunks of arbitrary length (each on its own pages): the page lists and the
+    tiles' KV block ranges follow the SLOT of a token (token index + the unused slots behind earlier chunks' tails).
+    Checked against a restatement that lays the stream out slot by slot."""
+    rng = np.random.default_rng(100 + P)
+    for trial in range(30):
+        n_chunks = int(rng.integers(2, 9))
+        chunks = [int(rng.choice([1, P - 1, P, P + 1, 100, 333, 700])) for _ in range(n_chunks)]
+        kv_len = sum(chunks)
+        q_len = int(rng.integers(1, kv_len + 1))
+        cls = int(rng.integers(0, 2))
+        W = int(rng.choice([1, 7, 128, 300, 5000]))
+        n_sink = int(rng.choice([0, 0, 4, 50])) if cls == LOCAL else 0
+        G = int(rng.choice([1, 4, 8]))
+        c = plan_cache(Hq=2 * G, Hkv=2, P=P, num_pages=2048)
+        # slot-by-slot layout: tok_of_slot[u] = token or -1
+        tok_of_slot, ids_all, next_id = [], [], 0
+        for n in chunks:
+            npg = (n + P - 1) // P
+            ids = list(range(next_id, next_id + npg))
+            next_id += npg
+            ids_all += ids
+            B.segpa_append_pages(c, 0, 1, 42, None, None, n, page_ids=ids)
+            base = len([t for t in tok_of_slot if t >= 0])
+            tok_of_slot += [base + o if o < n else -1 for o in range(npg * P)]
+        kv, got_ids = B.segpa_stream_info(c, 0, 1, 42)
+        assert kv == kv_len and list(got_ids) == ids_all
+        slot_of = {t: u for u, t in enumerate(tok_of_slot) if t >= 0}
+        segs = B.segpa_build_segments(c, 0, [(42, 1, cls, W, n_sink, 3, q_len)])
+        st = B.segpa_segments_stats(segs)
+        items = B.segpa_segments_items(segs)
+        first, pages = B.segpa_segments_pages(segs, 0)
+        ppb = 128 // P
+        # visible tokens of the whole segment and of each tile
+        def visible(i):
+            lo = 0 if cls == GLOBAL else max(0, i - W + 1)
+            sinks = range(0, min(n_sink, lo)) if (cls == LOCAL and kv_len > W) else range(0)
+            return list(sinks) + list(range(lo, i + 1))
+        need_pages = set()
+        pairs = 0
+        by_tile = {}
+        for it in items:
+            by_tile.setdefault(it["tile"], []).append(it)
+        for tile, parts in by_tile.items():
+            t0, n_tok = parts[0]["t0"], parts[0]["n_tok"]
+            need_blocks = set()
+            for t in range(t0, t0 + n_tok):
+                vis = visible(kv_len - q_len + t)
+                pairs += len(vis) * G
+                need_blocks.update(slot_of[j] // 128 for j in vis)
+                need_pages.update(slot_of[j] // P for j in vis)
+            got_blocks = set()
+            for pt in parts:
+                got_blocks.update(range(pt["kb_lo"], pt["kb_hi"]))
+            assert need_blocks <= got_blocks                      # every attended block is visited ...
+            assert got_blocks <= set(range(min(need_blocks), max(need_blocks) + 1))   # ... and nothing outside their hull
+        assert st["attended_pairs"] == pairs
+        # every page that holds a visible token is listed with its physical id; pages outside the hull are the zero page
+        for pg in need_pages:
+            assert pages[pg - first] == ids_all[pg], (trial, pg)
+        for k, pid in enumerate(pages):
+            assert pid == 2048 or pid == ids_all[first + k]
+        B.segpa_destroy(c)
 
 
 def test_split_kv_plan_for_decode():
