@@ -465,7 +465,11 @@ void fill_fwd_params(FwdParams& p, const segpa_cache* c, const segpa_segments* s
     p.n_items = (int)s->items.size();
     p.n_combs = (int)s->combs.size();
     p.comb_max_rows = 0;
-    for (const CombDev& cd : s->combs) p.comb_max_rows = std::max(p.comb_max_rows, cd.n_tok * c->G);
+    p.comb_max_parts = 0;
+    for (const CombDev& cd : s->combs) {
+        p.comb_max_rows = std::max(p.comb_max_rows, cd.n_tok * c->G);
+        p.comb_max_parts = std::max(p.comb_max_parts, cd.n_splits * ((cd.flags & 1) ? 2 : 1));
+    }
     p.counter = s->buf->counter;
     p.k_pool = c->k_pool;
     p.v_pool = c->v_pool;

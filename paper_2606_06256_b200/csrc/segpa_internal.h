@@ -96,6 +96,7 @@ struct FwdParams {
     int n_items;
     int n_combs;
     int comb_max_rows;           // most rows (tokens x G) any combine entry has
+    int comb_max_parts;          // most partials any combine entry merges
     int* counter;                // dynamic scheduler cursor (zeroed before launch)
     const uint8_t* k_pool;
     const uint8_t* v_pool;

@@ -167,18 +167,57 @@ cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, con
 // merged in ascending split order (deterministic).  Exactness of the merge: PAPER.md:302.
 // One warp per row.
 // ---------------------------------------------------------------------------------------------
-template <int D>
-__global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ FwdParams p) {
+// One warp folds partials s0, s0 + NW, ... (NB of them at a time, all loads issued before the first use) of a row into
+// its running state (M, L, acc): fixed order, so the result does not depend on timing.
+template <int D, int NB, int NW, class PartRow>
+__device__ __forceinline__ void fold_partials(const FwdParams& p, PartRow part_row, int warp, int lane, int n_part, float& M, float& L,
+                                              float (&acc)[D / 32]) {
+    constexpr int EPL = D / 32;
+    for (int s0 = warp; s0 < n_part; s0 += NW * NB) {
+        float2 ml[NB];
+        float ov[NB][EPL];
+#pragma unroll
+        for (int i = 0; i < NB; ++i) {
+            const int s = s0 + i * NW;
+            const bool ok = s < n_part;
+            const size_t base = part_row(ok ? s : s0);
+            ml[i] = ok ? *reinterpret_cast<const float2*>(p.ws_ml + base * 2) : make_float2(-INFINITY, 0.f);
+#pragma unroll
+            for (int k = 0; k < EPL; ++k) ov[i][k] = ok ? p.ws_o[base * D + lane + 32 * k] : 0.f;
+        }
+        float mb = M;
+#pragma unroll
+        for (int i = 0; i < NB; ++i) mb = fmaxf(mb, ml[i].x);
+        const float corr = (M == -INFINITY) ? 0.f : exp2f(M - mb);   // (mb = -inf only while every partial so far is empty)
+        L *= corr;
+#pragma unroll
+        for (int k = 0; k < EPL; ++k) acc[k] *= corr;
+        M = mb;
+#pragma unroll
+        for (int i = 0; i < NB; ++i) {
+            const float w = (ml[i].x == -INFINITY) ? 0.f : exp2f(ml[i].x - M);
+            L += w * ml[i].y;
+#pragma unroll
+            for (int k = 0; k < EPL; ++k) acc[k] += w * ov[i][k];
+        }
+    }
+}
+
+template <int D, int NW>
+__global__ void __launch_bounds__(NW * 32) combine_kernel(const __grid_constant__ FwdParams p) {
     constexpr int EPL = D / 32;   // elements per lane
-    constexpr int NW = 8;         // warps per block: warp w merges partials w, w + 8, ... of the block's row
+    // NW warps per block: warp w merges partials w, w + NW, ... of the block's row (8 when some tile has many
+    // partials, a long decode context cut over the whole grid; 2 when every tile has a few)
+    constexpr int NB = 12;        // partials a warp has in flight: all their loads are issued before the first is used
     __shared__ float s_acc[NW][D];
-    __shared__ float s_l[NW];
+    __shared__ float2 s_ml[NW];
     const int rows_per_slot = kTileRows * p.tiles_per_item;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     ptx::pdl_launch_dependents();
     ptx::pdl_wait();         // the partials are the attention kernel's
-    // block (x, y): comb x, rows y, y + gridDim.y, ...  One block per row: the chain of dependent loads of a
-    // row with many partials is cut eight ways; sums are formed in a fixed order (deterministic).
+    // block (x, y): comb x, rows y, y + gridDim.y, ...  One block per row.  Each warp folds its share of the row's
+    // partials into a state (M, L, acc) of its own -- no pass over all the maxima first, so a row with up to 96 partials
+    // costs ONE round trip to memory -- and warp 0 merges the NW states.  Every sum runs in a fixed order.
     const CombDev c = p.combs[blockIdx.x];
     const SegDev sg = p.segs[c.seg];
     const int rows = c.n_tok * p.G;
@@ -189,42 +228,31 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ Fw
         auto part_row = [&](int s) {
             return (size_t)(c.first_slot + s / per_slot) * rows_per_slot + (size_t)(s % per_slot) * kTileRows + r;
         };
-        // global max M: every warp forms it (lanes over partials, loads independent)
-        float M = -INFINITY;
-        for (int s = lane; s < n_part; s += 32) M = fmaxf(M, p.ws_ml[part_row(s) * 2]);
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) M = fmaxf(M, __shfl_xor_sync(0xffffffffu, M, o));
-        // this warp's partials, ascending
-        float L = 0.f;
+        float M = -INFINITY, L = 0.f;
         float acc[EPL];
 #pragma unroll
         for (int k = 0; k < EPL; ++k) acc[k] = 0.f;
-#pragma unroll 4
-        for (int s = warp; s < n_part; s += NW) {
-            const size_t base = part_row(s);
-            const float ms = p.ws_ml[base * 2], ls = p.ws_ml[base * 2 + 1];
-            float ov[EPL];
-#pragma unroll
-            for (int k = 0; k < EPL; ++k) ov[k] = p.ws_o[base * D + lane + 32 * k];
-            const float w = (ms == -INFINITY) ? 0.f : exp2f(ms - M);
-            L += w * ls;
-#pragma unroll
-            for (int k = 0; k < EPL; ++k) acc[k] += w * ov[k];
-        }
+        if (n_part <= 2 * NW) fold_partials<D, 2, NW>(p, part_row, warp, lane, n_part, M, L, acc);   // (most tiles: a strided item or two)
+        else fold_partials<D, NB, NW>(p, part_row, warp, lane, n_part, M, L, acc);
 #pragma unroll
         for (int k = 0; k < EPL; ++k) s_acc[warp][lane + 32 * k] = acc[k];
-        if (lane == 0) s_l[warp] = L;
+        if (lane == 0) s_ml[warp] = make_float2(M, L);
         __syncthreads();
         if (warp == 0) {
+            float Mt = -INFINITY;
+#pragma unroll
+            for (int w2 = 0; w2 < NW; ++w2) Mt = fmaxf(Mt, s_ml[w2].x);
             float Lt = 0.f;
             float tot[EPL];
 #pragma unroll
             for (int k = 0; k < EPL; ++k) tot[k] = 0.f;
 #pragma unroll
             for (int w2 = 0; w2 < NW; ++w2) {     // fixed order
-                Lt += s_l[w2];
+                const float2 ml = s_ml[w2];
+                const float w = (ml.x == -INFINITY) ? 0.f : exp2f(ml.x - Mt);
+                Lt += w * ml.y;
 #pragma unroll
-                for (int k = 0; k < EPL; ++k) tot[k] += s_acc[w2][lane + 32 * k];
+                for (int k = 0; k < EPL; ++k) tot[k] += w * s_acc[w2][lane + 32 * k];
             }
             const int t = c.t0 + r / p.G, head = sg.kv_head * p.G + r % p.G;
             const long long row = sg.q_row_start + t;
@@ -233,7 +261,7 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ Fw
             for (int k = 0; k < EPL; ++k)
                 p.out[row * p.out_row_stride + (long long)head * D + lane + 32 * k] =
                     __bfloat16_as_ushort(__float2bfloat16_rn(tot[k] * inv));
-            if (p.lse && lane == 0) p.lse[(long long)head * p.lse_stride + row] = (M + log2f(Lt)) * 0.6931471805599453f;
+            if (p.lse && lane == 0) p.lse[(long long)head * p.lse_stride + row] = (Mt + log2f(Lt)) * 0.6931471805599453f;
         }
         __syncthreads();
     }
@@ -242,7 +270,9 @@ __global__ void __launch_bounds__(256) combine_kernel(const __grid_constant__ Fw
 cudaError_t launch_combine(const FwdParams& p, cudaStream_t st) {
     if (p.n_combs == 0) return cudaSuccess;
     const dim3 grid((unsigned)p.n_combs, (unsigned)(p.comb_max_rows < 1 ? 1 : (p.comb_max_rows > 256 ? 256 : p.comb_max_rows)));
-    return p.D == 128 ? launch_pdl(combine_kernel<128>, grid, dim3(256), 0, st, p) : launch_pdl(combine_kernel<64>, grid, dim3(256), 0, st, p);
+    if (p.comb_max_parts <= 24)
+        return p.D == 128 ? launch_pdl(combine_kernel<128, 2>, grid, dim3(64), 0, st, p) : launch_pdl(combine_kernel<64, 2>, grid, dim3(64), 0, st, p);
+    return p.D == 128 ? launch_pdl(combine_kernel<128, 8>, grid, dim3(256), 0, st, p) : launch_pdl(combine_kernel<64, 8>, grid, dim3(256), 0, st, p);
 }
 
 // ---------------------------------------------------------------------------------------------
