@@ -897,13 +897,13 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
     if (c->planning_only) return fail(SEGPA_ERR_STATE, "rope_align: planning-only cache has no device");
     if (!(rope_base > 1.0)) return fail(SEGPA_ERR_INVALID, "rope_align: rope_base must be > 1");
     const int D = c->desc.head_dim, P = c->desc.page_size;
-    std::vector<RopeJob> jobs;
-    std::vector<int32_t> ids;
-    long long total_chunks = 0;
+    // Pass 1: streams, ranges, overlaps; count the jobs (pieces contiguous in slot space) and the page ids they list.
     // a token may be rotated once per batch: overlapping ranges would make the result order-dependent
-    struct Rng { StreamKey key; int64_t lo, hi; };
+    struct Rng { const StreamRec* rec; int64_t lo, hi; };
     std::vector<Rng> seen;
+    size_t n_jobs = 0, n_ids = 0;
     try {
+        seen.reserve((size_t)n);
         for (int32_t i = 0; i < n; ++i) {
             const segpa_rope_req_t& r = reqs[i];
             auto it = c->streams.find(StreamKey{r.layer, r.kv_head, r.seq_id});
@@ -912,26 +912,12 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
             if (r.first_token < 0 || r.n_tokens < 1 || r.first_token + r.n_tokens > rec.kv_len)
                 return fail(SEGPA_ERR_INVALID, "rope_align[%d]: token range outside the stream", i);
             for (const Rng& g : seen)
-                if (g.key == it->first && r.first_token < g.hi && g.lo < r.first_token + r.n_tokens)
+                if (g.rec == &rec && r.first_token < g.hi && g.lo < r.first_token + r.n_tokens)
                     return fail(SEGPA_ERR_INVALID, "rope_align[%d]: token range overlaps an earlier request of the batch", i);
-            seen.push_back(Rng{it->first, r.first_token, r.first_token + r.n_tokens});
-            const int64_t pg_lo = rec.slot_of(r.first_token) / P, pg_hi = rec.slot_of(r.first_token + r.n_tokens - 1) / P + 1;
-            for (int64_t pg = pg_lo; pg < pg_hi; ++pg) {
-                const int32_t id = rec.pages[(size_t)pg];
-                if (id < 0) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: the range touches an evicted page", i);
-                if (c->refcnt[id] > 1) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: page %d is shared with another stream", i, id);
-            }
-            // one job per piece that is contiguous in slot space (a range may span head segments with ragged tails)
+            seen.push_back(Rng{&rec, r.first_token, r.first_token + r.n_tokens});
             for_each_piece(rec, r.first_token, r.n_tokens, [&](int64_t, int64_t n_piece, int64_t slot_lo) {
-                RopeJob jb{};
-                jb.chunk_begin = total_chunks;
-                jb.page_off = (long long)ids.size();
-                jb.n_tokens = n_piece;
-                jb.delta_pos = r.delta_pos;   // R(p_on) R(p_off)^-1 = R(delta); the per-pair cos / sin are formed on the device in fp64
-                jb.first_slot = (int)(slot_lo % P);
-                ids.insert(ids.end(), rec.pages.begin() + slot_lo / P, rec.pages.begin() + (slot_lo + n_piece - 1) / P + 1);
-                total_chunks += n_piece * (D >> 4);
-                jobs.push_back(jb);
+                ++n_jobs;
+                n_ids += (size_t)((slot_lo + n_piece - 1) / P - slot_lo / P + 1);
             });
         }
     } catch (const std::bad_alloc&) {
@@ -942,17 +928,60 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
     Staging& sg = c->append_stage[c->append_turn];
     c->append_turn ^= 1;
     auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
-    const size_t off_tabs = al(jobs.size() * sizeof(RopeJob));
-    const size_t off_ids = al(off_tabs + jobs.size() * sizeof(RopeTable));   // (tables: device scratch, not uploaded)
-    const size_t bytes = off_ids + ids.size() * sizeof(int32_t);
+    const size_t off_tabs = al(n_jobs * sizeof(RopeJob));
+    const size_t off_ids = al(off_tabs + n_jobs * sizeof(RopeTable));   // (tables: device scratch, not uploaded)
+    const size_t bytes = off_ids + n_ids * sizeof(int32_t);
     cudaError_t e = staging_acquire(sg, bytes);
-    if (e == cudaSuccess) {
-        memcpy(sg.h, jobs.data(), jobs.size() * sizeof(RopeJob));
-        memcpy((uint8_t*)sg.h + off_ids, ids.data(), ids.size() * sizeof(int32_t));
-        e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "rope_align: %s", cudaGetErrorString(e)); }
+    // Pass 2: the jobs and their page ids are written straight into the pinned staging buffer; every page is checked on
+    // the way (evicted: id < 0; shared with another stream: rotating it would move that stream's keys too).  The
+    // reference counts are read in the (random) order of the ids: fetched ahead.
+    RopeJob* jobs = (RopeJob*)sg.h;
+    int32_t* ids = (int32_t*)((uint8_t*)sg.h + off_ids);
+    size_t nj = 0, ni = 0;
+    long long total_chunks = 0;
+    int32_t min_id = 0, max_ref = 0;
+    const int32_t* refcnt = c->refcnt.data();
+    const int32_t n_pool = (int32_t)c->desc.num_pages;
+    for (int32_t i = 0; i < n; ++i) {
+        const segpa_rope_req_t& r = reqs[i];
+        const StreamRec& rec = *seen[(size_t)i].rec;
+        for_each_piece(rec, r.first_token, r.n_tokens, [&](int64_t, int64_t n_piece, int64_t slot_lo) {
+            RopeJob jb{};
+            jb.chunk_begin = total_chunks;
+            jb.page_off = (long long)ni;
+            jb.n_tokens = n_piece;
+            jb.delta_pos = r.delta_pos;   // R(p_on) R(p_off)^-1 = R(delta); the per-pair cos / sin are formed on the device in fp64
+            jb.first_slot = (int)(slot_lo % P);
+            const int32_t* pg = rec.pages.data() + slot_lo / P;
+            const int64_t np = (slot_lo + n_piece - 1) / P - slot_lo / P + 1;
+            for (int64_t k = 0; k < np; ++k) {
+                const int32_t id = pg[k];
+                if (k + 16 < np && (uint32_t)pg[k + 16] < (uint32_t)n_pool) __builtin_prefetch(refcnt + pg[k + 16]);
+                min_id = std::min(min_id, id);
+                max_ref = std::max(max_ref, refcnt[id < 0 ? 0 : id]);
+                ids[ni++] = id;
+            }
+            total_chunks += n_piece * (D >> 4);
+            jobs[nj++] = jb;
+        });
     }
+    if (min_id < 0 || max_ref > 1) {   // (the search for the message only on failure; nothing has been launched)
+        for (int32_t i = 0; i < n; ++i) {
+            const segpa_rope_req_t& r = reqs[i];
+            const StreamRec& rec = *seen[(size_t)i].rec;
+            const int64_t pg_lo = rec.slot_of(r.first_token) / P, pg_hi = rec.slot_of(r.first_token + r.n_tokens - 1) / P + 1;
+            for (int64_t pg = pg_lo; pg < pg_hi; ++pg) {
+                const int32_t id = rec.pages[(size_t)pg];
+                if (id < 0) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: the range touches an evicted page", i);
+                if (c->refcnt[id] > 1) return fail(SEGPA_ERR_INVALID, "rope_align[%d]: page %d is shared with another stream", i, id);
+            }
+        }
+        return fail(SEGPA_ERR_INVALID, "rope_align: a page of a range is evicted or shared with another stream");
+    }
+    e = staging_upload(sg, bytes, c->up_stream, st);
     if (e == cudaSuccess)
-        e = launch_rope_align(c->k_pool, (const RopeJob*)sg.d, (RopeTable*)((uint8_t*)sg.d + off_tabs), (int)jobs.size(),
+        e = launch_rope_align(c->k_pool, (const RopeJob*)sg.d, (RopeTable*)((uint8_t*)sg.d + off_tabs), (int)n_jobs,
                               (const int*)((const uint8_t*)sg.d + off_ids), total_chunks, rope_base, D, P, st);
     if (e == cudaSuccess) staging_release(sg, st);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "rope_align: %s", cudaGetErrorString(e)); }

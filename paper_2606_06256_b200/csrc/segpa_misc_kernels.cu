@@ -64,6 +64,7 @@ cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const Scatter
 // fp32 argument reduction would cost ~1e-3 rad), rounded once to fp32
 __global__ void rope_table_kernel(const RopeJob* __restrict__ jobs, RopeTable* __restrict__ tabs, double rope_base, int D) {
     const int d = threadIdx.x;
+    ptx::pdl_launch_dependents();   // (the rotation kernel starts its prologue now and waits for this grid in pdl_wait)
     if (d >= D / 2) return;
     const double ang = (double)jobs[blockIdx.x].delta_pos * pow(rope_base, -2.0 * d / D);
     double sn, cs;
@@ -76,6 +77,8 @@ __global__ void rope_align_kernel(uint8_t* __restrict__ k_pool, const RopeJob* _
                                   const RopeTable* __restrict__ tabs, int n_jobs, const int* __restrict__ page_ids,
                                   long long total_chunks, int D, int P) {
     const int cph = D >> 4;  // 16-byte chunks per half row
+    ptx::pdl_launch_dependents();
+    ptx::pdl_wait();         // the cos / sin tables are the table kernel's; the K pages may still be read by the kernel before it
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total_chunks;
          idx += (long long)gridDim.x * blockDim.x) {
         int lo = 0, hi = n_jobs - 1;
@@ -127,8 +130,8 @@ cudaError_t launch_rope_align(uint8_t* k_pool, const RopeJob* jobs_dev, RopeTabl
     rope_table_kernel<<<n_jobs, 64, 0, st>>>(jobs_dev, tabs_dev, rope_base, D);
     long long blocks = (total_chunks + 255) / 256;
     if (blocks > 148 * 32) blocks = 148 * 32;
-    rope_align_kernel<<<(unsigned)blocks, 256, 0, st>>>(k_pool, jobs_dev, tabs_dev, n_jobs, page_ids_dev, total_chunks, D, P);
-    return cudaGetLastError();
+    return launch_pdl(rope_align_kernel, dim3((unsigned)blocks), dim3(256), 0, st, k_pool, jobs_dev, (const RopeTable*)tabs_dev, n_jobs, page_ids_dev,
+                      total_chunks, D, P);
 }
 
 // ---------------------------------------------------------------------------------------------
