@@ -45,17 +45,18 @@ def load_peaks():
 
 
 def ncu_traffic(workload: str):
-    """DRAM bytes (read + write) of one attention launch from the committed ncu --set full capture of this
-    workload (profiles/r1_traffic.csv), or None when none was taken."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    """(DRAM bytes read + written by one attention launch, what that launch was) from the committed ncu --set full
+    capture of this workload (profiles/r2_traffic.csv; commands in profiles/r2_ncu_full_attention_tc.md), or
+    (None, None) when none was taken."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     try:
         for line in open(p).read().splitlines()[1:]:
-            f = line.rsplit(",", 1)
-            if f[0].split(",")[0] == workload:
-                return int(f[1])
+            f = line.split(",")
+            if f[0] == workload:
+                return int(f[-1]), ",".join(f[1:-1])
     except Exception:
         pass
-    return None
+    return None, None
 
 
 def max_over_ranks(x: float, dist, device) -> float:
@@ -410,7 +411,7 @@ def measure(name: str, steps: int, warmup: int, dev, local_rank: int, world: int
         roof = {"bound": "tensor", "achieved": ach, "peak": pk, "unit": "TFLOP/s", "frac": ach / pk,
                 "frac_of_burst": ach / peaks["bf16_tflops"], "frac_of_sustained": ach / peaks["bf16_tflops_sustained"],
                 "peak_source": peaks_src + (", sustained figure (kernel timed inside a %.0f ms step)" % fwd_mean if long_step else ", burst figure")}
-    roof["traffic"] = ncu_traffic(w.name)
+    roof["traffic"], roof["traffic_capture"] = ncu_traffic(w.name)
     roof["kernel"] = "attention_tc_kernel (+ combine_kernel where the plan splits KV) = segpa_attention_fwd, mean over %d steps x %d layers, CUDA events on the launching stream" % (steps, w.num_layers)
     roof["algorithmic_bytes"] = alg_bytes
     roof["useful_flops"] = useful
