@@ -181,11 +181,212 @@ __device__ __forceinline__ ItemBlocks item_blocks(const ItemDev& it, const SegDe
     return b;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Softmax of a decode-shaped plan (instantiation NARROW: every tile of the plan holds <= 16 valid rows).
+// With one thread per query row the exponentials of a 4-row tile cost as much as those of a 128-row tile
+// (MUFU.EX2 occupies its pipe 8 cycles per warp instruction whatever the number of active lanes: measured), and the
+// chain QK^T -> softmax -> PV of a decode step was bound by them (1 500 of ~2 500 cycles per block), not by HBM.
+// Here a row is spread over FOUR threads: warp 0 of the tile's softmax warpgroup reads S with the 16x256b shape
+// (thread t: rows t/4 and t/4 + 8, columns 8i + 2(t%4), +1 of every 8), so a thread holds 32 columns of a row (64 with
+// rows 8..15 in use), reduces max / sum over its group of four with two shuffles, and writes bf16 P back with the
+// 16x128b shape, whose column 4i + t%4 is exactly the pair it has just packed.  Warps 1..3 of the warpgroup hold no row.
+// ---------------------------------------------------------------------------------------------
+template <int D, bool RG>
+__device__ __forceinline__ void softmax_narrow(const FwdParams& p, Bars& bars, float2 (&stats)[2][kTileRows], const uint32_t tmem,
+                                               const int tile, const int wq, const int lane, const int i_lo, const int i_hi,
+                                               const int TT, const int G) {
+    const uint32_t tS = tmem + tile * 128;            // lanes 0..15 of quadrant 0
+    const uint32_t tO = tmem + 256 + tile * 128;
+    const float sl2 = p.scale * 1.4426950408889634f;
+    const int g = lane >> 2, q = lane & 3;
+    uint32_t n_s = 0, n_st = 0;
+    for (int ii = i_lo; ii < i_hi; ++ii) {
+        const ItemDev it = p.items[ii];
+        const SegDev sg = p.segs[it.seg];
+        const TileRange tr = tile_range(it, sg, p.pads, tile, TT, G);
+        if (tr.n_rows == 0) continue;
+        const int nb = n_blocks(tr);
+        if (wq != 0) {   // no rows in this warp: keep the barriers' arrival counts
+            for (int kb = 0; kb < nb; ++kb) {
+                mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
+                ++n_s;
+                mbar_arrive(smem_u32(&bars.p_full[tile][0]));
+                mbar_arrive(smem_u32(&bars.p_full[tile][1]));
+            }
+            mbar_wait(smem_u32(&bars.stat_free[tile]), (n_st & 1) ^ 1);
+            ++n_st;
+            mbar_arrive(smem_u32(&bars.stat_full[tile]));
+            continue;
+        }
+        // rows X = 0: g, X = 1: g + 8 (rows past the end mirror the last valid row)
+        const bool useB = tr.n_rows > 8;
+        int pos[2], klo[2];
+        bool live[2];
+#pragma unroll
+        for (int X = 0; X < 2; ++X) {
+            const int row = g + 8 * X;
+            live[X] = row < tr.n_rows;
+            pos[X] = sg.kv_len - sg.q_len + tr.tok0 + min(row, tr.n_rows - 1) / G;
+            klo[X] = max(0, pos[X] - sg.window + 1);
+        }
+        const int pos_min = sg.kv_len - sg.q_len + tr.tok0, pos_max = pos_min + (tr.n_rows - 1) / G;
+        const int klo_max = max(0, pos_max - sg.window + 1);
+        float m[2] = {-INFINITY, -INFINITY}, l[2] = {0.f, 0.f};   // l: this thread's part of the row sum
+        for (int kb = 0; kb < nb; ++kb) {
+            const int j = block_at(tr, kb);
+            mbar_wait(smem_u32(&bars.s_full[tile]), n_s & 1);
+            ++n_s;
+            tc_fence_after();
+            int tokb = j * kBlockKeys;      // token of column 0 (see the one-thread-per-row path)
+            bool ragged_blk = false;
+            if (RG && sg.n_pads > 0) {
+                int padv = 0, prev = 0;
+                for (int k = 0; k < sg.n_pads; ++k) {
+                    const PadDev pd = p.pads[sg.pad_off + k];
+                    const int seg0 = pd.tok + pd.pad, tail = pd.tok + prev;
+                    if (seg0 <= j * kBlockKeys) padv = pd.pad;
+                    else if (tail < (j + 1) * kBlockKeys) ragged_blk = true;
+                    prev = pd.pad;
+                }
+                tokb -= padv;
+            }
+            // element (row X, repeat i, e) = s[4 i + 2 X + e], column 8 i + 2 q + e
+            uint32_t s[64];
+            tmem_ld_16x256b_x16(tS, s);
+            tmem_wait_ld();
+            const int csink = sg.n_sink - tokb;
+            const bool need_mask = pos_min - tokb < kBlockKeys - 1 || (klo_max - tokb > 0 && csink < kBlockKeys);
+            if (RG && ragged_blk) {
+#pragma unroll
+                for (int X = 0; X < 2; ++X) {
+                    uint32_t vis[4] = {0u, 0u, 0u, 0u};
+                    auto add_bits = [&vis](int a, int b) {
+#pragma unroll
+                        for (int w = 0; w < 4; ++w) {
+                            const int lo = min(max(a - 32 * w, 0), 32), hi = min(max(b - 32 * w, 0), 32);
+                            if (hi > lo) vis[w] |= (hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u);
+                        }
+                    };
+                    const int B = j * kBlockKeys;
+                    int start = 0, pad_c = 0;
+                    for (int k = 0; k <= sg.n_pads; ++k) {
+                        int end = INT_MAX, nstart = 0, npad = 0;
+                        if (k < sg.n_pads) {
+                            const PadDev pd = p.pads[sg.pad_off + k];
+                            end = pd.tok + pad_c;
+                            nstart = pd.tok + pd.pad;
+                            npad = pd.pad;
+                        }
+                        const int ra = max(start, B) - B, rb = min(end, B + kBlockKeys) - B;
+                        if (ra < rb) {
+                            const int off = B - pad_c;
+                            add_bits(max(ra, klo[X] - off), min(rb, pos[X] - off + 1));
+                            add_bits(ra, min(rb, min(sg.n_sink, pos[X] + 1) - off));
+                        }
+                        start = nstart;
+                        pad_c = npad;
+                    }
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int c = 8 * i + 2 * q + e;
+                            if (!((vis[c >> 5] >> (c & 31)) & 1u)) s[4 * i + 2 * X + e] = 0xff800000u;   // -inf
+                        }
+                }
+            } else if (need_mask) {
+                // visible columns of row X: c <= cmax and (c >= cmin or c < csink); also drops whatever a half of S that
+                // this block's QK^T did not write still holds
+#pragma unroll
+                for (int X = 0; X < 2; ++X) {
+                    const int cmin = klo[X] - tokb, cmax = pos[X] - tokb;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i)
+#pragma unroll
+                        for (int e = 0; e < 2; ++e) {
+                            const int c = 8 * i + 2 * q + e;
+                            if (c > cmax || (c < cmin && c >= csink)) s[4 * i + 2 * X + e] = 0xff800000u;
+                        }
+                }
+            }
+            // row max over the thread's columns, then over its group of four
+            float mx[2];
+#pragma unroll
+            for (int X = 0; X < 2; ++X) {
+                float ma = -INFINITY, mb = -INFINITY;
+#pragma unroll
+                for (int i = 0; i < 16; i += 2) {
+                    ma = max3(ma, __uint_as_float(s[4 * i + 2 * X]), __uint_as_float(s[4 * i + 2 * X + 1]));
+                    mb = max3(mb, __uint_as_float(s[4 * i + 4 + 2 * X]), __uint_as_float(s[4 * i + 4 + 2 * X + 1]));
+                }
+                float v = fmaxf(ma, mb);
+                v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 1));
+                v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, 2));
+                mx[X] = v * sl2;
+            }
+            // lazy rescale, as in the one-thread-per-row path (rows that hold nothing never ask for one)
+            const bool growA = live[0] && mx[0] > m[0] + kRescaleThreshold, growB = live[1] && mx[1] > m[1] + kRescaleThreshold;
+            if (__any_sync(0xffffffffu, growA || growB)) {
+                float corr[2] = {1.f, 1.f};
+                if (growA) { corr[0] = (m[0] == -INFINITY) ? 0.f : fast_exp2(m[0] - mx[0]); m[0] = mx[0]; l[0] *= corr[0]; }
+                if (growB) { corr[1] = (m[1] == -INFINITY) ? 0.f : fast_exp2(m[1] - mx[1]); m[1] = mx[1]; l[1] *= corr[1]; }
+                if (kb > 0) {
+                    uint32_t o[D / 2];
+                    if (D == 128) tmem_ld_16x256b_x16(tO, o); else tmem_ld_16x256b_x8(tO, o);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int i = 0; i < D / 8; ++i)
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) o[4 * i + e] = __float_as_uint(__uint_as_float(o[4 * i + e]) * corr[e >> 1]);
+                    if (D == 128) tmem_st_16x256b_x16(tO, o); else tmem_st_16x256b_x8(tO, o);
+                }
+            }
+            const float mref[2] = {(m[0] == -INFINITY) ? 0.f : m[0], (m[1] == -INFINITY) ? 0.f : m[1]};
+            // p = 2^(s*scale*log2e - m), bf16 pairs -> P (aliases S[0, 64)); keys [0, 64) first so that their PV can start
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                uint32_t pk[16];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int ib = 8 * h + i;
+#pragma unroll
+                    for (int X = 0; X < 2; ++X) {
+                        if (X == 1 && !useB) { pk[2 * i + 1] = 0u; continue; }
+                        const float p0 = fast_exp2(fmaf(__uint_as_float(s[4 * ib + 2 * X]), sl2, -mref[X]));
+                        const float p1 = fast_exp2(fmaf(__uint_as_float(s[4 * ib + 2 * X + 1]), sl2, -mref[X]));
+                        l[X] += p0 + p1;
+                        pk[2 * i + X] = pack_bf16x2(p0, p1);
+                    }
+                }
+                tmem_st_16x128b_x8(tS + 32 * h, pk);
+                tmem_wait_st();
+                tc_fence_before();
+                mbar_arrive(smem_u32(&bars.p_full[tile][h]));
+            }
+        }
+        // row sums over the groups of four (butterflies: every thread of a group ends with the same bits), then hand (m, l)
+        // of rows g and g + 8 to the epilogue warpgroup
+#pragma unroll
+        for (int X = 0; X < 2; ++X) {
+            l[X] += __shfl_xor_sync(0xffffffffu, l[X], 1);
+            l[X] += __shfl_xor_sync(0xffffffffu, l[X], 2);
+        }
+        mbar_wait(smem_u32(&bars.stat_free[tile]), (n_st & 1) ^ 1);
+        ++n_st;
+        if (q == 0) {
+            stats[tile][g] = make_float2(m[0], l[0]);
+            stats[tile][g + 8] = make_float2(m[1], l[1]);
+        }
+        mbar_arrive(smem_u32(&bars.stat_full[tile]));
+    }
+}
+
 }  // namespace
 
 // RG: the plan has ragged streams (head segments with partial last pages in mid-stream).  The dense
 // instantiation carries none of that code: inlined into the softmax loop it cost cfg2 3 % even when never taken.
-template <int D, int NT, bool RG>
+// NARROW: every tile of the plan holds <= 16 valid rows (a decode-shaped plan): the softmax spreads a row over four threads.
+template <int D, int NT, bool RG, bool NARROW>
 __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_constant__ FwdParams p) {
     using C = Cfg<D, NT>;
     extern __shared__ uint8_t smem_raw[];
@@ -477,7 +678,9 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
         // ------------------------------------------------------------------ softmax warpgroups
         reg_inc<kRegsSoftmax>();
         const int tile = (warp - kFirstSoftmaxWarp) >> 2;
-        if (tile < NT) {
+        if (NARROW) {
+            if (tile < NT) softmax_narrow<D, RG>(p, bars, stats, tmem, tile, warp & 3, lane, i_lo, i_hi, TT, G);
+        } else if (tile < NT) {
             const int wq = warp & 3;                       // TMEM lane quadrant this warp may access
             const int r = wq * 32 + lane;                  // row inside the tile
             const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
@@ -804,7 +1007,7 @@ __global__ void __launch_bounds__(kThreads, 1) attention_tc_kernel(const __grid_
 }
 
 // ---------------------------------------------------------------------------------------------
-template <int D, int NT, bool RG>
+template <int D, int NT, bool RG, bool NARROW>
 static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
     using C = Cfg<D, NT>;
     // the opt-in to > 48 KB of dynamic shared memory is per device: remember which devices have it
@@ -812,21 +1015,23 @@ static cudaError_t launch_one(const FwdParams& p, cudaStream_t st) {
     int dev = 0;
     cudaGetDevice(&dev);
     if (dev < 0 || dev >= 64 || !configured[dev]) {
-        cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<D, NT, RG>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+        cudaError_t e = cudaFuncSetAttribute(attention_tc_kernel<D, NT, RG, NARROW>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
         if (e != cudaSuccess) return e;
         if (dev >= 0 && dev < 64) configured[dev] = true;
     }
-    return launch_pdl(attention_tc_kernel<D, NT, RG>, dim3((unsigned)p.n_cta), dim3(kThreads), (size_t)C::kSmemBytes, st, p);
+    return launch_pdl(attention_tc_kernel<D, NT, RG, NARROW>, dim3((unsigned)p.n_cta), dim3(kThreads), (size_t)C::kSmemBytes, st, p);
+}
+
+template <int D, int NT>
+static cudaError_t launch_shape(const FwdParams& p, cudaStream_t st) {
+    if (p.narrow) return p.has_ragged ? launch_one<D, NT, true, true>(p, st) : launch_one<D, NT, false, true>(p, st);
+    return p.has_ragged ? launch_one<D, NT, true, false>(p, st) : launch_one<D, NT, false, false>(p, st);
 }
 
 cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st) {
     if (p.n_items == 0) return cudaSuccess;
-    if (p.has_ragged) {
-        if (p.tiles_per_item == 2) return p.D == 128 ? launch_one<128, 2, true>(p, st) : launch_one<64, 2, true>(p, st);
-        return p.D == 128 ? launch_one<128, 1, true>(p, st) : launch_one<64, 1, true>(p, st);
-    }
-    if (p.tiles_per_item == 2) return p.D == 128 ? launch_one<128, 2, false>(p, st) : launch_one<64, 2, false>(p, st);
-    return p.D == 128 ? launch_one<128, 1, false>(p, st) : launch_one<64, 1, false>(p, st);
+    if (p.tiles_per_item == 2) return p.D == 128 ? launch_shape<128, 2>(p, st) : launch_shape<64, 2>(p, st);
+    return p.D == 128 ? launch_shape<128, 1>(p, st) : launch_shape<64, 1>(p, st);
 }
 
 }  // namespace segpa

@@ -191,6 +191,7 @@ struct segpa_segments {
     std::vector<int32_t> cta_off;   // items of CTA q: [cta_off[q], cta_off[q+1])
     std::vector<int64_t> mass_off;  // [n + 1]: layout of the attention-mass array (kv_len rounded up to 128 per segment)
     bool has_ragged = false;             // some segment's stream has head segments with partial last pages
+    bool narrow = false;                 // every tile holds <= 16 rows (decode-shaped plan; FwdParams::narrow)
     mutable bool mass_planned = false;   // mass plan built and uploaded (lazily, by the first segpa_attention_mass)
     mutable int mass_n_cta = 0;
     mutable size_t m_off_items = 0, m_off_cta = 0, m_off_layout = 0, m_off_kvlen = 0;
@@ -216,7 +217,7 @@ struct segpa_segments {
     void reset() {
         cache = nullptr; layer = 0;
         reqs.clear(); segs.clear(); items.clear(); item_meta.clear(); pages.clear(); pads.clear(); combs.clear(); cta_off.clear(); mass_off.clear();
-        mass_planned = false; mass_n_cta = 0; has_ragged = false;
+        mass_planned = false; mass_n_cta = 0; has_ragged = false; narrow = false;
         hchunks.clear(); host_planned = false;
         m_off_items = m_off_cta = m_off_layout = m_off_kvlen = 0;
         stats = segpa_plan_stats_t{};
@@ -485,6 +486,7 @@ void fill_fwd_params(FwdParams& p, const segpa_cache* c, const segpa_segments* s
     p.page_bytes = c->page_bytes;
     p.num_sms = c->num_sms;
     p.has_ragged = s->has_ragged ? 1 : 0;
+    p.narrow = s->narrow ? 1 : 0;
 }
 
 }  // namespace
@@ -1264,6 +1266,8 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             }
         }
         const int64_t kv_blocks = lpt_assign(ps, S->items, &S->item_meta, c->num_sms, S->cta_off);
+        S->narrow = c->kernel_kind == 1;
+        for (const ItemDev& itd : S->items) S->narrow = S->narrow && itd.n_tok * G <= 16;
 
         segpa_plan_stats_t& stt = S->stats;
         stt.n_segments = n;

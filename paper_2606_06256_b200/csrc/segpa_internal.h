@@ -114,6 +114,8 @@ struct FwdParams {
     int tiles_per_item;
     int page_bytes;
     int num_sms;
+    int narrow;                  // every tile of the plan holds <= 16 rows (decode-shaped plan): the instantiation whose softmax
+                                 // spreads a row over four threads
     int has_ragged;              // some segment's stream is ragged (SegDev::n_pads > 0): the kernel instantiation with that code
 #ifdef SEGPA_TRACE
     unsigned long long* trace;   // [16 warps][kTraceCap] (tag << 56 | arg << 40 | clock) of CTA 0; debug builds only
