@@ -802,9 +802,14 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 const HostCopy& hc = host_copies[h];
                 uint16_t* kd = c->st_kv + (size_t)hc.off_rows * D;
                 uint16_t* vd = c->st_kv + (size_t)(host_rows_total + hc.off_rows) * D;
-                e = cudaMemcpy2DAsync(kd, (size_t)D * 2, hc.k, (size_t)hc.stride * 2, (size_t)D * 2, (size_t)hc.n, cudaMemcpyHostToDevice, st);
-                if (e == cudaSuccess)
-                    e = cudaMemcpy2DAsync(vd, (size_t)D * 2, hc.v, (size_t)hc.stride * 2, (size_t)D * 2, (size_t)hc.n, cudaMemcpyHostToDevice, st);
+                if (hc.stride == D) {   // contiguous rows: one plain copy each
+                    e = cudaMemcpyAsync(kd, hc.k, (size_t)hc.n * D * 2, cudaMemcpyHostToDevice, st);
+                    if (e == cudaSuccess) e = cudaMemcpyAsync(vd, hc.v, (size_t)hc.n * D * 2, cudaMemcpyHostToDevice, st);
+                } else {
+                    e = cudaMemcpy2DAsync(kd, (size_t)D * 2, hc.k, (size_t)hc.stride * 2, (size_t)D * 2, (size_t)hc.n, cudaMemcpyHostToDevice, st);
+                    if (e == cudaSuccess)
+                        e = cudaMemcpy2DAsync(vd, (size_t)D * 2, hc.v, (size_t)hc.stride * 2, (size_t)D * 2, (size_t)hc.n, cudaMemcpyHostToDevice, st);
+                }
             }
         }
         if (e == cudaSuccess)
@@ -1190,8 +1195,12 @@ segpa_status_t segpa_build_segments(segpa_cache_t* c, int32_t layer, const segpa
             vis_tokens += last_slot + 1 - first_vis_page * P + sink_pages * P;
             q_rows = std::max<int64_t>(q_rows, r.q_row_start + r.q_len);
             pairs += visible_pairs(kv_len - r.q_len, kv_len - 1, W);
-            if (has_sink)   // sink keys not already inside the window
-                for (int64_t i = kv_len - r.q_len; i < kv_len; ++i) pairs += std::max<int64_t>(0, std::min(ns, i - W + 1));
+            if (has_sink) {   // sink keys not already inside the window: sum over the queries i of clamp(i - W + 1, 0, ns)
+                const int64_t a = kv_len - r.q_len - W + 1, b = kv_len - W;          // x = i - W + 1 runs over [a, b]
+                const int64_t lo = std::max<int64_t>(a, 1), mid = std::min<int64_t>(b, ns);   // x in [lo, mid] contributes x, x > ns contributes ns
+                if (mid >= lo) pairs += (lo + mid) * (mid - lo + 1) / 2;
+                if (b > ns) pairs += (b - std::max<int64_t>(a, ns + 1) + 1) * ns;
+            }
             // tiles: exactly the KV blocks (of slots) the tile's rows attend to
             for (int64_t t0 = 0; t0 < r.q_len; t0 += item_tok) {
                 const int64_t n_tok = std::min<int64_t>(item_tok, r.q_len - t0);
@@ -1678,7 +1687,14 @@ namespace {
 
 // builds and uploads the attention-mass plan of a segments object (once)
 segpa_status_t plan_mass(segpa_cache* c, const segpa_segments* s, cudaStream_t st) {
-    if (s->mass_planned) return SEGPA_OK;
+    if (s->mass_planned) {
+        // the plan was uploaded by an earlier call, possibly on another stream: order this stream after that copy
+        if (s->buf->mass_blob.up && cudaStreamWaitEvent(st, s->buf->mass_blob.up, 0) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(SEGPA_ERR_CUDA, "attention_mass: cannot order the stream after the plan upload");
+        }
+        return SEGPA_OK;
+    }
     const int TT = kTileRows / c->G;
     std::vector<MassItem> items;
     for (size_t si = 0; si < s->segs.size(); ++si) {
@@ -1737,7 +1753,7 @@ segpa_status_t plan_mass(segpa_cache* c, const segpa_segments* s, cudaStream_t s
         memcpy(hb + s->m_off_cta, cta_off.data(), cta_off.size() * sizeof(int32_t));
         memcpy(hb + s->m_off_layout, s->mass_off.data(), s->mass_off.size() * sizeof(int64_t));
         memcpy(hb + s->m_off_kvlen, kv_lens.data(), kv_lens.size() * sizeof(int32_t));
-        e = cudaMemcpyAsync(sg.d, sg.h, bytes, cudaMemcpyHostToDevice, st);
+        e = staging_upload(sg, bytes, c->up_stream, st);   // (recorded in sg.up: calls on other streams wait for it, below)
     }
     if (e != cudaSuccess) { cudaGetLastError(); return fail(e == cudaErrorMemoryAllocation ? SEGPA_ERR_OOM : SEGPA_ERR_CUDA, "attention_mass: %s", cudaGetErrorString(e)); }
     s->mass_n_cta = n_cta;

@@ -5,7 +5,7 @@
 // exist in memory).  Transposed formulation so that the sum over queries is an in-thread sum:
 //     S^T = K_block Q_tile^T    (M = 128 keys = TMEM lanes, N = 128 query rows = columns)
 // tcgen05.mma with both operands K-major from shared memory (K pages by bulk copy, Q tiles by TMA), accumulator
-// double-buffered in TMEM; one thread per key applies the visibility rule and ex2 to its 128 columns and keeps the
+// four-deep in TMEM (all 512 columns), K block double-buffered; one thread per key applies the visibility rule and ex2 to its 128 columns and keeps the
 // running sum in a register.  A CTA owns a (segment, key block) item and loops over the query tiles that can see
 // it: every mass entry is written exactly once, by one thread (deterministic, no atomics).
 // Bound: the dense contraction is half of the attention kernel's (no PV) and the exponentials are the same, so the
@@ -30,13 +30,17 @@ struct alignas(16) MassAux {
     int pad[2];
 };
 
-constexpr int kQStages = 4;   // Q tiles in flight (the S accumulator and the per-column arrays are double-buffered)
+constexpr int kQStages = 4;   // Q tiles in flight
+constexpr int kSStages = 4;   // S accumulators in TMEM (4 x 128 columns) and per-column arrays: the MMA issuer and the LSE
+                              // warps run up to three tiles ahead of the exp warpgroups, which then never wait for a tile
+                              // (round 1 had two: MUFU pipe active 53 % of the time)
+constexpr int kKStages = 2;   // K blocks: the next item's block is loaded under the current item's last tiles
 
 struct MassBars {
-    uint64_t k_full, k_empty;
+    uint64_t k_full[kKStages], k_empty[kKStages];
     uint64_t q_full[kQStages], q_empty[kQStages];
-    uint64_t aux_full[2], aux_empty[2];
-    uint64_t s_full[2], s_empty[2];
+    uint64_t aux_full[kSStages], aux_empty[kSStages];
+    uint64_t s_full[kSStages], s_empty[kSStages];
     uint32_t tmem_base;
 };
 
@@ -49,23 +53,25 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
     constexpr uint32_t kSBO = kHalves * kAtomBytes;
     extern __shared__ uint8_t smem_raw[];
     __shared__ MassBars bars;
-    __shared__ MassAux aux[2];
+    __shared__ MassAux aux[kSStages];
     __shared__ float half_sum[kTileRows];   // partial mass of the second exp warpgroup, added by the first
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
-    const uint32_t sK = smem_u32(smem);
-    const uint32_t sQ = sK + kTileBytes;          // kQStages Q stages
+    const uint32_t sK = smem_u32(smem);           // kKStages K blocks
+    const uint32_t sQ = sK + kKStages * kTileBytes;   // kQStages Q stages
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
     const int i_lo = p.cta_off[blockIdx.x], i_hi = p.cta_off[blockIdx.x + 1];
 
     if (threadIdx.x == 0) {
-        mbar_init(smem_u32(&bars.k_full), 1);
-        mbar_init(smem_u32(&bars.k_empty), 1);
+        for (int s = 0; s < kKStages; ++s) {
+            mbar_init(smem_u32(&bars.k_full[s]), 1);
+            mbar_init(smem_u32(&bars.k_empty[s]), 1);
+        }
         for (int s = 0; s < kQStages; ++s) {
             mbar_init(smem_u32(&bars.q_full[s]), 1);
             mbar_init(smem_u32(&bars.q_empty[s]), 1);
         }
-        for (int s = 0; s < 2; ++s) {
+        for (int s = 0; s < kSStages; ++s) {
             mbar_init(smem_u32(&bars.aux_full[s]), 1);
             mbar_init(smem_u32(&bars.aux_empty[s]), 256);
             mbar_init(smem_u32(&bars.s_full[s]), 1);
@@ -74,7 +80,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
         fence_mbar_init();
     }
     if (warp == 3) {
-        tmem_alloc(smem_u32(&bars.tmem_base), 256);
+        tmem_alloc(smem_u32(&bars.tmem_base), 512);
         tmem_relinquish();
     }
     tc_fence_before();
@@ -89,14 +95,16 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
         for (int ii = i_lo; ii < i_hi; ++ii) {
             const MassItem it = p.items[ii];
             const SegDev sg = p.segs[it.seg];
+            const uint32_t ks = n_k % kKStages, kph = (n_k / kKStages) & 1;
             if (lane == 0) {
-                mbar_wait(smem_u32(&bars.k_empty), (n_k & 1) ^ 1);
-                mbar_arrive_expect_tx(smem_u32(&bars.k_full), kTileBytes);
+                mbar_wait(smem_u32(&bars.k_empty[ks]), kph ^ 1);
+                mbar_arrive_expect_tx(smem_u32(&bars.k_full[ks]), kTileBytes);
             }
             __syncwarp();
             if (lane < ppb) {
                 const int page = p.pages[sg.page_off + (long long)(it.kb * ppb - sg.first_page) + lane];
-                bulk_g2s(sK + lane * p.page_bytes, p.k_pool + (size_t)page * p.page_bytes, p.page_bytes, smem_u32(&bars.k_full));
+                bulk_g2s(sK + ks * kTileBytes + lane * p.page_bytes, p.k_pool + (size_t)page * p.page_bytes, p.page_bytes,
+                         smem_u32(&bars.k_full[ks]));
             }
             ++n_k;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
@@ -123,8 +131,8 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             const SegDev sg = p.segs[it.seg];
             const int p0 = sg.kv_len - sg.q_len;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
-                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
-                if ((int)st != warp - 2) continue;
+                const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
+                if ((int)(n_t & 1) != warp - 2) continue;
                 const int tok0 = ti * TT;
                 const int n_rows = min(TT, sg.q_len - tok0) * G;
                 // columns past the segment's rows: position -1 (their scores are garbage and never counted)
@@ -171,11 +179,13 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
         uint32_t n_k = 0, n_t = 0;
         for (int ii = i_lo; ii < i_hi; ++ii) {
             const MassItem it = p.items[ii];
-            mbar_wait(smem_u32(&bars.k_full), n_k & 1);
+            const uint32_t ks = n_k % kKStages;
+            mbar_wait(smem_u32(&bars.k_full[ks]), (n_k / kKStages) & 1);
             ++n_k;
+            const uint64_t dk = dk0 + (uint64_t)((ks * kTileBytes) >> 4);
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
                 const uint32_t qs = n_t % kQStages, qph = (n_t / kQStages) & 1;
-                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
                 mbar_wait(smem_u32(&bars.q_full[qs]), qph);
                 mbar_wait(smem_u32(&bars.s_empty[st]), ph ^ 1);
                 tc_fence_after();
@@ -185,11 +195,11 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                     for (int kk = 0; kk < D / 16; ++kk) {
                         const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
                         const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
-                        mma_ss(tmem + st * 128, dk0 + ok, dq + oq, idesc, kk > 0 ? 1u : 0u);
+                        mma_ss(tmem + st * 128, dk + ok, dq + oq, idesc, kk > 0 ? 1u : 0u);
                     }
                     tc_commit(smem_u32(&bars.s_full[st]));
                     tc_commit(smem_u32(&bars.q_empty[qs]));
-                    if (ti + 1 == it.t_hi) tc_commit(smem_u32(&bars.k_empty));
+                    if (ti + 1 == it.t_hi) tc_commit(smem_u32(&bars.k_empty[ks]));
                 }
                 __syncwarp();
             }
@@ -212,7 +222,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             const bool is_sink_key = key < sg.n_sink;
             float acc = 0.f;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
-                const uint32_t st = n_t & 1, ph = (n_t >> 1) & 1;
+                const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
                 mbar_wait(smem_u32(&bars.aux_full[st]), ph);
                 mbar_wait(smem_u32(&bars.s_full[st]), ph);
                 tc_fence_after();
@@ -265,12 +275,12 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
 
     tc_fence_before();
     __syncthreads();
-    if (warp == 3) tmem_dealloc(tmem, 256);
+    if (warp == 3) tmem_dealloc(tmem, 512);
 }
 
 template <int D>
 static cudaError_t launch_mass_one(const MassParams& p, cudaStream_t st) {
-    constexpr int smem = (1 + kQStages) * kTileRows * D * 2 + 1024;
+    constexpr int smem = (kKStages + kQStages) * kTileRows * D * 2 + 1024;
     // the opt-in to > 48 KB of dynamic shared memory is per device: remember which devices have it
     static bool configured[64] = {};
     int dev = 0;
