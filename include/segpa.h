@@ -209,6 +209,24 @@ segpa_status_t segpa_gather_rows(segpa_cache_t *cache, int32_t layer, int32_t kv
                                  int64_t first_token, int64_t n_tokens, void *k_dst, void *v_dst,
                                  int64_t dst_row_stride_elems, void *cuda_stream);
 
+/*
+ * segpa_gather_rows for callers that may not allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): same arguments, same result bit for bit, and the call makes NO cudaMalloc /
+ * cudaFree / allocating library call.  Its scratch -- the device copy of the page ids the token range covers, which
+ * segpa_gather_rows keeps in a staging buffer that grows on demand -- is a fixed array of SEGPA_NOALLOC_MAX_PAGES
+ * int32 entries (64 KB) inside the library image, held by every GPU that loads the library until the process exits.
+ * Limit: the range [first_token, first_token + n_tokens) may cover at most SEGPA_NOALLOC_MAX_PAGES pages of the stream
+ * (262144 tokens at page_size 16); a longer range is refused with SEGPA_ERR_INVALID and a message that says so (split it,
+ * or use segpa_gather_rows).  All calls share the one array, which keeps the last call's ids: each call overwrites the
+ * entries it uses in stream order (nothing needs clearing), so calls on ONE stream may follow each other freely, but
+ * two calls that can overlap on the GPU (different streams with no dependency between them) race on it.
+ * Other errors: as segpa_gather_rows.
+ */
+#define SEGPA_NOALLOC_MAX_PAGES 16384
+segpa_status_t segpa_gather_rows_noalloc(segpa_cache_t *cache, int32_t layer, int32_t kv_head, int64_t seq_id,
+                                         int64_t first_token, int64_t n_tokens, void *k_dst, void *v_dst,
+                                         int64_t dst_row_stride_elems, void *cuda_stream);
+
 /* Drop every stream of the cache (all pages return to the free list).  Segment objects built
  * earlier keep their translated page lists and must not be used afterwards. */
 segpa_status_t segpa_clear_streams(segpa_cache_t *cache);

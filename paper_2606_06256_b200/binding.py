@@ -22,7 +22,7 @@ _STATUS = {0: "OK", 1: "INVALID", 2: "OOM", 3: "CUDA", 4: "UNSUPPORTED", 5: "STA
 
 EXPORTS = [
     "segpa_pool_bytes", "segpa_create_cache", "segpa_append_pages", "segpa_append_pages_batch",
-    "segpa_clear_streams", "segpa_evict_pages", "segpa_rope_align", "segpa_rope_align_batch", "segpa_gather_rows", "segpa_free_stream",
+    "segpa_clear_streams", "segpa_evict_pages", "segpa_rope_align", "segpa_rope_align_batch", "segpa_gather_rows", "segpa_gather_rows_noalloc", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
     "segpa_attention_fwd_host", "segpa_merge", "segpa_segments_mass_layout", "segpa_attention_mass",
@@ -118,6 +118,7 @@ def lib():
         L.segpa_rope_align_batch.argtypes = [C.c_void_p, C.POINTER(RopeReq), C.c_int32, C.c_double, C.c_void_p]
         L.segpa_gather_rows.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int64, C.c_int64, C.c_void_p,
                                         C.c_void_p, C.c_int64, C.c_void_p]
+        L.segpa_gather_rows_noalloc.argtypes = L.segpa_gather_rows.argtypes
         L.segpa_evict_pages.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.c_int32, C.c_int32]
         L.segpa_free_stream.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64]
         L.segpa_stream_info.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int64, C.POINTER(C.c_int64),
@@ -266,6 +267,22 @@ def segpa_gather_rows(cache: int, layer: int, kv_head: int, seq_id: int, first_t
     _check(lib().segpa_gather_rows(cache, layer, kv_head, seq_id, first_token, n_tokens,
                                    k_dst.data_ptr() if k_dst is not None else None,
                                    v_dst.data_ptr() if v_dst is not None else None, ref.stride(0), _stream_ptr(stream)))
+
+
+NOALLOC_MAX_PAGES = 16384
+
+
+def segpa_gather_rows_noalloc(cache: int, layer: int, kv_head: int, seq_id: int, first_token: int, n_tokens: int,
+                              k_dst=None, v_dst=None, stream=None) -> None:
+    """segpa_gather_rows without any device allocation (fixed 64 KB scratch in the library; at most NOALLOC_MAX_PAGES
+    pages per call; calls that overlap on the GPU race on the scratch)."""
+    ref = k_dst if k_dst is not None else v_dst
+    assert ref is not None and ref.is_cuda and ref.stride(-1) == 1
+    if k_dst is not None and v_dst is not None:
+        assert k_dst.stride(0) == v_dst.stride(0)
+    _check(lib().segpa_gather_rows_noalloc(cache, layer, kv_head, seq_id, first_token, n_tokens,
+                                           k_dst.data_ptr() if k_dst is not None else None,
+                                           v_dst.data_ptr() if v_dst is not None else None, ref.stride(0), _stream_ptr(stream)))
 
 
 def segpa_clear_streams(cache: int) -> None:

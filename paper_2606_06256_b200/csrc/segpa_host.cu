@@ -340,6 +340,7 @@ const char* encode_q_map(TensorMap* out, const void* q, int64_t T, int Hq, int D
         fn = (EncodeTiledFn)f;
     }
     static_assert(sizeof(CUtensorMap) == sizeof(TensorMap), "tensor map size");
+    static_assert(SEGPA_NOALLOC_MAX_PAGES == kNoAllocMaxPages, "header and kernel file must agree on the scratch size");
     const cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)Hq, (cuuint64_t)T};
     const cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)row_stride_elems * 2};
     const cuuint32_t box[3] = {64u, (cuuint32_t)G, (cuuint32_t)tile_tokens};
@@ -1036,6 +1037,42 @@ segpa_status_t segpa_gather_rows(segpa_cache_t* c, int32_t layer, int32_t kv_hea
     });
     staging_release(*used, st);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "gather_rows: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
+segpa_status_t segpa_gather_rows_noalloc(segpa_cache_t* c, int32_t layer, int32_t kv_head, int64_t seq_id, int64_t first_token,
+                                         int64_t n_tokens, void* k_dst, void* v_dst, int64_t dst_row_stride_elems,
+                                         void* cuda_stream) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: null cache");
+    if (c->planning_only) return fail(SEGPA_ERR_STATE, "gather_rows_noalloc: planning-only cache has no device");
+    const int D = c->desc.head_dim, P = c->desc.page_size;
+    if (!k_dst && !v_dst) return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: give k_dst, v_dst or both");
+    if (dst_row_stride_elems < D || (dst_row_stride_elems % 8) || ((uintptr_t)k_dst % 16) || ((uintptr_t)v_dst % 16))
+        return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: destinations must be 16-byte aligned with a row stride >= head_dim, multiple of 8 elements");
+    auto it = c->streams.find(StreamKey{layer, kv_head, seq_id});
+    if (it == c->streams.end()) return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: no stream (%d, %d, %lld)", layer, kv_head, (long long)seq_id);
+    const StreamRec& rec = it->second;
+    if (first_token < 0 || n_tokens < 1 || first_token + n_tokens > rec.kv_len)
+        return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: token range outside the stream");
+    const int64_t pg_lo = rec.slot_of(first_token) / P, pg_hi = rec.slot_of(first_token + n_tokens - 1) / P + 1;
+    if (pg_hi - pg_lo > SEGPA_NOALLOC_MAX_PAGES)
+        return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: the range covers %lld pages; the fixed scratch of this entry point holds %d "
+                    "(%lld tokens at this page size): split the range, or use segpa_gather_rows", (long long)(pg_hi - pg_lo),
+                    SEGPA_NOALLOC_MAX_PAGES, (long long)SEGPA_NOALLOC_MAX_PAGES * P);
+    for (int64_t pg = pg_lo; pg < pg_hi; ++pg)
+        if (rec.pages[(size_t)pg] < 0) return fail(SEGPA_ERR_INVALID, "gather_rows_noalloc: the range touches an evicted page");
+    DeviceGuard g(c->desc.device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int* ids = nullptr;
+    cudaError_t e = noalloc_stage_page_ids(rec.pages.data() + pg_lo, (int)(pg_hi - pg_lo), st, &ids);
+    for_each_piece(rec, first_token, n_tokens, [&](int64_t tok_lo, int64_t n_piece, int64_t slot_lo) {
+        if (e != cudaSuccess) return;
+        uint16_t* kd = k_dst ? (uint16_t*)k_dst + (tok_lo - first_token) * dst_row_stride_elems : nullptr;
+        uint16_t* vd = v_dst ? (uint16_t*)v_dst + (tok_lo - first_token) * dst_row_stride_elems : nullptr;
+        e = launch_gather_rows(c->k_pool, c->v_pool, ids + (slot_lo / P - pg_lo), (int)(slot_lo % P), n_piece, kd, vd,
+                               dst_row_stride_elems, D, P, st);
+    });
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "gather_rows_noalloc: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;
 }
 

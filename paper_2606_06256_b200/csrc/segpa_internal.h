@@ -160,6 +160,10 @@ cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, con
                                long long n_tokens, uint16_t* k_dst, uint16_t* v_dst, long long dst_stride, int D, int P,
                                cudaStream_t st);
 
+// segpa_gather_rows_noalloc (segpa_misc_kernels.cu): page ids in a fixed device array of kNoAllocMaxPages entries
+constexpr int kNoAllocMaxPages = 16384;   // 64 KB per GPU; = SEGPA_NOALLOC_MAX_PAGES of include/segpa.h
+cudaError_t noalloc_stage_page_ids(const int* ids_host, int n_ids, cudaStream_t st, const int** ids_dev);
+
 cudaError_t launch_merge(const uint16_t* out_a, const float* lse_a, const uint16_t* out_b, const float* lse_b, uint16_t* out,
                          float* lse, long long row_stride, long long lse_stride, long long T, int Hq, int D, cudaStream_t st);
 

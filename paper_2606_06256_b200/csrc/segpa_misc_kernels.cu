@@ -166,6 +166,47 @@ cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, con
 }
 
 // ---------------------------------------------------------------------------------------------
+// segpa_gather_rows_noalloc: the same gather with its scratch -- the device copy of the page ids the range covers --
+// in a fixed file-scope array instead of a staging buffer that grows with cudaMalloc.  For callers that may not
+// allocate (code under CUDA graph capture, tight serving loops).  Every GPU that loads the library holds the array
+// (kNoAllocMaxPages x 4 B = 64 KB) until the process exits.  All calls share it and it keeps the last call's ids: a call
+// overwrites the entries it uses (nothing has to start at zero) in stream order, so calls on ONE stream are safe back to
+// back, while calls that overlap on the GPU (different streams, no dependency between them) race on it.
+// In host code `g_noalloc_page_ids` is a host-side stand-in for the symbol, not a device address: the address the kernel
+// gets comes from cudaGetSymbolAddress, asked once per device with that device current.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) int g_noalloc_page_ids[kNoAllocMaxPages];
+
+static cudaError_t noalloc_page_ids_ptr(int** out) {
+    static int* ptr_of_device[64] = {};
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!ptr_of_device[dev]) {
+        int* ptr = nullptr;
+        e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_page_ids);
+        if (e != cudaSuccess) return e;
+        ptr_of_device[dev] = ptr;
+    }
+    *out = ptr_of_device[dev];
+    return cudaSuccess;
+}
+
+// ids_host[0 .. n_ids): the page ids of the range (ordinary host memory: the copy stages them before it returns).
+// No allocation: one stream-ordered copy into the fixed array; *ids_dev is what the gather kernel is then given.
+cudaError_t noalloc_stage_page_ids(const int* ids_host, int n_ids, cudaStream_t st, const int** ids_dev) {
+    if (n_ids < 1 || n_ids > kNoAllocMaxPages) return cudaErrorInvalidValue;   // (the entry point has already refused it with a message)
+    int* ptr = nullptr;
+    cudaError_t e = noalloc_page_ids_ptr(&ptr);
+    if (e != cudaSuccess) return e;
+    e = cudaMemcpyAsync(ptr, ids_host, (size_t)n_ids * sizeof(int), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    *ids_dev = ptr;
+    return cudaSuccess;
+}
+
+// ---------------------------------------------------------------------------------------------
 // a7: split-KV combine.  Partials hold unnormalised O, running max m (log2 units) and sum l;
 // merged in ascending split order (deterministic).  Exactness of the merge: PAPER.md:302.
 // One warp per row.
