@@ -60,6 +60,7 @@ struct StreamRec {
     int64_t kv_len = 0;
     std::vector<PadPoint> pads;   // ascending; empty = the stream is dense (token j in page j / P, slot j % P)
     bool tail_open = false;       // the partial last page was started by a COPY append of this stream (it may be filled further)
+    int64_t n_holes = 0;          // evicted pages (entries -1 of `pages`)
     int64_t slot_len() const { return kv_len + (pads.empty() ? 0 : pads.back().pad); }
     int64_t slot_of(int64_t tok) const {
         int64_t pad = 0;
@@ -251,6 +252,7 @@ struct segpa_cache {
     std::vector<int32_t> free_list;  // may hold stale entries (refcnt != 0: pages taken by caller-given id): skipped on pop
     std::vector<uint8_t> in_free;    // page id is somewhere in free_list (so a release never adds a second entry)
     int64_t n_free = 0;
+    int64_t n_shared_pages = 0;      // pages with reference count > 1 (kept as the counts change): while it is 0 no stream shares a page
     std::unordered_map<StreamKey, StreamRec, StreamKeyHash> streams;
     std::vector<segpa_segments*> seg_objs;
     std::vector<SegBuf*> free_bufs;   // released device storage, oldest first
@@ -292,6 +294,7 @@ int32_t pop_free_page(segpa_cache* c) {
 }
 
 void release_page(segpa_cache* c, int32_t id) {
+    if (c->refcnt[id] == 2) --c->n_shared_pages;
     if (--c->refcnt[id] == 0) {
         if (!c->in_free[(size_t)id]) {
             c->free_list.push_back(id);
@@ -772,7 +775,7 @@ segpa_status_t segpa_append_pages_batch(segpa_cache_t* c, const segpa_append_req
                 }
                 ++undo.back().n_new;
                 if (c->refcnt[id] == 0) --c->n_free;
-                ++c->refcnt[id];
+                if (++c->refcnt[id] == 2) ++c->n_shared_pages;
                 rec.pages.push_back(id);
                 if (!attach) touched.push_back(id);
             }
@@ -863,6 +866,7 @@ segpa_status_t segpa_evict_pages(segpa_cache_t* c, int32_t layer, int32_t kv_hea
     for (int32_t i = 0; i < n_pages; ++i) {
         release_page(c, rec.pages[(size_t)first_page_index + i]);
         rec.pages[(size_t)first_page_index + i] = -1;
+        ++rec.n_holes;
     }
     return SEGPA_OK;
 }
@@ -963,6 +967,11 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
             jb.first_slot = (int)(slot_lo % P);
             const int32_t* pg = rec.pages.data() + slot_lo / P;
             const int64_t np = (slot_lo + n_piece - 1) / P - slot_lo / P + 1;
+            if (c->n_shared_pages == 0 && rec.n_holes == 0) {
+                // no page of the cache is shared and the stream has no hole: nothing to check page by page
+                memcpy(ids + ni, pg, (size_t)np * sizeof(int32_t));
+                ni += (size_t)np;
+            } else
             for (int64_t k = 0; k < np; ++k) {
                 const int32_t id = pg[k];
                 if (k + 16 < np && (uint32_t)pg[k + 16] < (uint32_t)n_pool) __builtin_prefetch(refcnt + pg[k + 16]);
@@ -1080,6 +1089,7 @@ segpa_status_t segpa_clear_streams(segpa_cache_t* c) {
     if (!c) return fail(SEGPA_ERR_INVALID, "clear_streams: null cache");
     c->streams.clear();
     std::fill(c->refcnt.begin(), c->refcnt.end(), 0);
+    c->n_shared_pages = 0;
     c->free_list.resize((size_t)c->desc.num_pages);
     for (int64_t i = 0; i < c->desc.num_pages; ++i) c->free_list[(size_t)i] = (int32_t)(c->desc.num_pages - 1 - i);
     std::fill(c->in_free.begin(), c->in_free.end(), 1);
