@@ -223,6 +223,33 @@ def test_decode_split_kv(kernel, tiles):
         g.close()
 
 
+NARROW = [
+    # Decode-shaped plans (every tile <= 16 rows): they run the NARROW instantiation, whose softmax spreads a row over four
+    # threads (16x256b / 16x128b TMEM shapes) and has its own mask code.  Hq, Hkv, D, P, requests.
+    # G = 1: one row per tile; W = 1, W inside one 64-key half, sinks, GLOBAL; kv_len around block and half edges
+    (2, 2, 128, 16, [{"kv_len": n, "heads": {0: (GLOBAL, 0, 0, 1), 1: (LOCAL, W, ns, 1)}}
+                     for n, W, ns in [(1, 1, 0), (64, 1, 0), (65, 40, 0), (128, 64, 4), (129, 65, 4), (700, 300, 70), (2049, 1, 0), (5000, 2048, 128)]]),
+    # G = 4, q_len 1..4 (4..16 rows: rows 8..15 live in the second register set), D = 64, P = 32
+    (8, 2, 64, 32, [{"kv_len": 900 + 77 * r, "heads": {0: (GLOBAL, 0, 0, 1 + r % 4), 1: (LOCAL, 129 + 64 * r, 4 * (r % 2), 1 + (r + 1) % 4)}} for r in range(6)]),
+    # G = 7 (14 rows with q_len 2), G = 16 (16 rows), G = 8 with q_len 2
+    (28, 4, 128, 32, [{"kv_len": 3000 + 501 * r, "heads": {0: (GLOBAL, 0, 0, 2), 1: (LOCAL, 1000, 0, 2), 2: (LOCAL, 4096, 128, 1), 3: (LOCAL, 63, 4, 2)}} for r in range(3)]),
+    (32, 2, 64, 16, [{"kv_len": 777, "heads": {0: (GLOBAL, 0, 0, 1), 1: (LOCAL, 200, 10, 1)}}]),
+    (16, 2, 128, 16, [{"kv_len": 12000, "heads": {0: (GLOBAL, 0, 0, 2), 1: (LOCAL, 3000, 200, 2)}}]),
+    # ragged stream under a narrow plan: tails inside the window, sinks in the first chunk
+    (8, 2, 128, 16, [{"kv_len": 1000, "chunks": [333, 200, 407, 60], "heads": {0: (GLOBAL, 0, 0, 3), 1: (LOCAL, 100, 40, 4)}}]),
+]
+
+
+@pytest.mark.parametrize("tiles", [1, 2])
+@pytest.mark.parametrize("case", range(len(NARROW)))
+def test_narrow_decode_shapes(case, tiles):
+    Hq, Hkv, D, P, reqs = NARROW[case]
+    w = wl.make_workload("narrow%d" % case, Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=1700 + case)
+    G = Hq // Hkv
+    assert all(s.q_len * G <= 16 for s in w.segments)          # what selects the instantiation
+    print(_run_full(w, "tc", tiles, "narrow%d" % case))
+
+
 @pytest.mark.parametrize("tiles", [1, 2])
 def test_determinism_and_page_permutation(tiles):
     """Run-to-run bit determinism, and bit-identical results under a different page placement of the
