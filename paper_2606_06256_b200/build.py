@@ -12,8 +12,8 @@ LIB = os.path.join(HERE, "libsegpa.so")
 # test build (-DSEGPA_BRINGUP): adds the SIMT cross-check attention kernel; loaded only by tests that ask for it
 BRINGUP_LIB = os.path.join(HERE, "libsegpa_bringup.so")
 BRINGUP_SOURCES = ["segpa_host.cu", "segpa_misc_kernels.cu"]     # the files that look at SEGPA_BRINGUP
-SOURCES = ["segpa_host.cu", "segpa_misc_kernels.cu", "segpa_attn_tc.cu", "segpa_mass.cu"]
-HEADERS = ["segpa_internal.h", "sm100_ptx.cuh", os.path.join("..", "..", "include", "segpa.h")]
+SOURCES = ["segpa_host.cu", "segpa_misc_kernels.cu", "segpa_attn_tc.cu", "segpa_attn_tc1.cu", "segpa_mass.cu"]
+HEADERS = ["segpa_internal.h", "sm100_ptx.cuh", "segpa_attn_common.cuh", os.path.join("..", "..", "include", "segpa.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "--use_fast_math"]
 

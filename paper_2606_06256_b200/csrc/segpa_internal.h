@@ -220,6 +220,7 @@ cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const Scatter
 cudaError_t launch_attention_simt(const FwdParams& p, cudaStream_t st);   // test build only (libsegpa_bringup.so)
 #endif
 cudaError_t launch_attention_tc(const FwdParams& p, cudaStream_t st);
+cudaError_t launch_attention_tc1(const FwdParams& p, cudaStream_t st);   // tiles_per_item == 1, not decode-shaped (segpa_attn_tc1.cu)
 cudaError_t launch_combine(const FwdParams& p, cudaStream_t st);
 
 }  // namespace segpa
