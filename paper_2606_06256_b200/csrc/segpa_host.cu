@@ -1849,8 +1849,22 @@ segpa_status_t segpa_attention_mass(segpa_cache_t* c, const segpa_segments_t* s,
     p.P = c->desc.page_size;
     p.tile_tokens = kTileRows / c->G;
     p.page_bytes = c->page_bytes;
+#ifdef SEGPA_TRACE
+    static unsigned long long* d_mtrace = nullptr;
+    if (!d_mtrace) cudaMalloc((void**)&d_mtrace, 32 * kTraceCap * 8);
+    cudaMemsetAsync(d_mtrace, 0, 32 * kTraceCap * 8, st);
+    p.trace = d_mtrace;
+#endif
     cudaError_t e = cudaMemsetAsync(mass, 0, (size_t)s->mass_off.back() * sizeof(float), st);
     if (e == cudaSuccess) e = launch_attention_mass(p, st);
+#ifdef SEGPA_TRACE
+    if (const char* tf = getenv("SEGPA_MASS_TRACE_FILE")) {
+        std::vector<unsigned long long> h(32 * kTraceCap);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(h.data(), d_mtrace, h.size() * 8, cudaMemcpyDeviceToHost);
+        if (FILE* f = fopen(tf, "wb")) { fwrite(h.data(), 8, h.size(), f); fclose(f); }
+    }
+#endif
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_mass: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;
 }

@@ -191,6 +191,7 @@ struct MassParams {
     float scale;
     int n_cta;
     int G, D, P, tile_tokens, page_bytes;
+    unsigned long long* trace;   // [32 warps][kTraceCap] records of CTA 0, as FwdParams::trace; debug builds only
 };
 cudaError_t launch_attention_mass(const MassParams& p, cudaStream_t st);
 cudaError_t launch_mass_select(const float* mass, const long long* mass_off_dev, const int* kv_len_dev, int n_segments, float tau,

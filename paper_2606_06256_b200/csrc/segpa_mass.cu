@@ -11,8 +11,17 @@
 // Bound: the dense contraction is half of the attention kernel's (no PV) and the exponentials are the same, so the
 // MUFU pipe (16 ex2 / clk / SM = 1024 clk per 128x128 tile) limits it at twice the MMA time.
 //
-// 12 warps: 0 loader (K block, Q tiles), 1 MMA issuer, 2-3 per-column LSE / position arrays (3 also owns TMEM), 4-7 and 8-11 the two
-// exp warpgroups (each takes half of a tile's query columns).
+// 20 warps: 0 loader (K block, Q tiles), 1 MMA issuer, 2-3 per-column LSE / position arrays (3 also owns TMEM), 4-19 four
+// exp warpgroups, warpgroup g on the tiles whose running number in the CTA's tile sequence is g mod 4 (accumulator
+// stage g), all 128 query columns of a key in one thread, in four chunks of 32 with the TMEM load of the next chunk
+// under the exponentials of the current one.
+// Why four tiles in flight (round 2; ncu source page and the -DSEGPA_TRACE timeline): a tile costs an
+// exp warp ~450-1100 cycles of serial latency around its exponentials (two mbarrier waits, the per-tile flags, the
+// first TMEM load, the drain -- each a round trip through the instruction queue the other warps' ex2 sit in).  With
+// two warpgroups that each took half of the columns of EVERY tile (round 1), all eight warps sat in that prologue
+// together and the MUFU pipe idled (56 % busy, 1850 cycles per tile); with the warpgroups on different tiles one's
+// prologue runs under the others' exponentials (1440-1540 cycles per tile, pipe 67-71 % busy).  What was tried on top
+// and did not pay is listed in DESIGN.md 5.7.
 #include "segpa_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -21,30 +30,46 @@ using namespace ptx;
 
 namespace {
 
-constexpr int kMassThreads = 384;   // 4 service warps + two exp warpgroups
+constexpr int kMassThreads = 640;   // 4 service warps + four exp warpgroups
+// register budgets (setmaxnreg): 128 * 56 + 512 * 104 = 60416 <= 640 * 96, the launch allocation
+constexpr int kRegsService = 56, kRegsExp = 104;
 
 struct alignas(16) MassAux {
     float lse2[kTileRows];   // LSE of column c in log2 units
     int pos[kTileRows];      // query position of column c; -1: no such row
     int pmin, pmax;          // over the valid columns
-    int pad[2];
+    int all_rows;            // every column has a row
+    int pad;
 };
 
 constexpr int kQStages = 4;   // Q tiles in flight
-constexpr int kSStages = 4;   // S accumulators in TMEM (4 x 128 columns) and per-column arrays: the MMA issuer and the LSE
-                              // warps run up to three tiles ahead of the exp warpgroups, which then never wait for a tile
-                              // (round 1 had two: MUFU pipe active 53 % of the time)
+constexpr int kSStages = 4;   // S accumulators in TMEM (4 x 128 columns), one per exp warpgroup
 constexpr int kKStages = 2;   // K blocks: the next item's block is loaded under the current item's last tiles
+constexpr int kAuxStages = 8; // per-column arrays: an exp warpgroup needs those of its next tile (four on) the moment it
+                              // finishes one, so the LSE warps must be able to run more than four tiles ahead
 
 struct MassBars {
     uint64_t k_full[kKStages], k_empty[kKStages];
     uint64_t q_full[kQStages], q_empty[kQStages];
-    uint64_t aux_full[kSStages], aux_empty[kSStages];
+    uint64_t aux_full[kAuxStages], aux_empty[kAuxStages];
     uint64_t s_full[kSStages], s_empty[kSStages];
     uint32_t tmem_base;
 };
 
 }  // namespace
+
+// Pipeline trace (debug builds with -DSEGPA_TRACE only): lane 0 of every warp of CTA 0 logs (tag, arg, SM clock) records.
+#ifdef SEGPA_TRACE
+#define TRACE(tag, arg)                                                                                          \
+    do {                                                                                                         \
+        if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && trace_n < kTraceCap)                                   \
+            p.trace[(threadIdx.x >> 5) * kTraceCap + trace_n++] =                                                \
+                ((unsigned long long)(tag) << 56) | ((unsigned long long)((arg) & 0xffff) << 40) |               \
+                ((unsigned long long)clock64() & 0xffffffffffull);                                               \
+    } while (0)
+#else
+#define TRACE(tag, arg) do { } while (0)
+#endif
 
 template <int D>
 __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const __grid_constant__ MassParams p) {
@@ -53,14 +78,17 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
     constexpr uint32_t kSBO = kHalves * kAtomBytes;
     extern __shared__ uint8_t smem_raw[];
     __shared__ MassBars bars;
-    __shared__ MassAux aux[kSStages];
-    __shared__ float half_sum[kTileRows];   // partial mass of the second exp warpgroup, added by the first
+    __shared__ MassAux aux[kAuxStages];
+    __shared__ float part_sum[3][kTileRows];   // partial masses of the other three exp warpgroups, added by the first in a fixed order
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
     const uint32_t sK = smem_u32(smem);           // kKStages K blocks
     const uint32_t sQ = sK + kKStages * kTileBytes;   // kQStages Q stages
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int G = p.G, TT = p.tile_tokens, ppb = kBlockKeys / p.P;
     const int i_lo = p.cta_off[blockIdx.x], i_hi = p.cta_off[blockIdx.x + 1];
+#ifdef SEGPA_TRACE
+    int trace_n = 0;
+#endif
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < kKStages; ++s) {
@@ -71,11 +99,13 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             mbar_init(smem_u32(&bars.q_full[s]), 1);
             mbar_init(smem_u32(&bars.q_empty[s]), 1);
         }
-        for (int s = 0; s < kSStages; ++s) {
+        for (int s = 0; s < kAuxStages; ++s) {
             mbar_init(smem_u32(&bars.aux_full[s]), 1);
-            mbar_init(smem_u32(&bars.aux_empty[s]), 256);
+            mbar_init(smem_u32(&bars.aux_empty[s]), 128);      // the one exp warpgroup that takes the tile
+        }
+        for (int s = 0; s < kSStages; ++s) {
             mbar_init(smem_u32(&bars.s_full[s]), 1);
-            mbar_init(smem_u32(&bars.s_empty[s]), 256);
+            mbar_init(smem_u32(&bars.s_empty[s]), 128);
         }
         fence_mbar_init();
     }
@@ -90,6 +120,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
 
     if (warp == 0) {
         // ------------------------------------------------------------------ loader
+        reg_dec<kRegsService>();
         uint32_t n_k = 0, n_t = 0;      // K fills, tile fills so far
         if (lane == 0) prefetch_tmap(&p.q_map);
         for (int ii = i_lo; ii < i_hi; ++ii) {
@@ -125,54 +156,101 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
         // ------------------------------------------------------------------ per-column LSE / position arrays of each tile
         // (two warps, one per stage: warp 2 serves the even tiles, warp 3 the odd ones -- a tile costs one
         // round trip to L2 for the LSE values, which one warp alone cannot hide)
-        uint32_t n_t = 0;
-        for (int ii = i_lo; ii < i_hi; ++ii) {
-            const MassItem it = p.items[ii];
+        reg_dec<kRegsService>();
+        // One tile ahead: the LSE loads of this warp's next tile are issued before the current tile's values are used,
+        // so the round trip to L2 runs under the current tile's work (without it each of the two warps was busy ~95 %
+        // of the time once the exp warps stopped being the limit).  cur / nxt walk the CTA's (item, tile) sequence,
+        // taking the tiles whose running number has this warp's parity.
+        struct Cursor {
+            int ii, ti, t_hi;
+            uint32_t n_t;
+            int q_len, p0, head0;          // of the item's segment: rows, position of row 0, first query head
+            long long row0;
+            bool valid;
+        };
+        const int par = warp - 2;
+        auto open_item = [&](Cursor& c) {
+            const MassItem it = p.items[c.ii];
             const SegDev sg = p.segs[it.seg];
-            const int p0 = sg.kv_len - sg.q_len;
-            for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
-                const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
-                if ((int)(n_t & 1) != warp - 2) continue;
-                const int tok0 = ti * TT;
-                const int n_rows = min(TT, sg.q_len - tok0) * G;
-                // columns past the segment's rows: position -1 (their scores are garbage and never counted)
-                int pos[4], pmin = INT32_MAX, pmax = -1;
-                float l2[4];
-                // the four LSE loads of a lane are issued together (clamped to a valid row), then used
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    const int cc = min(lane + 32 * u, n_rows - 1);
-                    const int tok = tok0 + cc / G, head = sg.kv_head * G + cc % G;
-                    pos[u] = p0 + tok;
-                    l2[u] = p.lse[(long long)head * p.lse_stride + sg.q_row_start + tok];
-                }
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    if (lane + 32 * u < n_rows) {
-                        l2[u] *= 1.4426950408889634f;
-                        pmin = min(pmin, pos[u]);
-                        pmax = max(pmax, pos[u]);
-                    } else {
-                        pos[u] = -1;
-                        l2[u] = 0.f;
-                    }
-                }
-                pmin = __reduce_min_sync(0xffffffffu, pmin);
-                pmax = __reduce_max_sync(0xffffffffu, pmax);
-                if (lane == 0) mbar_wait(smem_u32(&bars.aux_empty[st]), ph ^ 1);
-                __syncwarp();
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    aux[st].pos[lane + 32 * u] = pos[u];
-                    aux[st].lse2[lane + 32 * u] = l2[u];
-                }
-                if (lane == 0) { aux[st].pmin = pmin; aux[st].pmax = pmax; }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(smem_u32(&bars.aux_full[st]));
+            c.ti = it.t_lo; c.t_hi = it.t_hi;
+            c.q_len = sg.q_len; c.p0 = sg.kv_len - sg.q_len; c.head0 = sg.kv_head * G; c.row0 = sg.q_row_start;
+        };
+        auto step = [&](Cursor& c) {       // to the next tile of the sequence
+            ++c.n_t;
+            if (++c.ti == c.t_hi) {
+                if (++c.ii == i_hi) { c.valid = false; return; }
+                open_item(c);
             }
+        };
+        // column c of a full tile is token c / G, head c % G: per lane, once
+        int ctok[4], chead[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { ctok[u] = (lane + 32 * u) / G; chead[u] = (lane + 32 * u) % G; }
+        auto issue = [&](const Cursor& c, float (&l2)[4], int (&pos)[4]) {
+            const int tok0 = c.ti * TT;
+            const int n_rows = min(TT, c.q_len - tok0) * G;
+            // the four LSE loads of a lane are issued together (clamped to a valid row)
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                int tk = ctok[u], hd = chead[u];
+                if (lane + 32 * u >= n_rows) { tk = (n_rows - 1) / G; hd = (n_rows - 1) % G; }   // ragged last tile only
+                pos[u] = c.p0 + tok0 + tk;
+                l2[u] = p.lse[(long long)(c.head0 + hd) * p.lse_stride + c.row0 + tok0 + tk];
+            }
+        };
+        Cursor cur;
+        cur.ii = i_lo; cur.n_t = 0; cur.valid = i_lo < i_hi;
+        if (cur.valid) {
+            open_item(cur);
+            if (par == 1) step(cur);
+        }
+        float l2[4] = {0.f, 0.f, 0.f, 0.f};
+        int pos[4] = {0, 0, 0, 0};
+        if (cur.valid) issue(cur, l2, pos);
+        while (cur.valid) {
+            Cursor nxt = cur;
+            step(nxt);
+            if (nxt.valid) step(nxt);
+            float l2n[4] = {0.f, 0.f, 0.f, 0.f};
+            int posn[4] = {0, 0, 0, 0};
+            if (nxt.valid) issue(nxt, l2n, posn);
+            const uint32_t st = cur.n_t % kAuxStages, ph = (cur.n_t / kAuxStages) & 1;
+            const int n_rows = min(TT, cur.q_len - cur.ti * TT) * G;
+            // columns past the segment's rows: position -1 (their scores are garbage and never counted)
+            int pmin = INT32_MAX, pmax = -1;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                if (lane + 32 * u < n_rows) {
+                    l2[u] *= 1.4426950408889634f;
+                    pmin = min(pmin, pos[u]);
+                    pmax = max(pmax, pos[u]);
+                } else {
+                    pos[u] = -1;
+                    l2[u] = 0.f;
+                }
+            }
+            pmin = __reduce_min_sync(0xffffffffu, pmin);
+            pmax = __reduce_max_sync(0xffffffffu, pmax);
+            TRACE(30, cur.n_t);
+            if (lane == 0) mbar_wait(smem_u32(&bars.aux_empty[st]), ph ^ 1);
+            __syncwarp();
+            TRACE(31, cur.n_t);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                aux[st].pos[lane + 32 * u] = pos[u];
+                aux[st].lse2[lane + 32 * u] = l2[u];
+            }
+            if (lane == 0) { aux[st].pmin = pmin; aux[st].pmax = pmax; aux[st].all_rows = n_rows == kTileRows; }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(smem_u32(&bars.aux_full[st]));
+            TRACE(32, cur.n_t);
+            cur = nxt;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { l2[u] = l2n[u]; pos[u] = posn[u]; }
         }
     } else if (warp == 1) {
         // ------------------------------------------------------------------ MMA issuer: S^T = K Q^T
+        reg_dec<kRegsService>();
         constexpr uint32_t idesc = make_idesc_bf16(128, 128, 0, 0);
         const uint64_t dk0 = make_desc_sw128(sK, 16, kSBO);             // A: K block image (page layout)
         const uint64_t dq0 = make_desc_sw128(sQ, 16, kAtomBytes);       // B: Q tile image (TMA box layout)
@@ -186,8 +264,11 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
                 const uint32_t qs = n_t % kQStages, qph = (n_t / kQStages) & 1;
                 const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
+                TRACE(10, n_t);
                 mbar_wait(smem_u32(&bars.q_full[qs]), qph);
+                TRACE(11, n_t);
                 mbar_wait(smem_u32(&bars.s_empty[st]), ph ^ 1);
+                TRACE(12, n_t);
                 tc_fence_after();
                 if (elect_one()) {
                     const uint64_t dq = dq0 + (uint64_t)((qs * kTileBytes) >> 4);
@@ -205,13 +286,16 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             }
         }
     } else if (warp >= 4) {
-        // ------------------------------------------------------------------ exp warpgroups: thread = (key, half of the columns)
-        // warps 4-7 take the query columns [0, 64) of every tile, warps 8-11 the columns [64, 128): the per-tile
-        // chain (TMEM load, 64 ex2, sum) is half as long; the two partial sums of a key are added in a fixed order
+        // ------------------------------------------------------------------ exp warpgroups: thread = (key, every fourth tile)
+        // Warpgroup g (warps 4 + 4g ...) takes the tiles with running number = g mod 4: accumulator stage g.  A thread
+        // walks its key's 128 query columns in four chunks of 32, the TMEM load of the next chunk in flight under the
+        // exponentials of the current one; the accumulator stage goes back to the MMA issuer as soon as the last
+        // chunk is in registers.  The four partial sums of a key are added in a fixed order.
+        reg_inc<kRegsExp>();
         const int wq = warp & 3;
-        const int hf = (warp - 4) >> 2;                                  // which half of the columns
+        const int grp = (warp - 4) >> 2;
         const int kr = wq * 32 + lane;                                   // key row inside the block
-        const uint32_t lane_base = (uint32_t)(wq * 32) << 16;
+        const uint32_t t_base = tmem + ((uint32_t)(wq * 32) << 16) + grp * 128;
         const float sl2 = p.scale * 1.4426950408889634f;
         uint32_t n_t = 0;
         for (int ii = i_lo; ii < i_hi; ++ii) {
@@ -222,54 +306,78 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             const bool is_sink_key = key < sg.n_sink;
             float acc = 0.f;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
-                const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
-                mbar_wait(smem_u32(&bars.aux_full[st]), ph);
-                mbar_wait(smem_u32(&bars.s_full[st]), ph);
+                if ((int)(n_t & 3) != grp) continue;
+                static_assert(kSStages == 4, "accumulator stage = exp warpgroup");
+                const uint32_t ph = (n_t / kSStages) & 1;
+                const uint32_t as = n_t % kAuxStages, aph = (n_t / kAuxStages) & 1;
+                TRACE(20, n_t);
+                mbar_wait(smem_u32(&bars.aux_full[as]), aph);
+                TRACE(21, n_t);
+                mbar_wait(smem_u32(&bars.s_full[grp]), ph);
+                TRACE(22, n_t);
                 tc_fence_after();
-                const MassAux& ax = aux[st];
+                uint32_t sa[32], sb[32];
+                tmem_ld32(t_base, sa);
+                const MassAux& ax = aux[as];
                 // the whole block is visible to every valid column of the tile: causal (blk_hi <= pmin) and inside
                 // the window of the latest query (blk_lo > pmax - W); columns without a row have position -1
-                const bool all_rows = ax.pos[kTileRows - 1] >= 0;
-                const bool full = all_rows && blk_hi <= ax.pmin && blk_lo > ax.pmax - sg.window;
-                uint32_t s[64];
-                tmem_ld32(tmem + lane_base + st * 128 + hf * 64, s);
-                tmem_ld32(tmem + lane_base + st * 128 + hf * 64 + 32, s + 32);
-                tmem_wait_ld();
+                const int4 fl = *reinterpret_cast<const int4*>(&ax.pmin);
+                const bool full = fl.z != 0 && blk_hi <= fl.x && blk_lo > fl.y - sg.window;
                 float pa = 0.f, pb = 0.f, pc = 0.f, pd = 0.f;
-                if (full) {
+                auto chunk = [&](const uint32_t (&s)[32], const int c0) {
+                    if (full) {
 #pragma unroll
-                    for (int e = 0; e < 64; e += 4) {
-                        const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[hf * 64 + e]);
-                        pa += fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
-                        pb += fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
-                        pc += fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
-                        pd += fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
-                    }
-                } else {
+                        for (int e = 0; e < 32; e += 4) {
+                            const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[c0 + e]);
+                            pa += fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
+                            pb += fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
+                            pc += fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
+                            pd += fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
+                        }
+                    } else {
 #pragma unroll
-                    for (int e = 0; e < 64; e += 4) {
-                        const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[hf * 64 + e]);
-                        const int4 p4 = *reinterpret_cast<const int4*>(&ax.pos[hf * 64 + e]);
-                        const float e0 = fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
-                        const float e1 = fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
-                        const float e2 = fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
-                        const float e3 = fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
-                        pa += (key <= p4.x && (key > p4.x - sg.window || is_sink_key)) ? e0 : 0.f;
-                        pb += (key <= p4.y && (key > p4.y - sg.window || is_sink_key)) ? e1 : 0.f;
-                        pc += (key <= p4.z && (key > p4.z - sg.window || is_sink_key)) ? e2 : 0.f;
-                        pd += (key <= p4.w && (key > p4.w - sg.window || is_sink_key)) ? e3 : 0.f;
+                        for (int e = 0; e < 32; e += 4) {
+                            const float4 l4 = *reinterpret_cast<const float4*>(&ax.lse2[c0 + e]);
+                            const int4 p4 = *reinterpret_cast<const int4*>(&ax.pos[c0 + e]);
+                            const float e0 = fast_exp2(fmaf(__uint_as_float(s[e + 0]), sl2, -l4.x));
+                            const float e1 = fast_exp2(fmaf(__uint_as_float(s[e + 1]), sl2, -l4.y));
+                            const float e2 = fast_exp2(fmaf(__uint_as_float(s[e + 2]), sl2, -l4.z));
+                            const float e3 = fast_exp2(fmaf(__uint_as_float(s[e + 3]), sl2, -l4.w));
+                            pa += (key <= p4.x && (key > p4.x - sg.window || is_sink_key)) ? e0 : 0.f;
+                            pb += (key <= p4.y && (key > p4.y - sg.window || is_sink_key)) ? e1 : 0.f;
+                            pc += (key <= p4.z && (key > p4.z - sg.window || is_sink_key)) ? e2 : 0.f;
+                            pd += (key <= p4.w && (key > p4.w - sg.window || is_sink_key)) ? e3 : 0.f;
+                        }
                     }
-                }
-                acc += (pa + pb) + (pc + pd);
+                };
+                tmem_wait_ld();
+                TRACE(23, n_t);
+                tmem_ld32(t_base + 32, sb);
+                chunk(sa, 0);
+                tmem_wait_ld();
+                tmem_ld32(t_base + 64, sa);
+                chunk(sb, 32);
+                tmem_wait_ld();
+                tmem_ld32(t_base + 96, sb);
+                // the accumulator stage goes back at the half-way point, at the price of one exposed TMEM load (the
+                // other three warps of the scheduler fill it): the MMA of tile n_t + 4 takes ~1500-1900 cycles from
+                // this arrive to a visible s_full (wait latency + 8 MMAs + commit + wait latency), more than one chunk
+                tmem_wait_ld();
                 tc_fence_before();
-                mbar_arrive(smem_u32(&bars.s_empty[st]));
-                mbar_arrive(smem_u32(&bars.aux_empty[st]));
+                mbar_arrive(smem_u32(&bars.s_empty[grp]));
+                chunk(sa, 64);
+                chunk(sb, 96);
+                acc += (pa + pb) + (pc + pd);
+                TRACE(24 + (full ? 0 : 1), n_t);
+                mbar_arrive(smem_u32(&bars.aux_empty[as]));
             }
-            // mass = (columns [0, 64)) + (columns [64, 128)), added by the first warpgroup: one writer per entry
-            if (hf == 1) half_sum[kr] = acc;
-            asm volatile("bar.sync 1, 256;" ::: "memory");
-            if (hf == 0 && key < sg.kv_len) p.mass[p.mass_off[it.seg] + key] = acc + half_sum[kr];
-            asm volatile("bar.sync 2, 256;" ::: "memory");
+            // mass = ((tiles 0 mod 4) + (1 mod 4)) + ((2 mod 4) + (3 mod 4)), added by the first warpgroup: one writer
+            // per entry, one order
+            if (grp > 0) part_sum[grp - 1][kr] = acc;
+            asm volatile("bar.sync 1, 512;" ::: "memory");
+            if (grp == 0 && key < sg.kv_len)
+                p.mass[p.mass_off[it.seg] + key] = (acc + part_sum[0][kr]) + (part_sum[1][kr] + part_sum[2][kr]);
+            asm volatile("bar.sync 2, 512;" ::: "memory");
         }
     }
 
