@@ -940,8 +940,7 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
     Staging& sg = c->append_stage[c->append_turn];
     c->append_turn ^= 1;
     auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
-    const size_t off_tabs = al(n_jobs * sizeof(RopeJob));
-    const size_t off_ids = al(off_tabs + n_jobs * sizeof(RopeTable));   // (tables: device scratch, not uploaded)
+    const size_t off_ids = al(n_jobs * sizeof(RopeJob));
     const size_t bytes = off_ids + n_ids * sizeof(int32_t);
     cudaError_t e = staging_acquire(sg, bytes);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "rope_align: %s", cudaGetErrorString(e)); }
@@ -951,7 +950,7 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
     RopeJob* jobs = (RopeJob*)sg.h;
     int32_t* ids = (int32_t*)((uint8_t*)sg.h + off_ids);
     size_t nj = 0, ni = 0;
-    long long total_chunks = 0;
+    long long total_units = 0;                     // CTAs of the rotation kernel: kRopeUnitChunks half-row chunks of one job each
     int32_t min_id = 0, max_ref = 0;
     const int32_t* refcnt = c->refcnt.data();
     const int32_t n_pool = (int32_t)c->desc.num_pages;
@@ -960,7 +959,7 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
         const StreamRec& rec = *seen[(size_t)i].rec;
         for_each_piece(rec, r.first_token, r.n_tokens, [&](int64_t, int64_t n_piece, int64_t slot_lo) {
             RopeJob jb{};
-            jb.chunk_begin = total_chunks;
+            jb.unit_begin = (int)total_units;
             jb.page_off = (long long)ni;
             jb.n_tokens = n_piece;
             jb.delta_pos = r.delta_pos;   // R(p_on) R(p_off)^-1 = R(delta); the per-pair cos / sin are formed on the device in fp64
@@ -979,7 +978,7 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
                 max_ref = std::max(max_ref, refcnt[id < 0 ? 0 : id]);
                 ids[ni++] = id;
             }
-            total_chunks += n_piece * (D >> 4);
+            total_units += (n_piece * (D >> 4) + kRopeUnitChunks - 1) / kRopeUnitChunks;
             jobs[nj++] = jb;
         });
     }
@@ -998,8 +997,8 @@ segpa_status_t segpa_rope_align_batch(segpa_cache_t* c, const segpa_rope_req_t* 
     }
     e = staging_upload(sg, bytes, c->up_stream, st);
     if (e == cudaSuccess)
-        e = launch_rope_align(c->k_pool, (const RopeJob*)sg.d, (RopeTable*)((uint8_t*)sg.d + off_tabs), (int)n_jobs,
-                              (const int*)((const uint8_t*)sg.d + off_ids), total_chunks, rope_base, D, P, st);
+        e = launch_rope_align(c->k_pool, (const RopeJob*)sg.d, (int)n_jobs, (const int*)((const uint8_t*)sg.d + off_ids),
+                              (int)total_units, rope_base, D, P, st);
     if (e == cudaSuccess) staging_release(sg, st);
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "rope_align: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;

@@ -139,23 +139,18 @@ struct ScatterJob {
                                  // job of the same batch continues the stream inside this job's last page
 };
 
-// cos / sin of delta_pos * theta_d for the D/2 rotation pairs (host-computed in fp64)
-struct RopeTable {
-    float cs[64];
-    float sn[64];
-};
-// one chunk of a RoPEAlign batch
+// One job = a run of tokens contiguous in slot space, moved by one delta.  The rotation kernel runs one CTA per
+// unit of kRopeUnitChunks 16-byte half-row chunks of one job.
+constexpr int kRopeUnitChunks = 1024;   // (2048 in two rounds per CTA measured 10 % slower)
 struct RopeJob {
-    long long chunk_begin;       // first 16-byte half-row chunk of this job in the batch-wide index
     long long page_off;          // index of its first page id in the batch's id array
     long long n_tokens;
     long long delta_pos;         // p_on - p_off of the chunk
-    int first_slot;
-    int pad;
+    int first_slot;              // slot of its first token inside its first page
+    int unit_begin;              // first CTA (unit) of this job in the grid
 };
-// tabs_dev: scratch for n_jobs tables, filled on the device (fp64 sincos) before the rotation kernel runs
-cudaError_t launch_rope_align(uint8_t* k_pool, const RopeJob* jobs_dev, RopeTable* tabs_dev, int n_jobs,
-                              const int* page_ids_dev, long long total_chunks, double rope_base, int D, int P, cudaStream_t st);
+cudaError_t launch_rope_align(uint8_t* k_pool, const RopeJob* jobs_dev, int n_jobs, const int* page_ids_dev, int total_units,
+                              double rope_base, int D, int P, cudaStream_t st);
 cudaError_t launch_gather_rows(const uint8_t* k_pool, const uint8_t* v_pool, const int* page_ids_dev, int first_slot,
                                long long n_tokens, uint16_t* k_dst, uint16_t* v_dst, long long dst_stride, int D, int P,
                                cudaStream_t st);

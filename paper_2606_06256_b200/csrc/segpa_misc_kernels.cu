@@ -60,50 +60,69 @@ cudaError_t launch_scatter_pages(uint8_t* k_pool, uint8_t* v_pool, const Scatter
 // 16-byte chunk of the first half of the head dim): it holds the 8 pairs (d, d + D/2), d = 8c .. 8c+7.
 // HBM-bound: 2 * D * 2 bytes read + written per token.
 // ---------------------------------------------------------------------------------------------
-// cos / sin of delta * base^(-2d/D) per (job, pair d), in double precision (delta can be 10^5 and more:
-// fp32 argument reduction would cost ~1e-3 rad), rounded once to fp32
-__global__ void rope_table_kernel(const RopeJob* __restrict__ jobs, RopeTable* __restrict__ tabs, double rope_base, int D) {
-    const int d = threadIdx.x;
-    ptx::pdl_launch_dependents();   // (the rotation kernel starts its prologue now and waits for this grid in pdl_wait)
-    if (d >= D / 2) return;
-    const double ang = (double)jobs[blockIdx.x].delta_pos * pow(rope_base, -2.0 * d / D);
-    double sn, cs;
-    sincos(ang, &sn, &cs);
-    tabs[blockIdx.x].cs[d] = (float)cs;
-    tabs[blockIdx.x].sn[d] = (float)sn;
-}
-
-__global__ void rope_align_kernel(uint8_t* __restrict__ k_pool, const RopeJob* __restrict__ jobs,
-                                  const RopeTable* __restrict__ tabs, int n_jobs, const int* __restrict__ page_ids,
-                                  long long total_chunks, int D, int P) {
-    const int cph = D >> 4;  // 16-byte chunks per half row
+// One CTA per unit of kRopeUnitChunks chunks of one job (4 per thread, all eight loads of a thread in flight
+// together).  Its prologue, before the wait on the preceding kernel, forms the job's cos / sin of
+// delta * base^(-2d/D) in shared memory, in double precision (delta can be 10^5 and more: fp32 argument reduction
+// would cost ~1e-3 rad), rounded once to fp32.  Index arithmetic is shifts and masks on 32-bit values (D / 16 and P
+// are powers of two); round 2's first version (one chunk per thread, a binary search over the jobs and two 64-bit
+// divisions per chunk, a separate table kernel) was bound by instruction issue at 0.66 of the HBM rate.
+__global__ void __launch_bounds__(256, 4) rope_align_kernel(uint8_t* __restrict__ k_pool, const RopeJob* __restrict__ jobs, int n_jobs,
+                                                         const int* __restrict__ page_ids, double rope_base, int D, int p_shift) {
+    __shared__ float cs_s[64], sn_s[64];
+    const int cph = D >> 4;                        // 16-byte chunks per half row: 4 or 8
+    const int c_shift = cph == 8 ? 3 : 2;
+    int lo = 0, hi = n_jobs - 1;                   // this CTA's job (uniform)
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (jobs[mid].unit_begin <= (int)blockIdx.x) lo = mid; else hi = mid - 1;
+    }
+    const RopeJob jb = jobs[lo];
     ptx::pdl_launch_dependents();
-    ptx::pdl_wait();         // the cos / sin tables are the table kernel's; the K pages may still be read by the kernel before it
-    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < total_chunks;
-         idx += (long long)gridDim.x * blockDim.x) {
-        int lo = 0, hi = n_jobs - 1;
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (jobs[mid].chunk_begin <= idx) lo = mid; else hi = mid - 1;
+    if ((int)threadIdx.x < D / 2) {
+        // theta_d = base^(-2d/D) = 2^(-(2d/D) log2 base); the angle is brought into [-pi, pi] first (2 pi in two
+        // pieces: |delta * theta| < 2^40 leaves the reduced angle good to ~1e-9 rad) so that sincos takes its short path
+        const double theta = exp2(-2.0 * (int)threadIdx.x / D * log2(rope_base));
+        const double ang = (double)jb.delta_pos * theta;
+        const double k = rint(ang * 0.15915494309189535);                    // 1 / (2 pi)
+        const double r = fma(-k, 2.4492935982947064e-16, fma(-k, 6.283185307179586, ang));
+        double sn, cs;
+        sincos(r, &sn, &cs);
+        cs_s[threadIdx.x] = (float)cs;
+        sn_s[threadIdx.x] = (float)sn;
+    }
+    __syncthreads();
+    const int c = (int)threadIdx.x & (cph - 1);    // the same for the four chunks of a thread: 256 is a multiple of cph
+    float csv[8], snv[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { csv[i] = cs_s[c * 8 + i]; snv[i] = sn_s[c * 8 + i]; }
+    const unsigned job_chunks = (unsigned)jb.n_tokens << c_shift;
+    static_assert(kRopeUnitChunks == 4 * 256, "four chunks per thread");
+    const unsigned local0 = (unsigned)((int)blockIdx.x - jb.unit_begin) * kRopeUnitChunks + threadIdx.x;
+    const size_t page_bytes = ((size_t)D * 2) << p_shift;
+    ptx::pdl_wait();                               // the K pages may still be read or written by the kernel before this one
+    uint4* pa[4];
+    uint4* pb[4];
+    uint4 a4[4], b4[4];
+    bool ok[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const unsigned local = local0 + i * 256;
+        ok[i] = local < job_chunks;
+        const unsigned gs = (unsigned)jb.first_slot + (local >> c_shift);
+        if (ok[i]) {
+            const size_t page = (size_t)page_ids[jb.page_off + (gs >> p_shift)] * page_bytes;
+            const int slot = (int)(gs & ((1u << p_shift) - 1));
+            pa[i] = reinterpret_cast<uint4*>(k_pool + page + page_elem_offset_bytes(D, slot, c * 8));
+            pb[i] = reinterpret_cast<uint4*>(k_pool + page + page_elem_offset_bytes(D, slot, c * 8 + D / 2));
+            a4[i] = *pa[i];
+            b4[i] = *pb[i];
         }
-        const RopeJob jb = jobs[lo];
-        const float* cs_t = tabs[lo].cs;
-        const float* sn_t = tabs[lo].sn;
-        const long long local = idx - jb.chunk_begin;
-        const long long n = local / cph;
-        const int c = (int)(local % cph);
-        const long long gs = jb.first_slot + n;
-        const size_t page = (size_t)page_ids[jb.page_off + gs / P] * ((size_t)P * D * 2);
-        const int slot = (int)(gs % P);
-        uint4* pa = reinterpret_cast<uint4*>(k_pool + page + page_elem_offset_bytes(D, slot, c * 8));
-        uint4* pb = reinterpret_cast<uint4*>(k_pool + page + page_elem_offset_bytes(D, slot, c * 8 + D / 2));
-        uint4 a4 = *pa, b4 = *pb;
-        const float4 cs0 = *reinterpret_cast<const float4*>(cs_t + c * 8), cs1 = *reinterpret_cast<const float4*>(cs_t + c * 8 + 4);
-        const float4 sn0 = *reinterpret_cast<const float4*>(sn_t + c * 8), sn1 = *reinterpret_cast<const float4*>(sn_t + c * 8 + 4);
-        const float csv[8] = {cs0.x, cs0.y, cs0.z, cs0.w, cs1.x, cs1.y, cs1.z, cs1.w};
-        const float snv[8] = {sn0.x, sn0.y, sn0.z, sn0.w, sn1.x, sn1.y, sn1.z, sn1.w};
-        uint32_t* aw = reinterpret_cast<uint32_t*>(&a4);
-        uint32_t* bw = reinterpret_cast<uint32_t*>(&b4);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        if (!ok[i]) continue;
+        uint32_t* aw = reinterpret_cast<uint32_t*>(&a4[i]);
+        uint32_t* bw = reinterpret_cast<uint32_t*>(&b4[i]);
 #pragma unroll
         for (int w = 0; w < 4; ++w) {
             uint32_t ra = 0, rb = 0;
@@ -119,19 +138,16 @@ __global__ void rope_align_kernel(uint8_t* __restrict__ k_pool, const RopeJob* _
             aw[w] = ra;
             bw[w] = rb;
         }
-        *pa = a4;
-        *pb = b4;
+        *pa[i] = a4[i];
+        *pb[i] = b4[i];
     }
 }
 
-cudaError_t launch_rope_align(uint8_t* k_pool, const RopeJob* jobs_dev, RopeTable* tabs_dev, int n_jobs,
-                              const int* page_ids_dev, long long total_chunks, double rope_base, int D, int P, cudaStream_t st) {
-    if (total_chunks <= 0 || n_jobs <= 0) return cudaSuccess;
-    rope_table_kernel<<<n_jobs, 64, 0, st>>>(jobs_dev, tabs_dev, rope_base, D);
-    long long blocks = (total_chunks + 255) / 256;
-    if (blocks > 148 * 32) blocks = 148 * 32;
-    return launch_pdl(rope_align_kernel, dim3((unsigned)blocks), dim3(256), 0, st, k_pool, jobs_dev, (const RopeTable*)tabs_dev, n_jobs, page_ids_dev,
-                      total_chunks, D, P);
+cudaError_t launch_rope_align(uint8_t* k_pool, const RopeJob* jobs_dev, int n_jobs, const int* page_ids_dev, int total_units,
+                              double rope_base, int D, int P, cudaStream_t st) {
+    if (total_units <= 0 || n_jobs <= 0) return cudaSuccess;
+    return launch_pdl(rope_align_kernel, dim3((unsigned)total_units), dim3(256), 0, st, k_pool, jobs_dev, n_jobs, page_ids_dev,
+                      rope_base, D, P == 32 ? 5 : 4);
 }
 
 // ---------------------------------------------------------------------------------------------
