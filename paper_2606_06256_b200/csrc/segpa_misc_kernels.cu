@@ -274,12 +274,14 @@ __global__ void __launch_bounds__(NW * 32) combine_kernel(const __grid_constant_
     const int rows_per_slot = kTileRows * p.tiles_per_item;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     ptx::pdl_launch_dependents();
-    ptx::pdl_wait();         // the partials are the attention kernel's
     // block (x, y): comb x, rows y, y + gridDim.y, ...  One block per row.  Each warp folds its share of the row's
     // partials into a state (M, L, acc) of its own -- no pass over all the maxima first, so a row with up to 96 partials
     // costs ONE round trip to memory -- and warp 0 merges the NW states.  Every sum runs in a fixed order.
+    // The descriptors were uploaded before the attention kernel started: their two dependent loads run while this
+    // block still waits for that kernel (a decode-shaped layer is ~60 us, this kernel ~6 of them, all latency).
     const CombDev c = p.combs[blockIdx.x];
     const SegDev sg = p.segs[c.seg];
+    ptx::pdl_wait();         // the partials are the attention kernel's
     const int rows = c.n_tok * p.G;
     // partials of row r: slot first_slot + s at row r; strided items hold a second one at row r + 128
     const int per_slot = (c.flags & 1) ? 2 : 1;
