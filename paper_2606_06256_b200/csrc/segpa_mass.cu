@@ -4,24 +4,27 @@
 // recomputed from Q, the paged K and the LSE the fused attention wrote (the probabilities themselves never
 // exist in memory).  Transposed formulation so that the sum over queries is an in-thread sum:
 //     S^T = K_block Q_tile^T    (M = 128 keys = TMEM lanes, N = 128 query rows = columns)
-// tcgen05.mma with both operands K-major from shared memory (K pages by bulk copy, Q tiles by TMA), accumulator
-// four-deep in TMEM (all 512 columns), K block double-buffered; one thread per key applies the visibility rule and ex2 to its 128 columns and keeps the
-// running sum in a register.  A CTA owns a (segment, key block) item and loops over the query tiles that can see
-// it: every mass entry is written exactly once, by one thread (deterministic, no atomics).
+// tcgen05.mma, B (the Q tile, by TMA) K-major from shared memory and A (the K block) from TENSOR MEMORY: the block is the
+// same for every tile of an item, so it is copied once per item from its shared-memory page image into TMEM
+// (tcgen05.cp.128x256b with the same SWIZZLE_128B descriptors an SS-mode MMA would read it through, one copy per 16
+// head-dim columns; in order with the MMAs in the tensor pipe, so no barrier sits between copy and use and the copy of
+// item i + 2 cannot overtake item i's MMAs) and the MMAs read half as much from shared memory.  TMEM: two K-block
+// buffers [0, 128), three accumulator stages [128, 512).  One thread per key applies the visibility rule and ex2 to
+// its 128 columns and keeps the running sum in a register.  A CTA owns a (segment, key block) item and loops over the
+// query tiles that can see it: every mass entry is written exactly once, by one thread (deterministic, no atomics).
 // Bound: the dense contraction is half of the attention kernel's (no PV) and the exponentials are the same, so the
 // MUFU pipe (16 ex2 / clk / SM = 1024 clk per 128x128 tile) limits it at twice the MMA time.
 //
-// 20 warps: 0 loader (K block, Q tiles), 1 MMA issuer, 2-3 per-column LSE / position arrays (3 also owns TMEM), 4-19 four
-// exp warpgroups, warpgroup g on the tiles whose running number in the CTA's tile sequence is g mod 4 (accumulator
-// stage g), all 128 query columns of a key in one thread, in four chunks of 32 with the TMEM load of the next chunk
-// under the exponentials of the current one.
-// Why four tiles in flight (round 2; ncu source page and the -DSEGPA_TRACE timeline): a tile costs an
+// 16 warps: 0 loader (K block, Q tiles), 1 MMA issuer (and the K-block copies), 2-3 per-column LSE / position arrays (3
+// also owns TMEM), 4-15 three exp warpgroups, warpgroup g on the tiles whose running number in the CTA's tile sequence
+// is g mod 3 (accumulator stage g), all 128 query columns of a key in one thread, in four chunks of 32 with the TMEM
+// load of the next chunk under the exponentials of the current one.
+// Why several tiles in flight (round 2; ncu source page and the -DSEGPA_TRACE timeline): a tile costs an
 // exp warp ~450-1100 cycles of serial latency around its exponentials (two mbarrier waits, the per-tile flags, the
 // first TMEM load, the drain -- each a round trip through the instruction queue the other warps' ex2 sit in).  With
 // two warpgroups that each took half of the columns of EVERY tile (round 1), all eight warps sat in that prologue
 // together and the MUFU pipe idled (56 % busy, 1850 cycles per tile); with the warpgroups on different tiles one's
-// prologue runs under the others' exponentials (1440-1540 cycles per tile, pipe 67-71 % busy).  What was tried on top
-// and did not pay is listed in DESIGN.md 5.7.
+// prologue runs under the others' exponentials.  What was tried on top and did not pay is listed in DESIGN.md 5.7.
 #include "segpa_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -30,9 +33,13 @@ using namespace ptx;
 
 namespace {
 
-constexpr int kMassThreads = 640;   // 4 service warps + four exp warpgroups
-// register budgets (setmaxnreg): 128 * 56 + 512 * 104 = 60416 <= 640 * 96, the launch allocation
-constexpr int kRegsService = 56, kRegsExp = 104;
+constexpr int kExpGroups = 3;        // exp warpgroups = accumulator stages
+constexpr int kMassThreads = 128 + 128 * kExpGroups;   // 4 service warps + the exp warpgroups
+// register budgets (setmaxnreg): 128 * 56 + 384 * 144 = 62464 <= 512 * 128, the launch allocation
+constexpr int kRegsService = 56, kRegsExp = 144;
+// TMEM columns: the K block of the current and the next item as the MMA's A operand (bf16, D / 2 columns each), then the
+// accumulator stages
+constexpr uint32_t kColA = 0, kColS = 128;
 
 struct alignas(16) MassAux {
     float lse2[kTileRows];   // LSE of column c in log2 units
@@ -43,10 +50,10 @@ struct alignas(16) MassAux {
 };
 
 constexpr int kQStages = 4;   // Q tiles in flight
-constexpr int kSStages = 4;   // S accumulators in TMEM (4 x 128 columns), one per exp warpgroup
+constexpr int kSStages = kExpGroups;   // S accumulators in TMEM (128 columns each), one per exp warpgroup
 constexpr int kKStages = 2;   // K blocks: the next item's block is loaded under the current item's last tiles
-constexpr int kAuxStages = 8; // per-column arrays: an exp warpgroup needs those of its next tile (four on) the moment it
-                              // finishes one, so the LSE warps must be able to run more than four tiles ahead
+constexpr int kAuxStages = 8; // per-column arrays: an exp warpgroup needs those of its next tile (three on) the moment it
+                              // finishes one, so the LSE warps must be able to run more than three tiles ahead
 
 struct MassBars {
     uint64_t k_full[kKStages], k_empty[kKStages];
@@ -79,7 +86,7 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
     extern __shared__ uint8_t smem_raw[];
     __shared__ MassBars bars;
     __shared__ MassAux aux[kAuxStages];
-    __shared__ float part_sum[3][kTileRows];   // partial masses of the other three exp warpgroups, added by the first in a fixed order
+    __shared__ float part_sum[kExpGroups - 1][kTileRows];   // partial masses of the other three exp warpgroups, added by the first in a fixed order
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
     const uint32_t sK = smem_u32(smem);           // kKStages K blocks
     const uint32_t sQ = sK + kKStages * kTileBytes;   // kQStages Q stages
@@ -261,6 +268,19 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             mbar_wait(smem_u32(&bars.k_full[ks]), (n_k / kKStages) & 1);
             ++n_k;
             const uint64_t dk = dk0 + (uint64_t)((ks * kTileBytes) >> 4);
+            // The K block is the A operand of every tile of the item: copied once into TMEM (tcgen05.cp, in order with the
+            // MMAs in the tensor pipe: no barrier between them, and the copy for item i + 2 cannot overtake item i's MMAs),
+            // so that the MMAs read only the Q tile from shared memory -- half of the operand traffic.
+            const uint32_t tA = tmem + kColA + ((n_k - 1) & 1) * 64;
+            if (elect_one()) {
+#pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk) {
+                    const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
+                    tmem_cp_128x256b(tA + kk * 8, dk + ok);
+                }
+                tc_commit(smem_u32(&bars.k_empty[ks]));      // the K stage is free as soon as the copies have completed
+            }
+            __syncwarp();
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
                 const uint32_t qs = n_t % kQStages, qph = (n_t / kQStages) & 1;
                 const uint32_t st = n_t % kSStages, ph = (n_t / kSStages) & 1;
@@ -275,27 +295,25 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
 #pragma unroll
                     for (int kk = 0; kk < D / 16; ++kk) {
                         const uint32_t oq = ((kk / 4) * (kTileRows * 128) + (kk % 4) * 32) >> 4;
-                        const uint32_t ok = ((kk / 4) * kAtomBytes + (kk % 4) * 32) >> 4;
-                        mma_ss(tmem + st * 128, dk + ok, dq + oq, idesc, kk > 0 ? 1u : 0u);
+                        mma_ts(tmem + kColS + st * 128, tA + kk * 8, dq + oq, idesc, kk > 0 ? 1u : 0u);
                     }
                     tc_commit(smem_u32(&bars.s_full[st]));
                     tc_commit(smem_u32(&bars.q_empty[qs]));
-                    if (ti + 1 == it.t_hi) tc_commit(smem_u32(&bars.k_empty[ks]));
                 }
                 __syncwarp();
             }
         }
     } else if (warp >= 4) {
-        // ------------------------------------------------------------------ exp warpgroups: thread = (key, every fourth tile)
-        // Warpgroup g (warps 4 + 4g ...) takes the tiles with running number = g mod 4: accumulator stage g.  A thread
+        // ------------------------------------------------------------------ exp warpgroups: thread = (key, every third tile)
+        // Warpgroup g (warps 4 + 4g ...) takes the tiles with running number = g mod 3: accumulator stage g.  A thread
         // walks its key's 128 query columns in four chunks of 32, the TMEM load of the next chunk in flight under the
         // exponentials of the current one; the accumulator stage goes back to the MMA issuer as soon as the last
-        // chunk is in registers.  The four partial sums of a key are added in a fixed order.
+        // chunk is in registers.  The partial sums of a key are added in a fixed order.
         reg_inc<kRegsExp>();
         const int wq = warp & 3;
         const int grp = (warp - 4) >> 2;
         const int kr = wq * 32 + lane;                                   // key row inside the block
-        const uint32_t t_base = tmem + ((uint32_t)(wq * 32) << 16) + grp * 128;
+        const uint32_t t_base = tmem + ((uint32_t)(wq * 32) << 16) + kColS + grp * 128;
         const float sl2 = p.scale * 1.4426950408889634f;
         uint32_t n_t = 0;
         for (int ii = i_lo; ii < i_hi; ++ii) {
@@ -306,8 +324,8 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
             const bool is_sink_key = key < sg.n_sink;
             float acc = 0.f;
             for (int ti = it.t_lo; ti < it.t_hi; ++ti, ++n_t) {
-                if ((int)(n_t & 3) != grp) continue;
-                static_assert(kSStages == 4, "accumulator stage = exp warpgroup");
+                if ((int)(n_t % kExpGroups) != grp) continue;
+                static_assert(kSStages == kExpGroups, "accumulator stage = exp warpgroup");
                 const uint32_t ph = (n_t / kSStages) & 1;
                 const uint32_t as = n_t % kAuxStages, aph = (n_t / kAuxStages) & 1;
                 TRACE(20, n_t);
@@ -360,8 +378,8 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                 tmem_wait_ld();
                 tmem_ld32(t_base + 96, sb);
                 // the accumulator stage goes back at the half-way point, at the price of one exposed TMEM load (the
-                // other three warps of the scheduler fill it): the MMA of tile n_t + 4 takes ~1500-1900 cycles from
-                // this arrive to a visible s_full (wait latency + 8 MMAs + commit + wait latency), more than one chunk
+                // other warps of the scheduler fill it): the MMA of the stage's next tile takes ~1500 cycles from this
+                // arrive to a visible s_full (wait latency + the MMAs + commit + wait latency), more than one chunk
                 tmem_wait_ld();
                 tc_fence_before();
                 mbar_arrive(smem_u32(&bars.s_empty[grp]));
@@ -371,13 +389,12 @@ __global__ void __launch_bounds__(kMassThreads, 1) attention_mass_kernel(const _
                 TRACE(24 + (full ? 0 : 1), n_t);
                 mbar_arrive(smem_u32(&bars.aux_empty[as]));
             }
-            // mass = ((tiles 0 mod 4) + (1 mod 4)) + ((2 mod 4) + (3 mod 4)), added by the first warpgroup: one writer
-            // per entry, one order
+            // mass = ((tiles 0 mod 3) + (1 mod 3)) + (2 mod 3), added by the first warpgroup: one writer per entry, one order
             if (grp > 0) part_sum[grp - 1][kr] = acc;
-            asm volatile("bar.sync 1, 512;" ::: "memory");
+            asm volatile("bar.sync 1, 384;" ::: "memory");
             if (grp == 0 && key < sg.kv_len)
-                p.mass[p.mass_off[it.seg] + key] = (acc + part_sum[0][kr]) + (part_sum[1][kr] + part_sum[2][kr]);
-            asm volatile("bar.sync 2, 512;" ::: "memory");
+                p.mass[p.mass_off[it.seg] + key] = (acc + part_sum[0][kr]) + part_sum[1][kr];
+            asm volatile("bar.sync 2, 384;" ::: "memory");
         }
     }
 

@@ -144,6 +144,12 @@ __device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_
         : "memory");
 }
 
+// shared memory -> TMEM: 128 rows x 256 bits of the matrix the descriptor names (same descriptor format as the MMA's
+// operands) into lanes 0..127, 8 columns; asynchronous, in order with the tcgen05.mma of the issuing thread
+__device__ __forceinline__ void tmem_cp_128x256b(uint32_t taddr, uint64_t s_desc) {
+    asm volatile("tcgen05.cp.cta_group::1.128x256b [%0], %1;" ::"r"(taddr), "l"(s_desc) : "memory");
+}
+
 // TMEM -> registers: this thread's lane (row), 32 consecutive 32-bit columns
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t* r) {
     asm volatile(
