@@ -472,18 +472,43 @@ __global__ void mass_select_kernel(const float* __restrict__ mass, const long lo
         ties_needed = rest > 0.f ? (int)ceilf(rest / tval) : 0;
     }
     __syncthreads();
-    // sequential over positions for the tie rule (one thread; n is a stream length, the pass is a few microseconds)
+    // The tie rule is positional: key j at the threshold is taken when fewer than ties_needed threshold keys lie before
+    // it.  Every thread takes a contiguous range of positions, counts the threshold keys in it, a block-wide exclusive
+    // scan of those counts gives the number before the range, and the thread then walks its range.  (One thread walking
+    // the whole stream took ~80 us of the kernel's 190 on cfg2's 4 800-key segments.)
+    __shared__ int wsum[32];
+    const int per = (n + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int j0 = min(n, (int)threadIdx.x * per), j1 = min(n, j0 + per);
+    int mine = 0;
+    for (int j = j0; j < j1; ++j) mine += __float_as_uint(m[j]) == lo;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int incl = mine;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += up;
+    }
+    if (lane == 31) wsum[warp] = incl;
+    __syncthreads();
+    int before = incl - mine;
+    for (int w2 = 0; w2 < warp; ++w2) before += wsum[w2];
+    int taken = before, cnt = 0;
+    for (int j = j0; j < j1; ++j) {
+        const unsigned b = __float_as_uint(m[j]);
+        unsigned char sv = 0;
+        if (b > lo) sv = 1;
+        else if (b == lo && taken < ties_needed) sv = 1;
+        taken += b == lo;
+        sel[j] = sv;
+        cnt += sv;
+    }
+    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    __syncthreads();
+    if (lane == 0) wsum[warp] = cnt;
+    __syncthreads();
     if (threadIdx.x == 0) {
-        int taken = 0, cnt = 0;
-        for (int j = 0; j < n; ++j) {
-            const unsigned b = __float_as_uint(m[j]);
-            unsigned char s = 0;
-            if (b > lo) s = 1;
-            else if (b == lo && taken < ties_needed) { s = 1; ++taken; }
-            sel[j] = s;
-            cnt += s;
-        }
-        n_selected[seg] = cnt;
+        int tot_sel = 0;
+        for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) tot_sel += wsum[w2];
+        n_selected[seg] = tot_sel;
     }
 }
 

@@ -140,3 +140,54 @@ def test_mass_select_is_the_smallest_covering_set(tau):
             assert abs(int(cn[si]) - min(k_star, kv)) <= 1
     finally:
         g.close()
+
+
+def test_mass_select_takes_ties_lowest_position_first():
+    """Keys of equal mass at the threshold: the lowest positions are taken, exactly as many as are needed (the tie
+    rule of segpa.h; the pass that applies it is spread over the block, each thread with a range of positions and the
+    number of threshold keys before it).  Synthetic masses on the segments of a real plan."""
+    Hq, Hkv, D, P, reqs = CASES[0]
+    w = wl.make_workload("selties", Hq=Hq, Hkv=Hkv, D=D, P=P, requests=reqs, seed=601)
+    g = GpuRun(w, "tc", 2)
+    try:
+        g.layer(0)
+        segs = g.segs[0]
+        offs = B.segpa_segments_mass_layout(segs)
+        sm = w.stream_map()
+        kvs = [sm[(0, s.kv_head, s.seq_id)].kv_len for s in w.layer_segments(0)]
+        rng = np.random.default_rng(11)
+        for variant in range(4):
+            mass = np.zeros((int(offs[-1]),), dtype=np.float32)
+            want = np.zeros_like(mass, dtype=np.uint8)
+            tau = [0.5, 0.3, 0.77, 1.0][variant]
+            for si, kv in enumerate(kvs):
+                if variant == 0:
+                    mm = np.ones(kv, dtype=np.float32)                       # all equal
+                elif variant == 1:
+                    mm = rng.choice(np.array([0.25, 0.5, 1.0, 2.0], dtype=np.float32), size=kv)   # four levels, many ties
+                elif variant == 2:
+                    mm = np.where(np.arange(kv) % 7 == 3, 4.0, 0.5).astype(np.float32)
+                else:
+                    mm = rng.choice(np.array([0.0, 1.0], dtype=np.float32), size=kv)              # tau = 1: every key with mass
+                mass[offs[si]:offs[si] + kv] = mm
+                # reference: heaviest first, ties by position, until tau of the total is covered (exact in fp64 for these values)
+                need = np.float32(tau) * np.float32(mm.sum(dtype=np.float64))
+                order = np.lexsort((np.arange(kv), -mm))
+                csum = np.cumsum(mm[order].astype(np.float64))
+                k = int(np.searchsorted(csum, float(need) - 1e-9) + 1)
+                k = min(k, kv)
+                if variant == 3:
+                    k = int((mm > 0).sum())
+                want[offs[si] + order[:k]] = 1
+            md = torch.from_numpy(mass).to(g.dev)
+            sel = torch.full((int(offs[-1]),), 7, dtype=torch.uint8, device=g.dev)
+            cnt = torch.zeros((len(offs) - 1,), dtype=torch.int32, device=g.dev)
+            B.segpa_mass_select(g.cache, segs, md, tau, sel, cnt)
+            torch.cuda.synchronize()
+            got = sel.cpu().numpy()
+            for si, kv in enumerate(kvs):
+                a, b = got[offs[si]:offs[si] + kv], want[offs[si]:offs[si] + kv]
+                assert np.array_equal(a, b), (variant, si, int(a.sum()), int(b.sum()), np.flatnonzero(a != b)[:8])
+                assert int(cnt[si]) == int(b.sum())
+    finally:
+        g.close()
