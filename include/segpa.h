@@ -379,8 +379,8 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t *cache, const segpa_segmen
  * softmax over their union"): (out_a, lse_a) and (out_b, lse_b) are attention results of the SAME queries over
  * two DISJOINT key sets (e.g. an offline-cached part and an online part); writes the result over the union:
  *     lse = ln(e^lse_a + e^lse_b),   out = (e^lse_a out_a + e^lse_b out_b) / (e^lse_a + e^lse_b).
- * Layouts as in segpa_attention_fwd (out_*: device bf16 [T][Hq][D] with one common row stride; lse_*: device
- * fp32 [Hq][lse_stride]).  A (row, head) whose lse is -inf on one side takes the other side's result; out / lse
+ * Layouts as in segpa_attention_fwd (out_*: device bf16 [T][Hq][D] with one common row stride, a multiple of 8
+ * elements, 16-byte aligned; lse_*: device fp32 [Hq][lse_stride]).  A (row, head) whose lse is -inf on one side takes the other side's result; out / lse
  * may alias out_a / lse_a.  Asynchronous on cuda_stream.  Errors: INVALID, STATE (planning-only cache), CUDA.
  */
 segpa_status_t segpa_merge(segpa_cache_t *cache, const void *out_a, const float *lse_a, const void *out_b,

@@ -1714,6 +1714,8 @@ segpa_status_t segpa_merge(segpa_cache_t* c, const void* out_a, const float* lse
     if (c->planning_only) return fail(SEGPA_ERR_STATE, "merge: planning-only cache has no device");
     const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
     if (T < 1 || row_stride < (int64_t)Hq * D || lse_stride < T) return fail(SEGPA_ERR_INVALID, "merge: bad T / strides");
+    if ((row_stride % 8) || ((uintptr_t)out_a % 16) || ((uintptr_t)out_b % 16) || ((uintptr_t)out % 16))
+        return fail(SEGPA_ERR_INVALID, "merge: out_a / out_b / out must be 16-byte aligned with a row stride multiple of 8 elements (as in attention_fwd)");
     DeviceGuard g(c->desc.device);
     cudaError_t e = launch_merge((const uint16_t*)out_a, lse_a, (const uint16_t*)out_b, lse_b, (uint16_t*)out, lse, row_stride,
                                  lse_stride, T, Hq, D, (cudaStream_t)cuda_stream);

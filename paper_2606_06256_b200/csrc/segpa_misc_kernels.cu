@@ -3,6 +3,8 @@
 #include "segpa_internal.h"
 #include "sm100_ptx.cuh"
 
+#include <type_traits>
+
 #include <cuda_bf16.h>
 
 namespace segpa {
@@ -341,41 +343,86 @@ cudaError_t launch_combine(const FwdParams& p, cudaStream_t st) {
 // LSE merge of two results over disjoint key sets.  One warp per (row, head), lanes over D.
 // HBM-bound: 2 * D * 2 bytes read + D * 2 written per (row, head).
 // ---------------------------------------------------------------------------------------------
-__global__ void merge_kernel(const uint16_t* __restrict__ out_a, const float* __restrict__ lse_a,
-                             const uint16_t* __restrict__ out_b, const float* __restrict__ lse_b, uint16_t* out, float* lse,
-                             long long row_stride, long long lse_stride, long long T, int Hq, int D) {
+// A warp takes 32 consecutive (row, head) units at a time: lane i loads the two LSE values of unit i and forms its
+// weights (one load instruction per side for the 32 scattered values, lse being [Hq][T]), then the warp walks the units
+// two at a time, every lane moving its D / 32 consecutive elements of the unit's rows with one load per side (8 bytes at
+// D = 128).  The rows do not wait for the LSE values: a side whose weight turns out to be 0 is loaded and dropped.
+template <int EPL>   // elements per lane: D / 32 = 2 or 4
+__global__ void __launch_bounds__(256) merge_kernel(const uint16_t* __restrict__ out_a, const float* __restrict__ lse_a,
+                                                    const uint16_t* __restrict__ out_b, const float* __restrict__ lse_b, uint16_t* out,
+                                                    float* lse, long long row_stride, long long lse_stride, long long T, int Hq) {
+    constexpr int D = EPL * 32;
+    using Vec = typename std::conditional<EPL == 4, uint2, uint32_t>::type;
     const int lane = threadIdx.x & 31;
     const long long wid = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5, nw = ((long long)gridDim.x * blockDim.x) >> 5;
-    for (long long u = wid; u < T * Hq; u += nw) {
-        const long long row = u / Hq;
-        const int head = (int)(u % Hq);
-        const float la = lse_a[(long long)head * lse_stride + row], lb = lse_b[(long long)head * lse_stride + row];
+    const long long n_units = T * Hq;
+    for (long long g0 = wid * 32; g0 < n_units; g0 += nw * 32) {
+        // this lane's unit: weights and merged LSE
+        const long long um = g0 + lane;
+        const bool okm = um < n_units;
+        const long long rowm = okm ? um / Hq : 0;
+        const int headm = okm ? (int)(um - rowm * Hq) : 0;
+        const long long lidx = (long long)headm * lse_stride + rowm;
+        const float la = okm ? lse_a[lidx] : -INFINITY, lb = okm ? lse_b[lidx] : -INFINITY;
+        const long long basem = rowm * row_stride + (long long)headm * D;
         const float m = fmaxf(la, lb);
-        float wa = 0.f, wb = 0.f, l = -INFINITY;
+        float wam = 0.f, wbm = 0.f, l = -INFINITY;
         if (m != -INFINITY) {
             const float ea = expf(la - m), eb = expf(lb - m);     // exp(-inf) = 0
-            wa = ea / (ea + eb);
-            wb = eb / (ea + eb);
+            wam = ea / (ea + eb);
+            wbm = eb / (ea + eb);
             l = m + logf(ea + eb);
         }
-        const long long base = row * row_stride + (long long)head * D;
-        for (int d = lane; d < D; d += 32) {
-            // a side with weight 0 (lse = -inf) may hold anything, NaN included: it is not read into the sum
-            const float a = wa != 0.f ? __bfloat162float(__ushort_as_bfloat16(out_a[base + d])) : 0.f;
-            const float b = wb != 0.f ? __bfloat162float(__ushort_as_bfloat16(out_b[base + d])) : 0.f;
-            out[base + d] = __bfloat16_as_ushort(__float2bfloat16_rn(wa * a + wb * b));
+        if (okm) lse[lidx] = l;
+        const int n_here = (int)min((long long)32, n_units - g0);
+#pragma unroll 1
+        for (int i0 = 0; i0 < n_here; i0 += 2) {
+            float wa[2], wb[2];
+            long long base[2];
+            Vec va[2], vb[2];
+            bool ok[2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int src = min(i0 + i, 31);
+                ok[i] = i0 + i < n_here;
+                base[i] = __shfl_sync(0xffffffffu, basem, src) + lane * EPL;
+                wa[i] = __shfl_sync(0xffffffffu, wam, src);
+                wb[i] = __shfl_sync(0xffffffffu, wbm, src);
+                va[i] = *reinterpret_cast<const Vec*>(out_a + base[i]);      // (unit min(i, last): always inside the arrays)
+                vb[i] = *reinterpret_cast<const Vec*>(out_b + base[i]);
+            }
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                if (!ok[i]) continue;
+                // a side with weight 0 (lse = -inf) may hold anything, NaN included: it is not read into the sum
+                if (wa[i] == 0.f) va[i] = Vec{};
+                if (wb[i] == 0.f) vb[i] = Vec{};
+                const uint32_t* pa = reinterpret_cast<const uint32_t*>(&va[i]);
+                const uint32_t* pb = reinterpret_cast<const uint32_t*>(&vb[i]);
+                Vec vo;
+                uint32_t* po = reinterpret_cast<uint32_t*>(&vo);
+#pragma unroll
+                for (int w = 0; w < EPL / 2; ++w) {
+                    const float a0 = __uint_as_float(pa[w] << 16), a1 = __uint_as_float(pa[w] & 0xffff0000u);
+                    const float b0 = __uint_as_float(pb[w] << 16), b1 = __uint_as_float(pb[w] & 0xffff0000u);
+                    const uint32_t r0 = __bfloat16_as_ushort(__float2bfloat16_rn(wa[i] * a0 + wb[i] * b0));
+                    const uint32_t r1 = __bfloat16_as_ushort(__float2bfloat16_rn(wa[i] * a1 + wb[i] * b1));
+                    po[w] = r0 | (r1 << 16);
+                }
+                *reinterpret_cast<Vec*>(out + base[i]) = vo;
+            }
         }
-        if (lane == 0) lse[(long long)head * lse_stride + row] = l;
     }
 }
 
 cudaError_t launch_merge(const uint16_t* out_a, const float* lse_a, const uint16_t* out_b, const float* lse_b, uint16_t* out,
                          float* lse, long long row_stride, long long lse_stride, long long T, int Hq, int D, cudaStream_t st) {
-    const long long warps = T * Hq;
+    const long long warps = (T * Hq + 31) / 32;
     if (warps <= 0) return cudaSuccess;
     long long blocks = (warps + 7) / 8;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    merge_kernel<<<(unsigned)blocks, 256, 0, st>>>(out_a, lse_a, out_b, lse_b, out, lse, row_stride, lse_stride, T, Hq, D);
+    if (D == 128) merge_kernel<4><<<(unsigned)blocks, 256, 0, st>>>(out_a, lse_a, out_b, lse_b, out, lse, row_stride, lse_stride, T, Hq);
+    else merge_kernel<2><<<(unsigned)blocks, 256, 0, st>>>(out_a, lse_a, out_b, lse_b, out, lse, row_stride, lse_stride, T, Hq);
     return cudaGetLastError();
 }
 

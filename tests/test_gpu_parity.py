@@ -720,6 +720,64 @@ def test_lse_merge_of_split_key_sets(j0):
         g.close()
 
 
+@pytest.mark.parametrize("T,Hq,D,pad", [(1, 8, 128, 0), (5, 3, 64, 0), (37, 28, 128, 64), (1000, 7, 64, 8), (4099, 4, 128, 0)])
+def test_merge_over_shapes(T, Hq, D, pad):
+    """segpa_merge against its definition (segpa.h) written out in fp64, over shapes whose number of
+    (row, head) units is not a multiple of the 32 a warp takes at a time, both head dims, a padded row stride, and
+    lse = -inf on either side (that side may hold NaN) or on both.  Tolerance: one bf16 rounding of a convex combination
+    (|result| <= max(|a|, |b|)), fp32 weights: 2^-8 * max(|a|, |b|) + 1e-6; lse: 1e-5."""
+    dev = torch.device("cuda:0")
+    cache = B.segpa_create_cache(num_layers=1, num_q_heads=Hq, num_kv_heads=4 if Hq > 16 else 1, head_dim=D, page_size=16,
+                                 num_pages=8, device=0)
+    try:
+        rs = Hq * D + pad
+        def rows(seed):
+            buf = wl.randn_bf16((T, rs), seed, dev)
+            return buf, buf.as_strided((T, Hq, D), (rs, D, 1))
+        _, oa = rows(71)
+        _, ob = rows(72)
+        g = torch.Generator(device="cpu").manual_seed(73)
+        la = (torch.randn((Hq, T), generator=g) * 3).to(dev)
+        lb = (torch.randn((Hq, T), generator=g) * 3).to(dev)
+        kill = torch.rand((Hq, T), generator=g).to(dev)
+        la = torch.where(kill < 0.15, torch.full_like(la, float("-inf")), la)
+        lb = torch.where((kill > 0.1) & (kill < 0.3), torch.full_like(lb, float("-inf")), lb)      # 0.10-0.15: both sides
+        oa = torch.where((la == float("-inf")).t().unsqueeze(-1), torch.full_like(oa, float("nan")), oa)
+        ob = torch.where((lb == float("-inf")).t().unsqueeze(-1), torch.full_like(ob, float("nan")), ob)
+        bufa = torch.zeros((T, rs), dtype=torch.bfloat16, device=dev); bufb = torch.zeros_like(bufa)
+        va, vb = bufa.as_strided((T, Hq, D), (rs, D, 1)), bufb.as_strided((T, Hq, D), (rs, D, 1))
+        va.copy_(oa); vb.copy_(ob)
+        bufo = torch.full((T, rs), 7.0, dtype=torch.bfloat16, device=dev)
+        vo = bufo.as_strided((T, Hq, D), (rs, D, 1))
+        lo = torch.zeros_like(la)
+        B.segpa_merge(cache, va, la, vb, lb, vo, lo)
+        torch.cuda.synchronize()
+        a64, b64 = va.to(torch.float64).cpu().numpy(), vb.to(torch.float64).cpu().numpy()
+        la64, lb64 = la.to(torch.float64).cpu().numpy().T[:, :, None], lb.to(torch.float64).cpu().numpy().T[:, :, None]   # [T][Hq][1]
+        with np.errstate(invalid="ignore", divide="ignore"):
+            m = np.maximum(la64, lb64)
+            ea, eb = np.exp(la64 - np.where(np.isfinite(m), m, 0.0)), np.exp(lb64 - np.where(np.isfinite(m), m, 0.0))
+            wa, wb = ea / (ea + eb), eb / (ea + eb)
+            want = np.where(wa > 0, wa * np.nan_to_num(a64), 0.0) + np.where(wb > 0, wb * np.nan_to_num(b64), 0.0)
+            want_l = np.where(np.isfinite(m), m + np.log(ea + eb), -np.inf)
+        both = ~np.isfinite(m)
+        want = np.where(both, 0.0, want)
+        got = vo.to(torch.float64).cpu().numpy()
+        bound = 2.0 ** -8 * np.maximum(np.abs(np.nan_to_num(a64)), np.abs(np.nan_to_num(b64))) + 1e-6
+        assert np.all(np.abs(got - want) <= bound), np.abs(got - want).max()
+        got_l = lo.to(torch.float64).cpu().numpy().T[:, :, None]
+        assert np.array_equal(np.isfinite(got_l), np.isfinite(want_l))
+        fin = np.isfinite(want_l)
+        assert np.all(np.abs(got_l[fin] - want_l[fin]) <= 1e-5)
+        if pad:
+            assert bool((bufo[:, Hq * D:] == 7.0).all())          # the padding of the row stride is not written
+        big = torch.zeros((T * rs + 8,), dtype=torch.bfloat16, device=dev)
+        with pytest.raises(B.SegpaError):
+            B.segpa_merge(cache, va, la, vb, lb, big[1:].as_strided((T, Hq, D), (rs, D, 1)), lo)   # out not 16-byte aligned
+    finally:
+        B.segpa_destroy(cache)
+
+
 @pytest.mark.parametrize("seed", range(12))
 def test_random_workloads(seed):
     """Seeded random small workloads over the whole argument space (shape, page size, lengths, class, window,
