@@ -467,7 +467,9 @@ def measure(name: str, steps: int, warmup: int, dev, local_rank: int, world: int
             for l in range(w.num_layers):
                 segs = B.segpa_build_segments(cache, l, seg_batches[l], stream=stream)
                 seg_objs.append(segs)
-                B.segpa_attention_fwd_host(cache, segs, h_q[l], w.scale, h_out[l], h_lse[l], stream=stream)
+                # (several layers: asynchronous calls, so that layer l+1's rows go up while layer l's results come down)
+                B.segpa_attention_fwd_host(cache, segs, h_q[l], w.scale, h_out[l], h_lse[l], stream=stream, wait=w.num_layers == 1)
+            B.segpa_host_wait(cache)          # every layer's out / lse rows are in host memory
             torch.cuda.synchronize()
 
         e2e_step()
@@ -479,7 +481,7 @@ def measure(name: str, steps: int, warmup: int, dev, local_rank: int, world: int
         pcie = max(h2d, d2h) / (e2e_s) / 1e9
         rec["e2e"] = {"value": world * useful / e2e_s / 1e12, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                       "ms_per_step": 1e3 * e2e_s, "steps": n_e2e,
-                      "how": "segpa_append_pages_batch(src_is_host) + segpa_build_segments + segpa_attention_fwd_host per layer, pinned host buffers, wall clock around whole steps",
+                      "how": "segpa_append_pages_batch(src_is_host) + (segpa_build_segments + segpa_attention_fwd_host_async) per layer + segpa_host_wait, pinned host buffers, wall clock around whole steps",
                       "larger_direction_gbs": pcie}
         del h_q, h_out, h_lse, keep, h_batch
 

@@ -375,6 +375,21 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t *cache, const segpa_segmen
                                         float *lse_host, int64_t T, void *cuda_stream);
 
 /*
+ * segpa_attention_fwd_host without the wait at the end: the call returns once everything is enqueued, and out_host /
+ * lse_host are complete only after segpa_host_wait(cache) (or after a later synchronous segpa_attention_fwd_host on
+ * the cache has returned).  Consecutive calls (the layers of a step) then overlap: the cache holds two sets of staging
+ * buffers, so the q rows of call k+1 go up while the kernels and the copies back of call k still run, and the link is
+ * busy in both directions across layer boundaries.  At most two calls are in flight; a third waits (on the device) for
+ * the first to finish.  q_host must stay valid and out_host / lse_host untouched until the wait.  Same results, bit for
+ * bit, same errors.  segpa_host_wait: blocks the host until every asynchronous call on the cache has completed;
+ * Errors: INVALID (null), CUDA.
+ */
+segpa_status_t segpa_attention_fwd_host_async(segpa_cache_t *cache, const segpa_segments_t *segs,
+                                              const void *q_host, float softmax_scale, void *out_host,
+                                              float *lse_host, int64_t T, void *cuda_stream);
+segpa_status_t segpa_host_wait(segpa_cache_t *cache);
+
+/*
  * LSE merge ("splitting the key set ... and merging them with LSE gives the same result as
  * softmax over their union"): (out_a, lse_a) and (out_b, lse_b) are attention results of the SAME queries over
  * two DISJOINT key sets (e.g. an offline-cached part and an online part); writes the result over the union:

@@ -25,7 +25,7 @@ EXPORTS = [
     "segpa_clear_streams", "segpa_evict_pages", "segpa_rope_align", "segpa_rope_align_batch", "segpa_gather_rows", "segpa_gather_rows_noalloc", "segpa_free_stream",
     "segpa_stream_info", "segpa_pool_stats", "segpa_build_segments", "segpa_free_segments",
     "segpa_segments_stats", "segpa_segments_items", "segpa_segments_pages", "segpa_attention_fwd",
-    "segpa_attention_fwd_host", "segpa_merge", "segpa_segments_mass_layout", "segpa_attention_mass",
+    "segpa_attention_fwd_host", "segpa_attention_fwd_host_async", "segpa_host_wait", "segpa_merge", "segpa_segments_mass_layout", "segpa_attention_mass",
     "segpa_mass_select", "segpa_last_launch_count", "segpa_destroy", "segpa_last_error",
     "segpa_version",
 ]
@@ -135,6 +135,8 @@ def lib():
                                           C.c_int64, C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
         L.segpa_attention_fwd_host.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
                                                C.c_void_p, C.c_int64, C.c_void_p]
+        L.segpa_attention_fwd_host_async.argtypes = L.segpa_attention_fwd_host.argtypes
+        L.segpa_host_wait.argtypes = [C.c_void_p]
         L.segpa_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64,
                                   C.c_int64, C.c_int64, C.c_void_p]
         L.segpa_segments_mass_layout.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_int32)]
@@ -369,16 +371,25 @@ def segpa_attention_fwd(cache: int, segs: int, q, softmax_scale: float, out, lse
 
 
 def segpa_attention_fwd_host(cache: int, segs: int, q_host, softmax_scale: float, out_host, lse_host=None,
-                             stream=None) -> None:
-    """q_host, out_host: CPU torch bf16 tensors [T][Hq][D] contiguous (pinned for speed); lse_host fp32 [Hq][T]."""
+                             stream=None, wait: bool = True) -> None:
+    """q_host, out_host: CPU torch bf16 tensors [T][Hq][D] contiguous (pinned for speed); lse_host fp32 [Hq][T].
+    wait=False: segpa_attention_fwd_host_async (results complete after segpa_host_wait)."""
     assert (not q_host.is_cuda) and (not out_host.is_cuda) and q_host.is_contiguous() and out_host.is_contiguous()
     T = q_host.shape[0]
     lp = None
     if lse_host is not None:
         assert (not lse_host.is_cuda) and lse_host.is_contiguous()
         lp = lse_host.data_ptr()
-    _check(lib().segpa_attention_fwd_host(cache, segs, q_host.data_ptr(), softmax_scale, out_host.data_ptr(), lp, T,
-                                          _stream_ptr(stream)))
+    fn = lib().segpa_attention_fwd_host if wait else lib().segpa_attention_fwd_host_async
+    _check(fn(cache, segs, q_host.data_ptr(), softmax_scale, out_host.data_ptr(), lp, T, _stream_ptr(stream)))
+
+
+def segpa_attention_fwd_host_async(cache: int, segs: int, q_host, softmax_scale: float, out_host, lse_host=None, stream=None) -> None:
+    segpa_attention_fwd_host(cache, segs, q_host, softmax_scale, out_host, lse_host, stream=stream, wait=False)
+
+
+def segpa_host_wait(cache: int) -> None:
+    _check(lib().segpa_host_wait(cache))
 
 
 def segpa_merge(cache: int, out_a, lse_a, out_b, lse_b, out, lse, stream=None) -> None:

@@ -269,10 +269,17 @@ struct segpa_cache {
     int tiles_per_item = 2;   // 128-row tiles per work item (desc.tiles_per_item; fixed at create)
     int last_launches = 0;
     // host-buffer entry points: device staging, copy streams and events
-    uint16_t* st_q = nullptr;
-    uint16_t* st_out = nullptr;
-    float* st_lse = nullptr;
-    size_t st_q_bytes = 0, st_lse_bytes = 0;
+    // Q / out / LSE staging of segpa_attention_fwd_host: two sets, so that a call may be enqueued (the _async entry
+    // point) while the copies back of the previous one are still running.  The synchronous entry point uses set 0.
+    struct HostStage {
+        uint16_t* q = nullptr;
+        uint16_t* out = nullptr;
+        float* lse = nullptr;
+        size_t q_bytes = 0, lse_bytes = 0;
+        cudaEvent_t done = nullptr;      // recorded on d2h_stream after the set's last copy back
+        bool pending = false;            // done has been recorded and not yet waited for by the host
+    } hs[2];
+    int hs_turn = 0;
     uint16_t* st_kv = nullptr;          // K / V rows of host-source append requests (src_is_host)
     size_t st_kv_bytes = 0;
     cudaEvent_t st_kv_ev = nullptr;     // the scatter that last read st_kv has completed
@@ -598,9 +605,12 @@ segpa_status_t segpa_destroy(segpa_cache_t* c) {
     staging_free(c->append_stage[0]);
     staging_free(c->append_stage[1]);
     if (c->up_stream) cudaStreamDestroy(c->up_stream);
-    if (c->st_q) cudaFree(c->st_q);
-    if (c->st_out) cudaFree(c->st_out);
-    if (c->st_lse) cudaFree(c->st_lse);
+    for (auto& h : c->hs) {
+        if (h.q) cudaFree(h.q);
+        if (h.out) cudaFree(h.out);
+        if (h.lse) cudaFree(h.lse);
+        if (h.done) cudaEventDestroy(h.done);
+    }
     if (c->st_kv) cudaFree(c->st_kv);
     if (c->st_kv_ev) cudaEventDestroy(c->st_kv_ev);
     if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
@@ -1595,9 +1605,10 @@ segpa_status_t plan_host_chunks(segpa_cache* c, const segpa_segments* s, int64_t
 
 }  // namespace
 
-segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t* s, const void* q_host,
-                                        float scale, void* out_host, float* lse_host, int64_t T,
-                                        void* cuda_stream) {
+namespace {
+
+segpa_status_t attention_fwd_host_impl(segpa_cache_t* c, const segpa_segments_t* s, const void* q_host, float scale, void* out_host,
+                                       float* lse_host, int64_t T, void* cuda_stream, const bool async) {
     if (!c || !s || !q_host || !out_host) return fail(SEGPA_ERR_INVALID, "attention_fwd_host: null argument");
     if (c->planning_only) return fail(SEGPA_ERR_STATE, "attention_fwd_host: planning-only cache has no device; there is no CPU fallback");
     if (s->cache != c || std::find(c->seg_objs.begin(), c->seg_objs.end(), s) == c->seg_objs.end())
@@ -1611,20 +1622,30 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t
     cudaStream_t st = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(SEGPA_ERR_CUDA, "attention_fwd_host: earlier asynchronous failure: %s", cudaGetErrorString(e));
-    if (qb > c->st_q_bytes) {
-        if (c->st_q) { cudaStreamSynchronize(st); cudaFree(c->st_q); cudaFree(c->st_out); c->st_q = c->st_out = nullptr; c->st_q_bytes = 0; }
-        if (cudaMalloc((void**)&c->st_q, qb) != cudaSuccess || cudaMalloc((void**)&c->st_out, qb) != cudaSuccess) {
+    segpa_cache::HostStage& hs = c->hs[async ? (c->hs_turn++ & 1) : 0];
+    if (!hs.done && cudaEventCreateWithFlags(&hs.done, cudaEventDisableTiming) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(SEGPA_ERR_CUDA, "attention_fwd_host: cannot create events");
+    }
+    if (qb > hs.q_bytes || lb > hs.lse_bytes) {
+        // (growing the set: its last user must have finished with it)
+        if (hs.pending) { cudaEventSynchronize(hs.done); hs.pending = false; }
+        cudaStreamSynchronize(st);
+    }
+    if (qb > hs.q_bytes) {
+        if (hs.q) { cudaFree(hs.q); cudaFree(hs.out); hs.q = hs.out = nullptr; hs.q_bytes = 0; }
+        if (cudaMalloc((void**)&hs.q, qb) != cudaSuccess || cudaMalloc((void**)&hs.out, qb) != cudaSuccess) {
             cudaGetLastError();
-            if (c->st_q) cudaFree(c->st_q);
-            c->st_q = c->st_out = nullptr;
+            if (hs.q) cudaFree(hs.q);
+            hs.q = hs.out = nullptr;
             return fail(SEGPA_ERR_OOM, "attention_fwd_host: staging allocation of 2 x %zu bytes failed", qb);
         }
-        c->st_q_bytes = qb;
+        hs.q_bytes = qb;
     }
-    if (lb > c->st_lse_bytes) {
-        if (c->st_lse) { cudaStreamSynchronize(st); cudaFree(c->st_lse); c->st_lse = nullptr; c->st_lse_bytes = 0; }
-        if (cudaMalloc((void**)&c->st_lse, lb) != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_OOM, "attention_fwd_host: staging allocation failed"); }
-        c->st_lse_bytes = lb;
+    if (lb > hs.lse_bytes) {
+        if (hs.lse) { cudaFree(hs.lse); hs.lse = nullptr; hs.lse_bytes = 0; }
+        if (cudaMalloc((void**)&hs.lse, lb) != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_OOM, "attention_fwd_host: staging allocation failed"); }
+        hs.lse_bytes = lb;
     }
     if (!c->h2d_stream && (cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking) != cudaSuccess ||
                            cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking) != cudaSuccess)) {
@@ -1650,22 +1671,31 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t
     // (row, head) pairs no segment covers come back as zeros: the staging rows are cleared first.
     FwdParams base{};
     fill_fwd_params(base, c, s);
-    const char* why = encode_q_map(&base.q_map, c->st_q, T, Hq, D, c->G, base.tile_tokens, (int64_t)Hq * D);
+    const char* why = encode_q_map(&base.q_map, hs.q, T, Hq, D, c->G, base.tile_tokens, (int64_t)Hq * D);
     if (why) return fail(SEGPA_ERR_CUDA, "attention_fwd_host: %s", why);
-    base.q = c->st_q;
-    base.out = c->st_out;
-    base.lse = c->st_lse;
+    base.q = hs.q;
+    base.out = hs.out;
+    base.lse = hs.lse;
     base.q_row_stride = base.out_row_stride = (int64_t)Hq * D;
     base.lse_stride = T;
     base.scale = scale;
     const uint8_t* hb = (const uint8_t*)s->buf->host_blob.d;
-    e = cudaMemsetAsync(c->st_out, 0, qb, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->st_lse, 0, lb, st);
-    if (e == cudaSuccess) e = cudaEventRecord(ev_start, st);                  // earlier work on the caller's stream (K/V stores) is ordered before
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(c->h2d_stream, ev_start, 0);   // ... the first copy, so a step's uploads do not overtake the previous step's reads
+    // the set's previous user (two asynchronous calls ago) must have finished: its kernels with hs.q, its copies back with
+    // hs.out / hs.lse; done was recorded behind all of them
+    e = cudaSuccess;
+    if (hs.pending) {
+        e = cudaStreamWaitEvent(st, hs.done, 0);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c->h2d_stream, hs.done, 0);
+    }
+    if (e == cudaSuccess) e = cudaMemsetAsync(hs.out, 0, qb, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(hs.lse, 0, lb, st);
+    if (!async) {
+        if (e == cudaSuccess) e = cudaEventRecord(ev_start, st);                  // earlier work on the caller's stream is ordered before
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(c->h2d_stream, ev_start, 0);   // ... the first copy
+    }   // (asynchronous calls: the Q rows may go up while the kernels of the call before still run -- they use the other set)
     for (size_t k = 0; k < n_ch && e == cudaSuccess; ++k) {
         const segpa_segments::HostChunk& hc = s->hchunks[k];
-        e = cudaMemcpyAsync((uint8_t*)c->st_q + (size_t)hc.row_lo * row_bytes, (const uint8_t*)q_host + (size_t)hc.row_lo * row_bytes,
+        e = cudaMemcpyAsync((uint8_t*)hs.q + (size_t)hc.row_lo * row_bytes, (const uint8_t*)q_host + (size_t)hc.row_lo * row_bytes,
                             (size_t)(hc.row_hi - hc.row_lo) * row_bytes, cudaMemcpyHostToDevice, c->h2d_stream);
         if (e == cudaSuccess) e = cudaEventRecord(ev_in[k], c->h2d_stream);
     }
@@ -1692,21 +1722,53 @@ segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t
         // rows of chunk k are final once the kernels of chunk k have run (items of chunk k-1 that reach into it ran before)
         if (e == cudaSuccess) e = cudaStreamWaitEvent(c->d2h_stream, ev_done[k], 0);
         if (e == cudaSuccess)
-            e = cudaMemcpyAsync((uint8_t*)out_host + (size_t)hc.row_lo * row_bytes, (const uint8_t*)c->st_out + (size_t)hc.row_lo * row_bytes,
+            e = cudaMemcpyAsync((uint8_t*)out_host + (size_t)hc.row_lo * row_bytes, (const uint8_t*)hs.out + (size_t)hc.row_lo * row_bytes,
                                 (size_t)(hc.row_hi - hc.row_lo) * row_bytes, cudaMemcpyDeviceToHost, c->d2h_stream);
         if (e == cudaSuccess && lse_host)
-            e = cudaMemcpy2DAsync(lse_host + hc.row_lo, (size_t)T * 4, c->st_lse + hc.row_lo, (size_t)T * 4, (size_t)(hc.row_hi - hc.row_lo) * 4,
+            e = cudaMemcpy2DAsync(lse_host + hc.row_lo, (size_t)T * 4, hs.lse + hc.row_lo, (size_t)T * 4, (size_t)(hc.row_hi - hc.row_lo) * 4,
                                   (size_t)Hq, cudaMemcpyDeviceToHost, c->d2h_stream);
     }
     c->last_launches = launches;
-    // the call is synchronous: wait for the last copy back (and leave the caller's stream ordered after it)
-    if (e == cudaSuccess) e = cudaEventRecord(ev_start, c->d2h_stream);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_start, 0);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(c->d2h_stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e == cudaSuccess) e = cudaEventRecord(hs.done, c->d2h_stream);
+    if (e == cudaSuccess) hs.pending = true;
+    if (!async) {
+        // the call is synchronous: wait for the last copy back (and leave the caller's stream ordered after it)
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(st, hs.done, 0);
+        if (e == cudaSuccess) e = cudaEventSynchronize(hs.done);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        hs.pending = false;
+    }
     if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "attention_fwd_host: %s", cudaGetErrorString(e)); }
     return SEGPA_OK;
 }
+
+}  // namespace
+
+segpa_status_t segpa_attention_fwd_host(segpa_cache_t* c, const segpa_segments_t* s, const void* q_host, float scale, void* out_host,
+                                        float* lse_host, int64_t T, void* cuda_stream) {
+    return attention_fwd_host_impl(c, s, q_host, scale, out_host, lse_host, T, cuda_stream, false);
+}
+
+segpa_status_t segpa_attention_fwd_host_async(segpa_cache_t* c, const segpa_segments_t* s, const void* q_host, float scale,
+                                              void* out_host, float* lse_host, int64_t T, void* cuda_stream) {
+    return attention_fwd_host_impl(c, s, q_host, scale, out_host, lse_host, T, cuda_stream, true);
+}
+
+segpa_status_t segpa_host_wait(segpa_cache_t* c) {
+    if (!c) return fail(SEGPA_ERR_INVALID, "host_wait: null cache");
+    if (c->planning_only) return SEGPA_OK;
+    DeviceGuard g(c->desc.device);
+    cudaError_t e = cudaSuccess;
+    for (auto& h : c->hs)
+        if (h.pending) {
+            const cudaError_t e2 = cudaEventSynchronize(h.done);
+            if (e == cudaSuccess) e = e2;
+            h.pending = false;
+        }
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(SEGPA_ERR_CUDA, "host_wait: %s", cudaGetErrorString(e)); }
+    return SEGPA_OK;
+}
+
 
 segpa_status_t segpa_merge(segpa_cache_t* c, const void* out_a, const float* lse_a, const void* out_b, const float* lse_b,
                            void* out, float* lse, int64_t row_stride, int64_t lse_stride, int64_t T, void* cuda_stream) {

@@ -553,6 +553,49 @@ def test_host_entry_points_pipelined_chunks_and_host_source_append():
         g.close()
 
 
+def test_host_entry_point_async_calls_overlap_and_match():
+    """segpa_attention_fwd_host_async: five calls in a row with different queries (more than the two staging sets, so the
+    third and later calls reuse a set whose previous copies back may still be running), one segpa_host_wait, every result
+    bit-identical to the synchronous entry point's; then synchronous and asynchronous calls mixed."""
+    reqs = [{"kv_len": 5000, "heads": {h: ((GLOBAL, 0, 0, 5000) if h == 0 else (LOCAL, 700, 4 * (h % 2), 5000 if h < 6 else 333)) for h in range(8)}},
+            {"kv_len": 9000, "heads": {h: ((GLOBAL, 0, 0, 1) if h % 3 == 0 else (LOCAL, 2048, 0, 1)) for h in range(8)}}]
+    w = wl.make_workload("hostasync", Hq=32, Hkv=8, D=128, P=16, requests=reqs, seed=62)
+    dev = torch.device("cuda:0")
+    g = GpuRun(w, "tc", 2)
+    try:
+        g.layer(0)
+        segs = g.segs[0]
+        T = w.T[0]
+        gen = torch.Generator().manual_seed(5)
+        qs = [torch.randn((T, w.Hq, w.D), generator=gen).to(torch.bfloat16).pin_memory() for _ in range(5)]
+        want = []
+        for qh in qs:
+            oh = torch.full_like(qh, 3.0).pin_memory()
+            lh = torch.full((w.Hq, T), 3.0, dtype=torch.float32).pin_memory()
+            B.segpa_attention_fwd_host(g.cache, segs, qh, w.scale, oh, lh)
+            want.append((oh.clone(), lh.clone()))
+        outs = [(torch.full_like(qh, 5.0).pin_memory(), torch.full((w.Hq, T), 5.0, dtype=torch.float32).pin_memory()) for qh in qs]
+        for qh, (oh, lh) in zip(qs, outs):
+            B.segpa_attention_fwd_host_async(g.cache, segs, qh, w.scale, oh, lh)
+        B.segpa_host_wait(g.cache)
+        for (oh, lh), (ow, lw) in zip(outs, want):
+            assert torch.equal(oh, ow) and torch.equal(lh, lw)
+        # mixed: async, sync (which must wait for the set the async call holds), async; a wait with nothing pending
+        o0, l0 = torch.full_like(qs[0], 5.0).pin_memory(), torch.full((w.Hq, T), 5.0, dtype=torch.float32).pin_memory()
+        o1, l1 = torch.full_like(qs[1], 5.0).pin_memory(), torch.full((w.Hq, T), 5.0, dtype=torch.float32).pin_memory()
+        o2, l2 = torch.full_like(qs[2], 5.0).pin_memory(), torch.full((w.Hq, T), 5.0, dtype=torch.float32).pin_memory()
+        B.segpa_attention_fwd_host_async(g.cache, segs, qs[0], w.scale, o0, l0)
+        B.segpa_attention_fwd_host(g.cache, segs, qs[1], w.scale, o1, l1)
+        assert torch.equal(o1, want[1][0]) and torch.equal(l1, want[1][1])
+        B.segpa_attention_fwd_host_async(g.cache, segs, qs[2], w.scale, o2, l2)
+        B.segpa_host_wait(g.cache)
+        B.segpa_host_wait(g.cache)
+        assert torch.equal(o0, want[0][0]) and torch.equal(l0, want[0][1])
+        assert torch.equal(o2, want[2][0]) and torch.equal(l2, want[2][1])
+    finally:
+        g.close()
+
+
 def test_no_dense_allocation():
     """'No dense [B,H,L,D] tensor and no additive mask is built': device memory taken by
     build_segments + attention_fwd stays far below one [L, L] mask."""
