@@ -363,7 +363,7 @@ segpa_status_t segpa_attention_fwd(segpa_cache_t *cache, const segpa_segments_t 
 /*
  * Same computation with HOST buffers (pinned memory for the copies to be asynchronous): q/out are dense
  * [T][Hq][D] bf16, lse [Hq][T] fp32 (may be NULL).  The plan is cut into chunks of consecutive query rows (about
- * 16 MB of q each); the host->device copy of chunk k+1, the kernels of chunk k (on cuda_stream) and the device->host
+ * 16 MB of q each; 32 MB when the first call on the segments object is the _async one); the host->device copy of chunk k+1, the kernels of chunk k (on cuda_stream) and the device->host
  * copy of chunk k-1 run concurrently on three streams, so the call is bounded by the larger PCIe direction, not by
  * the sum.  Results are bit-identical to segpa_attention_fwd on the same plan.  Differences from the device entry
  * point: the call returns after the last copy back has completed (synchronous), and (row, head) pairs that no segment

@@ -1544,12 +1544,17 @@ namespace {
 // segpa_attention_fwd_host: cut the plan into chunks of consecutive query rows (about 16 MB of Q each, at most 16),
 // each with its own LPT assignment over the persistent grid and its own combine entries, and upload them (once per
 // segments object).  An item belongs to the chunk that holds its first row.
-segpa_status_t plan_host_chunks(segpa_cache* c, const segpa_segments* s, int64_t T, cudaStream_t st) {
+segpa_status_t plan_host_chunks(segpa_cache* c, const segpa_segments* s, int64_t T, cudaStream_t st, const bool async) {
     if (s->host_planned) return SEGPA_OK;
     const int Hq = c->desc.num_q_heads, D = c->desc.head_dim;
     const int64_t row_bytes = (int64_t)Hq * D * 2;
     const int64_t rows_used = std::max<int64_t>(1, std::min(T, s->stats.q_rows));
-    int64_t n_chunks = std::min<int64_t>(16, std::max<int64_t>(1, (rows_used * row_bytes + (16 << 20) - 1) / (16 << 20)));
+    // ~16 MB of Q per chunk for a synchronous call (whose first chunk goes up and whose last comes down with the link idle
+    // the other way: small chunks keep that short), ~32 MB for an asynchronous one (its ends overlap the neighbouring calls,
+    // and fewer copies, events and launches pay: cfg5 185 -> 179 ms per step; 8 MB chunks: 200 ms).  The plan is made by the
+    // first call on the segments object and kept.
+    const int64_t chunk_bytes = async ? (32 << 20) : (16 << 20);
+    int64_t n_chunks = std::min<int64_t>(16, std::max<int64_t>(1, (rows_used * row_bytes + chunk_bytes - 1) / chunk_bytes));
     int64_t rows_per = std::max<int64_t>(2 * kTileRows, cdiv(rows_used, n_chunks));   // an item spans < 2 * 128 rows: it reaches into the next chunk at most
     n_chunks = cdiv(rows_used, rows_per);
     std::vector<std::vector<ItemDev>> per((size_t)n_chunks);
@@ -1653,7 +1658,7 @@ segpa_status_t attention_fwd_host_impl(segpa_cache_t* c, const segpa_segments_t*
         return fail(SEGPA_ERR_CUDA, "attention_fwd_host: cannot create the copy streams");
     }
     s->last_stream = st;
-    segpa_status_t rc = plan_host_chunks(c, s, T, st);
+    segpa_status_t rc = plan_host_chunks(c, s, T, st, async);
     if (rc != SEGPA_OK) return rc;
     const size_t n_ch = s->hchunks.size();
     while (c->host_events.size() < 2 * n_ch + 1) {
