@@ -473,6 +473,16 @@ def measure(name: str, steps: int, warmup: int, dev, local_rank: int, world: int
             torch.cuda.synchronize()
 
         e2e_step()
+        # the host-buffer results of the warm-up step against the device entry point (first and last layer, bit for bit;
+        # pairs no segment covers are zeros on both sides): an e2e figure from wrong results would be worthless
+        for l in sorted({0, w.num_layers - 1}):
+            chk = torch.zeros_like(qs[l])
+            chk_lse = torch.zeros((w.Hq, w.T[l]), dtype=torch.float32, device=dev)
+            B.segpa_attention_fwd(cache, seg_objs[l - w.num_layers], qs[l], w.scale, chk, chk_lse, stream=stream)
+            torch.cuda.synchronize()
+            if not (torch.equal(chk.cpu(), h_out[l]) and torch.equal(chk_lse.cpu(), h_lse[l])):
+                raise RuntimeError("e2e: host-buffer results of layer %d differ from the device entry point" % l)
+            del chk, chk_lse
         n_e2e = max(2, min(steps, 5))
         t0 = time.perf_counter()
         for _ in range(n_e2e):
