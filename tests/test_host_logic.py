@@ -58,6 +58,11 @@ def test_no_cpu_fallback_without_gpu():
     rc = B.lib().segpa_attention_fwd(c, segs, ctypes.c_void_p(16), 1024, ctypes.c_float(1.0), ctypes.c_void_p(16), 1024,
                                      None, 0, 1, None)
     assert rc == B.ERR_STATE
+    # the host-buffer entry points too: no device, no result (and nothing to wait for)
+    for fn in (B.lib().segpa_attention_fwd_host, B.lib().segpa_attention_fwd_host_async):
+        assert fn(c, segs, ctypes.c_void_p(16), ctypes.c_float(1.0), ctypes.c_void_p(16), None, 1, None) == B.ERR_STATE
+    B.segpa_host_wait(c)
+    assert B.lib().segpa_host_wait(None) == B.ERR_INVALID
     B.segpa_destroy(c)
 
 
